@@ -1,0 +1,510 @@
+// md_oracle.cpp -- CPU ORACLE for the multiple-double GEMM hot path of arxiv/paper_2607_06881
+// ("Multiple Double Arithmetic on NVIDIA Tensor Cores", Chen & Verschelde).
+//
+// THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and the
+// cpu_baseline / --impl reference legs of bench.py may load it.  It shares no code, header,
+// table or helper with paper_2607_06881_b200/csrc (the CUDA path) and neither includes the other.
+// It is deliberately plain and slow: straight loops in the paper's order and notation, fp64
+// with contraction disabled (-ffp-contract=off), exact arithmetic done with a long accumulator.
+// The only parallelism is an OpenMP `parallel for` over output rows (no blocking, no fusion).
+//
+// Citations are "PAPER.md:<line>" plus section / equation; "DESIGN.md Rn"
+// names a reading of the paper listed in DESIGN.md section 3.
+//
+// Parts (all pinned by tests/test_oracle_*.py against things other than themselves -- exact
+// rational arithmetic in Python, closed forms, hand-derived special cases, the paper's constants):
+//   O1  oracle_exact_*      exact product  C = A*B of multiple-double matrices (plain definition)
+//   O2  oracle_split        Algorithm S: exponent vectors + 13-bit quarters
+//   O3  oracle_orders_*     order matrices C^(s) = sum_{p+q=s} A_p B_q  (eq. 3-4)
+//   O4  oracle_renorm       sum of the S order values -> L non-overlapping limbs
+//   O5  oracle_classic_gemm classical multiple-double GEMM on "regular cores", cross-check
+//   --  oracle_md_gemm      O2 -> O3 (fp64 route) -> O4, the paper's 5-step algorithm
+// Parity status: every function above has an independent pin; none is "parity unpinned".
+
+#include <cmath>
+#include <cstdint>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef unsigned __int128 u128;
+
+// =====================================================================================================
+// Long accumulator: an exact fixed-point two's-complement integer of NW 32-bit digits (stored in int64
+// words with deferred carries).  Bit 0 has weight 2^-BIAS.  Every finite double and every product of two
+// finite doubles is an integer multiple of 2^-2148 below 2^2048, so with BIAS = 2240 and 4608 bits nothing
+// is ever rounded: sums of such terms are exact (a Kulisch accumulator).
+// =====================================================================================================
+namespace {
+
+const int BIAS = 2240;
+const int NW = 144;  // 144 * 32 = 4608 bits
+
+struct LongAcc {
+  int64_t w[NW];
+  int pending;  // additions since the last carry propagation
+
+  LongAcc() { clear(); }
+  void clear() {
+    std::memset(w, 0, sizeof(w));
+    pending = 0;
+  }
+
+  // Carry propagation: afterwards every word except the top one is in [0, 2^32); the top word carries the sign.
+  void normalize() {
+    int64_t carry = 0;
+    for (int i = 0; i < NW; i++) {
+      int64_t v = w[i] + carry;
+      int64_t lo = v & 0xffffffffLL;
+      carry = (v - lo) >> 32;  // arithmetic shift: floor division by 2^32
+      w[i] = lo;
+    }
+    w[NW - 1] += carry << 32;  // keep the sign in the top word
+    pending = 0;
+  }
+
+  // Add sign * mag * 2^e, with mag < 2^106.
+  void add_scaled(u128 mag, int e, int sign) {
+    if (mag == 0) return;
+    int pos = e + BIAS;  // bit position of mag's bit 0
+    int idx = pos >> 5, sh = pos & 31;
+    // mag << sh spans at most 138 bits: three 64-bit words {v2, v1, v0}, i.e. five 32-bit digits.
+    const uint64_t lo = (uint64_t)mag, hi = (uint64_t)(mag >> 64);  // hi < 2^42
+    const u128 low = (u128)lo << sh;                                // < 2^95, weight 2^0
+    const u128 mid = (low >> 64) + ((u128)hi << sh);                // < 2^74, weight 2^64
+    const uint64_t v0 = (uint64_t)low, v1 = (uint64_t)mid, v2 = (uint64_t)(mid >> 64);
+    uint64_t d[5];
+    d[0] = v0 & 0xffffffffULL;
+    d[1] = v0 >> 32;
+    d[2] = v1 & 0xffffffffULL;
+    d[3] = v1 >> 32;
+    d[4] = v2 & 0xffffffffULL;
+    for (int t = 0; t < 5; t++) {
+      if (sign > 0)
+        w[idx + t] += (int64_t)d[t];
+      else
+        w[idx + t] -= (int64_t)d[t];
+    }
+    if (++pending >= (1 << 28)) normalize();
+  }
+
+  // Decompose a finite double: x = sign * mant * 2^e with mant < 2^53 an integer.
+  static void decompose(double x, uint64_t* mant, int* e, int* sign) {
+    uint64_t b;
+    std::memcpy(&b, &x, 8);
+    *sign = (b >> 63) ? -1 : 1;
+    int be = (int)((b >> 52) & 0x7ff);
+    uint64_t f = b & 0xfffffffffffffULL;
+    if (be == 0) {
+      *mant = f;
+      *e = -1074;
+    } else {
+      *mant = f | (1ULL << 52);
+      *e = be - 1075;
+    }
+  }
+
+  void add_double(double x, int sgn = 1) {
+    uint64_t m;
+    int e, s;
+    decompose(x, &m, &e, &s);
+    add_scaled((u128)m, e, s * sgn);
+  }
+
+  void add_product(double a, double b, int sgn = 1) {
+    uint64_t ma, mb;
+    int ea, eb, sa, sb;
+    decompose(a, &ma, &ea, &sa);
+    decompose(b, &mb, &eb, &sb);
+    add_scaled((u128)ma * (u128)mb, ea + eb, sa * sb * sgn);
+  }
+
+  // sign of the value (-1, 0, +1); normalises first.
+  int signum() {
+    normalize();
+    if (w[NW - 1] < 0) return -1;
+    for (int i = 0; i < NW; i++)
+      if (w[i] != 0) return 1;
+    return 0;
+  }
+
+  // Round to nearest double, ties to even (the value must be within double range).  Does not modify *this
+  // except for normalisation.
+  double to_double() {
+    normalize();
+    bool neg = w[NW - 1] < 0;
+    // magnitude digits
+    uint32_t mag[NW];
+    if (!neg) {
+      for (int i = 0; i < NW; i++) mag[i] = (uint32_t)w[i];
+    } else {
+      // two's complement negate of the NW-digit number (top word holds sign-extended value)
+      uint64_t carry = 1;
+      for (int i = 0; i < NW; i++) {
+        uint32_t digit = (uint32_t)(w[i] & 0xffffffffLL);
+        uint64_t v = (uint64_t)(uint32_t)(~digit) + carry;
+        mag[i] = (uint32_t)v;
+        carry = v >> 32;
+      }
+    }
+    int top = -1;
+    for (int i = NW - 1; i >= 0 && top < 0; i--)
+      if (mag[i]) {
+        int b = 31;
+        while (!((mag[i] >> b) & 1)) b--;
+        top = i * 32 + b;
+      }
+    if (top < 0) return 0.0;
+    // lowest bit position we keep: 53 significant bits, but never below the subnormal grid 2^-1074
+    int low = top - 52;
+    int min_low = -1074 + BIAS;
+    if (low < min_low) low = min_low;
+    auto bit = [&](int p) -> int { return p < 0 ? 0 : (int)((mag[p >> 5] >> (p & 31)) & 1); };
+    uint64_t m = 0;
+    for (int p = top; p >= low; p--) m = (m << 1) | (uint64_t)bit(p);
+    int round_bit = bit(low - 1);
+    bool sticky = false;
+    for (int p = low - 2; p >= 0 && !sticky; p--) {
+      if ((p & 31) == 31 && mag[p >> 5] == 0) {
+        p -= 31;
+        continue;
+      }
+      if (bit(p)) sticky = true;
+    }
+    if (round_bit && (sticky || (m & 1))) m++;
+    double r = std::ldexp((double)m, low - BIAS);  // exact: m <= 2^53, result representable
+    return neg ? -r : r;
+  }
+};
+
+// --- error-free transformations (textbook: Knuth TwoSum, Dekker FastTwoSum, TwoProd by fma; PAPER.md refs [2],[15]) ---
+inline void two_sum(double a, double b, double* s, double* e) {
+  double sum = a + b;
+  double bb = sum - a;
+  double err = (a - (sum - bb)) + (b - bb);
+  *s = sum;
+  *e = err;
+}
+inline void fast_two_sum(double a, double b, double* s, double* e) {  // needs |a| >= |b| or a == 0
+  double sum = a + b;
+  *e = b - (sum - a);
+  *s = sum;
+}
+inline void two_prod(double a, double b, double* p, double* e) {
+  double prod = a * b;
+  *e = std::fma(a, b, -prod);
+  *p = prod;
+}
+
+}  // namespace
+
+extern "C" {
+
+// =====================================================================================================
+// O2 -- Algorithm S: exponent vectors and quarters.
+//   PAPER.md:47-49 (section 2): the bits of a double are distributed over 13-bit parts, the quarters, with
+//   exponents 0, -13, -26, -39 relative to the number; a double double gives 8 quarter matrices, the
+//   quarters of the high double first; the exponents must lie on an equally spaced grid ("balanced");
+//   PAPER.md:124-142 (section 3, eq. 7-8): bits are moved between neighbouring parts, without changing the value,
+//   until every part sits on the grid; a zero part is an "unnormalized zero with the desired exponent".
+//   Reading (R1, R2, R4; BASELINE.json north_star): the grid is common to a row of A (axis 0) or a column
+//   of B (axis 1): E_g = ilogb(max |leading limb| over the group) + 1 and quarter q of every element of the group is
+//   an integer multiple of u_q = 2^(E_g - 13(q+1)), the nearest one to what is left of the element (ties to even on
+//   the leading remainder limb), so |digit| <= 2^13 for q = 0 and <= 2^12 after.  All operations are error free.
+//
+//   planes          [limbs][rows][cols]  fp64, input
+//   quarter_planes  [quarters][rows][cols] fp64, output, true-valued quarters d_q = D_q * u_q
+//   exps            int32[rows] (axis 0) or int32[cols] (axis 1), output
+//   remainder       [limbs][rows][cols] or NULL: what is left after the last quarter (sum of quarters + remainder
+//                   == element, exactly)
+// =====================================================================================================
+void oracle_split(int rows, int cols, int limbs, int quarters, int axis, const double* planes,
+                  double* quarter_planes, int32_t* exps, double* remainder) {
+  const size_t plane = (size_t)rows * cols;
+  const int groups = axis == 0 ? rows : cols;
+  // S0: the exponent of each scale group, from the leading limb only.
+  for (int g = 0; g < groups; g++) {
+    double M = 0.0;
+    const int len = axis == 0 ? cols : rows;
+    for (int t = 0; t < len; t++) {
+      size_t at = axis == 0 ? (size_t)g * cols + t : (size_t)t * cols + g;
+      double v = std::fabs(planes[at]);
+      if (v > M) M = v;
+    }
+    exps[g] = (M == 0.0) ? 0 : std::ilogb(M) + 1;  // 2^(E-1) <= M < 2^E
+  }
+  // S1: per element, peel off one quarter at a time.
+#pragma omp parallel for schedule(static)
+  for (int i = 0; i < rows; i++) {
+    std::vector<double> r(limbs);
+    for (int j = 0; j < cols; j++) {
+      const size_t at = (size_t)i * cols + j;
+      const int E = exps[axis == 0 ? i : j];
+      for (int l = 0; l < limbs; l++) r[l] = planes[l * plane + at];
+      for (int q = 0; q < quarters; q++) {
+        const double u = std::ldexp(1.0, E - 13 * (q + 1));  // the unit of quarter q
+        const double c = 6755399441055744.0 * u;            // 3 * 2^51 * u: ulp(c) == u, so r0 + c rounds r0 to a multiple of u
+        const double t = r[0] + c;
+        const double d = t - c;   // exact; the quarter
+        r[0] = r[0] - d;          // exact; |r0| <= u/2 now
+        for (int l = 0; l + 1 < limbs; l++) two_sum(r[l], r[l + 1], &r[l], &r[l + 1]);  // carry into the next limbs
+        quarter_planes[(size_t)q * plane + at] = d;
+      }
+      if (remainder)
+        for (int l = 0; l < limbs; l++) remainder[l * plane + at] = r[l];
+    }
+  }
+}
+
+// =====================================================================================================
+// O3 -- order matrices C^(s)[i,j] = sum_k sum_{p+q=s} A_p[i,k] * B_q[k,j], s = 0..orders-1 (the paper's C_{s+1}).
+//   PAPER.md:66-71 eq. (3): "the convolutions with the sum of the last two indices ... equal to the index of the
+//   quarter"; eq. (4): Cbar = [C_1 ... C_8] = Abar * Bbar with Bbar block upper triangular Toeplitz.
+//   Two routes that must agree bit for bit (that IS the exactness claim of PAPER.md:51-54 and :95-99):
+//   * oracle_orders_int: on the integer digits D = d / u in int64, scaled by 2^(E_i + F_j - 13(s+2)) at the end;
+//   * oracle_orders_fp64: the same sums in plain fp64, k innermost, products in the order p = 0..s.
+//   Aq [quarters][m][k], Bq [quarters][k][n], order_planes [orders][m][n] (true values).
+// =====================================================================================================
+void oracle_orders_int(int m, int n, int k, int quarters, int orders, const double* Aq, const int32_t* expA,
+                       const double* Bq, const int32_t* expB, double* order_planes, int64_t* raw_sums) {
+  const size_t pa = (size_t)m * k, pb = (size_t)k * n, pc = (size_t)m * n;
+  // integer digits
+  std::vector<int32_t> DA((size_t)quarters * pa), DB((size_t)quarters * pb);
+  for (int q = 0; q < quarters; q++) {
+    for (int i = 0; i < m; i++)
+      for (int t = 0; t < k; t++)
+        DA[q * pa + (size_t)i * k + t] = (int32_t)std::ldexp(Aq[q * pa + (size_t)i * k + t], -(expA[i] - 13 * (q + 1)));
+    for (int t = 0; t < k; t++)
+      for (int j = 0; j < n; j++)
+        DB[q * pb + (size_t)t * n + j] = (int32_t)std::ldexp(Bq[q * pb + (size_t)t * n + j], -(expB[j] - 13 * (q + 1)));
+  }
+#pragma omp parallel for schedule(static)
+  for (int i = 0; i < m; i++)
+    for (int j = 0; j < n; j++)
+      for (int s = 0; s < orders; s++) {
+        int64_t acc = 0;
+        for (int p = 0; p <= s; p++) {
+          const int q = s - p;
+          if (p >= quarters || q >= quarters) continue;
+          for (int t = 0; t < k; t++)
+            acc += (int64_t)DA[p * pa + (size_t)i * k + t] * (int64_t)DB[q * pb + (size_t)t * n + j];
+        }
+        if (raw_sums) raw_sums[s * pc + (size_t)i * n + j] = acc;
+        // |acc| < 2^53 under the k-budget (R6), so the conversion and the scaling are exact.
+        order_planes[s * pc + (size_t)i * n + j] = std::ldexp((double)acc, expA[i] + expB[j] - 13 * (s + 2));
+      }
+}
+
+// The same integer route at sampled output positions only (for full-size matrices): out[t*orders + s] = C^(s)[si[t], sj[t]].
+void oracle_orders_int_samples(int m, int n, int k, int quarters, int orders, const double* Aq, const int32_t* expA,
+                               const double* Bq, const int32_t* expB, int64_t nsamples, const int64_t* si,
+                               const int64_t* sj, double* out) {
+  const size_t pa = (size_t)m * k, pb = (size_t)k * n;
+#pragma omp parallel for schedule(dynamic, 16)
+  for (int64_t t = 0; t < nsamples; t++) {
+    const int64_t i = si[t], j = sj[t];
+    for (int s = 0; s < orders; s++) {
+      int64_t acc = 0;
+      for (int p = 0; p <= s; p++) {
+        const int q = s - p;
+        if (p >= quarters || q >= quarters) continue;
+        for (int kk = 0; kk < k; kk++) {
+          const int64_t da = (int64_t)std::ldexp(Aq[p * pa + (size_t)i * k + kk], -(expA[i] - 13 * (p + 1)));
+          const int64_t db = (int64_t)std::ldexp(Bq[q * pb + (size_t)kk * n + j], -(expB[j] - 13 * (q + 1)));
+          acc += da * db;
+        }
+      }
+      out[t * orders + s] = std::ldexp((double)acc, expA[i] + expB[j] - 13 * (s + 2));
+    }
+  }
+}
+
+void oracle_orders_fp64(int m, int n, int k, int quarters, int orders, const double* Aq, const double* Bq,
+                        double* order_planes) {
+  const size_t pa = (size_t)m * k, pb = (size_t)k * n, pc = (size_t)m * n;
+#pragma omp parallel for schedule(static)
+  for (int i = 0; i < m; i++)
+    for (int j = 0; j < n; j++)
+      for (int s = 0; s < orders; s++) {
+        double acc = 0.0;
+        for (int p = 0; p <= s; p++) {
+          const int q = s - p;
+          if (p >= quarters || q >= quarters) continue;
+          for (int t = 0; t < k; t++) acc += Aq[p * pa + (size_t)i * k + t] * Bq[q * pb + (size_t)t * n + j];
+        }
+        order_planes[s * pc + (size_t)i * n + j] = acc;
+      }
+}
+
+// =====================================================================================================
+// O4 -- recombination.  PAPER.md:88-91 steps 4-5: "Add the parts of the product into a double double matrix ...
+//   summing 8 doubles into one double double for each element".  The oracle's result is the plain definition: the
+//   exact sum of the `orders` values, rounded to `limbs` limbs one after another, limb_l = RN(sum - limb_0 - ... -
+//   limb_{l-1}).  Several results are acceptable for an implementation (R9); this one is the best possible.
+// =====================================================================================================
+void oracle_renorm(int m, int n, int limbs, int orders, const double* order_planes, double* C_planes) {
+  const size_t pc = (size_t)m * n;
+#pragma omp parallel for schedule(static)
+  for (int i = 0; i < m; i++) {
+    LongAcc acc;
+    for (int j = 0; j < n; j++) {
+      const size_t at = (size_t)i * n + j;
+      acc.clear();
+      for (int s = 0; s < orders; s++) acc.add_double(order_planes[s * pc + at]);
+      for (int l = 0; l < limbs; l++) {
+        const double v = acc.to_double();
+        C_planes[l * pc + at] = v;
+        acc.add_double(v, -1);
+      }
+    }
+  }
+}
+
+// =====================================================================================================
+// O1 -- the exact product (the plain definition of what the whole path must reach).
+//   a_ik = sum_l A_l[i,k], b_kj = sum_l B_l[k,j] (Definition 1.1: a multiple double is the unevaluated
+//   sum of its doubles); C_exact[i,j] = sum_k a_ik * b_kj, W[i,j] = sum_k |a_ik| |b_kj| = (|A||B|)_ij, all exact.
+//   For each sampled position (si[t], sj[t]):
+//     Cexact_limbs[t*out_limbs + l]  the exact value rounded to out_limbs limbs (if not NULL)
+//     W[t]                            (|A||B|)_ij rounded to double (if not NULL)
+//     err[t]                          | sum_l C_l[i,j] - C_exact[i,j] | evaluated exactly, then rounded (if C not NULL)
+//   A [limbs][m][k], B [limbs][k][n], C [limbs][m][n].
+// =====================================================================================================
+void oracle_exact_samples(int m, int n, int k, int limbs, const double* A, const double* B, const double* C,
+                          int64_t nsamples, const int64_t* si, const int64_t* sj, double* err, double* W,
+                          double* Cexact_limbs, int out_limbs) {
+  const size_t pa = (size_t)m * k, pb = (size_t)k * n, pc = (size_t)m * n;
+#pragma omp parallel for schedule(dynamic, 16)
+  for (int64_t t = 0; t < nsamples; t++) {
+    const int64_t i = si[t], j = sj[t];
+    LongAcc acc, wacc, aabs, babs;
+    for (int kk = 0; kk < k; kk++) {
+      for (int la = 0; la < limbs; la++)
+        for (int lb = 0; lb < limbs; lb++)
+          acc.add_product(A[la * pa + (size_t)i * k + kk], B[lb * pb + (size_t)kk * n + j]);
+      if (W) {
+        // |a_ik| * |b_kj| = sign(a) sign(b) * a * b with the signs of the exact sums of limbs
+        aabs.clear();
+        babs.clear();
+        for (int la = 0; la < limbs; la++) aabs.add_double(A[la * pa + (size_t)i * k + kk]);
+        for (int lb = 0; lb < limbs; lb++) babs.add_double(B[lb * pb + (size_t)kk * n + j]);
+        const int sg = aabs.signum() * babs.signum();
+        if (sg != 0)
+          for (int la = 0; la < limbs; la++)
+            for (int lb = 0; lb < limbs; lb++)
+              wacc.add_product(A[la * pa + (size_t)i * k + kk], B[lb * pb + (size_t)kk * n + j], sg);
+      }
+    }
+    if (W) W[t] = wacc.to_double();
+    if (Cexact_limbs) {
+      LongAcc tmp = acc;
+      for (int l = 0; l < out_limbs; l++) {
+        const double v = tmp.to_double();
+        Cexact_limbs[t * out_limbs + l] = v;
+        tmp.add_double(v, -1);
+      }
+    }
+    if (C && err) {
+      for (int l = 0; l < limbs; l++) acc.add_double(C[l * pc + (size_t)i * n + j], -1);
+      err[t] = std::fabs(acc.to_double());
+    }
+  }
+}
+
+// Exact sum of `count` doubles rounded to `limbs` limbs (used by tests to examine the accumulator itself).
+void oracle_exact_sum(int count, const double* x, int limbs, double* out) {
+  LongAcc acc;
+  for (int i = 0; i < count; i++) acc.add_double(x[i]);
+  for (int l = 0; l < limbs; l++) {
+    out[l] = acc.to_double();
+    acc.add_double(out[l], -1);
+  }
+}
+
+// Exact dot product sum_i x[i]*y[i] rounded to `limbs` limbs.
+void oracle_exact_dot(int count, const double* x, const double* y, int limbs, double* out) {
+  LongAcc acc;
+  for (int i = 0; i < count; i++) acc.add_product(x[i], y[i]);
+  for (int l = 0; l < limbs; l++) {
+    out[l] = acc.to_double();
+    acc.add_double(out[l], -1);
+  }
+}
+
+// =====================================================================================================
+// O5 -- classical multiple-double GEMM, "a single thread executes an inner product" in multiple-double arithmetic on
+//   regular cores (the paper's C_CUDA of eq. 9).  Built from the textbook error-free transformations
+//   only (refs [2], [3], [15]: TwoSum, FastTwoSum, TwoProd): every partial product a_la * b_lb with la + lb < limbs
+//   is formed exactly by TwoProd, those with la + lb == limbs in plain fp64, and each term is added into a
+//   (limbs+1)-term accumulator by a TwoSum cascade, followed by a renormalising sweep.  Its own error is about
+//   k * 2^-(53*limbs - 2) * (|A||B|)_ij, so it is a cross-check with that threshold, not the ground truth.
+// =====================================================================================================
+static void md_cascade_add(double* acc, int terms, double x) {
+  for (int l = 0; l < terms; l++) two_sum(acc[l], x, &acc[l], &x);  // what is left in x is below the last term
+}
+static void md_renormalise(double* acc, int terms) {
+  // bottom-up then top-down sweep of FastTwoSum/TwoSum: leaves a non-overlapping, decreasing expansion
+  for (int l = terms - 1; l > 0; l--) two_sum(acc[l - 1], acc[l], &acc[l - 1], &acc[l]);
+  for (int l = 0; l + 1 < terms; l++) two_sum(acc[l], acc[l + 1], &acc[l], &acc[l + 1]);
+}
+
+void oracle_classic_gemm(int m, int n, int k, int limbs, const double* A, const double* B, double* C) {
+  const size_t pa = (size_t)m * k, pb = (size_t)k * n, pc = (size_t)m * n;
+  const int terms = limbs + 1;
+#pragma omp parallel for schedule(static)
+  for (int i = 0; i < m; i++) {
+    std::vector<double> acc(terms);
+    for (int j = 0; j < n; j++) {
+      for (int l = 0; l < terms; l++) acc[l] = 0.0;
+      for (int kk = 0; kk < k; kk++) {
+        for (int la = 0; la < limbs; la++)
+          for (int lb = 0; la + lb <= limbs && lb < limbs; lb++) {
+            const double a = A[la * pa + (size_t)i * k + kk], b = B[lb * pb + (size_t)kk * n + j];
+            if (la + lb < limbs) {
+              double p, e;
+              two_prod(a, b, &p, &e);
+              md_cascade_add(acc.data(), terms, p);
+              md_cascade_add(acc.data(), terms, e);
+            } else {
+              md_cascade_add(acc.data(), terms, a * b);
+            }
+          }
+        md_renormalise(acc.data(), terms);
+      }
+      for (int l = 0; l < limbs; l++) C[l * pc + (size_t)i * n + j] = acc[l];
+    }
+  }
+}
+
+// =====================================================================================================
+// The paper's five steps end to end: split -> (rewrite) -> quarter products -> (extract) -> add the
+// parts.  Steps 2 and 4 are index bookkeeping only (Abar/Bbar are never stored).  Computes rows [row0,row1) of C
+// into C_rows [limbs][row1-row0][n]; B's quarters are computed for the whole of B every call.
+// =====================================================================================================
+void oracle_md_gemm_rows(int m, int n, int k, int limbs, int quarters, int orders, const double* A, const double* B,
+                         int row0, int row1, double* C_rows) {
+  const int mr = row1 - row0;
+  std::vector<double> Arows((size_t)limbs * mr * k);
+  for (int l = 0; l < limbs; l++)
+    std::memcpy(&Arows[(size_t)l * mr * k], &A[(size_t)l * m * k + (size_t)row0 * k], sizeof(double) * (size_t)mr * k);
+  std::vector<double> Aq((size_t)quarters * mr * k), Bq((size_t)quarters * k * n), ord((size_t)orders * mr * n);
+  std::vector<int32_t> eA(mr), eB(n);
+  oracle_split(mr, k, limbs, quarters, 0, Arows.data(), Aq.data(), eA.data(), nullptr);
+  oracle_split(k, n, limbs, quarters, 1, B, Bq.data(), eB.data(), nullptr);
+  oracle_orders_fp64(mr, n, k, quarters, orders, Aq.data(), Bq.data(), ord.data());
+  oracle_renorm(mr, n, limbs, orders, ord.data(), C_rows);
+}
+
+int oracle_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+}  // extern "C"
