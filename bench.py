@@ -1,0 +1,314 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the multiple-double GEMM hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 2]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
+        bench.py --gpus N --steps K --warmup W
+
+A "step" is one pass of the whole hot path (md_gemm: exponent vectors + split of A and B + fused quarter GEMM with the
+renormalising epilogue) over one seeded synthetic problem.  The workload at N = 1 is
+BASELINE.json configs[2], the config its metric is quoted on: double-double 4096^3, hi ~ N(0,1), lo = hi*2^-53*U[-1,1].
+With N > 1 the rows of A are sharded (rank r owns rows [r*4096, (r+1)*4096) of an (N*4096) x 4096 A, B replicated): no
+data-path collective is needed because a row's exponent depends on that row only -> weak scaling.
+
+Rank 0 prints ONE JSON line.  value = whole-job double-double GFLOP/s (2mnk per problem) with inputs resident in HBM;
+e2e = the same through md_gemm_host with pinned HOST buffers (H2D of A, B and D2H of C inside the timed region);
+roofline = the fused quarter-GEMM kernel's issued FP64 flops (T*2mnk, T = 36) / its CUDA-event duration against the FP64
+tensor (DMMA) peak; cpu_baseline = the CPU oracle (oracle/, as it stands) on a bounded sample, same run, rank 0, N = 1.
+--impl reference times that oracle alone (there is no reference implementation to install: /root/reference holds only
+the paper's text).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "effective double-double GFLOP/s at n=4096 on 1 B200; % of FP64 tensor peak"
+UNIT = "GFLOP/s (double-double, 2mnk)"
+# FP64 tensor (DMMA) peak of B200: 128 flop/clk/SM x 148 SMs x 1.965 GHz (clocks.max.sm).  MEASURED_PEAKS.json holds
+# no FP64 figure; a register-only mma.sync.m8n8k4.f64 loop on this pool's B200 measured 128.0 flop/clk/SM and
+# 37.07 TFLOP/s at 1.957 GHz (profiles/r01_dmma_peak.md), cuBLAS DGEMM 8192^3 35.5 TFLOP/s.  DESIGN.md section 6.
+FP64_TENSOR_PEAK_TFLOPS = 128 * 148 * 1.965e9 / 1e12
+# The paper's own figure for this metric and workload (double double, n = 4096, whole pipeline t_TC = 7.93621 s ->
+# 2*4096^3 / t = 17.3 GFLOP/s; Table 1; hardware A100 or RTX 4080, the paper does not say): context only.
+PAPER_DD_4096_GFLOPS = 2 * 4096 ** 3 / 7.93621 / 1e9
+CPU_SAMPLE_ROWS = 16
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (default 2: the headline)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+class ClockSampler(threading.Thread):
+    """Samples nvidia-smi clocks / throttle reasons of one GPU every 200 ms while running."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        super().__init__(daemon=True)
+        self.gpu_index = gpu_index
+        self.samples = []
+        self.proc = None
+
+    def run(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.gpu_index), f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits",
+                 "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            for line in self.proc.stdout:
+                parts = [p.strip() for p in line.split(",")]
+                if len(parts) == 7:
+                    self.samples.append(parts)
+        except Exception:
+            pass
+
+    def stop(self):
+        if self.proc is not None:
+            self.proc.terminate()
+
+    def summary(self, t0: float = 0.0):
+        sm, reasons, mx, power = [], set(), None, []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for s in self.samples:
+            try:
+                sm.append(float(s[0]))
+                mx = float(s[1])
+                power.append(float(s[2]))
+            except ValueError:
+                continue
+            for name, val in zip(names, s[3:]):
+                if val == "Active":
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        busy = [c for c, p in zip(sm, power) if p > 0.5 * max(power)] or sm  # samples under load
+        return {"sm_mhz": statistics.median(busy), "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "power_w_max": max(power), "samples": len(sm)}
+
+
+def cpu_oracle_sample(cfg, rows: int):
+    """The oracle's five-step pipeline on the first `rows` rows of A (all of B): returns (GFLOP/s, seconds, threads)."""
+    from oracle import md_oracle as orc
+    from paper_2607_06881_b200 import inputs
+    A = inputs.generate(cfg, "A", 0, rows)
+    B = inputs.generate(cfg, "B")
+    threads = min(orc.num_threads(), rows)
+    t0 = time.perf_counter()
+    orc.md_gemm_rows(A, B, quarters=cfg.quarters)
+    dt = time.perf_counter() - t0
+    return 2.0 * rows * cfg.n * cfg.k / dt / 1e9, dt, threads
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from paper_2607_06881_b200 import inputs
+    cfg = inputs.CONFIGS[args.config]
+    rows = CPU_SAMPLE_ROWS
+    for _ in range(min(args.warmup, 1)):
+        cpu_oracle_sample(cfg, 2)
+    steps = max(1, min(args.steps, 3))  # each step is ~10-20 s of CPU work; keep the run within minutes
+    vals, secs, threads = [], [], 1
+    for _ in range(steps):
+        v, dt, threads = cpu_oracle_sample(cfg, rows)
+        vals.append(v)
+        secs.append(dt)
+    value = 2.0 * rows * cfg.n * cfg.k * steps / sum(secs) / 1e9
+    sample = (f"first {rows} rows of A ({rows}x{cfg.n} outputs of the {cfg.m}x{cfg.n}x{cfg.k} problem), all of B; "
+              f"oracle split + {cfg.products} plain fp64 quarter GEMM loops + exact renorm; {steps} step(s) timed "
+              f"(--steps capped at 3)")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+        "warmup": min(args.warmup, 1), "ms_per_step": 1e3 * sum(secs) / steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": value / PAPER_DD_4096_GFLOPS if args.config == 2 else None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{cfg.index}] {cfg.name}: {cfg.m}x{cfg.n}x{cfg.k}, limbs={cfg.limbs}, "
+                               f"quarters={cfg.quarters}, seed {cfg.seed}", "kind": "CPU oracle (no GPU work)"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2607_06881_b200 import binding as md
+    from paper_2607_06881_b200 import inputs
+    from paper_2607_06881_b200 import shard
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback")
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}; launch with torch.distributed.run")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    md.lib()  # fail loudly now if the extension is missing
+
+    base = inputs.CONFIGS[args.config]
+    # weak scaling: the global A has world * m rows, rank r owns one block of m rows (no collective on the data path)
+    cfg = base.with_shape(m=base.m * world)
+    row0, row1 = shard.row_block(cfg.m, world, rank)
+    m, n, k, L, Q = row1 - row0, cfg.n, cfg.k, cfg.limbs, cfg.quarters
+    A_host = torch.from_numpy(inputs.generate(cfg, "A", row0, row1)).pin_memory()
+    B_host = torch.from_numpy(inputs.generate(cfg, "B")).pin_memory()
+    C_host = torch.empty((L, m, n), dtype=torch.float64).pin_memory()
+    A, B = A_host.cuda(), B_host.cuda()
+    C = torch.empty((L, m, n), dtype=torch.float64, device="cuda")
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x: float) -> float:
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    sampler = ClockSampler(local_rank)
+    with md.Workspace(m, n, k, L, Q):
+        for _ in range(args.warmup):
+            md.md_gemm(A, B, C)
+        barrier()
+        sampler.start()
+        md.md_profile_enable(args.steps)
+        launches0 = md.md_launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record(stream)
+        for _ in range(args.steps):
+            md.md_gemm(A, B, C)
+        e1.record(stream)
+        barrier()
+        ms_total = max_over_ranks(e0.elapsed_time(e1))
+        launches = md.md_launch_count() - launches0
+        split_ms, gemm_ms = md.md_profile_read(args.steps)
+        md.md_profile_enable(0)
+        flags = md.md_read_flags()
+    clocks_after_device_loop = len(sampler.samples)
+
+    # end to end: pinned host buffers through md_gemm_host (H2D A, B + the whole path + D2H C, synchronous)
+    e2e = None
+    if not args.no_e2e:
+        scratch = torch.empty(md.md_host_scratch_bytes(m, n, k, L), dtype=torch.uint8, device="cuda")
+        md.md_set_option(md.MD_OPT_QUARTERS, 0 if Q == 4 * L else Q)
+        for _ in range(min(args.warmup, 2)):
+            md.md_gemm_host(A_host, B_host, C_host, scratch)
+        barrier()
+        launches_e2e0 = md.md_launch_count()
+        t0 = time.perf_counter()
+        e0.record(stream)
+        for _ in range(args.steps):
+            md.md_gemm_host(A_host, B_host, C_host, scratch)
+        e1.record(stream)
+        barrier()
+        e2e_ms = max_over_ranks(e0.elapsed_time(e1))
+        wall_ms = max_over_ranks((time.perf_counter() - t0) * 1e3)
+        md.md_set_option(md.MD_OPT_QUARTERS, 0)
+        e2e = {"value": world * base.md_flops * args.steps / (max(e2e_ms, wall_ms) * 1e-3) / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": A_host.numel() * 8 + B_host.numel() * 8, "d2h_bytes_per_step": C_host.numel() * 8,
+               "ms_per_step": max(e2e_ms, wall_ms) / args.steps, "launches": md.md_launch_count() - launches_e2e0,
+               "matches_device_path": bool((C_host == C.cpu()).all())}
+        del scratch
+    sampler.stop()
+    clocks = sampler.summary()
+    clocks["samples_in_device_loop"] = clocks_after_device_loop
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    ms_per_step = ms_total / args.steps
+    value = world * base.md_flops / (ms_per_step * 1e-3) / 1e9
+    gemm_avg_ms = sum(gemm_ms) / len(gemm_ms)
+    issued_flops = base.fp64_flops  # T * 2mnk per launch (per rank)
+    achieved = issued_flops / (gemm_avg_ms * 1e-3) / 1e12
+    roofline = {
+        "bound": "tensor", "kernel": "qgemm_kernel (fused triangular quarter GEMM + renormalising epilogue)",
+        "achieved": achieved, "peak": FP64_TENSOR_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_TENSOR_PEAK_TFLOPS,
+        "peak_source": "FP64 DMMA: 128 flop/clk/SM x 148 SMs x 1.965 GHz (MEASURED_PEAKS.json has no FP64 entry; "
+                       "microbenchmark on this pool measured 37.07 TFLOP/s, profiles/r01_dmma_peak.md)",
+        "algorithmic_flops_per_launch": issued_flops, "kernel_ms": gemm_avg_ms, "split_ms": sum(split_ms) / len(split_ms),
+        "kernel_share_of_step": gemm_avg_ms / ms_per_step,
+        "traffic": None,
+    }
+    traffic_file = os.path.join(ROOT, "profiles", "r01_qgemm_traffic.json")
+    if os.path.exists(traffic_file) and args.config == 2:
+        try:
+            roofline["traffic"] = json.load(open(traffic_file))["dram_bytes_per_launch"]
+        except Exception:
+            pass
+
+    cpu_baseline = None
+    if world == 1 and not args.no_cpu_baseline:
+        v, dt, threads = cpu_oracle_sample(base, CPU_SAMPLE_ROWS)
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "seconds": dt,
+                        "sample": f"first {CPU_SAMPLE_ROWS} rows of A ({CPU_SAMPLE_ROWS}x{base.n} outputs of the "
+                                  f"{base.m}x{base.n}x{base.k} problem), all of B; oracle split + {base.products} plain "
+                                  f"fp64 quarter GEMM loops + exact renorm, OpenMP over rows"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": value / PAPER_DD_4096_GFLOPS if args.config == 2 else None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {
+            "workload": f"BASELINE.json configs[{base.index}] {base.name}: m={base.m} n={base.n} k={base.k} per GPU, "
+                        f"limbs={L}, quarters={Q} (T={base.products} quarter products), seed {base.seed}",
+            "parallelism": "single GPU" if world == 1 else f"rows of A sharded over {world} GPUs, B replicated, no collective",
+            "l2": "inputs (%.0f MiB) and quarter planes (%.0f MiB) exceed the 126 MB L2; no explicit flush" % (
+                (A.numel() + B.numel()) * 8 / 2 ** 20, 8.0 * Q * (m * k + k * n) / 2 ** 20),
+            "paper_baseline": "PAPER.md:184 Table 1 t_TC(dd, n=4096) = 7.93621 s = 17.3 GFLOP/s on A100 or RTX 4080 (unstated)",
+        },
+        "fp64_tflops_issued": world * base.fp64_flops / (ms_per_step * 1e-3) / 1e12,
+        "pct_of_fp64_tensor_peak": 100.0 * base.fp64_flops / (ms_per_step * 1e-3) / 1e12 / FP64_TENSOR_PEAK_TFLOPS,
+        "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": launches,
+        "clocks": clocks, "status_flags": flags,
+    }
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

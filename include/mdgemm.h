@@ -1,0 +1,165 @@
+/* mdgemm.h -- C-ABI boundary of the B200 (sm_100a) multiple-double matrix multiplication library.
+ *
+ * Hot path of "Multiple Double Arithmetic on NVIDIA Tensor Cores" (Chen & Verschelde, arxiv/paper_2607_06881):
+ *   C = A * B for matrices whose elements are multiple doubles (Definition 1.1: an unevaluated sum of
+ *   non-overlapping doubles), stored as `limbs` fp64 LIMB PLANES (double-double: A_hi, A_lo; quad-double:
+ *   4 planes).  The five steps of PAPER.md:82-89 are:
+ *     1. split every element into 13-bit "quarters"                                   -> md_split      (a1 + a2)
+ *     2./3. multiply the quarter matrices on the FP64 tensor pipe, exactly            -> md_qgemm      (a3)
+ *     4./5. extract the parts C_1..C_S and add them into a multiple-double matrix     -> md_renorm     (a4)
+ *   and md_gemm runs all of them (steps 3-5 fused in one kernel: the stacked matrices Abar, Bbar of eq. (4),
+ *   PAPER.md:75, are never built).  Citations "PAPER.md:<line>" refer to /root/reference/PAPER.md; "DESIGN.md Rn" to
+ *   the readings of the paper listed in DESIGN.md section 3.
+ *
+ * Conventions for every entry point
+ *   - No torch / C++ types: plain pointers and sizes.  Unless a parameter says "host", every data pointer is a DEVICE
+ *     pointer (cudaMalloc'ed or a torch CUDA tensor's data_ptr) on the current device, 8-byte aligned (16-byte
+ *     alignment together with even column counts enables the vectorised paths; anything else still works).
+ *   - Matrices are dense, row-major planes: a multiple-double matrix X (rows x cols) with `limbs` limbs is
+ *     limbs * rows * cols doubles, plane l at X + l*rows*cols, element (i,j) of plane l at X[l*rows*cols + i*cols + j]
+ *     (a contiguous torch tensor [limbs, rows, cols]).  Plane 0 is the leading (high) double.
+ *   - `stream` is a cudaStream_t passed as an opaque pointer (NULL = the legacy default stream).  Calls ENQUEUE work on
+ *     it and return without synchronising (md_gemm_host and md_read_flags excepted); they are safe to capture in a
+ *     CUDA graph.  The library never allocates device memory; the caller owns every buffer, and must keep it alive until
+ *     the stream has run the work.  Inputs are read-only; outputs must not alias inputs or the workspace.
+ *   - Return value: MD_OK (0) or a negative md_status.  Errors are detected from the ARGUMENTS only, synchronously,
+ *     and nothing has been enqueued when one is returned (MD_ERR_CUDA: a launch failed; cudaGetLastError is preserved).
+ *   - Data preconditions (cannot be seen without a sync, so they are not return codes): inputs finite; the leading limb
+ *     is the largest in magnitude and |limb_{l+1}| <= ulp(limb_l); every group exponent (below) within [-900, 900].
+ *     Violations set bits in a device status word (md_read_flags) and give unspecified values, never a fault.
+ *   - Not thread-safe with respect to md_set_option / md_set_workspace (process-wide state); otherwise re-entrant.
+ */
+#ifndef MDGEMM_H_
+#define MDGEMM_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef int md_status;
+enum {
+  MD_OK = 0,
+  MD_ERR_BAD_ARG = -1,      /* null pointer, dimension <= 0, misaligned pointer, limbs/quarters/orders unsupported */
+  MD_ERR_K_TOO_LARGE = -2,  /* k exceeds the exactness budget k * orders <= 2^27 (eq. 5; R6) */
+  MD_ERR_WORKSPACE = -3,    /* no workspace registered, or it is too small (md_workspace_bytes) */
+  MD_ERR_CUDA = -4,         /* a CUDA call failed */
+  MD_ERR_UNSUPPORTED = -5   /* combination of (limbs, quarters, orders) that has no kernel instantiation */
+};
+
+typedef void* md_stream;    /* a cudaStream_t */
+
+/* Options (process-wide).  value 0 restores the default. */
+enum {
+  MD_OPT_QUARTERS = 1,  /* quarters per element used by md_gemm / md_gemm_orders / md_gemm_host.  Default 4*limbs, the
+                           paper's count (8 for double double, 16 for quad double).  Supported:
+                           limbs=2: 8, 9, 10; limbs=4: 16, 17, 18 (R5). */
+  MD_OPT_ORDERS = 2     /* kept product orders S (the paper's C_1..C_S).  Default = quarters.  Must equal
+                           quarters in this version. */
+};
+md_status md_set_option(int key, int value);
+int md_get_option(int key); /* current value (0 = default), or -1 for an unknown key */
+
+/* ---------------------------------------------------------------------------------------------------------------------
+ * md_split -- steps a1 + a2: exponent vectors ("balancing") and quarter planes.
+ *   PAPER.md:47-49 (section 2): the bits of a double are distributed over parts of 13 bits, the QUARTERS, doubles with
+ *   exponents 0, -13, -26, -39; a double double gives 8 quarter matrices; exactness needs the
+ *   exponents on an equally spaced grid; PAPER.md:124-142 (section 3): bits are moved between parts, value unchanged,
+ *   until they are; zeros are "unnormalized zeros with the desired exponent".  Reading (R1-R4): one exponent
+ *   per ROW (axis = 0, use for A) or per COLUMN (axis = 1, use for B):
+ *       exps[g]  = E_g = ilogb(max over the group of |leading limb|) + 1   (0 for an all-zero group)
+ *       quarter q of an element of group g = D * 2^(E_g - 13(q+1)), D an integer, |D| <= 2^13 (q = 0), 2^12 (q > 0),
+ *       chosen nearest to what is left of the element after quarters 0..q-1 (ties to even on the leading remainder
+ *       limb).  The element equals the sum of its quarters plus a remainder of at most 2^(E_g - 13*quarters - 1)
+ *       (1 + 2^-27) in magnitude; the remainder is zero when the element fits the 13*quarters-bit window below 2^E_g.
+ *   planes          in   [limbs][rows][cols]
+ *   quarter_planes  out  [quarters][rows][cols]  true-valued quarters (not the integers D)
+ *   exps            out  int32[rows] (axis 0) / int32[cols] (axis 1)
+ *   limbs in {1, 2, 4}; 1 <= quarters <= 24; rows, cols >= 1.  Bit-exact against the oracle's Algorithm S.
+ * ------------------------------------------------------------------------------------------------------------------ */
+md_status md_split(int rows, int cols, int limbs, int quarters, int axis, const double* planes,
+                   double* quarter_planes, int32_t* exps, md_stream stream);
+
+/* ---------------------------------------------------------------------------------------------------------------------
+ * md_qgemm -- steps a3 (+ a4): the triangular set of quarter products on the FP64 tensor pipe (DMMA).
+ *   PAPER.md:66-71 eq. (3) and :75-78 eq. (4): C^(s) = sum_{p+q=s} A_p * B_q for s = 0..orders-1 (the paper's C_{s+1}),
+ *   orders*(orders+1)/2 quarter GEMMs (36 for double double) instead of the 64 blocks of Abar*Bbar.  Every fp64
+ *   accumulation is exact, so the result does not depend on any summation order.
+ *   Aq            in   [quarters][m][k]  quarter planes of A (md_split axis 0)
+ *   Bq            in   [quarters][k][n]  quarter planes of B (md_split axis 1)
+ *   order_planes  out  [orders][m][n] fp64, C^(s) true-valued; may be NULL
+ *   C_planes      out  [limbs][m][n]: the orders summed error-free into `limbs` limbs in the kernel's epilogue
+ *                      (same arithmetic as md_renorm); may be NULL.  Not both NULL.
+ *   Needs orders == quarters, (limbs, quarters) as listed at MD_OPT_QUARTERS, k * orders <= 2^27.
+ * ------------------------------------------------------------------------------------------------------------------ */
+md_status md_qgemm(int m, int n, int k, int limbs, int quarters, int orders, const double* Aq, const double* Bq,
+                   double* order_planes, double* C_planes, md_stream stream);
+
+/* ---------------------------------------------------------------------------------------------------------------------
+ * md_renorm -- step a4: recombination.  PAPER.md:88-91 steps 4-5: "summing 8 doubles into one double double for each
+ *   element of the product ... in double double arithmetic ... on regular cores".
+ *   order_planes  in   [orders][m][n]
+ *   C_planes      out  [limbs][m][n]:  sum_s C^(s) as `limbs` non-overlapping doubles (|limb_{l+1}| <= ulp(limb_l)/2),
+ *                      within 2^-(53*limbs - 3) * sum_s |C^(s)| of the exact sum (R9).
+ *   limbs in {1, 2, 4}; 1 <= orders <= 24.
+ * ------------------------------------------------------------------------------------------------------------------ */
+md_status md_renorm(int m, int n, int limbs, int orders, const double* order_planes, double* C_planes,
+                    md_stream stream);
+
+/* ---------------------------------------------------------------------------------------------------------------------
+ * md_gemm -- the whole hot path: C = A * B (all five steps), A: m x k, B: k x n, C: m x n, each with
+ *   `limbs` limb planes.  Splits A by rows and B by columns into the registered workspace, then one fused kernel does
+ *   the quarter products and writes the renormalised C once.  limbs in {2, 4}.
+ *   Accuracy: |C - A*B|_ij <= k (Q+1) 2^(E_i + F_j - 13Q - 2) + 2^-(53*limbs - 3) |C|_ij for any input (Q = quarters; E, F
+ *   the exponent vectors of A's rows and B's columns); on the BASELINE.json workloads this is within 1e-28 (|A||B|)_ij
+ *   (double double) and 1e-58 (|A||B|)_ij (quad double).
+ *   md_gemm_orders is the debug/parity variant: same split, then writes the order matrices C^(s) [orders][m][n] instead.
+ * ------------------------------------------------------------------------------------------------------------------ */
+md_status md_gemm(int m, int n, int k, int limbs, const double* A_planes, const double* B_planes, double* C_planes,
+                  md_stream stream);
+md_status md_gemm_orders(int m, int n, int k, int limbs, const double* A_planes, const double* B_planes,
+                         double* order_planes, md_stream stream);
+
+/* Workspace for md_gemm / md_gemm_orders: quarter planes of A and B, exponent vectors and the status word, for the
+ * CURRENT option values.  The caller allocates (device memory, 256-byte aligned) and registers it; the library keeps
+ * the pointer until it is replaced (ptr = NULL, bytes = 0 unregisters).  md_workspace_bytes returns 0 on bad arguments. */
+size_t md_workspace_bytes(int m, int n, int k, int limbs);
+md_status md_set_workspace(void* dev_ptr, size_t bytes);
+
+/* Device status word of the registered workspace, copied to *flags_host (host pointer); SYNCHRONISES `stream`.
+ * bit 0: a non-finite input was seen; bit 1: a group exponent outside [-900, 900].  The word is cleared by md_set_workspace
+ * and accumulates until then. */
+md_status md_read_flags(uint32_t* flags_host, md_stream stream);
+
+/* ---------------------------------------------------------------------------------------------------------------------
+ * md_gemm_host -- md_gemm on HOST buffers (end-to-end path).  A_host, B_host, C_host are HOST pointers (pinned memory
+ *   makes the copies asynchronous and fast; pageable works).  dev_scratch is DEVICE memory of at least
+ *   md_host_scratch_bytes(m,n,k,limbs) bytes, 256-byte aligned, owned by the caller; it receives the device copies of
+ *   A, B, C and the workspace.  Copies A and B to the device, runs md_gemm, copies C back, all on `stream`, then
+ *   SYNCHRONISES the stream: C_host is complete on return.
+ * ------------------------------------------------------------------------------------------------------------------ */
+size_t md_host_scratch_bytes(int m, int n, int k, int limbs);
+md_status md_gemm_host(int m, int n, int k, int limbs, const double* A_host, const double* B_host, double* C_host,
+                       void* dev_scratch, size_t scratch_bytes, md_stream stream);
+
+/* Per-call device timing of md_gemm / md_gemm_orders / md_gemm_host, for roofline accounting (bench.py).
+ * md_profile_enable(capacity > 0): each following call records CUDA events on its stream before its first kernel, before
+ * the fused quarter-GEMM kernel and after it, for up to `capacity` calls (further calls are not recorded); calling it again
+ * restarts the record; capacity = 0 disables and frees the events.  Do not enable while capturing a CUDA graph.
+ * md_profile_read synchronises the recorded events and returns how many calls were recorded (<= capacity, or a negative
+ * md_status); for call i it stores the split time (exponent + split kernels) in split_ms_host[i] and the fused GEMM
+ * kernel time in gemm_ms_host[i] (HOST arrays of at least `capacity` floats; either may be NULL). */
+md_status md_profile_enable(int capacity);
+int md_profile_read(float* split_ms_host, float* gemm_ms_host, int capacity);
+
+/* Number of kernels this library has launched since load (all entry points), for launch accounting. */
+uint64_t md_launch_count(void);
+
+const char* md_status_string(md_status status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MDGEMM_H_ */

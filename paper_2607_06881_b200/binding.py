@@ -1,0 +1,214 @@
+"""Thin Python binding of libmdgemm.so (include/mdgemm.h): same names, argument marshalling only.
+
+Every step of the hot path runs in the library's CUDA kernels; torch is used for device memory and streams.  There is
+no CPU fallback: if the shared library is missing (run `python -m paper_2607_06881_b200.build`) or a call fails, an
+exception is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmdgemm.so")
+
+MD_OK = 0
+MD_ERR_BAD_ARG, MD_ERR_K_TOO_LARGE, MD_ERR_WORKSPACE, MD_ERR_CUDA, MD_ERR_UNSUPPORTED = -1, -2, -3, -4, -5
+MD_OPT_QUARTERS, MD_OPT_ORDERS = 1, 2
+
+# every symbol include/mdgemm.h declares: name -> (restype, argtypes)
+_c = ctypes
+_SIGNATURES = {
+    "md_set_option": (_c.c_int, [_c.c_int, _c.c_int]),
+    "md_get_option": (_c.c_int, [_c.c_int]),
+    "md_split": (_c.c_int, [_c.c_int] * 5 + [_c.c_void_p] * 4),
+    "md_qgemm": (_c.c_int, [_c.c_int] * 6 + [_c.c_void_p] * 5),
+    "md_renorm": (_c.c_int, [_c.c_int] * 4 + [_c.c_void_p] * 3),
+    "md_gemm": (_c.c_int, [_c.c_int] * 4 + [_c.c_void_p] * 4),
+    "md_gemm_orders": (_c.c_int, [_c.c_int] * 4 + [_c.c_void_p] * 4),
+    "md_workspace_bytes": (_c.c_size_t, [_c.c_int] * 4),
+    "md_set_workspace": (_c.c_int, [_c.c_void_p, _c.c_size_t]),
+    "md_read_flags": (_c.c_int, [_c.c_void_p, _c.c_void_p]),
+    "md_host_scratch_bytes": (_c.c_size_t, [_c.c_int] * 4),
+    "md_gemm_host": (_c.c_int, [_c.c_int] * 4 + [_c.c_void_p] * 4 + [_c.c_size_t, _c.c_void_p]),
+    "md_profile_enable": (_c.c_int, [_c.c_int]),
+    "md_profile_read": (_c.c_int, [_c.c_void_p, _c.c_void_p, _c.c_int]),
+    "md_launch_count": (_c.c_uint64, []),
+    "md_status_string": (_c.c_char_p, [_c.c_int]),
+}
+EXPORTED_SYMBOLS = tuple(_SIGNATURES)
+
+_lib = None
+
+
+class MdError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {lib().md_status_string(status).decode()} ({status})")
+
+
+def lib() -> ctypes.CDLL:
+    """Load libmdgemm.so (once).  Raises if it has not been built: there is no fallback path."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} not found: build it with `python -m paper_2607_06881_b200.build` "
+                              "(the CUDA extension is the product; there is no CPU fallback)")
+        handle = ctypes.CDLL(LIB_PATH)
+        for name, (res, args) in _SIGNATURES.items():
+            fn = getattr(handle, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = handle
+    return _lib
+
+
+def _check(status: int, where: str):
+    if status != MD_OK:
+        raise MdError(status, where)
+
+
+def _dev(t: torch.Tensor, dtype=torch.float64) -> int:
+    if not (t.is_cuda and t.is_contiguous() and t.dtype == dtype):
+        raise ValueError("expected a contiguous CUDA tensor of dtype %s" % dtype)
+    return t.data_ptr()
+
+
+def _stream(stream) -> int:
+    s = torch.cuda.current_stream() if stream is None else stream
+    return s.cuda_stream
+
+
+def md_set_option(key: int, value: int):
+    _check(lib().md_set_option(key, value), "md_set_option")
+
+
+def md_get_option(key: int) -> int:
+    return lib().md_get_option(key)
+
+
+def md_workspace_bytes(m, n, k, limbs) -> int:
+    return lib().md_workspace_bytes(m, n, k, limbs)
+
+
+def md_set_workspace(ws: torch.Tensor | None):
+    """Register a uint8 CUDA tensor (or None) as the library workspace.  The caller keeps it alive."""
+    if ws is None:
+        _check(lib().md_set_workspace(None, 0), "md_set_workspace")
+    else:
+        _check(lib().md_set_workspace(_dev(ws, torch.uint8), ws.numel()), "md_set_workspace")
+
+
+def md_read_flags(stream=None) -> int:
+    out = ctypes.c_uint32(0)
+    _check(lib().md_read_flags(ctypes.addressof(out), _stream(stream)), "md_read_flags")
+    return out.value
+
+
+def md_split(planes: torch.Tensor, axis: int, quarters: int | None = None, stream=None):
+    """planes [limbs, rows, cols] -> (quarter_planes [Q, rows, cols], exps int32[rows or cols])."""
+    limbs, rows, cols = planes.shape
+    Q = 4 * limbs if quarters is None else quarters
+    qp = torch.empty((Q, rows, cols), dtype=torch.float64, device=planes.device)
+    exps = torch.empty(rows if axis == 0 else cols, dtype=torch.int32, device=planes.device)
+    _check(lib().md_split(rows, cols, limbs, Q, axis, _dev(planes), _dev(qp), _dev(exps, torch.int32),
+                          _stream(stream)), "md_split")
+    return qp, exps
+
+
+def md_qgemm(Aq: torch.Tensor, Bq: torch.Tensor, limbs: int, want_orders: bool = False, want_C: bool = True,
+             stream=None):
+    """Aq [Q, m, k], Bq [Q, k, n] -> (order_planes [Q, m, n] or None, C_planes [limbs, m, n] or None)."""
+    Q, m, k = Aq.shape
+    n = Bq.shape[2]
+    assert Bq.shape[0] == Q and Bq.shape[1] == k
+    orders = torch.empty((Q, m, n), dtype=torch.float64, device=Aq.device) if want_orders else None
+    C = torch.empty((limbs, m, n), dtype=torch.float64, device=Aq.device) if want_C else None
+    _check(lib().md_qgemm(m, n, k, limbs, Q, Q, _dev(Aq), _dev(Bq), None if orders is None else _dev(orders),
+                          None if C is None else _dev(C), _stream(stream)), "md_qgemm")
+    return orders, C
+
+
+def md_renorm(order_planes: torch.Tensor, limbs: int, stream=None) -> torch.Tensor:
+    S, m, n = order_planes.shape
+    C = torch.empty((limbs, m, n), dtype=torch.float64, device=order_planes.device)
+    _check(lib().md_renorm(m, n, limbs, S, _dev(order_planes), _dev(C), _stream(stream)), "md_renorm")
+    return C
+
+
+def md_gemm(A: torch.Tensor, B: torch.Tensor, C: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+    """C = A * B on limb planes: A [limbs, m, k], B [limbs, k, n] -> C [limbs, m, n].  Needs a registered workspace."""
+    limbs, m, k = A.shape
+    n = B.shape[2]
+    assert B.shape[0] == limbs and B.shape[1] == k
+    if C is None:
+        C = torch.empty((limbs, m, n), dtype=torch.float64, device=A.device)
+    _check(lib().md_gemm(m, n, k, limbs, _dev(A), _dev(B), _dev(C), _stream(stream)), "md_gemm")
+    return C
+
+
+def md_gemm_orders(A: torch.Tensor, B: torch.Tensor, stream=None) -> torch.Tensor:
+    limbs, m, k = A.shape
+    n = B.shape[2]
+    S = md_get_option(MD_OPT_ORDERS) or md_get_option(MD_OPT_QUARTERS) or 4 * limbs
+    out = torch.empty((S, m, n), dtype=torch.float64, device=A.device)
+    _check(lib().md_gemm_orders(m, n, k, limbs, _dev(A), _dev(B), _dev(out), _stream(stream)), "md_gemm_orders")
+    return out
+
+
+def md_host_scratch_bytes(m, n, k, limbs) -> int:
+    return lib().md_host_scratch_bytes(m, n, k, limbs)
+
+
+def md_gemm_host(A_host: torch.Tensor, B_host: torch.Tensor, C_host: torch.Tensor, scratch: torch.Tensor, stream=None):
+    """End-to-end call on HOST tensors (pinned recommended); `scratch` is a uint8 CUDA tensor."""
+    limbs, m, k = A_host.shape
+    n = B_host.shape[2]
+    for t in (A_host, B_host, C_host):
+        if t.is_cuda or not t.is_contiguous() or t.dtype != torch.float64:
+            raise ValueError("md_gemm_host takes contiguous float64 HOST tensors")
+    _check(lib().md_gemm_host(m, n, k, limbs, A_host.data_ptr(), B_host.data_ptr(), C_host.data_ptr(),
+                              _dev(scratch, torch.uint8), scratch.numel(), _stream(stream)), "md_gemm_host")
+    return C_host
+
+
+def md_profile_enable(capacity: int):
+    _check(lib().md_profile_enable(capacity), "md_profile_enable")
+
+
+def md_profile_read(capacity: int):
+    """Returns (split_ms list, gemm_ms list) for the calls recorded since md_profile_enable."""
+    split = (ctypes.c_float * max(capacity, 1))()
+    gemm = (ctypes.c_float * max(capacity, 1))()
+    count = lib().md_profile_read(split, gemm, capacity)
+    if count < 0:
+        raise MdError(count, "md_profile_read")
+    return list(split[:count]), list(gemm[:count])
+
+
+def md_launch_count() -> int:
+    return lib().md_launch_count()
+
+
+class Workspace:
+    """Allocates and registers the md_gemm workspace for one problem shape (context manager)."""
+
+    def __init__(self, m, n, k, limbs, quarters: int = 0, device="cuda"):
+        md_set_option(MD_OPT_QUARTERS, 0 if quarters == 4 * limbs else quarters)
+        nbytes = md_workspace_bytes(m, n, k, limbs)
+        if nbytes == 0:
+            raise ValueError("bad shape for workspace")
+        self.buffer = torch.empty(nbytes, dtype=torch.uint8, device=device)
+        md_set_workspace(self.buffer)
+
+    def close(self):
+        md_set_workspace(None)
+        md_set_option(MD_OPT_QUARTERS, 0)
+        self.buffer = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()

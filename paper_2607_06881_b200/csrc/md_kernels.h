@@ -1,0 +1,21 @@
+// md_kernels.h -- internal launcher declarations of libmdgemm (host side).  Each launcher enqueues on `stream`, returns
+// the cudaError_t of the launch, and adds the number of kernels it launched to *launches.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace md {
+
+cudaError_t launch_exponents(int rows, int cols, int axis, const double* lead_plane, int32_t* exps, uint32_t* flags,
+                             cudaStream_t stream, uint64_t* launches);
+cudaError_t launch_split(int rows, int cols, int limbs, int quarters, int axis, const double* planes,
+                         double* quarter_planes, const int32_t* exps, uint32_t* flags, cudaStream_t stream,
+                         uint64_t* launches);
+cudaError_t launch_renorm(int m, int n, int limbs, int orders, const double* order_planes, double* C_planes,
+                          cudaStream_t stream, uint64_t* launches);
+// returns cudaErrorInvalidValue when (limbs, quarters) has no instantiation
+cudaError_t launch_qgemm(int m, int n, int k, int limbs, int quarters, const double* Aq, const double* Bq,
+                         double* order_planes, double* C_planes, cudaStream_t stream, uint64_t* launches);
+bool qgemm_supported(int limbs, int quarters);
+
+}  // namespace md

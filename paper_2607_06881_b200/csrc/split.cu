@@ -1,0 +1,162 @@
+// split.cu -- steps a1 + a2 of the hot path: exponent vectors and quarter planes (include/mdgemm.h: md_split).
+//   PAPER.md:47-49 (13-bit quarters with exponents 0,-13,-26,-39), :95 (balanced = exponents on an equally spaced grid),
+//   :124-142 (moving bits between parts without changing the value; zeros keep the desired exponent).
+// HBM-bound: reads 8*limbs and writes 8*quarters bytes per element, once.
+#include "md_common.cuh"
+#include "md_kernels.h"
+
+namespace md {
+namespace {
+
+__device__ __forceinline__ uint32_t abs_hi32(double x) { return (uint32_t)(__double_as_longlong(x) >> 32) & 0x7fffffffu; }
+
+// hi32 of the group maximum -> E = ilogb(max)+1 (0 for a zero group); flags out-of-range / non-finite maxima.
+__device__ __forceinline__ int exponent_from_hi32(uint32_t hi, uint32_t* flags) {
+  const int biased = (int)(hi >> 20);
+  if (biased == 0) return 0;  // zero group (subnormal maxima are outside the documented range and count as zero)
+  const int E = biased - 1022;
+  if (flags) {
+    if (biased == 0x7ff) atomicOr(flags, FLAG_NONFINITE);
+    else if (E < -EXP_LIMIT || E > EXP_LIMIT) atomicOr(flags, FLAG_EXP_RANGE);
+  }
+  return E;
+}
+
+// axis 0: one block per row of the leading limb plane.
+__global__ void __launch_bounds__(256) row_exponent_kernel(int rows, int cols, const double* __restrict__ lead,
+                                                           int32_t* __restrict__ exps, uint32_t* flags) {
+  __shared__ uint32_t warp_max[8];
+  for (int row = blockIdx.x; row < rows; row += gridDim.x) {
+    const double* p = lead + (size_t)row * cols;
+    uint32_t mx = 0;
+    for (int j = threadIdx.x; j < cols; j += blockDim.x) mx = max(mx, abs_hi32(p[j]));
+    mx = __reduce_max_sync(0xffffffffu, mx);
+    if ((threadIdx.x & 31) == 0) warp_max[threadIdx.x >> 5] = mx;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      uint32_t v = warp_max[0];
+#pragma unroll
+      for (int w = 1; w < 8; w++) v = max(v, warp_max[w]);
+      exps[row] = exponent_from_hi32(v, flags);
+    }
+    __syncthreads();
+  }
+}
+
+// axis 1: a thread per column walks a chunk of rows (coalesced across the warp) and folds its maximum into exps[]
+// (pre-zeroed, used as uint32 scratch); the finalize kernel turns the maxima into exponents in place.
+__global__ void __launch_bounds__(256) col_max_kernel(int rows, int cols, int rows_per_block,
+                                                      const double* __restrict__ lead, int32_t* exps) {
+  const int col = blockIdx.x * blockDim.x + threadIdx.x;
+  if (col >= cols) return;
+  const int r0 = blockIdx.y * rows_per_block;
+  const int r1 = min(rows, r0 + rows_per_block);
+  uint32_t mx = 0;
+  for (int r = r0; r < r1; r++) mx = max(mx, abs_hi32(lead[(size_t)r * cols + col]));
+  if (mx) atomicMax(reinterpret_cast<unsigned int*>(exps) + col, mx);
+}
+__global__ void col_exponent_finalize_kernel(int cols, int32_t* exps, uint32_t* flags) {
+  const int col = blockIdx.x * blockDim.x + threadIdx.x;
+  if (col < cols) exps[col] = exponent_from_hi32((uint32_t)exps[col], flags);
+}
+
+// Algorithm S, step S1: per element, for q = 0..Q-1:
+//   c = 3*2^51 * u_q (so that ulp(c) = u_q = 2^(E - 13(q+1)));  d_q = (r_0 + c) - c;  r_0 -= d_q;  carry r through the limbs.
+// Every operation is exact except r_0 + c, whose rounding IS the digit selection.  VEC elements per thread.
+template <int L, int VEC>
+__global__ void __launch_bounds__(256) split_kernel(size_t rows, size_t cols, int Q, int axis,
+                                                    const double* __restrict__ planes, double* __restrict__ qplanes,
+                                                    const int32_t* __restrict__ exps, uint32_t* flags) {
+  const size_t plane = rows * cols;
+  const size_t idx = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) * VEC;
+  if (idx >= plane) return;
+  const size_t row = idx / cols, col = idx - row * cols;  // VEC == 2 only when cols is even: both elements in one row
+
+  double r[VEC][L];
+  if (VEC == 2) {
+#pragma unroll
+    for (int l = 0; l < L; l++) {
+      const double2 v = *reinterpret_cast<const double2*>(planes + l * plane + idx);
+      r[0][l] = v.x;
+      r[VEC - 1][l] = v.y;
+    }
+  } else {
+#pragma unroll
+    for (int l = 0; l < L; l++) r[0][l] = planes[l * plane + idx];
+  }
+  int E[VEC];
+  bool bad = false;
+#pragma unroll
+  for (int v = 0; v < VEC; v++) {
+    E[v] = axis == 0 ? exps[row] : exps[col + v];
+#pragma unroll
+    for (int l = 0; l < L; l++) bad |= (abs_hi32(r[v][l]) >> 20) == 0x7ffu;
+  }
+  if (bad && flags) atomicOr(flags, FLAG_NONFINITE);
+
+  for (int q = 0; q < Q; q++) {
+    double d[VEC];
+#pragma unroll
+    for (int v = 0; v < VEC; v++) {
+      // c = 1.5 * 2^(E - 13(q+1) + 52): exponent field + the top mantissa bit
+      const long long cbits = ((long long)(E[v] - 13 * (q + 1) + 52 + 1023) << 52) | (1ll << 51);
+      const double c = __longlong_as_double(cbits);
+      const double t = __dadd_rn(r[v][0], c);
+      d[v] = __dsub_rn(t, c);
+      r[v][0] = __dsub_rn(r[v][0], d[v]);
+#pragma unroll
+      for (int l = 0; l + 1 < L; l++) two_sum(r[v][l], r[v][l + 1], r[v][l], r[v][l + 1]);
+    }
+    if (VEC == 2)
+      *reinterpret_cast<double2*>(qplanes + (size_t)q * plane + idx) = make_double2(d[0], d[VEC - 1]);
+    else
+      qplanes[(size_t)q * plane + idx] = d[0];
+  }
+}
+
+}  // namespace
+
+cudaError_t launch_exponents(int rows, int cols, int axis, const double* lead, int32_t* exps, uint32_t* flags,
+                             cudaStream_t stream, uint64_t* launches) {
+  if (axis == 0) {
+    row_exponent_kernel<<<min(rows, 148 * 64), 256, 0, stream>>>(rows, cols, lead, exps, flags);
+    *launches += 1;
+    return cudaGetLastError();
+  }
+  cudaError_t err = cudaMemsetAsync(exps, 0, sizeof(int32_t) * (size_t)cols, stream);
+  if (err != cudaSuccess) return err;
+  const int col_blocks = (cols + 255) / 256;
+  // enough row chunks to fill the machine, at least 16 rows each
+  int chunks = max(1, min((rows + 15) / 16, (148 * 8 + col_blocks - 1) / col_blocks));
+  chunks = min(chunks, 65535);
+  const int rows_per_block = (rows + chunks - 1) / chunks;
+  chunks = (rows + rows_per_block - 1) / rows_per_block;
+  col_max_kernel<<<dim3(col_blocks, chunks), 256, 0, stream>>>(rows, cols, rows_per_block, lead, exps);
+  if ((err = cudaGetLastError()) != cudaSuccess) return err;
+  col_exponent_finalize_kernel<<<col_blocks, 256, 0, stream>>>(cols, exps, flags);
+  *launches += 2;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_split(int rows, int cols, int limbs, int quarters, int axis, const double* planes,
+                         double* qplanes, const int32_t* exps, uint32_t* flags, cudaStream_t stream,
+                         uint64_t* launches) {
+  const size_t total = (size_t)rows * cols;
+  const bool vec = (cols % 2 == 0) && ((reinterpret_cast<uintptr_t>(planes) | reinterpret_cast<uintptr_t>(qplanes)) % 16 == 0);
+  const size_t threads = vec ? total / 2 : total;
+  const unsigned blocks = (unsigned)((threads + 255) / 256);
+#define MD_SPLIT(L_)                                                                                              \
+  if (vec) split_kernel<L_, 2><<<blocks, 256, 0, stream>>>(rows, cols, quarters, axis, planes, qplanes, exps, flags); \
+  else split_kernel<L_, 1><<<blocks, 256, 0, stream>>>(rows, cols, quarters, axis, planes, qplanes, exps, flags);
+  switch (limbs) {
+    case 1: MD_SPLIT(1) break;
+    case 2: MD_SPLIT(2) break;
+    case 4: MD_SPLIT(4) break;
+    default: return cudaErrorInvalidValue;
+  }
+#undef MD_SPLIT
+  *launches += 1;
+  return cudaGetLastError();
+}
+
+}  // namespace md

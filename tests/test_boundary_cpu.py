@@ -1,0 +1,73 @@
+"""CPU-only checks of the boundary: libmdgemm.so loads, exports every symbol include/mdgemm.h declares, and rejects bad
+arguments before touching the GPU (no compute calls here)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+from paper_2607_06881_b200 import binding as md
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2607_06881_b200 import build
+    build.build()
+    return md.lib()
+
+
+def header_symbols():
+    text = open(os.path.join(ROOT, "include", "mdgemm.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(md_[a-z_]+)\s*\(", text)))
+
+
+def test_every_declared_symbol_is_exported_and_bound(lib):
+    declared = header_symbols()
+    assert len(declared) >= 14
+    for name in declared:
+        assert hasattr(lib, name), name
+    assert sorted(md.EXPORTED_SYMBOLS) == declared  # the binding covers exactly the header
+
+
+def test_status_strings(lib):
+    for code in (0, -1, -2, -3, -4, -5):
+        assert lib.md_status_string(code)
+    assert b"unknown" in lib.md_status_string(-99)
+
+
+def test_argument_errors_need_no_gpu(lib):
+    fake = ctypes.c_void_p(4096)  # non-null, aligned, never dereferenced: errors are argument-only
+    assert lib.md_gemm(0, 4, 4, 2, fake, fake, fake, None) == md.MD_ERR_BAD_ARG
+    assert lib.md_gemm(4, 4, 4, 3, fake, fake, fake, None) == md.MD_ERR_BAD_ARG
+    assert lib.md_gemm(4, 4, 4, 2, None, fake, fake, None) == md.MD_ERR_BAD_ARG
+    assert lib.md_gemm(4, 4, 4, 2, ctypes.c_void_p(4100), fake, fake, None) == md.MD_ERR_BAD_ARG  # misaligned
+    # k budget: k * S <= 2^27 (eq. 5 generalised, R6): 2^24 passes the check, 2^24 + 1 does not
+    assert lib.md_gemm(1, 1, 2 ** 24 + 1, 2, fake, fake, fake, None) == md.MD_ERR_K_TOO_LARGE
+    assert lib.md_gemm(1, 1, 2 ** 23 + 1, 4, fake, fake, fake, None) == md.MD_ERR_K_TOO_LARGE
+    assert lib.md_gemm(1, 1, 2 ** 24, 2, fake, fake, fake, None) == md.MD_ERR_WORKSPACE  # passes the checks; no workspace
+    assert lib.md_split(4, 4, 3, 8, 0, fake, fake, fake, None) == md.MD_ERR_BAD_ARG
+    assert lib.md_split(4, 4, 2, 8, 2, fake, fake, fake, None) == md.MD_ERR_BAD_ARG
+    assert lib.md_split(4, 4, 2, 25, 0, fake, fake, fake, None) == md.MD_ERR_BAD_ARG
+    assert lib.md_renorm(4, 4, 2, 0, fake, fake, None) == md.MD_ERR_BAD_ARG
+    assert lib.md_qgemm(4, 4, 4, 2, 8, 7, fake, fake, fake, fake, None) == md.MD_ERR_UNSUPPORTED
+    assert lib.md_qgemm(4, 4, 4, 2, 12, 12, fake, fake, fake, fake, None) == md.MD_ERR_UNSUPPORTED
+    assert lib.md_qgemm(4, 4, 4, 2, 8, 8, fake, fake, None, None, None) == md.MD_ERR_BAD_ARG
+
+
+def test_options_and_workspace_sizes(lib):
+    assert lib.md_get_option(md.MD_OPT_QUARTERS) == 0 and lib.md_get_option(99) == -1
+    base = lib.md_workspace_bytes(64, 64, 64, 2)
+    # a quartered double double matrix has 8 times the size of a matrix of doubles
+    assert base >= 2 * 8 * 64 * 64 * 8 and base < 2 * 8 * 64 * 64 * 8 + 4096
+    assert lib.md_set_option(md.MD_OPT_QUARTERS, 9) == 0
+    assert lib.md_workspace_bytes(64, 64, 64, 2) >= 2 * 9 * 64 * 64 * 8
+    assert lib.md_set_option(md.MD_OPT_QUARTERS, 0) == 0
+    assert lib.md_workspace_bytes(64, 64, 64, 4) >= 2 * 16 * 64 * 64 * 8  # quad double: 16 times
+    assert lib.md_workspace_bytes(0, 64, 64, 2) == 0 and lib.md_workspace_bytes(64, 64, 64, 3) == 0
+    assert lib.md_host_scratch_bytes(64, 64, 64, 2) >= base + 3 * 2 * 64 * 64 * 8
+    assert lib.md_set_option(99, 1) == md.MD_ERR_BAD_ARG and lib.md_set_option(md.MD_OPT_QUARTERS, 99) == md.MD_ERR_BAD_ARG
+    assert lib.md_set_workspace(None, 16) == md.MD_ERR_BAD_ARG
+    assert lib.md_set_workspace(None, 0) == 0
