@@ -37,14 +37,16 @@ if ROOT not in sys.path:
 
 METRIC = "effective double-double GFLOP/s at n=4096 on 1 B200; % of FP64 tensor peak"
 UNIT = "GFLOP/s (double-double, 2mnk)"
-# FP64 tensor (DMMA) peak of B200: 128 flop/clk/SM x 148 SMs x 1.965 GHz (clocks.max.sm).  MEASURED_PEAKS.json holds
-# no FP64 figure; a register-only mma.sync.m8n8k4.f64 loop on this pool's B200 measured 128.0 flop/clk/SM and
-# 37.07 TFLOP/s at 1.957 GHz (profiles/r01_dmma_peak.md), cuBLAS DGEMM 8192^3 35.5 TFLOP/s.  DESIGN.md section 6.
+# FP64 tensor (DMMA) peak of B200: 128 flop/clk/SM x 148 SMs x 1.965 GHz (clocks.max.sm) = 37.22 TFLOP/s.
+# MEASURED_PEAKS.json holds no FP64 figure, so the denominator is this unit-count x clock figure;
+# it is cross-checked LIVE in every run by md_probe_dmma, a register-only mma.sync.m8n8k4.f64 loop (measure_dmma_peak
+# below; profiles/r01_dmma_peak.md), and the probe's number is reported beside it.
 FP64_TENSOR_PEAK_TFLOPS = 128 * 148 * 1.965e9 / 1e12
 # The paper's own figure for this metric and workload (double double, n = 4096, whole pipeline t_TC = 7.93621 s ->
 # 2*4096^3 / t = 17.3 GFLOP/s; Table 1; hardware A100 or RTX 4080, the paper does not say): context only.
 PAPER_DD_4096_GFLOPS = 2 * 4096 ** 3 / 7.93621 / 1e9
-CPU_SAMPLE_ROWS = 16
+CPU_SAMPLE_ROWS = 16            # cpu_baseline leg of the default run: 16 rows x all columns (~10 s on 16 cores)
+REF_ROWS, REF_COLS = 16, 1024   # --impl reference: per step (~2.5 s on 16 cores)
 
 
 def parse_args():
@@ -107,17 +109,39 @@ class ClockSampler(threading.Thread):
                 "power_w_max": max(power), "samples": len(sm)}
 
 
-def cpu_oracle_sample(cfg, rows: int):
-    """The oracle's five-step pipeline on the first `rows` rows of A (all of B): returns (GFLOP/s, seconds, threads)."""
+def measure_dmma_peak(md, torch, warps_per_block: int = 8, reps: int = 5):
+    """FP64 tensor peak measured now, on this GPU: md_probe_dmma (one CTA per SM, register-only DMMA) timed with CUDA
+    events on the launching stream; best of `reps` after one warm-up.  Returns TFLOP/s."""
+    sms = torch.cuda.get_device_properties(torch.cuda.current_device()).multi_processor_count
+    stream = torch.cuda.current_stream()
+    iters = 100_000
+    md.md_probe_dmma(sms, warps_per_block, 1000)
+    best = 0.0
+    for _ in range(reps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        flops = md.md_probe_dmma(sms, warps_per_block, iters)
+        e1.record(stream)
+        e1.synchronize()
+        best = max(best, flops / (e0.elapsed_time(e1) * 1e-3) / 1e12)
+    return best
+
+
+def cpu_oracle_sample(cfg, rows: int, cols: int | None = None):
+    """The oracle's five-step pipeline on the first `rows` rows of A and the first `cols` columns of B (default: all):
+    a rows x cols block of C, exactly as the full problem would compute it (a row's / column's exponent depends on
+    that row / column only).  Returns (GFLOP/s, seconds, threads)."""
     from oracle import md_oracle as orc
     from paper_2607_06881_b200 import inputs
+    cols = cfg.n if cols is None else min(cols, cfg.n)
+    rows = min(rows, cfg.m)
     A = inputs.generate(cfg, "A", 0, rows)
-    B = inputs.generate(cfg, "B")
+    B = np.ascontiguousarray(inputs.generate(cfg, "B", 0, None, 0, cols))
     threads = min(orc.num_threads(), rows)
     t0 = time.perf_counter()
     orc.md_gemm_rows(A, B, quarters=cfg.quarters)
     dt = time.perf_counter() - t0
-    return 2.0 * rows * cfg.n * cfg.k / dt / 1e9, dt, threads
+    return 2.0 * rows * cols * cfg.k / dt / 1e9, dt, threads
 
 
 def run_reference(args):
@@ -126,22 +150,23 @@ def run_reference(args):
         return
     from paper_2607_06881_b200 import inputs
     cfg = inputs.CONFIGS[args.config]
-    rows = CPU_SAMPLE_ROWS
-    for _ in range(min(args.warmup, 1)):
-        cpu_oracle_sample(cfg, 2)
-    steps = max(1, min(args.steps, 3))  # each step is ~10-20 s of CPU work; keep the run within minutes
-    vals, secs, threads = [], [], 1
+    # one step = a bounded sample: a REF_ROWS x REF_COLS block of C over the full k (a few seconds of CPU work per
+    # step, one row per OpenMP thread), so that W + K steps end within minutes
+    rows, cols = min(REF_ROWS, cfg.m), min(REF_COLS, cfg.n)
+    for _ in range(args.warmup):
+        cpu_oracle_sample(cfg, rows, cols)
+    steps = args.steps
+    secs, threads = [], 1
     for _ in range(steps):
-        v, dt, threads = cpu_oracle_sample(cfg, rows)
-        vals.append(v)
+        _, dt, threads = cpu_oracle_sample(cfg, rows, cols)
         secs.append(dt)
-    value = 2.0 * rows * cfg.n * cfg.k * steps / sum(secs) / 1e9
-    sample = (f"first {rows} rows of A ({rows}x{cfg.n} outputs of the {cfg.m}x{cfg.n}x{cfg.k} problem), all of B; "
-              f"oracle split + {cfg.products} plain fp64 quarter GEMM loops + exact renorm; {steps} step(s) timed "
-              f"(--steps capped at 3)")
+    value = 2.0 * rows * cols * cfg.k * steps / sum(secs) / 1e9
+    sample = (f"per step: first {rows} rows of A x first {cols} columns of B over the full k ({rows}x{cols} outputs of "
+              f"the {cfg.m}x{cfg.n}x{cfg.k} problem); oracle split + {cfg.products} plain fp64 quarter GEMM loops + exact "
+              f"renorm, OpenMP over rows; {steps} steps timed")
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
-        "warmup": min(args.warmup, 1), "ms_per_step": 1e3 * sum(secs) / steps, "higher_is_better": True,
+        "warmup": args.warmup, "ms_per_step": 1e3 * sum(secs) / steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": value / PAPER_DD_4096_GFLOPS if args.config == 2 else None, "dtype": "f64",
         "data": "synthetic",
         "config": {"workload": f"BASELINE.json configs[{cfg.index}] {cfg.name}: {cfg.m}x{cfg.n}x{cfg.k}, limbs={cfg.limbs}, "
@@ -217,12 +242,15 @@ def run_ours(args):
         md.md_profile_enable(0)
         flags = md.md_read_flags()
     clocks_after_device_loop = len(sampler.samples)
+    probe_launches0 = md.md_launch_count()
+    dmma_probe_tflops = measure_dmma_peak(md, torch)
+    probe_launches = md.md_launch_count() - probe_launches0
 
     # end to end: pinned host buffers through md_gemm_host (H2D A, B + the whole path + D2H C, synchronous)
     e2e = None
     if not args.no_e2e:
+        md.md_set_option(md.MD_OPT_QUARTERS, 0 if Q == 4 * L else Q)  # before sizing the scratch: it depends on Q
         scratch = torch.empty(md.md_host_scratch_bytes(m, n, k, L), dtype=torch.uint8, device="cuda")
-        md.md_set_option(md.MD_OPT_QUARTERS, 0 if Q == 4 * L else Q)
         for _ in range(min(args.warmup, 2)):
             md.md_gemm_host(A_host, B_host, C_host, scratch)
         barrier()
@@ -259,17 +287,19 @@ def run_ours(args):
         "bound": "tensor", "kernel": "qgemm_kernel (fused triangular quarter GEMM + renormalising epilogue)",
         "achieved": achieved, "peak": FP64_TENSOR_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_TENSOR_PEAK_TFLOPS,
         "peak_source": "FP64 DMMA: 128 flop/clk/SM x 148 SMs x 1.965 GHz (MEASURED_PEAKS.json has no FP64 entry; "
-                       "microbenchmark on this pool measured 37.07 TFLOP/s, profiles/r01_dmma_peak.md)",
+                       "DESIGN.md section 6); cross-checked in this run by md_probe_dmma (peak_probe_measured)",
+        "peak_probe_measured": dmma_probe_tflops, "frac_of_probe": achieved / dmma_probe_tflops,
+        "probe_launches_outside_timed_region": probe_launches,
         "algorithmic_flops_per_launch": issued_flops, "kernel_ms": gemm_avg_ms, "split_ms": sum(split_ms) / len(split_ms),
         "kernel_share_of_step": gemm_avg_ms / ms_per_step,
         "traffic": None,
     }
-    traffic_file = os.path.join(ROOT, "profiles", "r01_qgemm_traffic.json")
+    # DRAM bytes of one launch of this kernel from the committed ncu --set full capture (cfg2 only), else null
+    traffic_file = os.path.join(ROOT, "profiles", "qgemm_traffic.txt")
     if os.path.exists(traffic_file) and args.config == 2:
-        try:
-            roofline["traffic"] = json.load(open(traffic_file))["dram_bytes_per_launch"]
-        except Exception:
-            pass
+        for ln in open(traffic_file):
+            if ln.startswith("dram_bytes_per_launch"):
+                roofline["traffic"] = int(ln.split("=")[1])
 
     cpu_baseline = None
     if world == 1 and not args.no_cpu_baseline:

@@ -154,6 +154,17 @@ md_status md_gemm_host(int m, int n, int k, int limbs, const double* A_host, con
 md_status md_profile_enable(int capacity);
 int md_profile_read(float* split_ms_host, float* gemm_ms_host, int capacity);
 
+/* ---------------------------------------------------------------------------------------------------------------------
+ * md_probe_dmma -- calibration, not a step of the path: enqueues ONE kernel in which `blocks` CTAs of `warps_per_block`
+ *   warps each issue iters * 8 register-only mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4, the instruction md_qgemm computes
+ *   with; "double precision tensor cores").  Timed by the caller with CUDA events it gives the FP64
+ *   tensor peak of this device, the roofline denominator of md_qgemm.
+ *   sink            out  device, blocks * warps_per_block * 32 doubles, or NULL (nothing is written)
+ *   flops_host      out  HOST pointer: FP64 flops the launch issues = blocks * warps_per_block * iters * 8 * 512
+ *   1 <= blocks; 1 <= warps_per_block <= 32; 1 <= iters < 2^25.
+ * ------------------------------------------------------------------------------------------------------------------ */
+md_status md_probe_dmma(int blocks, int warps_per_block, int iters, double* sink, uint64_t* flops_host, md_stream stream);
+
 /* Number of kernels this library has launched since load (all entry points), for launch accounting. */
 uint64_t md_launch_count(void);
 

@@ -35,6 +35,7 @@ _SIGNATURES = {
     "md_gemm_host": (_c.c_int, [_c.c_int] * 4 + [_c.c_void_p] * 4 + [_c.c_size_t, _c.c_void_p]),
     "md_profile_enable": (_c.c_int, [_c.c_int]),
     "md_profile_read": (_c.c_int, [_c.c_void_p, _c.c_void_p, _c.c_int]),
+    "md_probe_dmma": (_c.c_int, [_c.c_int] * 3 + [_c.c_void_p] * 3),
     "md_launch_count": (_c.c_uint64, []),
     "md_status_string": (_c.c_char_p, [_c.c_int]),
 }
@@ -185,6 +186,14 @@ def md_profile_read(capacity: int):
     if count < 0:
         raise MdError(count, "md_profile_read")
     return list(split[:count]), list(gemm[:count])
+
+
+def md_probe_dmma(blocks: int, warps_per_block: int, iters: int, sink: torch.Tensor | None = None, stream=None) -> int:
+    """Enqueue the register-only DMMA calibration kernel; returns the FP64 flops it issues (time it with CUDA events)."""
+    flops = ctypes.c_uint64(0)
+    _check(lib().md_probe_dmma(blocks, warps_per_block, iters, None if sink is None else _dev(sink),
+                               ctypes.addressof(flops), _stream(stream)), "md_probe_dmma")
+    return flops.value
 
 
 def md_launch_count() -> int:

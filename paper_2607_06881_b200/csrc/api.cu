@@ -259,6 +259,17 @@ int md_profile_read(float* split_ms_host, float* gemm_ms_host, int capacity) {
   return g_prof.count;
 }
 
+md_status md_probe_dmma(int blocks, int warps_per_block, int iters, double* sink, uint64_t* flops_host, md_stream stream) {
+  if (blocks < 1 || warps_per_block < 1 || warps_per_block > 32 || iters < 1 || iters >= (1 << 25) || !flops_host)
+    return MD_ERR_BAD_ARG;
+  if (!aligned8(sink)) return MD_ERR_BAD_ARG;
+  uint64_t launches = 0;
+  cudaError_t err = md::launch_dmma_probe(blocks, warps_per_block, iters, sink, static_cast<cudaStream_t>(stream),
+                                          &launches, flops_host);
+  g_launches += launches;
+  return err == cudaSuccess ? MD_OK : MD_ERR_CUDA;
+}
+
 uint64_t md_launch_count(void) { return g_launches.load(); }
 
 const char* md_status_string(md_status status) {

@@ -17,5 +17,8 @@ cudaError_t launch_renorm(int m, int n, int limbs, int orders, const double* ord
 cudaError_t launch_qgemm(int m, int n, int k, int limbs, int quarters, const double* Aq, const double* Bq,
                          double* order_planes, double* C_planes, cudaStream_t stream, uint64_t* launches);
 bool qgemm_supported(int limbs, int quarters);
+// calibration (probe.cu): register-only DMMA loop; *flops receives the FP64 flops the launch issues
+cudaError_t launch_dmma_probe(int blocks, int warps_per_block, int iters, double* sink, cudaStream_t stream,
+                              uint64_t* launches, uint64_t* flops);
 
 }  // namespace md
