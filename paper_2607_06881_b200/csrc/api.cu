@@ -7,6 +7,7 @@
 #include "../../include/mdgemm.h"
 #include "md_common.cuh"
 #include "md_kernels.h"
+#include "md_packed.cuh"
 
 namespace {
 
@@ -32,7 +33,8 @@ inline size_t round_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 inline int quarters_for(int limbs) { return g_state.opt_quarters ? g_state.opt_quarters : 4 * limbs; }
 inline int orders_for(int limbs) { return g_state.opt_orders ? g_state.opt_orders : quarters_for(limbs); }
 
-// Workspace layout: [status word | expA int32[m] | expB int32[n] | Aq Q*m*k doubles | Bq Q*k*n doubles]
+// Workspace layout: [status word | expA int32[m] | expB int32[n] | Aq | Bq], Aq / Bq = the packed quarter planes of A / B
+// (md_packed.cuh: zero padded to whole CTA tiles and k-slabs)
 struct Carve {
   uint32_t* flags;
   int32_t* expA;
@@ -41,7 +43,7 @@ struct Carve {
   double* Bq;
   size_t total;
 };
-Carve carve(void* base, int m, int n, int k, int quarters) {
+Carve carve(void* base, int m, int n, int k, int limbs, int quarters) {
   Carve c;
   size_t off = 0;
   char* p = static_cast<char*>(base);
@@ -52,9 +54,9 @@ Carve carve(void* base, int m, int n, int k, int quarters) {
   c.expB = reinterpret_cast<int32_t*>(p + off);
   off += round_up(sizeof(int32_t) * (size_t)n);
   c.Aq = reinterpret_cast<double*>(p + off);
-  off += round_up(sizeof(double) * (size_t)quarters * m * k);
+  off += round_up(sizeof(double) * md::packed_doubles(m, k, md::pack_bx(limbs, 0), quarters));
   c.Bq = reinterpret_cast<double*>(p + off);
-  off += round_up(sizeof(double) * (size_t)quarters * k * n);
+  off += round_up(sizeof(double) * md::packed_doubles(n, k, md::pack_bx(limbs, 1), quarters));
   c.total = off;
   return c;
 }
@@ -73,22 +75,23 @@ md_status check_gemm_args(int m, int n, int k, int limbs, const void* A, const v
   return MD_OK;
 }
 
-// split A (rows) and B (columns) into the carved workspace, then the fused quarter GEMM.
+// split A (rows) and B (columns) into the packed quarter planes of the carved workspace, then the fused quarter GEMM.
 md_status gemm_impl(int m, int n, int k, int limbs, const double* A, const double* B, double* C_planes,
                     double* order_planes, void* ws, size_t ws_bytes, cudaStream_t stream) {
   const int Q = quarters_for(limbs);
   if (!ws) return MD_ERR_WORKSPACE;
-  const Carve c = carve(ws, m, n, k, Q);
+  const Carve c = carve(ws, m, n, k, limbs, Q);
   if (c.total > ws_bytes) return MD_ERR_WORKSPACE;
   uint64_t launches = 0;
   cudaEvent_t* ev = (g_prof.count < g_prof.capacity) ? &g_prof.ev[3 * (size_t)g_prof.count] : nullptr;
   if (ev) cudaEventRecord(ev[0], stream);
   cudaError_t err = md::launch_exponents(m, k, 0, A, c.expA, c.flags, stream, &launches);
   if (err == cudaSuccess) err = md::launch_exponents(k, n, 1, B, c.expB, c.flags, stream, &launches);
-  if (err == cudaSuccess) err = md::launch_split(m, k, limbs, Q, 0, A, c.Aq, c.expA, c.flags, stream, &launches);
-  if (err == cudaSuccess) err = md::launch_split(k, n, limbs, Q, 1, B, c.Bq, c.expB, c.flags, stream, &launches);
+  if (err == cudaSuccess) err = md::launch_split_packed(m, k, limbs, Q, 0, A, c.Aq, c.expA, c.flags, stream, &launches);
+  if (err == cudaSuccess) err = md::launch_split_packed(k, n, limbs, Q, 1, B, c.Bq, c.expB, c.flags, stream, &launches);
   if (ev) cudaEventRecord(ev[1], stream);
-  if (err == cudaSuccess) err = md::launch_qgemm(m, n, k, limbs, Q, c.Aq, c.Bq, order_planes, C_planes, stream, &launches);
+  if (err == cudaSuccess)
+    err = md::launch_qgemm_packed(m, n, k, limbs, Q, c.Aq, c.Bq, order_planes, C_planes, stream, &launches);
   if (ev) {
     cudaEventRecord(ev[2], stream);
     if (err == cudaSuccess) g_prof.count++;
@@ -161,7 +164,7 @@ md_status md_renorm(int m, int n, int limbs, int orders, const double* order_pla
 
 size_t md_workspace_bytes(int m, int n, int k, int limbs) {
   if (m <= 0 || n <= 0 || k <= 0 || (limbs != 2 && limbs != 4)) return 0;
-  return carve(nullptr, m, n, k, quarters_for(limbs)).total;
+  return carve(nullptr, m, n, k, limbs, quarters_for(limbs)).total;
 }
 
 md_status md_set_workspace(void* dev_ptr, size_t bytes) {

@@ -17,6 +17,13 @@ cudaError_t launch_renorm(int m, int n, int limbs, int orders, const double* ord
 cudaError_t launch_qgemm(int m, int n, int k, int limbs, int quarters, const double* Aq, const double* Bq,
                          double* order_planes, double* C_planes, cudaStream_t stream, uint64_t* launches);
 bool qgemm_supported(int limbs, int quarters);
+// md_gemm's internal pair: splitter writing the fragment-major packed layout (md_packed.cuh) and the bulk-copy /
+// mbarrier pipelined fused GEMM reading it.  Same (limbs, quarters) support as launch_qgemm.
+cudaError_t launch_split_packed(int rows, int cols, int limbs, int quarters, int axis, const double* planes,
+                                double* packed, const int32_t* exps, uint32_t* flags, cudaStream_t stream,
+                                uint64_t* launches);
+cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, const double* Ap, const double* Bp,
+                                double* order_planes, double* C_planes, cudaStream_t stream, uint64_t* launches);
 // calibration (probe.cu): register-only DMMA loop; *flops receives the FP64 flops the launch issues
 cudaError_t launch_dmma_probe(int blocks, int warps_per_block, int iters, double* sink, cudaStream_t stream,
                               uint64_t* launches, uint64_t* flops);

@@ -1,0 +1,40 @@
+// md_packed.cuh -- the FRAGMENT-MAJOR PACKED layout of quarter planes inside the md_gemm workspace.
+// Written by split_packed_kernel (split.cu), read by qgemm_packed_kernel (qgemm_packed.cu); internal to libmdgemm -- the
+// public md_split / md_qgemm keep the plain [quarters][rows][cols] layout.
+//
+// An operand is seen as X groups (rows of A, axis 0 / columns of B, axis 1: the index that carries the exponent) by K
+// contraction indices.  X is cut into tiles of BX (the CTA tile: BM for A, BN for B), K into slabs of PACK_BK; both are
+// zero padded to whole tiles / slabs (zero quarters are harmless).  Memory order, slowest to fastest:
+//
+//     [x tile][k slab]  [quarter q][k4 = (k % BK) / 4][x8 = (x % BX) / 8]  [g = x % 8][t4 = k % 4]
+//      \___ chunk ___/   \_______________ inside a chunk _______________/   \__ one DMMA fragment: 32 doubles __/
+//
+// so that (1) the Q * BK * BX doubles a CTA needs per k-slab are contiguous -> one cp.async.bulk; (2) consecutive slabs
+// of a tile are contiguous -> a CTA streams through one region; (3) lane 4g + t4 of a warp finds its element of the
+// 8x4 (A: row g, k t4) or 4x8 (B: k t4, column g) mma.m8n8k4 operand fragment at fragment base + lane.
+#pragma once
+#include <stddef.h>
+
+namespace md {
+
+constexpr int PACK_BK = 8;  // k-slab depth (two DMMA k-steps)
+
+// CTA tile extent along the group index: BM (axis 0) or BN (axis 1) of the qgemm_packed_kernel configuration for `limbs`.
+__host__ __device__ constexpr int pack_bx(int limbs, int axis) {
+  return limbs == 2 ? (axis == 0 ? 64 : 32) : (axis == 0 ? 32 : 16);
+}
+
+// doubles in the packed image of an operand with X groups and K contraction indices
+__host__ __device__ inline size_t packed_doubles(int X, int K, int bx, int quarters) {
+  const size_t xt = ((size_t)X + bx - 1) / bx, ks = ((size_t)K + PACK_BK - 1) / PACK_BK;
+  return xt * ks * (size_t)quarters * PACK_BK * bx;
+}
+
+// offset (in doubles) of quarter q of element (x, k); KS = number of k slabs
+__host__ __device__ inline size_t packed_offset(int x, int k, int q, int bx, int quarters, int KS) {
+  const int xt = x / bx, xin = x % bx, ks = k / PACK_BK, kin = k % PACK_BK;
+  const size_t chunk = ((size_t)xt * KS + ks) * ((size_t)quarters * PACK_BK * bx);
+  return chunk + ((size_t)(q * (PACK_BK / 4) + kin / 4) * (bx / 8) + xin / 8) * 32 + (xin % 8) * 4 + (kin % 4);
+}
+
+}  // namespace md

@@ -18,19 +18,11 @@
 // Exactness: quarters are integers |D| <= 2^13 times the group unit, products are <= 2^26 units, and with k*S <= 2^27 every
 // partial sum stays below 2^53 units, so each fp64 FMA inside DMMA is exact and the result is independent of the
 // order in which the hardware or this kernel adds things (eq. 5; R6).
-#include "md_common.cuh"
 #include "md_kernels.h"
+#include "qgemm_common.cuh"
 
 namespace md {
 namespace {
-
-constexpr int SMEM_LIMIT = 232448;  // 227 KB usable per CTA on sm_100a
-
-__device__ __forceinline__ void dmma_8x8x4(double (&c)[2], double a, double b) {
-  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-      : "+d"(c[0]), "+d"(c[1])
-      : "d"(a), "d"(b));
-}
 
 // cp.async of BYTES (8 or 16) with zero fill when !valid (src-size 0: nothing is read).
 template <int BYTES>
@@ -107,14 +99,8 @@ qgemm_kernel(int m, int n, int k, int tiles_m, int tiles_n, const double* __rest
   const int wm = warp / C::WN, wn = warp % C::WN;
   const int g = lane >> 2, t4 = lane & 3;  // DMMA fragment coordinates: A[g][t4], B[t4][g], C[g][2*t4 + {0,1}]
 
-  // Tile rasterisation: groups of GROUP_M tile rows are swept along n, so the ~148 CTAs in flight cover a near-square
-  // patch of C and share their A / B slabs through L2.
-  constexpr int GROUP_M = 8;
-  const int bid = blockIdx.x;
-  const int per_group = GROUP_M * tiles_n;
-  const int first_m = (bid / per_group) * GROUP_M;
-  const int gsize = min(tiles_m - first_m, GROUP_M);
-  const int tm = first_m + (bid % per_group) % gsize, tn = (bid % per_group) / gsize;
+  int tm, tn;
+  raster_tile(blockIdx.x, tiles_m, tiles_n, tm, tn);
   const int m0 = tm * C::BM, n0 = tn * C::BN;
 
   double acc[S][MT][NT][2];
@@ -168,50 +154,7 @@ qgemm_kernel(int m, int n, int k, int tiles_m, int tiles_n, const double* __rest
   }
   cp_async_wait<0>();
 
-  // Epilogue: this thread holds, for each 8x8 tile, the S order values of C[row][col], C[row][col+1].
-  const size_t planeC = (size_t)m * n;
-  const bool vec_ok = (n % 2 == 0) && (((uintptr_t)C_planes | (uintptr_t)order_planes) % 16 == 0);
-#pragma unroll
-  for (int i = 0; i < MT; i++) {
-    const int row = m0 + wm * MT * 8 + i * 8 + g;
-#pragma unroll
-    for (int j = 0; j < NT; j++) {
-      const int col = n0 + wn * NT * 8 + j * 8 + 2 * t4;
-      if (row >= m || col >= n) continue;
-      const size_t at = (size_t)row * n + col;
-      const bool two = col + 1 < n;
-      if (order_planes) {
-#pragma unroll
-        for (int s = 0; s < S; s++) {
-          if (vec_ok) {
-            *reinterpret_cast<double2*>(order_planes + s * planeC + at) = make_double2(acc[s][i][j][0], acc[s][i][j][1]);
-          } else {
-            order_planes[s * planeC + at] = acc[s][i][j][0];
-            if (two) order_planes[s * planeC + at + 1] = acc[s][i][j][1];
-          }
-        }
-      }
-      if (C_planes) {
-        double c0[S], c1[S], o0[L], o1[L];
-#pragma unroll
-        for (int s = 0; s < S; s++) {
-          c0[s] = acc[s][i][j][0];
-          c1[s] = acc[s][i][j][1];
-        }
-        renorm_orders<L, S>(c0, o0);
-        renorm_orders<L, S>(c1, o1);
-#pragma unroll
-        for (int l = 0; l < L; l++) {
-          if (vec_ok) {
-            *reinterpret_cast<double2*>(C_planes + l * planeC + at) = make_double2(o0[l], o1[l]);
-          } else {
-            C_planes[l * planeC + at] = o0[l];
-            if (two) C_planes[l * planeC + at + 1] = o1[l];
-          }
-        }
-      }
-    }
-  }
+  qgemm_epilogue<S, L, MT, NT>(acc, m, n, m0 + wm * MT * 8, n0 + wn * NT * 8, lane, order_planes, C_planes);
 }
 
 template <class C>

@@ -1,0 +1,215 @@
+// qgemm_packed.cu -- steps a3 + a4 of the hot path, the kernel behind md_gemm / md_gemm_orders.
+//
+//   For s = 0..S-1:  C^(s) = sum_{p+q=s} A_p * B_q      (PAPER.md:66-71 eq. 3; :75-78 eq. 4: the paper's C_{s+1})
+//   C = sum_s C^(s), summed error free into L limbs     (PAPER.md:88-91 steps 4-5)
+//
+// Same arithmetic as qgemm.cu (all T = S(S+1)/2 quarter products of a tile issued on DMMA.8x8x4 from one staging of the
+// Q quarter tiles, one register accumulator set per order, renormalising epilogue), but fed from the FRAGMENT-MAJOR
+// PACKED quarter planes the splitter writes for md_gemm (md_packed.cuh):
+//   * everything a CTA needs for one k-slab of its A block (all Q quarters) is ONE contiguous chunk of global memory, and
+//     so is its B block: a slab is staged with two cp.async.bulk copies (SASS UBLKCP) issued by one thread, completing
+//     on an mbarrier -- no per-thread address arithmetic, no LDGSTS, no register traffic in the DMMA stream;
+//   * inside a chunk every 8x4 (A) / 4x8 (B) DMMA operand fragment is 32 consecutive doubles in lane order, so a
+//     fragment load is one conflict-free LDS.64 at base + 8*lane with an immediate offset, no padding;
+//   * stages are handed back through per-stage "empty" mbarriers (one arrive per warp) instead of a block-wide
+//     __syncthreads, so the two warps of an SM sub-partition drift apart and one's LDS / barrier latency hides behind
+//     the other's DMMA stream.  The refill of a stage is issued two slabs after its last read, when its empty barrier
+//     has long completed, so the issuing thread never actually waits.
+// The r01 ncu capture of the cp.async kernel (profiles/r01_qgemm_ncu.md) showed exactly these three costs as the gap
+// between 88 % and the DMMA peak.
+//
+// Exactness (eq. 5; R6): quarters are integers |D| <= 2^13 times the group unit and
+// k*S <= 2^27, so every partial sum is an integer below 2^53 units: each FMA inside DMMA is exact and the result does not
+// depend on the order in which warps, slabs or the hardware add things.  Zero padding is harmless.
+#include "md_kernels.h"
+#include "md_packed.cuh"
+#include "qgemm_common.cuh"
+
+namespace md {
+namespace {
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred P1;\n"
+      "LAB_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+      "@P1 bra DONE;\n"
+      "bra LAB_WAIT;\n"
+      "DONE:\n"
+      "}" ::"r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+}
+// global -> shared bulk copy (bytes % 16 == 0, both addresses 16-byte aligned); completion = complete_tx on `bar`.
+__device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gmem_src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_u32(smem_dst)),
+               "l"(gmem_src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+
+// A warp owns an (8*MT) x (8*NT) block of C and Q (= S) accumulator sets for it; WM x WN warps tile the CTA block.
+template <int Q_, int L_, int WM_, int WN_, int MT_, int NT_>
+struct PCfg {
+  static constexpr int Q = Q_, S = Q_, L = L_, WM = WM_, WN = WN_, MT = MT_, NT = NT_;
+  static constexpr int BM = WM * MT * 8, BN = WN * NT * 8, BK = PACK_BK;
+  static constexpr int WARPS = WM * WN, THREADS = WARPS * 32;
+  static constexpr int K4 = BK / 4, R8 = BM / 8, N8 = BN / 8;
+  static constexpr int A_CHUNK = Q * BK * BM, B_CHUNK = Q * BK * BN;  // doubles per k-slab
+  static constexpr int STAGE_BYTES = (A_CHUNK + B_CHUNK) * 8;
+  static constexpr int BAR_BYTES = 128;
+  static constexpr int STAGES = ((SMEM_LIMIT - BAR_BYTES) / STAGE_BYTES) < 6 ? ((SMEM_LIMIT - BAR_BYTES) / STAGE_BYTES) : 6;
+  static constexpr int AHEAD = STAGES - 2;  // slabs in flight beyond the one being consumed
+  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES;
+  static_assert(STAGES >= 3, "the non-blocking refill needs at least 3 stages");
+  static_assert(2 * STAGES * 8 <= BAR_BYTES, "barrier area");
+  static_assert(STAGE_BYTES % 128 == 0, "stage alignment");
+};
+
+template <class C>
+__global__ void __launch_bounds__(C::THREADS, 1)
+qgemm_packed_kernel(int m, int n, int KS, int tiles_m, int tiles_n, const double* __restrict__ Ap,
+                    const double* __restrict__ Bp, double* __restrict__ order_planes, double* __restrict__ C_planes) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  constexpr int Q = C::Q, S = C::S, L = C::L, MT = C::MT, NT = C::NT, STAGES = C::STAGES;
+  double* const stages = reinterpret_cast<double*>(smem_raw);
+  uint64_t* const full = reinterpret_cast<uint64_t*>(smem_raw + STAGES * C::STAGE_BYTES);
+  uint64_t* const empty = full + STAGES;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int wm = warp / C::WN, wn = warp % C::WN;
+
+  int tm, tn;
+  raster_tile(blockIdx.x, tiles_m, tiles_n, tm, tn);
+  // this CTA's operand streams: KS consecutive chunks each
+  const double* const Asrc = Ap + (size_t)tm * KS * C::A_CHUNK;
+  const double* const Bsrc = Bp + (size_t)tn * KS * C::B_CHUNK;
+
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < STAGES; s++) {
+      mbar_init(&full[s], 1);
+      mbar_init(&empty[s], C::WARPS);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  auto issue = [&](int slab, int st) {  // one thread: arm the stage's full barrier and start the two bulk copies
+    double* dst = stages + (size_t)st * (C::A_CHUNK + C::B_CHUNK);
+    mbar_expect_tx(&full[st], C::STAGE_BYTES);
+    bulk_g2s(dst, Asrc + (size_t)slab * C::A_CHUNK, C::A_CHUNK * 8, &full[st]);
+    bulk_g2s(dst + C::A_CHUNK, Bsrc + (size_t)slab * C::B_CHUNK, C::B_CHUNK * 8, &full[st]);
+  };
+  if (tid == 0) {
+#pragma unroll
+    for (int j = 0; j < C::AHEAD; j++)
+      if (j < KS) issue(j, j);
+  }
+
+  double acc[S][MT][NT][2];
+#pragma unroll
+  for (int s = 0; s < S; s++)
+#pragma unroll
+    for (int i = 0; i < MT; i++)
+#pragma unroll
+      for (int j = 0; j < NT; j++) acc[s][i][j][0] = acc[s][i][j][1] = 0.0;
+
+  int st = 0;               // stage of slab kt
+  uint32_t phase = 0;       // parity of that stage's current fill
+  int pst = C::AHEAD % STAGES;  // stage of slab kt + AHEAD (producer side, thread 0 only)
+  for (int kt = 0; kt < KS; kt++) {
+    if (tid == 0) {
+      const int slab = kt + C::AHEAD;
+      if (slab < KS) {
+        // the stage was last read for slab (slab - STAGES) = kt - 2: wait for its release (completed long ago)
+        if (slab >= STAGES) mbar_wait(&empty[pst], ((slab / STAGES) + 1) & 1);
+        issue(slab, pst);
+      }
+    }
+    pst = (pst + 1 == STAGES) ? 0 : pst + 1;
+
+    mbar_wait(&full[st], phase);
+    const double* As = stages + (size_t)st * (C::A_CHUNK + C::B_CHUNK) + (wm * MT) * 32 + lane;
+    const double* Bs = stages + (size_t)st * (C::A_CHUNK + C::B_CHUNK) + C::A_CHUNK + (wn * NT) * 32 + lane;
+#pragma unroll
+    for (int k4 = 0; k4 < C::K4; k4++) {
+      double a[Q][MT];
+#pragma unroll
+      for (int p = 0; p < Q; p++)
+#pragma unroll
+        for (int i = 0; i < MT; i++) a[p][i] = As[((p * C::K4 + k4) * C::R8 + i) * 32];
+#pragma unroll
+      for (int q = 0; q < Q; q++) {
+        double b[NT];
+#pragma unroll
+        for (int j = 0; j < NT; j++) b[j] = Bs[((q * C::K4 + k4) * C::N8 + j) * 32];
+#pragma unroll
+        for (int p = 0; p + q < S; p++)  // product (p, q) goes to order s = p + q: consecutive DMMAs hit different accumulators
+#pragma unroll
+          for (int i = 0; i < MT; i++)
+#pragma unroll
+            for (int j = 0; j < NT; j++) dmma_8x8x4(acc[p + q][i][j], a[p][i], b[j]);
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty[st]);  // this warp is done reading the stage
+    if (++st == STAGES) {
+      st = 0;
+      phase ^= 1;
+    }
+  }
+
+  qgemm_epilogue<S, L, MT, NT>(acc, m, n, tm * C::BM + wm * MT * 8, tn * C::BN + wn * NT * 8, lane, order_planes,
+                               C_planes);
+}
+
+template <class C>
+cudaError_t launch_cfg(int m, int n, int k, const double* Ap, const double* Bp, double* order_planes, double* C_planes,
+                       cudaStream_t stream) {
+  static_assert(C::BM == pack_bx(C::L, 0) && C::BN == pack_bx(C::L, 1), "tile shape must match the packed layout");
+  const int tiles_m = (m + C::BM - 1) / C::BM, tiles_n = (n + C::BN - 1) / C::BN;
+  const long long tiles = (long long)tiles_m * tiles_n;
+  if (tiles > 0x7fffffffLL) return cudaErrorInvalidValue;
+  const int KS = (k + C::BK - 1) / C::BK;
+  auto kern = qgemm_packed_kernel<C>;
+  cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+  if (err != cudaSuccess) return err;
+  kern<<<(unsigned)tiles, C::THREADS, C::SMEM_BYTES, stream>>>(m, n, KS, tiles_m, tiles_n, Ap, Bp, order_planes, C_planes);
+  return cudaGetLastError();
+}
+
+// double double: 64 x 32 CTA tile, 8 warps (4 x 2), 16 x 16 warp tile.  quad double: 32 x 16 CTA tile, 8 x 8 warp tile
+// (16 orders x 2 registers per 8x8 tile).
+template <int Q> using PCfgDD = PCfg<Q, 2, 4, 2, 2, 2>;
+template <int Q> using PCfgQD = PCfg<Q, 4, 4, 2, 1, 1>;
+
+}  // namespace
+
+cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, const double* Ap, const double* Bp,
+                                double* order_planes, double* C_planes, cudaStream_t stream, uint64_t* launches) {
+  cudaError_t err = cudaErrorInvalidValue;
+  if (limbs == 2) {
+    if (quarters == 8) err = launch_cfg<PCfgDD<8>>(m, n, k, Ap, Bp, order_planes, C_planes, stream);
+    if (quarters == 9) err = launch_cfg<PCfgDD<9>>(m, n, k, Ap, Bp, order_planes, C_planes, stream);
+    if (quarters == 10) err = launch_cfg<PCfgDD<10>>(m, n, k, Ap, Bp, order_planes, C_planes, stream);
+  } else if (limbs == 4) {
+    if (quarters == 16) err = launch_cfg<PCfgQD<16>>(m, n, k, Ap, Bp, order_planes, C_planes, stream);
+    if (quarters == 17) err = launch_cfg<PCfgQD<17>>(m, n, k, Ap, Bp, order_planes, C_planes, stream);
+    if (quarters == 18) err = launch_cfg<PCfgQD<18>>(m, n, k, Ap, Bp, order_planes, C_planes, stream);
+  }
+  if (err == cudaSuccess) *launches += 1;
+  return err;
+}
+
+}  // namespace md

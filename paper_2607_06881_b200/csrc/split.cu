@@ -4,6 +4,7 @@
 // HBM-bound: reads 8*limbs and writes 8*quarters bytes per element, once.
 #include "md_common.cuh"
 #include "md_kernels.h"
+#include "md_packed.cuh"
 
 namespace md {
 namespace {
@@ -60,9 +61,31 @@ __global__ void col_exponent_finalize_kernel(int cols, int32_t* exps, uint32_t* 
   if (col < cols) exps[col] = exponent_from_hi32((uint32_t)exps[col], flags);
 }
 
-// Algorithm S, step S1: per element, for q = 0..Q-1:
+// Algorithm S, step S1 (DESIGN.md section 3 R4): digit q of the element whose remainder limbs are r[0..L-1], group exponent E:
 //   c = 3*2^51 * u_q (so that ulp(c) = u_q = 2^(E - 13(q+1)));  d_q = (r_0 + c) - c;  r_0 -= d_q;  carry r through the limbs.
-// Every operation is exact except r_0 + c, whose rounding IS the digit selection.  VEC elements per thread.
+// Every operation is exact except r_0 + c, whose rounding IS the digit selection.
+template <int L>
+__device__ __forceinline__ double extract_digit(double (&r)[L], int E, int q) {
+  // c = 1.5 * 2^(E - 13(q+1) + 52): exponent field + the top mantissa bit
+  const long long cbits = ((long long)(E - 13 * (q + 1) + 52 + 1023) << 52) | (1ll << 51);
+  const double c = __longlong_as_double(cbits);
+  const double t = __dadd_rn(r[0], c);
+  const double d = __dsub_rn(t, c);
+  r[0] = __dsub_rn(r[0], d);
+#pragma unroll
+  for (int l = 0; l + 1 < L; l++) two_sum(r[l], r[l + 1], r[l], r[l + 1]);
+  return d;
+}
+
+template <int L>
+__device__ __forceinline__ bool any_nonfinite(const double (&r)[L]) {
+  bool bad = false;
+#pragma unroll
+  for (int l = 0; l < L; l++) bad |= (abs_hi32(r[l]) >> 20) == 0x7ffu;
+  return bad;
+}
+
+// md_split: plain [quarters][rows][cols] output.  VEC elements per thread.
 template <int L, int VEC>
 __global__ void __launch_bounds__(256) split_kernel(size_t rows, size_t cols, int Q, int axis,
                                                     const double* __restrict__ planes, double* __restrict__ qplanes,
@@ -89,28 +112,76 @@ __global__ void __launch_bounds__(256) split_kernel(size_t rows, size_t cols, in
 #pragma unroll
   for (int v = 0; v < VEC; v++) {
     E[v] = axis == 0 ? exps[row] : exps[col + v];
-#pragma unroll
-    for (int l = 0; l < L; l++) bad |= (abs_hi32(r[v][l]) >> 20) == 0x7ffu;
+    bad |= any_nonfinite<L>(r[v]);
   }
   if (bad && flags) atomicOr(flags, FLAG_NONFINITE);
 
   for (int q = 0; q < Q; q++) {
     double d[VEC];
 #pragma unroll
-    for (int v = 0; v < VEC; v++) {
-      // c = 1.5 * 2^(E - 13(q+1) + 52): exponent field + the top mantissa bit
-      const long long cbits = ((long long)(E[v] - 13 * (q + 1) + 52 + 1023) << 52) | (1ll << 51);
-      const double c = __longlong_as_double(cbits);
-      const double t = __dadd_rn(r[v][0], c);
-      d[v] = __dsub_rn(t, c);
-      r[v][0] = __dsub_rn(r[v][0], d[v]);
-#pragma unroll
-      for (int l = 0; l + 1 < L; l++) two_sum(r[v][l], r[v][l + 1], r[v][l], r[v][l + 1]);
-    }
+    for (int v = 0; v < VEC; v++) d[v] = extract_digit<L>(r[v], E[v], q);
     if (VEC == 2)
       *reinterpret_cast<double2*>(qplanes + (size_t)q * plane + idx) = make_double2(d[0], d[VEC - 1]);
     else
       qplanes[(size_t)q * plane + idx] = d[0];
+  }
+}
+
+// md_gemm's splitter: same digits, written in the fragment-major packed layout of md_packed.cuh (zero padded to whole
+// tiles and k-slabs).  A thread owns one fragment row: group x (row of A, AXIS 0 / column of B, AXIS 1) and the four
+// contraction indices k = 4*k4g .. 4*k4g+3, i.e. 32 contiguous output bytes per quarter; the 32 lanes of a warp take 32
+// consecutive x, so a warp writes 1 KB contiguous per quarter (and, for B, reads 256 contiguous bytes per row).
+template <int L, int AXIS>
+__global__ void __launch_bounds__(256) split_packed_kernel(int rows, int cols, int Q, int bx, int x_blocks, int KS,
+                                                           const double* __restrict__ planes,
+                                                           double* __restrict__ packed,
+                                                           const int32_t* __restrict__ exps, uint32_t* flags) {
+  const int X = AXIS == 0 ? rows : cols, K = AXIS == 0 ? cols : rows;
+  const int x = (blockIdx.x % x_blocks) * 32 + (threadIdx.x & 31);
+  const int k4g = (blockIdx.x / x_blocks) * 8 + (threadIdx.x >> 5);  // group of four k
+  const int XP = (X + bx - 1) / bx * bx;                             // padded to whole tiles
+  if (k4g >= KS * (PACK_BK / 4) || x >= XP) return;
+  const int k0 = k4g * 4;
+  const size_t plane = (size_t)rows * cols;
+
+  double r[4][L];
+  const bool x_ok = x < X;
+  if (AXIS == 0) {
+    const bool vec = x_ok && (k0 + 4 <= K) && (cols % 2 == 0) && ((reinterpret_cast<uintptr_t>(planes) & 15) == 0);
+    const double* src = planes + (size_t)(x_ok ? x : 0) * cols + k0;
+#pragma unroll
+    for (int l = 0; l < L; l++) {
+      if (vec) {
+        const double2 v0 = *reinterpret_cast<const double2*>(src + l * plane);
+        const double2 v1 = *reinterpret_cast<const double2*>(src + l * plane + 2);
+        r[0][l] = v0.x, r[1][l] = v0.y, r[2][l] = v1.x, r[3][l] = v1.y;
+      } else {
+#pragma unroll
+        for (int t = 0; t < 4; t++) r[t][l] = (x_ok && k0 + t < K) ? src[l * plane + t] : 0.0;
+      }
+    }
+  } else {
+#pragma unroll
+    for (int l = 0; l < L; l++)
+#pragma unroll
+      for (int t = 0; t < 4; t++)
+        r[t][l] = (x_ok && k0 + t < K) ? planes[l * plane + (size_t)(k0 + t) * cols + x] : 0.0;
+  }
+  const int E = x_ok ? exps[x] : 0;
+  bool bad = false;
+#pragma unroll
+  for (int t = 0; t < 4; t++) bad |= any_nonfinite<L>(r[t]);
+  if (bad && flags) atomicOr(flags, FLAG_NONFINITE);
+
+  // element (x, k0) of quarter 0; quarter q is q * (BK/4) * (bx/8) fragments further
+  double* dst = packed + packed_offset(x, k0, 0, bx, Q, KS);
+  const size_t q_stride = (size_t)(PACK_BK / 4) * (bx / 8) * 32;
+  for (int q = 0; q < Q; q++) {
+    double d[4];
+#pragma unroll
+    for (int t = 0; t < 4; t++) d[t] = extract_digit<L>(r[t], E, q);
+    *reinterpret_cast<double2*>(dst + q * q_stride) = make_double2(d[0], d[1]);
+    *reinterpret_cast<double2*>(dst + q * q_stride + 2) = make_double2(d[2], d[3]);
   }
 }
 
@@ -155,6 +226,29 @@ cudaError_t launch_split(int rows, int cols, int limbs, int quarters, int axis, 
     default: return cudaErrorInvalidValue;
   }
 #undef MD_SPLIT
+  *launches += 1;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_split_packed(int rows, int cols, int limbs, int quarters, int axis, const double* planes,
+                                double* packed, const int32_t* exps, uint32_t* flags, cudaStream_t stream,
+                                uint64_t* launches) {
+  const int X = axis == 0 ? rows : cols, K = axis == 0 ? cols : rows;
+  const int bx = pack_bx(limbs, axis);
+  const int KS = (K + PACK_BK - 1) / PACK_BK;
+  const int x_blocks = ((X + bx - 1) / bx * bx + 31) / 32;  // 32 groups per block over the padded extent
+  const long long k_blocks = ((long long)KS * (PACK_BK / 4) + 7) / 8;
+  const long long blocks = (long long)x_blocks * k_blocks;
+  if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
+#define MD_SPLITP(L_, AX_)                                                                                           \
+  split_packed_kernel<L_, AX_><<<(unsigned)blocks, 256, 0, stream>>>(rows, cols, quarters, bx, x_blocks, KS, planes, \
+                                                                     packed, exps, flags)
+  if (limbs == 2 && axis == 0) MD_SPLITP(2, 0);
+  else if (limbs == 2 && axis == 1) MD_SPLITP(2, 1);
+  else if (limbs == 4 && axis == 0) MD_SPLITP(4, 0);
+  else if (limbs == 4 && axis == 1) MD_SPLITP(4, 1);
+  else return cudaErrorInvalidValue;
+#undef MD_SPLITP
   *launches += 1;
   return cudaGetLastError();
 }
