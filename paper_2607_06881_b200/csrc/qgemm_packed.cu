@@ -30,16 +30,18 @@ namespace {
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+// mbarrier / bulk-copy wrappers; barriers and shared destinations are passed as 32-bit shared-window addresses that the
+// kernel computes once (a generic->shared conversion inside the k loop costs an S2R + LEA chain per slab).
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
 }
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   asm volatile(
       "{\n"
       ".reg .pred P1;\n"
@@ -48,14 +50,13 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
       "@P1 bra DONE;\n"
       "bra LAB_WAIT;\n"
       "DONE:\n"
-      "}" ::"r"(smem_u32(bar)), "r"(parity)
+      "}" ::"r"(bar), "r"(parity)
       : "memory");
 }
 // global -> shared bulk copy (bytes % 16 == 0, both addresses 16-byte aligned); completion = complete_tx on `bar`.
-__device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gmem_src, uint32_t bytes, uint64_t* bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                   smem_u32(smem_dst)),
-               "l"(gmem_src), "r"(bytes), "r"(smem_u32(bar))
+__device__ __forceinline__ void bulk_g2s(uint32_t smem_dst, const void* gmem_src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_dst),
+               "l"(gmem_src), "r"(bytes), "r"(bar)
                : "memory");
 }
 
@@ -71,6 +72,8 @@ struct PCfg {
   static constexpr int BAR_BYTES = 128;
   static constexpr int STAGES = ((SMEM_LIMIT - BAR_BYTES) / STAGE_BYTES) < 6 ? ((SMEM_LIMIT - BAR_BYTES) / STAGE_BYTES) : 6;
   static constexpr int AHEAD = STAGES - 2;  // slabs in flight beyond the one being consumed
+  // second register set of operand fragments (software pipelining across k-steps and slabs) where 255 registers allow
+  static constexpr bool PREFETCH = (S * MT * NT * 4 + 2 * (Q * MT + NT) * 2) <= 200;
   static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES;
   static_assert(STAGES >= 3, "the non-blocking refill needs at least 3 stages");
   static_assert(2 * STAGES * 8 <= BAR_BYTES, "barrier area");
@@ -95,21 +98,23 @@ qgemm_packed_kernel(int m, int n, int KS, int tiles_m, int tiles_n, const double
   const double* const Asrc = Ap + (size_t)tm * KS * C::A_CHUNK;
   const double* const Bsrc = Bp + (size_t)tn * KS * C::B_CHUNK;
 
+  const uint32_t stages_u32 = smem_u32(stages);
+  const uint32_t full_u32 = smem_u32(full), empty_u32 = smem_u32(empty);  // barrier s at + 8 * s
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s < STAGES; s++) {
-      mbar_init(&full[s], 1);
-      mbar_init(&empty[s], C::WARPS);
+      mbar_init(full_u32 + 8 * s, 1);
+      mbar_init(empty_u32 + 8 * s, C::WARPS);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
 
   auto issue = [&](int slab, int st) {  // one thread: arm the stage's full barrier and start the two bulk copies
-    double* dst = stages + (size_t)st * (C::A_CHUNK + C::B_CHUNK);
-    mbar_expect_tx(&full[st], C::STAGE_BYTES);
-    bulk_g2s(dst, Asrc + (size_t)slab * C::A_CHUNK, C::A_CHUNK * 8, &full[st]);
-    bulk_g2s(dst + C::A_CHUNK, Bsrc + (size_t)slab * C::B_CHUNK, C::B_CHUNK * 8, &full[st]);
+    const uint32_t dst = stages_u32 + st * C::STAGE_BYTES;
+    mbar_expect_tx(full_u32 + 8 * st, C::STAGE_BYTES);
+    bulk_g2s(dst, Asrc + (size_t)slab * C::A_CHUNK, C::A_CHUNK * 8, full_u32 + 8 * st);
+    bulk_g2s(dst + C::A_CHUNK * 8, Bsrc + (size_t)slab * C::B_CHUNK, C::B_CHUNK * 8, full_u32 + 8 * st);
   };
   if (tid == 0) {
 #pragma unroll
@@ -125,48 +130,95 @@ qgemm_packed_kernel(int m, int n, int KS, int tiles_m, int tiles_n, const double
 #pragma unroll
       for (int j = 0; j < NT; j++) acc[s][i][j][0] = acc[s][i][j][1] = 0.0;
 
-  int st = 0;               // stage of slab kt
-  uint32_t phase = 0;       // parity of that stage's current fill
-  int pst = C::AHEAD % STAGES;  // stage of slab kt + AHEAD (producer side, thread 0 only)
-  for (int kt = 0; kt < KS; kt++) {
-    if (tid == 0) {
-      const int slab = kt + C::AHEAD;
-      if (slab < KS) {
-        // the stage was last read for slab (slab - STAGES) = kt - 2: wait for its release (completed long ago)
-        if (slab >= STAGES) mbar_wait(&empty[pst], ((slab / STAGES) + 1) & 1);
-        issue(slab, pst);
-      }
+  // Operand fragments of one DMMA k-step held in registers: all Q quarters of the warp's MT row blocks of A, and the
+  // quarter-0 fragments of its NT column blocks of B (the B fragments of quarters 1.. are loaded inside the step).
+  // Two sets: while the DMMAs of one k-step issue, the next step's set is already being loaded -- across the slab
+  // boundary too, so no LDS latency is exposed at the hand-over between stages.
+  struct Frags {
+    double a[Q][MT];
+    double b0[NT];
+  };
+  auto load_frags = [&](Frags& f, const double* As, const double* Bs, int k4) {
+#pragma unroll
+    for (int p = 0; p < Q; p++)
+#pragma unroll
+      for (int i = 0; i < MT; i++) f.a[p][i] = As[((p * C::K4 + k4) * C::R8 + i) * 32];
+#pragma unroll
+    for (int j = 0; j < NT; j++) f.b0[j] = Bs[(k4 * C::N8 + j) * 32];
+  };
+  auto k_step = [&](const Frags& f, const double* Bs, int k4) {
+#pragma unroll
+    for (int q = 0; q < Q; q++) {
+      double b[NT];
+#pragma unroll
+      for (int j = 0; j < NT; j++) b[j] = q == 0 ? f.b0[j] : Bs[((q * C::K4 + k4) * C::N8 + j) * 32];
+#pragma unroll
+      for (int p = 0; p + q < S; p++)  // product (p, q) goes to order s = p + q: consecutive DMMAs hit different accumulators
+#pragma unroll
+        for (int i = 0; i < MT; i++)
+#pragma unroll
+          for (int j = 0; j < NT; j++) dmma_8x8x4(acc[p + q][i][j], f.a[p][i], b[j]);
     }
-    pst = (pst + 1 == STAGES) ? 0 : pst + 1;
+  };
+  static_assert(C::K4 == 2, "the k loop below is written for two DMMA k-steps per slab");
+  const int a_off = (wm * MT) * 32 + lane, b_off = C::A_CHUNK + (wn * NT) * 32 + lane;
 
-    mbar_wait(&full[st], phase);
-    const double* As = stages + (size_t)st * (C::A_CHUNK + C::B_CHUNK) + (wm * MT) * 32 + lane;
-    const double* Bs = stages + (size_t)st * (C::A_CHUNK + C::B_CHUNK) + C::A_CHUNK + (wn * NT) * 32 + lane;
-#pragma unroll
-    for (int k4 = 0; k4 < C::K4; k4++) {
-      double a[Q][MT];
-#pragma unroll
-      for (int p = 0; p < Q; p++)
-#pragma unroll
-        for (int i = 0; i < MT; i++) a[p][i] = As[((p * C::K4 + k4) * C::R8 + i) * 32];
-#pragma unroll
-      for (int q = 0; q < Q; q++) {
-        double b[NT];
-#pragma unroll
-        for (int j = 0; j < NT; j++) b[j] = Bs[((q * C::K4 + k4) * C::N8 + j) * 32];
-#pragma unroll
-        for (int p = 0; p + q < S; p++)  // product (p, q) goes to order s = p + q: consecutive DMMAs hit different accumulators
-#pragma unroll
-          for (int i = 0; i < MT; i++)
-#pragma unroll
-            for (int j = 0; j < NT; j++) dmma_8x8x4(acc[p + q][i][j], a[p][i], b[j]);
-      }
+  int st = 0;                   // stage of slab kt
+  uint32_t phase = 0;           // parity of that stage's current fill
+  int pst = C::AHEAD % STAGES;  // stage of slab kt + AHEAD (producer side, thread 0 only)
+  auto produce = [&](int kt) {  // thread 0: refill for slab kt + AHEAD
+    const int slab = kt + C::AHEAD;
+    if (slab < KS) {
+      // the stage was last read for slab (slab - STAGES) = kt - 2: wait for its release (completed long ago)
+      if (slab >= STAGES) mbar_wait(empty_u32 + 8 * pst, ((slab / STAGES) + 1) & 1);
+      issue(slab, pst);
     }
-    __syncwarp();
-    if (lane == 0) mbar_arrive(&empty[st]);  // this warp is done reading the stage
-    if (++st == STAGES) {
-      st = 0;
-      phase ^= 1;
+  };
+  if constexpr (C::PREFETCH) {
+    Frags f0, f1;
+    mbar_wait(full_u32, 0);
+    load_frags(f0, stages + a_off, stages + b_off, 0);
+    for (int kt = 0; kt < KS; kt++) {
+      if (tid == 0) produce(kt);
+      pst = (pst + 1 == STAGES) ? 0 : pst + 1;
+
+      const double* As = stages + (size_t)st * (C::A_CHUNK + C::B_CHUNK) + a_off;
+      const double* Bs = stages + (size_t)st * (C::A_CHUNK + C::B_CHUNK) + b_off;
+      load_frags(f1, As, Bs, 1);
+      k_step(f0, Bs, 0);
+
+      const int nst = (st + 1 == STAGES) ? 0 : st + 1;
+      const uint32_t nphase = (st + 1 == STAGES) ? phase ^ 1 : phase;
+      if (kt + 1 < KS) {  // next slab: its first k-step's fragments are fetched under this slab's second k-step
+        mbar_wait(full_u32 + 8 * nst, nphase);
+        load_frags(f0, stages + (size_t)nst * (C::A_CHUNK + C::B_CHUNK) + a_off,
+                   stages + (size_t)nst * (C::A_CHUNK + C::B_CHUNK) + b_off, 0);
+      }
+      k_step(f1, Bs, 1);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(empty_u32 + 8 * st);  // this warp is done reading the stage
+      st = nst;
+      phase = nphase;
+    }
+  } else {  // one fragment set (register budget): loads of a k-step are issued at its start
+    for (int kt = 0; kt < KS; kt++) {
+      if (tid == 0) produce(kt);
+      pst = (pst + 1 == STAGES) ? 0 : pst + 1;
+      mbar_wait(full_u32 + 8 * st, phase);
+      const double* As = stages + (size_t)st * (C::A_CHUNK + C::B_CHUNK) + a_off;
+      const double* Bs = stages + (size_t)st * (C::A_CHUNK + C::B_CHUNK) + b_off;
+#pragma unroll
+      for (int k4 = 0; k4 < C::K4; k4++) {
+        Frags f;
+        load_frags(f, As, Bs, k4);
+        k_step(f, Bs, k4);
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(empty_u32 + 8 * st);
+      if (++st == STAGES) {
+        st = 0;
+        phase ^= 1;
+      }
     }
   }
 
