@@ -34,13 +34,14 @@ inline int quarters_for(int limbs) { return g_state.opt_quarters ? g_state.opt_q
 inline int orders_for(int limbs) { return g_state.opt_orders ? g_state.opt_orders : quarters_for(limbs); }
 
 // Workspace layout: [status word | expA int32[m] | expB int32[n] | Aq | Bq], Aq / Bq = the packed quarter planes of A / B
-// (md_packed.cuh: zero padded to whole CTA tiles and k-slabs)
+// (md_packed.cuh: zero padded to whole CTA tiles and k-slabs), then the stream-K scratch of the fused GEMM
 struct Carve {
   uint32_t* flags;
   int32_t* expA;
   int32_t* expB;
   double* Aq;
   double* Bq;
+  void* sk;  // stream-K scratch of the fused GEMM
   size_t total;
 };
 Carve carve(void* base, int m, int n, int k, int limbs, int quarters) {
@@ -57,6 +58,8 @@ Carve carve(void* base, int m, int n, int k, int limbs, int quarters) {
   off += round_up(sizeof(double) * md::packed_doubles(m, k, md::pack_bx(limbs, 0), quarters));
   c.Bq = reinterpret_cast<double*>(p + off);
   off += round_up(sizeof(double) * md::packed_doubles(n, k, md::pack_bx(limbs, 1), quarters));
+  c.sk = p + off;
+  off += round_up(md::sk_workspace_bytes(limbs, quarters));
   c.total = off;
   return c;
 }
@@ -91,7 +94,7 @@ md_status gemm_impl(int m, int n, int k, int limbs, const double* A, const doubl
   if (err == cudaSuccess) err = md::launch_split_packed(k, n, limbs, Q, 1, B, c.Bq, c.expB, c.flags, stream, &launches);
   if (ev) cudaEventRecord(ev[1], stream);
   if (err == cudaSuccess)
-    err = md::launch_qgemm_packed(m, n, k, limbs, Q, c.Aq, c.Bq, order_planes, C_planes, stream, &launches);
+    err = md::launch_qgemm_packed(m, n, k, limbs, Q, c.Aq, c.Bq, order_planes, C_planes, c.sk, stream, &launches);
   if (ev) {
     cudaEventRecord(ev[2], stream);
     if (err == cudaSuccess) g_prof.count++;

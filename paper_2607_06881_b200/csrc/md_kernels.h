@@ -22,8 +22,15 @@ bool qgemm_supported(int limbs, int quarters);
 cudaError_t launch_split_packed(int rows, int cols, int limbs, int quarters, int axis, const double* planes,
                                 double* packed, const int32_t* exps, uint32_t* flags, cudaStream_t stream,
                                 uint64_t* launches);
+// sk_ws: sk_workspace_bytes(limbs, quarters) bytes of device scratch for the stream-K tail (slab counters + one
+// order-plane tile per stream-K tile); zeroed by the launcher (a memset node on `stream`) as far as it is used.
+constexpr int SK_MAX_TILES = 256;
+constexpr size_t SK_COUNTER_BYTES = 1024;  // SK_MAX_TILES unsigned ints
+size_t sk_workspace_bytes(int limbs, int quarters);
+int sk_grid();
 cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, const double* Ap, const double* Bp,
-                                double* order_planes, double* C_planes, cudaStream_t stream, uint64_t* launches);
+                                double* order_planes, double* C_planes, void* sk_ws, cudaStream_t stream,
+                                uint64_t* launches);
 // calibration (probe.cu): register-only DMMA loop; *flops receives the FP64 flops the launch issues
 cudaError_t launch_dmma_probe(int blocks, int warps_per_block, int iters, double* sink, cudaStream_t stream,
                               uint64_t* launches, uint64_t* flops);

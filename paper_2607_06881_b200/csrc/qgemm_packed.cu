@@ -76,27 +76,62 @@ struct PCfg {
   static constexpr bool PREFETCH = (S * MT * NT * 4 + 2 * (Q * MT + NT) * 2) <= 200;
   static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES;
   static_assert(STAGES >= 3, "the non-blocking refill needs at least 3 stages");
-  static_assert(2 * STAGES * 8 <= BAR_BYTES, "barrier area");
+  static_assert(2 * STAGES * 8 <= BAR_BYTES - 8, "barrier area (its last 8 bytes hold the stream-K flag)");
   static_assert(STAGE_BYTES % 128 == 0, "stage alignment");
+};
+
+// Persistent kernel: gridDim.x = G CTAs (one per SM), each walks a private list of SEGMENTS = (tile, slab range):
+//   * stream-K part first: the sk_tiles tiles that do not fill a whole wave of G CTAs are cut along k into G nearly equal
+//     runs of slabs (CTA b owns global slab iterations [b*ipc, (b+1)*ipc) of the sk_tiles * KS), so that the last wave costs
+//     sk_tiles*KS/G slab-times instead of KS.  A CTA adds its partial order sums into the tile's scratch with fp64
+//     red.global.add -- EXACT here, every partial sum being an integer below 2^53 units (R6), hence the result is
+//     bit-identical whatever the arrival order -- then bumps the tile's slab counter; whoever completes the count re-reads
+//     the scratch and runs the epilogue.  Nobody ever waits for another CTA.
+//   * then dp_waves whole tiles, ids b, b + G, b + 2G, ... (tile ids are rasterised, so at any time the G CTAs cover a
+//     compact patch of C), accumulated and renormalised entirely in registers.
+// The stage ring runs straight through segment boundaries: the refill thread is AHEAD slabs ahead, possibly already in the
+// next tile, so the pipeline never drains between tiles.
+struct SkPlan {
+  int KS;                // k slabs per tile
+  int tiles_m, tiles_n;
+  int dp_waves;          // whole tiles per CTA
+  int sk_tiles;          // tiles dp_waves*G .. dp_waves*G + sk_tiles - 1 are processed stream-K
+  int sk_iters_per_cta;  // ipc
 };
 
 template <class C>
 __global__ void __launch_bounds__(C::THREADS, 1)
-qgemm_packed_kernel(int m, int n, int KS, int tiles_m, int tiles_n, const double* __restrict__ Ap,
-                    const double* __restrict__ Bp, double* __restrict__ order_planes, double* __restrict__ C_planes) {
+qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, const double* __restrict__ Bp,
+                    double* __restrict__ order_planes, double* __restrict__ C_planes, double* __restrict__ sk_scratch,
+                    unsigned int* __restrict__ sk_counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   constexpr int Q = C::Q, S = C::S, L = C::L, MT = C::MT, NT = C::NT, STAGES = C::STAGES;
   double* const stages = reinterpret_cast<double*>(smem_raw);
   uint64_t* const full = reinterpret_cast<uint64_t*>(smem_raw + STAGES * C::STAGE_BYTES);
   uint64_t* const empty = full + STAGES;
+  volatile int* const last_flag = reinterpret_cast<volatile int*>(smem_raw + STAGES * C::STAGE_BYTES + C::BAR_BYTES - 8);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int wm = warp / C::WN, wn = warp % C::WN;
+  const int G = gridDim.x, cta = blockIdx.x, KS = plan.KS;
 
-  int tm, tn;
-  raster_tile(blockIdx.x, tiles_m, tiles_n, tm, tn);
-  // this CTA's operand streams: KS consecutive chunks each
-  const double* const Asrc = Ap + (size_t)tm * KS * C::A_CHUNK;
-  const double* const Bsrc = Bp + (size_t)tn * KS * C::B_CHUNK;
+  // ---- this CTA's segment list ---------------------------------------------------------------------------------------
+  const int sk_total = plan.sk_tiles * KS;
+  const int g0 = min(cta * plan.sk_iters_per_cta, sk_total), g1 = min(g0 + plan.sk_iters_per_cta, sk_total);
+  const int n_sk = g1 > g0 ? (g1 - 1) / KS - g0 / KS + 1 : 0;
+  const int n_seg = n_sk + plan.dp_waves;
+  const int total_slabs = (g1 - g0) + plan.dp_waves * KS;
+  auto segment = [&](int i, int& tile, int& s0, int& s1) {
+    if (i < n_sk) {
+      const int r = g0 / KS + i;
+      tile = plan.dp_waves * G + r;
+      s0 = i == 0 ? g0 - r * KS : 0;
+      s1 = min(KS, g1 - r * KS);
+    } else {
+      tile = (i - n_sk) * G + cta;
+      s0 = 0;
+      s1 = KS;
+    }
+  };
 
   const uint32_t stages_u32 = smem_u32(stages);
   const uint32_t full_u32 = smem_u32(full), empty_u32 = smem_u32(empty);  // barrier s at + 8 * s
@@ -109,26 +144,53 @@ qgemm_packed_kernel(int m, int n, int KS, int tiles_m, int tiles_n, const double
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
+  if (total_slabs == 0) return;
 
-  auto issue = [&](int slab, int st) {  // one thread: arm the stage's full barrier and start the two bulk copies
-    const uint32_t dst = stages_u32 + st * C::STAGE_BYTES;
-    mbar_expect_tx(full_u32 + 8 * st, C::STAGE_BYTES);
-    bulk_g2s(dst, Asrc + (size_t)slab * C::A_CHUNK, C::A_CHUNK * 8, full_u32 + 8 * st);
-    bulk_g2s(dst + C::A_CHUNK * 8, Bsrc + (size_t)slab * C::B_CHUNK, C::B_CHUNK * 8, full_u32 + 8 * st);
+  // ---- producer side (thread 0): a cursor over the flat slab sequence, AHEAD slabs ahead of the consumers -------------
+  int p_seg = -1, p_left = 0, p_flat = 0, pst = 0;
+  const double *p_A = nullptr, *p_B = nullptr;
+  auto produce_one = [&]() {  // issue the bulk copies of flat slab p_flat into stage pst (its empty barrier has completed)
+    if (p_left == 0) {
+      int tile, s0, s1, tm, tn;
+      segment(++p_seg, tile, s0, s1);
+      raster_tile(tile, plan.tiles_m, plan.tiles_n, tm, tn);
+      p_A = Ap + ((size_t)tm * KS + s0) * C::A_CHUNK;
+      p_B = Bp + ((size_t)tn * KS + s0) * C::B_CHUNK;
+      p_left = s1 - s0;
+    }
+    const uint32_t dst = stages_u32 + pst * C::STAGE_BYTES, bar = full_u32 + 8 * pst;
+    mbar_expect_tx(bar, C::STAGE_BYTES);
+    bulk_g2s(dst, p_A, C::A_CHUNK * 8, bar);
+    bulk_g2s(dst + C::A_CHUNK * 8, p_B, C::B_CHUNK * 8, bar);
+    p_A += C::A_CHUNK;
+    p_B += C::B_CHUNK;
+    p_left--;
+    p_flat++;
+    pst = (pst + 1 == STAGES) ? 0 : pst + 1;
   };
   if (tid == 0) {
 #pragma unroll
     for (int j = 0; j < C::AHEAD; j++)
-      if (j < KS) issue(j, j);
+      if (p_flat < total_slabs) produce_one();
   }
+  auto produce = [&]() {  // top of consumer iteration `it`: refill for flat slab it + AHEAD
+    if (p_flat < total_slabs) {
+      // the stage was last read for flat slab (p_flat - STAGES) = it - 2: wait for its release (completed long ago)
+      if (p_flat >= STAGES) mbar_wait(empty_u32 + 8 * pst, ((p_flat / STAGES) + 1) & 1);
+      produce_one();
+    }
+  };
 
   double acc[S][MT][NT][2];
+  auto zero_acc = [&]() {
 #pragma unroll
-  for (int s = 0; s < S; s++)
+    for (int s = 0; s < S; s++)
 #pragma unroll
-    for (int i = 0; i < MT; i++)
+      for (int i = 0; i < MT; i++)
 #pragma unroll
-      for (int j = 0; j < NT; j++) acc[s][i][j][0] = acc[s][i][j][1] = 0.0;
+        for (int j = 0; j < NT; j++) acc[s][i][j][0] = acc[s][i][j][1] = 0.0;
+  };
+  zero_acc();
 
   // Operand fragments of one DMMA k-step held in registers: all Q quarters of the warp's MT row blocks of A, and the
   // quarter-0 fragments of its NT column blocks of B (the B fragments of quarters 1.. are loaded inside the step).
@@ -163,25 +225,65 @@ qgemm_packed_kernel(int m, int n, int KS, int tiles_m, int tiles_n, const double
   static_assert(C::K4 == 2, "the k loop below is written for two DMMA k-steps per slab");
   const int a_off = (wm * MT) * 32 + lane, b_off = C::A_CHUNK + (wn * NT) * 32 + lane;
 
-  int st = 0;                   // stage of slab kt
-  uint32_t phase = 0;           // parity of that stage's current fill
-  int pst = C::AHEAD % STAGES;  // stage of slab kt + AHEAD (producer side, thread 0 only)
-  auto produce = [&](int kt) {  // thread 0: refill for slab kt + AHEAD
-    const int slab = kt + C::AHEAD;
-    if (slab < KS) {
-      // the stage was last read for slab (slab - STAGES) = kt - 2: wait for its release (completed long ago)
-      if (slab >= STAGES) mbar_wait(empty_u32 + 8 * pst, ((slab / STAGES) + 1) & 1);
-      issue(slab, pst);
+  // ---- consumer side: segment bookkeeping and the end-of-segment epilogue ----------------------------------------------
+  int c_seg = 0, c_tile, c_s0, c_s1;
+  segment(0, c_tile, c_s0, c_s1);
+  int c_left = c_s1 - c_s0;
+  auto end_of_segment = [&]() {
+    int tm, tn;
+    raster_tile(c_tile, plan.tiles_m, plan.tiles_n, tm, tn);
+    const int row_base = tm * C::BM + wm * MT * 8, col_base = tn * C::BN + wn * NT * 8;
+    if (c_s1 - c_s0 == KS) {  // whole tile in registers
+      qgemm_epilogue<S, L, MT, NT>(acc, m, n, row_base, col_base, lane, order_planes, C_planes);
+    } else {                  // partial sums of a stream-K tile: exact fp64 reduction through the tile's scratch
+      const int r = c_tile - plan.dp_waves * G;
+      double* sc = sk_scratch + (size_t)r * (S * C::BM * C::BN) + (size_t)warp * (S * MT * NT * 64) + lane * 2;
+#pragma unroll
+      for (int s = 0; s < S; s++)
+#pragma unroll
+        for (int i = 0; i < MT; i++)
+#pragma unroll
+          for (int j = 0; j < NT; j++) {
+            atomicAdd(sc + ((s * MT + i) * NT + j) * 64, acc[s][i][j][0]);
+            atomicAdd(sc + ((s * MT + i) * NT + j) * 64 + 1, acc[s][i][j][1]);
+          }
+      __threadfence();
+      __syncthreads();
+      if (tid == 0) {
+        const unsigned int mine = (unsigned int)(c_s1 - c_s0);
+        *last_flag = (atomicAdd(&sk_counters[r], mine) + mine == (unsigned int)KS);
+      }
+      __syncthreads();
+      if (*last_flag) {  // every slab of the tile has been added: read the totals back and finish the tile
+        __threadfence();
+#pragma unroll
+        for (int s = 0; s < S; s++)
+#pragma unroll
+          for (int i = 0; i < MT; i++)
+#pragma unroll
+            for (int j = 0; j < NT; j++) {
+              const double2 v = __ldcg(reinterpret_cast<const double2*>(sc + ((s * MT + i) * NT + j) * 64));
+              acc[s][i][j][0] = v.x;
+              acc[s][i][j][1] = v.y;
+            }
+        qgemm_epilogue<S, L, MT, NT>(acc, m, n, row_base, col_base, lane, order_planes, C_planes);
+      }
+    }
+    zero_acc();
+    if (++c_seg < n_seg) {
+      segment(c_seg, c_tile, c_s0, c_s1);
+      c_left = c_s1 - c_s0;
     }
   };
+
+  int st = 0;          // stage of the slab being consumed
+  uint32_t phase = 0;  // parity of that stage's current fill
   if constexpr (C::PREFETCH) {
     Frags f0, f1;
     mbar_wait(full_u32, 0);
     load_frags(f0, stages + a_off, stages + b_off, 0);
-    for (int kt = 0; kt < KS; kt++) {
-      if (tid == 0) produce(kt);
-      pst = (pst + 1 == STAGES) ? 0 : pst + 1;
-
+    for (int it = 0; it < total_slabs; it++) {
+      if (tid == 0) produce();
       const double* As = stages + (size_t)st * (C::A_CHUNK + C::B_CHUNK) + a_off;
       const double* Bs = stages + (size_t)st * (C::A_CHUNK + C::B_CHUNK) + b_off;
       load_frags(f1, As, Bs, 1);
@@ -189,7 +291,7 @@ qgemm_packed_kernel(int m, int n, int KS, int tiles_m, int tiles_n, const double
 
       const int nst = (st + 1 == STAGES) ? 0 : st + 1;
       const uint32_t nphase = (st + 1 == STAGES) ? phase ^ 1 : phase;
-      if (kt + 1 < KS) {  // next slab: its first k-step's fragments are fetched under this slab's second k-step
+      if (it + 1 < total_slabs) {  // next slab: its first k-step's fragments are fetched under this slab's second k-step
         mbar_wait(full_u32 + 8 * nst, nphase);
         load_frags(f0, stages + (size_t)nst * (C::A_CHUNK + C::B_CHUNK) + a_off,
                    stages + (size_t)nst * (C::A_CHUNK + C::B_CHUNK) + b_off, 0);
@@ -199,11 +301,11 @@ qgemm_packed_kernel(int m, int n, int KS, int tiles_m, int tiles_n, const double
       if (lane == 0) mbar_arrive(empty_u32 + 8 * st);  // this warp is done reading the stage
       st = nst;
       phase = nphase;
+      if (--c_left == 0) end_of_segment();
     }
   } else {  // one fragment set (register budget): loads of a k-step are issued at its start
-    for (int kt = 0; kt < KS; kt++) {
-      if (tid == 0) produce(kt);
-      pst = (pst + 1 == STAGES) ? 0 : pst + 1;
+    for (int it = 0; it < total_slabs; it++) {
+      if (tid == 0) produce();
       mbar_wait(full_u32 + 8 * st, phase);
       const double* As = stages + (size_t)st * (C::A_CHUNK + C::B_CHUNK) + a_off;
       const double* Bs = stages + (size_t)st * (C::A_CHUNK + C::B_CHUNK) + b_off;
@@ -219,25 +321,38 @@ qgemm_packed_kernel(int m, int n, int KS, int tiles_m, int tiles_n, const double
         st = 0;
         phase ^= 1;
       }
+      if (--c_left == 0) end_of_segment();
     }
   }
-
-  qgemm_epilogue<S, L, MT, NT>(acc, m, n, tm * C::BM + wm * MT * 8, tn * C::BN + wn * NT * 8, lane, order_planes,
-                               C_planes);
 }
 
 template <class C>
 cudaError_t launch_cfg(int m, int n, int k, const double* Ap, const double* Bp, double* order_planes, double* C_planes,
-                       cudaStream_t stream) {
+                       void* sk_ws, cudaStream_t stream) {
   static_assert(C::BM == pack_bx(C::L, 0) && C::BN == pack_bx(C::L, 1), "tile shape must match the packed layout");
   const int tiles_m = (m + C::BM - 1) / C::BM, tiles_n = (n + C::BN - 1) / C::BN;
   const long long tiles = (long long)tiles_m * tiles_n;
   if (tiles > 0x7fffffffLL) return cudaErrorInvalidValue;
-  const int KS = (k + C::BK - 1) / C::BK;
+  const int G = sk_grid();
+  if (G <= 0) return cudaErrorInvalidDevice;
+  SkPlan plan;
+  plan.KS = (k + C::BK - 1) / C::BK;
+  plan.tiles_m = tiles_m;
+  plan.tiles_n = tiles_n;
+  plan.dp_waves = (int)(tiles / G);
+  plan.sk_tiles = (int)(tiles % G);
+  plan.sk_iters_per_cta = (int)(((long long)plan.sk_tiles * plan.KS + G - 1) / G);
+  unsigned int* counters = static_cast<unsigned int*>(sk_ws);
+  double* scratch = reinterpret_cast<double*>(static_cast<char*>(sk_ws) + SK_COUNTER_BYTES);
+  cudaError_t err;
+  if (plan.sk_tiles > 0) {  // counters and the scratch tiles in use start at zero (one contiguous region)
+    err = cudaMemsetAsync(sk_ws, 0, SK_COUNTER_BYTES + sizeof(double) * (size_t)plan.sk_tiles * C::S * C::BM * C::BN, stream);
+    if (err != cudaSuccess) return err;
+  }
   auto kern = qgemm_packed_kernel<C>;
-  cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+  err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
   if (err != cudaSuccess) return err;
-  kern<<<(unsigned)tiles, C::THREADS, C::SMEM_BYTES, stream>>>(m, n, KS, tiles_m, tiles_n, Ap, Bp, order_planes, C_planes);
+  kern<<<G, C::THREADS, C::SMEM_BYTES, stream>>>(m, n, plan, Ap, Bp, order_planes, C_planes, scratch, counters);
   return cudaGetLastError();
 }
 
@@ -248,17 +363,34 @@ template <int Q> using PCfgQD = PCfg<Q, 4, 4, 2, 1, 1>;
 
 }  // namespace
 
+// CTAs of the persistent grid: one per SM, at most SK_MAX_TILES (the scratch holds one tile per stream-K tile, < grid)
+int sk_grid() {
+  static int sms = 0;
+  if (sms == 0) {
+    int dev = 0, v = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+      return -1;
+    sms = v;
+  }
+  return sms < SK_MAX_TILES ? sms : SK_MAX_TILES;
+}
+
+size_t sk_workspace_bytes(int limbs, int quarters) {
+  return SK_COUNTER_BYTES + sizeof(double) * (size_t)SK_MAX_TILES * quarters * pack_bx(limbs, 0) * pack_bx(limbs, 1);
+}
+
 cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, const double* Ap, const double* Bp,
-                                double* order_planes, double* C_planes, cudaStream_t stream, uint64_t* launches) {
+                                double* order_planes, double* C_planes, void* sk_ws, cudaStream_t stream,
+                                uint64_t* launches) {
   cudaError_t err = cudaErrorInvalidValue;
   if (limbs == 2) {
-    if (quarters == 8) err = launch_cfg<PCfgDD<8>>(m, n, k, Ap, Bp, order_planes, C_planes, stream);
-    if (quarters == 9) err = launch_cfg<PCfgDD<9>>(m, n, k, Ap, Bp, order_planes, C_planes, stream);
-    if (quarters == 10) err = launch_cfg<PCfgDD<10>>(m, n, k, Ap, Bp, order_planes, C_planes, stream);
+    if (quarters == 8) err = launch_cfg<PCfgDD<8>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
+    if (quarters == 9) err = launch_cfg<PCfgDD<9>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
+    if (quarters == 10) err = launch_cfg<PCfgDD<10>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
   } else if (limbs == 4) {
-    if (quarters == 16) err = launch_cfg<PCfgQD<16>>(m, n, k, Ap, Bp, order_planes, C_planes, stream);
-    if (quarters == 17) err = launch_cfg<PCfgQD<17>>(m, n, k, Ap, Bp, order_planes, C_planes, stream);
-    if (quarters == 18) err = launch_cfg<PCfgQD<18>>(m, n, k, Ap, Bp, order_planes, C_planes, stream);
+    if (quarters == 16) err = launch_cfg<PCfgQD<16>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
+    if (quarters == 17) err = launch_cfg<PCfgQD<17>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
+    if (quarters == 18) err = launch_cfg<PCfgQD<18>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
   }
   if (err == cudaSuccess) *launches += 1;
   return err;

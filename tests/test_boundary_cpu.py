@@ -61,7 +61,11 @@ def test_options_and_workspace_sizes(lib):
     assert lib.md_get_option(md.MD_OPT_QUARTERS) == 0 and lib.md_get_option(99) == -1
     base = lib.md_workspace_bytes(64, 64, 64, 2)
     # a quartered double double matrix has 8 times the size of a matrix of doubles
-    assert base >= 2 * 8 * 64 * 64 * 8 and base < 2 * 8 * 64 * 64 * 8 + 4096
+    # plus the fixed stream-K scratch of the fused GEMM: 256 tiles of 8 orders x 64 x 32 doubles + slab counters
+    sk = 1024 + 256 * 8 * 64 * 32 * 8
+    assert base >= 2 * 8 * 64 * 64 * 8 + sk and base < 2 * 8 * 64 * 64 * 8 + sk + 4096
+    # the packed quarter planes are zero padded to whole CTA tiles (64 rows of A, 32 columns of B) and k-slabs of 8
+    assert lib.md_workspace_bytes(65, 33, 9, 2) - lib.md_workspace_bytes(64, 32, 8, 2) == 8 * 8 * (128 * 16 + 64 * 16 - 64 * 8 - 32 * 8) + 256
     assert lib.md_set_option(md.MD_OPT_QUARTERS, 9) == 0
     assert lib.md_workspace_bytes(64, 64, 64, 2) >= 2 * 9 * 64 * 64 * 8
     assert lib.md_set_option(md.MD_OPT_QUARTERS, 0) == 0
