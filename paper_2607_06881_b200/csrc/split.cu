@@ -127,6 +127,16 @@ __global__ void __launch_bounds__(256) split_kernel(size_t rows, size_t cols, in
   }
 }
 
+// 256-bit global accesses (sm_100: LDG.E.ENL2.256 / STG.E.ENL2.256); p must be 32-byte aligned.  A fragment row of the
+// packed layout is 4 doubles, so one store per quarter per thread fills whole 32-byte sectors (two 16-byte stores at a
+// 32-byte lane stride half-fill 32 sectors each and made the kernel L1-bound: profiles/r01c_split_ncu.md).
+__device__ __forceinline__ void ldg_256(const double* p, double& a, double& b, double& c, double& d) {
+  asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
+}
+__device__ __forceinline__ void stg_256(double* p, double a, double b, double c, double d) {
+  asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
+}
+
 // md_gemm's splitter: same digits, written in the fragment-major packed layout of md_packed.cuh (zero padded to whole
 // tiles and k-slabs).  A thread owns one fragment row: group x (row of A, AXIS 0 / column of B, AXIS 1) and the four
 // contraction indices k = 4*k4g .. 4*k4g+3, i.e. 32 contiguous output bytes per quarter; the 32 lanes of a warp take 32
@@ -147,14 +157,13 @@ __global__ void __launch_bounds__(256) split_packed_kernel(int rows, int cols, i
   double r[4][L];
   const bool x_ok = x < X;
   if (AXIS == 0) {
-    const bool vec = x_ok && (k0 + 4 <= K) && (cols % 2 == 0) && ((reinterpret_cast<uintptr_t>(planes) & 15) == 0);
+    // rows of every limb plane 32-byte aligned -> one 256-bit load per limb (k0 is a multiple of 4)
+    const bool vec = x_ok && (k0 + 4 <= K) && (cols % 4 == 0) && ((reinterpret_cast<uintptr_t>(planes) & 31) == 0);
     const double* src = planes + (size_t)(x_ok ? x : 0) * cols + k0;
 #pragma unroll
     for (int l = 0; l < L; l++) {
       if (vec) {
-        const double2 v0 = *reinterpret_cast<const double2*>(src + l * plane);
-        const double2 v1 = *reinterpret_cast<const double2*>(src + l * plane + 2);
-        r[0][l] = v0.x, r[1][l] = v0.y, r[2][l] = v1.x, r[3][l] = v1.y;
+        ldg_256(src + l * plane, r[0][l], r[1][l], r[2][l], r[3][l]);
       } else {
 #pragma unroll
         for (int t = 0; t < 4; t++) r[t][l] = (x_ok && k0 + t < K) ? src[l * plane + t] : 0.0;
@@ -180,8 +189,7 @@ __global__ void __launch_bounds__(256) split_packed_kernel(int rows, int cols, i
     double d[4];
 #pragma unroll
     for (int t = 0; t < 4; t++) d[t] = extract_digit<L>(r[t], E, q);
-    *reinterpret_cast<double2*>(dst + q * q_stride) = make_double2(d[0], d[1]);
-    *reinterpret_cast<double2*>(dst + q * q_stride + 2) = make_double2(d[2], d[3]);
+    stg_256(dst + q * q_stride, d[0], d[1], d[2], d[3]);  // a fragment row; the warp writes 1 KB contiguous
   }
 }
 
