@@ -1,4 +1,4 @@
-"""Seeded synthetic inputs for the five BASELINE.json configs.
+"""Seeded synthetic inputs for the five BASELINE.json configs (plus two wider-format configs, CONFIGS[5:]).
 
 This module is shared by the CPU oracle's tests and by the CUDA path's tests / bench.  It holds
 NONE of the method's arithmetic (no splitting, no products, no renormalisation): only a stateless
@@ -66,6 +66,10 @@ CONFIGS = (
     Config(2, "dd_4096_normal", 4096, 4096, 4096, 2, 2, "normal"),
     Config(3, "dd_8192x8192x2048_wide30", 8192, 8192, 2048, 2, 3, "wide30", quarters=9),
     Config(4, "qd_2048", 2048, 2048, 2048, 4, 4, "uniform"),
+    # Beyond BASELINE.json: the two wider formats of the paper's Table 2 (PAPER.md:196-205,
+    # octo double = 8 limbs / 32 quarters, hexa double = 16 limbs / 64 quarters), same recipe as configs[4].
+    Config(5, "od_1024", 1024, 1024, 1024, 8, 5, "uniform"),
+    Config(6, "hd_512", 512, 512, 512, 16, 6, "uniform"),
 )
 
 
