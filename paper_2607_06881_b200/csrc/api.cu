@@ -28,6 +28,7 @@ Profile g_prof;
 std::atomic<uint64_t> g_launches{0};
 
 constexpr size_t ALIGN = 256;
+constexpr int MD_MAX_QUARTERS = 72;  // md_split accepts up to 4 * 16 + 8 quarters; md_renorm up to twice as many orders
 inline size_t round_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 inline int quarters_for(int limbs) { return g_state.opt_quarters ? g_state.opt_quarters : 4 * limbs; }
@@ -55,9 +56,9 @@ Carve carve(void* base, int m, int n, int k, int limbs, int quarters) {
   c.expB = reinterpret_cast<int32_t*>(p + off);
   off += round_up(sizeof(int32_t) * (size_t)n);
   c.Aq = reinterpret_cast<double*>(p + off);
-  off += round_up(sizeof(double) * md::packed_doubles(m, k, md::pack_bx(limbs, 0), quarters));
+  off += round_up(sizeof(double) * md::packed_doubles(m, k, md::pack_bx(limbs, 0), md::pack_bk(limbs), quarters));
   c.Bq = reinterpret_cast<double*>(p + off);
-  off += round_up(sizeof(double) * md::packed_doubles(n, k, md::pack_bx(limbs, 1), quarters));
+  off += round_up(sizeof(double) * md::packed_doubles(n, k, md::pack_bx(limbs, 1), md::pack_bk(limbs), quarters));
   c.sk = p + off;
   off += round_up(md::sk_workspace_bytes(limbs, quarters));
   c.total = off;
@@ -69,9 +70,9 @@ inline bool aligned8(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 7
 md_status check_gemm_args(int m, int n, int k, int limbs, const void* A, const void* B, const void* C) {
   if (m <= 0 || n <= 0 || k <= 0 || !A || !B || !C) return MD_ERR_BAD_ARG;
   if (!aligned8(A) || !aligned8(B) || !aligned8(C)) return MD_ERR_BAD_ARG;
-  if (limbs != 2 && limbs != 4) return MD_ERR_BAD_ARG;
+  if (limbs != 2 && limbs != 4 && limbs != 8 && limbs != 16) return MD_ERR_BAD_ARG;
   const int Q = quarters_for(limbs), S = orders_for(limbs);
-  if (S != Q || !md::qgemm_supported(limbs, Q)) return MD_ERR_UNSUPPORTED;
+  if (S != Q || !(md::qgemm_supported(limbs, Q) || md::qgemm_wide_supported(limbs, Q))) return MD_ERR_UNSUPPORTED;
   // exactness budget: every partial sum of an order is below k * S * 2^26 units, which must not exceed 2^53
   // (eq. 5 generalised to S products per k; R6)
   if ((long long)k * S > (1ll << 27)) return MD_ERR_K_TOO_LARGE;
@@ -88,13 +89,14 @@ md_status gemm_impl(int m, int n, int k, int limbs, const double* A, const doubl
   uint64_t launches = 0;
   cudaEvent_t* ev = (g_prof.count < g_prof.capacity) ? &g_prof.ev[3 * (size_t)g_prof.count] : nullptr;
   if (ev) cudaEventRecord(ev[0], stream);
-  cudaError_t err = md::launch_exponents(m, k, 0, A, c.expA, c.flags, stream, &launches);
-  if (err == cudaSuccess) err = md::launch_exponents(k, n, 1, B, c.expB, c.flags, stream, &launches);
+  cudaError_t err = md::launch_exponents(m, k, 0, Q, A, c.expA, c.flags, stream, &launches);
+  if (err == cudaSuccess) err = md::launch_exponents(k, n, 1, Q, B, c.expB, c.flags, stream, &launches);
   if (err == cudaSuccess) err = md::launch_split_packed(m, k, limbs, Q, 0, A, c.Aq, c.expA, c.flags, stream, &launches);
   if (err == cudaSuccess) err = md::launch_split_packed(k, n, limbs, Q, 1, B, c.Bq, c.expB, c.flags, stream, &launches);
   if (ev) cudaEventRecord(ev[1], stream);
   if (err == cudaSuccess)
-    err = md::launch_qgemm_packed(m, n, k, limbs, Q, c.Aq, c.Bq, order_planes, C_planes, c.sk, stream, &launches);
+    err = limbs <= 4 ? md::launch_qgemm_packed(m, n, k, limbs, Q, c.Aq, c.Bq, order_planes, C_planes, c.sk, stream, &launches)
+                     : md::launch_qgemm_wide(m, n, k, limbs, Q, c.Aq, c.Bq, order_planes, C_planes, c.sk, stream, &launches);
   if (ev) {
     cudaEventRecord(ev[2], stream);
     if (err == cudaSuccess) g_prof.count++;
@@ -108,7 +110,7 @@ md_status gemm_impl(int m, int n, int k, int limbs, const double* A, const doubl
 extern "C" {
 
 md_status md_set_option(int key, int value) {
-  if (value < 0 || value > 24) return MD_ERR_BAD_ARG;
+  if (value < 0 || value > MD_MAX_QUARTERS) return MD_ERR_BAD_ARG;
   switch (key) {
     case MD_OPT_QUARTERS: g_state.opt_quarters = value; return MD_OK;
     case MD_OPT_ORDERS: g_state.opt_orders = value; return MD_OK;
@@ -127,13 +129,13 @@ int md_get_option(int key) {
 md_status md_split(int rows, int cols, int limbs, int quarters, int axis, const double* planes, double* quarter_planes,
                    int32_t* exps, md_stream stream) {
   if (rows <= 0 || cols <= 0 || !planes || !quarter_planes || !exps) return MD_ERR_BAD_ARG;
-  if (limbs != 1 && limbs != 2 && limbs != 4) return MD_ERR_BAD_ARG;
-  if (quarters < 1 || quarters > 24 || (axis != 0 && axis != 1)) return MD_ERR_BAD_ARG;
+  if (limbs != 1 && limbs != 2 && limbs != 4 && limbs != 8 && limbs != 16) return MD_ERR_BAD_ARG;
+  if (quarters < 1 || quarters > MD_MAX_QUARTERS || (axis != 0 && axis != 1)) return MD_ERR_BAD_ARG;
   if (!aligned8(planes) || !aligned8(quarter_planes) || (reinterpret_cast<uintptr_t>(exps) & 3)) return MD_ERR_BAD_ARG;
   uint32_t* flags = g_state.ws ? static_cast<uint32_t*>(g_state.ws) : nullptr;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   uint64_t launches = 0;
-  cudaError_t err = md::launch_exponents(rows, cols, axis, planes, exps, flags, st, &launches);
+  cudaError_t err = md::launch_exponents(rows, cols, axis, quarters, planes, exps, flags, st, &launches);
   if (err == cudaSuccess)
     err = md::launch_split(rows, cols, limbs, quarters, axis, planes, quarter_planes, exps, flags, st, &launches);
   g_launches += launches;
@@ -144,7 +146,8 @@ md_status md_qgemm(int m, int n, int k, int limbs, int quarters, int orders, con
                    double* order_planes, double* C_planes, md_stream stream) {
   if (m <= 0 || n <= 0 || k <= 0 || !Aq || !Bq || (!order_planes && !C_planes)) return MD_ERR_BAD_ARG;
   if (!aligned8(Aq) || !aligned8(Bq) || !aligned8(order_planes) || !aligned8(C_planes)) return MD_ERR_BAD_ARG;
-  if (limbs != 2 && limbs != 4) return MD_ERR_BAD_ARG;
+  if (limbs != 2 && limbs != 4 && limbs != 8 && limbs != 16) return MD_ERR_BAD_ARG;
+  // plain-layout quarter planes: double / quad double only (octo / hexa double go through md_gemm's packed operands)
   if (orders != quarters || !md::qgemm_supported(limbs, quarters)) return MD_ERR_UNSUPPORTED;
   if ((long long)k * orders > (1ll << 27)) return MD_ERR_K_TOO_LARGE;
   uint64_t launches = 0;
@@ -157,8 +160,8 @@ md_status md_qgemm(int m, int n, int k, int limbs, int quarters, int orders, con
 md_status md_renorm(int m, int n, int limbs, int orders, const double* order_planes, double* C_planes,
                     md_stream stream) {
   if (m <= 0 || n <= 0 || !order_planes || !C_planes) return MD_ERR_BAD_ARG;
-  if (limbs != 1 && limbs != 2 && limbs != 4) return MD_ERR_BAD_ARG;
-  if (orders < 1 || orders > 24 || !aligned8(order_planes) || !aligned8(C_planes)) return MD_ERR_BAD_ARG;
+  if (limbs != 1 && limbs != 2 && limbs != 4 && limbs != 8 && limbs != 16) return MD_ERR_BAD_ARG;
+  if (orders < 1 || orders > 2 * MD_MAX_QUARTERS || !aligned8(order_planes) || !aligned8(C_planes)) return MD_ERR_BAD_ARG;
   uint64_t launches = 0;
   cudaError_t err = md::launch_renorm(m, n, limbs, orders, order_planes, C_planes, static_cast<cudaStream_t>(stream), &launches);
   g_launches += launches;
@@ -166,7 +169,7 @@ md_status md_renorm(int m, int n, int limbs, int orders, const double* order_pla
 }
 
 size_t md_workspace_bytes(int m, int n, int k, int limbs) {
-  if (m <= 0 || n <= 0 || k <= 0 || (limbs != 2 && limbs != 4)) return 0;
+  if (m <= 0 || n <= 0 || k <= 0 || (limbs != 2 && limbs != 4 && limbs != 8 && limbs != 16)) return 0;
   return carve(nullptr, m, n, k, limbs, quarters_for(limbs)).total;
 }
 

@@ -35,29 +35,38 @@ __device__ __forceinline__ double pow2(int e) { return __longlong_as_double((lon
 // kinds of error-free sweeps bring the accumulator to a non-overlapping expansion: limb_{l} = fl(limb_l + limb_{l+1}).
 // Error: <= 2^-(53L+40) * sum|c| from the guard term + what the dropped (L+1)-th term holds (< 2^-53L |sum|).
 // ----------------------------------------------------------------------------------------------------------------------
-template <int L, int S>
-__device__ __forceinline__ void renorm_orders(const double (&c)[S], double (&out)[L]) {
-  double r[L + 1];
+// The three pieces of renorm_orders, usable separately (the standalone kernel streams the orders from memory; the hexa
+// double GEMM hands the (L+1)-term accumulator from warp to warp, qgemm_wide.cu).  r has L+1 terms, starts at zero.
+template <int L>
+__device__ __forceinline__ void renorm_add(double (&r)[L + 1], double x) {
 #pragma unroll
-  for (int l = 0; l <= L; l++) r[l] = 0.0;
-#pragma unroll
-  for (int s = S - 1; s >= 0; s--) {
-    double x = c[s];
-#pragma unroll
-    for (int l = 0; l < L; l++) two_sum(r[l], x, r[l], x);
-    r[L] = __dadd_rn(r[L], x);
-  }
+  for (int l = 0; l < L; l++) two_sum(r[l], x, r[l], x);
+  r[L] = __dadd_rn(r[L], x);
+}
+template <int L>
+__device__ __forceinline__ void renorm_finish(double (&r)[L + 1], double (&out)[L]) {
   // bottom-up: r[0] becomes fl(total), the rest the successive rounding errors
 #pragma unroll
   for (int l = L; l >= 1; l--) two_sum(r[l - 1], r[l], r[l - 1], r[l]);
-  // top-down sweeps: each makes r[l] = fl(r[l] + r[l+1]) and pushes the error (and interior zeros) one place down
-#pragma unroll
+  // top-down sweeps: each makes r[l] = fl(r[l] + r[l+1]) and pushes the error (and interior zeros) one place down.
+  // Not unrolled for the wide formats (L*L TwoSums: 1536 instructions at L = 16); same operations either way.
+#pragma unroll(L <= 4 ? L : 1)
   for (int sweep = 0; sweep < L; sweep++) {
 #pragma unroll
     for (int l = 0; l < L; l++) two_sum(r[l], r[l + 1], r[l], r[l + 1]);
   }
 #pragma unroll
   for (int l = 0; l < L; l++) out[l] = r[l];
+}
+
+template <int L, int S>
+__device__ __forceinline__ void renorm_orders(const double (&c)[S], double (&out)[L]) {
+  double r[L + 1];
+#pragma unroll
+  for (int l = 0; l <= L; l++) r[l] = 0.0;
+#pragma unroll
+  for (int s = S - 1; s >= 0; s--) renorm_add<L>(r, c[s]);
+  renorm_finish<L>(r, out);
 }
 
 }  // namespace md

@@ -6,8 +6,10 @@
 
 namespace md {
 
-cudaError_t launch_exponents(int rows, int cols, int axis, const double* lead_plane, int32_t* exps, uint32_t* flags,
-                             cudaStream_t stream, uint64_t* launches);
+// `quarters` only sets the lower bound of the exponent range that is flagged (exponent_floor)
+cudaError_t launch_exponents(int rows, int cols, int axis, int quarters, const double* lead_plane, int32_t* exps,
+                             uint32_t* flags, cudaStream_t stream, uint64_t* launches);
+int exponent_floor(int quarters);
 cudaError_t launch_split(int rows, int cols, int limbs, int quarters, int axis, const double* planes,
                          double* quarter_planes, const int32_t* exps, uint32_t* flags, cudaStream_t stream,
                          uint64_t* launches);
@@ -31,6 +33,11 @@ int sk_grid();
 cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, const double* Ap, const double* Bp,
                                 double* order_planes, double* C_planes, void* sk_ws, cudaStream_t stream,
                                 uint64_t* launches);
+// octo / hexa double (qgemm_wide.cu): same packed operands (k-slab depth 4), same stream-K scratch convention
+bool qgemm_wide_supported(int limbs, int quarters);
+cudaError_t launch_qgemm_wide(int m, int n, int k, int limbs, int quarters, const double* Ap, const double* Bp,
+                              double* order_planes, double* C_planes, void* sk_ws, cudaStream_t stream,
+                              uint64_t* launches);
 // calibration (probe.cu): register-only DMMA loop; *flops receives the FP64 flops the launch issues
 cudaError_t launch_dmma_probe(int blocks, int warps_per_block, int iters, double* sink, cudaStream_t stream,
                               uint64_t* launches, uint64_t* flops);

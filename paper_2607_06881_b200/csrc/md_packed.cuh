@@ -3,7 +3,7 @@
 // public md_split / md_qgemm keep the plain [quarters][rows][cols] layout.
 //
 // An operand is seen as X groups (rows of A, axis 0 / columns of B, axis 1: the index that carries the exponent) by K
-// contraction indices.  X is cut into tiles of BX (the CTA tile: BM for A, BN for B), K into slabs of PACK_BK; both are
+// contraction indices.  X is cut into tiles of BX (the CTA tile: BM for A, BN for B), K into slabs of BK = pack_bk(limbs); both are
 // zero padded to whole tiles / slabs (zero quarters are harmless).  Memory order, slowest to fastest:
 //
 //     [x tile][k slab]  [quarter q][k4 = (k % BK) / 4][x8 = (x % BX) / 8]  [g = x % 8][t4 = k % 4]
@@ -17,24 +17,28 @@
 
 namespace md {
 
-constexpr int PACK_BK = 8;  // k-slab depth (two DMMA k-steps)
+// k-slab depth BK: two DMMA k-steps for double / quad double (qgemm_packed.cu), one for octo / hexa double
+// (qgemm_wide.cu: 32 / 64 quarters per element make a slab of 8 too large for a multi-stage ring in 227 KB).
+constexpr int PACK_BK = 8, PACK_BK_WIDE = 4;
+__host__ __device__ constexpr int pack_bk(int limbs) { return limbs <= 4 ? PACK_BK : PACK_BK_WIDE; }
 
-// CTA tile extent along the group index: BM (axis 0) or BN (axis 1) of the qgemm_packed_kernel configuration for `limbs`.
+// CTA tile extent along the group index: BM (axis 0) or BN (axis 1) of the fused GEMM configuration for `limbs`
+// (dd 64 x 32, qd 32 x 16: qgemm_packed.cu; od 32 x 16, hd 16 x 8: qgemm_wide.cu).
 __host__ __device__ constexpr int pack_bx(int limbs, int axis) {
-  return limbs == 2 ? (axis == 0 ? 64 : 32) : (axis == 0 ? 32 : 16);
+  return limbs == 2 ? (axis == 0 ? 64 : 32) : limbs == 16 ? (axis == 0 ? 16 : 8) : (axis == 0 ? 32 : 16);
 }
 
 // doubles in the packed image of an operand with X groups and K contraction indices
-__host__ __device__ inline size_t packed_doubles(int X, int K, int bx, int quarters) {
-  const size_t xt = ((size_t)X + bx - 1) / bx, ks = ((size_t)K + PACK_BK - 1) / PACK_BK;
-  return xt * ks * (size_t)quarters * PACK_BK * bx;
+__host__ __device__ inline size_t packed_doubles(int X, int K, int bx, int bk, int quarters) {
+  const size_t xt = ((size_t)X + bx - 1) / bx, ks = ((size_t)K + bk - 1) / bk;
+  return xt * ks * (size_t)quarters * bk * bx;
 }
 
 // offset (in doubles) of quarter q of element (x, k); KS = number of k slabs
-__host__ __device__ inline size_t packed_offset(int x, int k, int q, int bx, int quarters, int KS) {
-  const int xt = x / bx, xin = x % bx, ks = k / PACK_BK, kin = k % PACK_BK;
-  const size_t chunk = ((size_t)xt * KS + ks) * ((size_t)quarters * PACK_BK * bx);
-  return chunk + ((size_t)(q * (PACK_BK / 4) + kin / 4) * (bx / 8) + xin / 8) * 32 + (xin % 8) * 4 + (kin % 4);
+__host__ __device__ inline size_t packed_offset(int x, int k, int q, int bx, int bk, int quarters, int KS) {
+  const int xt = x / bx, xin = x % bx, ks = k / bk, kin = k % bk;
+  const size_t chunk = ((size_t)xt * KS + ks) * ((size_t)quarters * bk * bx);
+  return chunk + ((size_t)(q * (bk / 4) + kin / 4) * (bx / 8) + xin / 8) * 32 + (xin % 8) * 4 + (kin % 4);
 }
 
 }  // namespace md

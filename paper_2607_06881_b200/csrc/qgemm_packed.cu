@@ -24,41 +24,10 @@
 #include "md_kernels.h"
 #include "md_packed.cuh"
 #include "qgemm_common.cuh"
+#include "qgemm_pipeline.cuh"
 
 namespace md {
 namespace {
-
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-// mbarrier / bulk-copy wrappers; barriers and shared destinations are passed as 32-bit shared-window addresses that the
-// kernel computes once (a generic->shared conversion inside the k loop costs an S2R + LEA chain per slab).
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  asm volatile(
-      "{\n"
-      ".reg .pred P1;\n"
-      "LAB_WAIT:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
-      "@P1 bra DONE;\n"
-      "bra LAB_WAIT;\n"
-      "DONE:\n"
-      "}" ::"r"(bar), "r"(parity)
-      : "memory");
-}
-// global -> shared bulk copy (bytes % 16 == 0, both addresses 16-byte aligned); completion = complete_tx on `bar`.
-__device__ __forceinline__ void bulk_g2s(uint32_t smem_dst, const void* gmem_src, uint32_t bytes, uint32_t bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_dst),
-               "l"(gmem_src), "r"(bytes), "r"(bar)
-               : "memory");
-}
 
 // A warp owns an (8*MT) x (8*NT) block of C and Q (= S) accumulator sets for it; WM x WN warps tile the CTA block.
 template <int Q_, int L_, int WM_, int WN_, int MT_, int NT_>
@@ -78,25 +47,6 @@ struct PCfg {
   static_assert(STAGES >= 3, "the non-blocking refill needs at least 3 stages");
   static_assert(2 * STAGES * 8 <= BAR_BYTES - 8, "barrier area (its last 8 bytes hold the stream-K flag)");
   static_assert(STAGE_BYTES % 128 == 0, "stage alignment");
-};
-
-// Persistent kernel: gridDim.x = G CTAs (one per SM), each walks a private list of SEGMENTS = (tile, slab range):
-//   * stream-K part first: the sk_tiles tiles that do not fill a whole wave of G CTAs are cut along k into G nearly equal
-//     runs of slabs (CTA b owns global slab iterations [b*ipc, (b+1)*ipc) of the sk_tiles * KS), so that the last wave costs
-//     sk_tiles*KS/G slab-times instead of KS.  A CTA adds its partial order sums into the tile's scratch with fp64
-//     red.global.add -- EXACT here, every partial sum being an integer below 2^53 units (R6), hence the result is
-//     bit-identical whatever the arrival order -- then bumps the tile's slab counter; whoever completes the count re-reads
-//     the scratch and runs the epilogue.  Nobody ever waits for another CTA.
-//   * then dp_waves whole tiles, ids b, b + G, b + 2G, ... (tile ids are rasterised, so at any time the G CTAs cover a
-//     compact patch of C), accumulated and renormalised entirely in registers.
-// The stage ring runs straight through segment boundaries: the refill thread is AHEAD slabs ahead, possibly already in the
-// next tile, so the pipeline never drains between tiles.
-struct SkPlan {
-  int KS;                // k slabs per tile
-  int tiles_m, tiles_n;
-  int dp_waves;          // whole tiles per CTA
-  int sk_tiles;          // tiles dp_waves*G .. dp_waves*G + sk_tiles - 1 are processed stream-K
-  int sk_iters_per_cta;  // ipc
 };
 
 template <class C>

@@ -1,0 +1,386 @@
+// qgemm_wide.cu -- steps a3 + a4 for the two wider formats of the paper's Table 2: octo double
+// (8 limbs, Q = S = 32 quarters / orders, T = 528 quarter products) and hexa double (16 limbs, Q = S = 64, T = 2080).
+//
+//   For s = 0..S-1:  C^(s) = sum_{p+q=s} A_p * B_q      (PAPER.md:66-71 eq. 3; :75-78 eq. 4: the paper's C_{s+1})
+//   C = sum_s C^(s), summed error free into L limbs     (PAPER.md:88-91 steps 4-5)
+//
+// Same method, same packed operand layout (md_packed.cuh, k-slab depth 4), same persistent stream-K bulk-copy / mbarrier
+// pipeline as qgemm_packed.cu.  What changes is where the S accumulator sets live: an 8x8 DMMA tile needs 2 doubles per
+// order per thread, so 32 orders fill 128 registers and 64 orders do not fit a thread at all.  Hence
+//   * a warp owns ONE 8x8 tile of C and a contiguous ORDER RANGE [S0, S1) of at most 32 orders;
+//   * octo double: one range [0, 32) per tile, 8 tiles (32 x 16) per CTA;
+//   * hexa double: four ranges [0,32) [32,45) [45,55) [55,64) -- 528 / 507 / 505 / 540 products, balanced -- so the 8 warps
+//     of a CTA are 2 tiles (16 x 8) x 4 ranges, all fed from the same staged quarter tiles, and ranges are paired on the
+//     SM sub-partitions so that each issues 1035 or 1045 DMMAs per k-step (ideal 1040);
+//   * inside a k-step a range walks q = 0, 1, ... and needs the A fragments p in [S0-q, S1-1-q]: a window of S1-S0 quarters
+//     that slides down by one per q, kept in a register ring (one new LDS per q, issued one step ahead);
+//   * the recombination of a hexa double element is a chain over its four warps: the (L+1)-term accumulator of
+//     renorm_add (md_common.cuh) goes from the warp with the smallest orders to the warp with the largest through a
+//     lane-private slot of shared memory, which performs exactly the operation sequence of the standalone md_renorm.
+//
+// Exactness as in qgemm_packed.cu: k * S <= 2^27 keeps every partial sum an integer below 2^53 units (PAPER.md:95-99
+// eq. 5; R6), so the result does not depend on the order in which warps, slabs or the hardware add things.
+#include "md_kernels.h"
+#include "md_packed.cuh"
+#include "qgemm_common.cuh"
+#include "qgemm_pipeline.cuh"
+
+namespace md {
+namespace {
+
+// TM x TN 8x8 tiles per CTA, R order ranges per tile: TM * TN * R = 8 warps.
+template <int Q_, int L_, int TM_, int TN_, int R_>
+struct WCfg {
+  static constexpr int Q = Q_, S = Q_, L = L_, TM = TM_, TN = TN_, R = R_;
+  static constexpr int BM = TM * 8, BN = TN * 8, BK = PACK_BK_WIDE;
+  static constexpr int TILES = TM * TN, WARPS = TILES * R, THREADS = WARPS * 32;
+  static constexpr int A_CHUNK = Q * BK * BM, B_CHUNK = Q * BK * BN;  // doubles per k-slab
+  static constexpr int STAGE_BYTES = (A_CHUNK + B_CHUNK) * 8;
+  static constexpr int BAR_BYTES = 128;
+  // hand-over slots of the recombination chain: per tile, per lane, two elements of L+1 terms
+  static constexpr int XCHG_BYTES = R > 1 ? TILES * 2 * (L + 1) * 32 * 8 : 0;
+  static constexpr int STAGES =
+      ((SMEM_LIMIT - BAR_BYTES - XCHG_BYTES) / STAGE_BYTES) < 6 ? ((SMEM_LIMIT - BAR_BYTES - XCHG_BYTES) / STAGE_BYTES) : 6;
+  static constexpr int AHEAD = STAGES - 2;
+  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + XCHG_BYTES;
+  static_assert(WARPS == 8, "8 warps per CTA (2 per SM sub-partition)");
+  static_assert(R == 1 || R == 4, "order ranges: 1 (octo double) or 4 (hexa double)");
+  static_assert(STAGES >= 3, "the non-blocking refill needs at least 3 stages");
+  static_assert(2 * STAGES * 8 <= BAR_BYTES - 8, "barrier area (its last 8 bytes hold the stream-K flag)");
+  static_assert(STAGE_BYTES % 128 == 0 && XCHG_BYTES % 128 == 0, "alignment");
+  // order range r = [lo(r), hi(r))
+  __host__ __device__ static constexpr int lo(int r) { return R == 1 ? 0 : (r == 0 ? 0 : r == 1 ? 32 : r == 2 ? 45 : 55); }
+  __host__ __device__ static constexpr int hi(int r) { return R == 1 ? S : (r == 0 ? 32 : r == 1 ? 45 : r == 2 ? 55 : 64); }
+  // warp -> (tile, range).  Warps w and w + 4 share an SM sub-partition: pair ranges (0,1) and (2,3) there.
+  __host__ __device__ static constexpr int tile_of(int w) { return R == 1 ? w : w / 4; }
+  __host__ __device__ static constexpr int range_of(int w) {
+    return R == 1 ? 0 : (w < 4 ? (w == 0 ? 0 : w == 1 ? 2 : w == 2 ? 1 : 3) : (w == 4 ? 1 : w == 5 ? 3 : w == 6 ? 0 : 2));
+  }
+};
+
+// What a warp needs to know about the CTA's pipeline and work list (built once in the kernel).
+struct WideCtx {
+  int m, n, G, cta, KS;
+  SkPlan plan;
+  int g0, g1, n_sk, n_seg, total_slabs;  // this CTA's segment list (see qgemm_pipeline.cuh)
+  const double *Ap, *Bp;
+  double *order_planes, *C_planes, *sk_scratch;
+  unsigned int* sk_counters;
+  double* stages;
+  uint32_t stages_u32, full_u32, empty_u32;
+  volatile int* last_flag;
+  double* xchg;
+  __device__ __forceinline__ void segment(int i, int& tile, int& s0, int& s1) const {
+    if (i < n_sk) {
+      const int r = g0 / KS + i;
+      tile = plan.dp_waves * G + r;
+      s0 = i == 0 ? g0 - r * KS : 0;
+      s1 = min(KS, g1 - r * KS);
+    } else {
+      tile = (i - n_sk) * G + cta;
+      s0 = 0;
+      s1 = KS;
+    }
+  }
+};
+
+// One DMMA k-step (4 contraction indices) of order range [S0, S1) on the warp's 8x8 tile: every product (p, q) with
+// S0 <= p + q < S1 goes to accumulator p + q - S0.  As / Bs point at the lane's element of the quarter-0 fragment of the
+// warp's row block / column block in the staged slab; quarter p of A is p * AQ doubles further, quarter q of B q * BQ.
+// Fully unrolled: every register index below is a compile-time constant.
+template <int Q, int S0, int S1, int AQ, int BQ>
+__device__ __forceinline__ void k_step_range(double (&acc)[S1 - S0][2], const double* __restrict__ As,
+                                             const double* __restrict__ Bs) {
+  constexpr int W = S1 - S0;
+  constexpr int RW = S0 == 0 ? W : W + 1;                   // ring slots (one spare for the fragment fetched ahead)
+  constexpr int QMAX = S1 - 1 < Q - 1 ? S1 - 1 : Q - 1;     // last q with a product in the range
+  double a[RW];
+#pragma unroll
+  for (int p = S0; p <= (S1 - 1 < Q - 1 ? S1 - 1 : Q - 1); p++) a[p % RW] = As[p * AQ];  // window of q = 0
+  double b = Bs[0];
+#pragma unroll
+  for (int q = 0; q <= QMAX; q++) {
+    double b_next = 0.0;
+    if (q + 1 <= QMAX) {                                     // operands of step q + 1, issued before step q's DMMAs
+      b_next = Bs[(q + 1) * BQ];
+      if (S0 - (q + 1) >= 0) a[(S0 - (q + 1)) % RW] = As[(S0 - (q + 1)) * AQ];
+    }
+    const int lo = S0 - q > 0 ? S0 - q : 0;
+    const int hi = S1 - 1 - q < Q - 1 ? S1 - 1 - q : Q - 1;
+#pragma unroll
+    for (int p = lo; p <= hi; p++) dmma_8x8x4(acc[p + q - S0], a[p % RW], b);
+    b = b_next;
+  }
+}
+
+// Producer cursor (thread 0 only): walks the CTA's flat slab sequence AHEAD slabs in front of the consumers.
+template <class C>
+struct WideProducer {
+  int p_seg = -1, p_left = 0, p_flat = 0, pst = 0;
+  const double *p_A = nullptr, *p_B = nullptr;
+  __device__ __forceinline__ void produce_one(const WideCtx& x) {
+    if (p_left == 0) {
+      int tile, s0, s1, tm, tn;
+      x.segment(++p_seg, tile, s0, s1);
+      raster_tile(tile, x.plan.tiles_m, x.plan.tiles_n, tm, tn);
+      p_A = x.Ap + ((size_t)tm * x.KS + s0) * C::A_CHUNK;
+      p_B = x.Bp + ((size_t)tn * x.KS + s0) * C::B_CHUNK;
+      p_left = s1 - s0;
+    }
+    const uint32_t dst = x.stages_u32 + pst * C::STAGE_BYTES, bar = x.full_u32 + 8 * pst;
+    mbar_expect_tx(bar, C::STAGE_BYTES);
+    bulk_g2s(dst, p_A, C::A_CHUNK * 8, bar);
+    bulk_g2s(dst + C::A_CHUNK * 8, p_B, C::B_CHUNK * 8, bar);
+    p_A += C::A_CHUNK;
+    p_B += C::B_CHUNK;
+    p_left--;
+    p_flat++;
+    pst = (pst + 1 == C::STAGES) ? 0 : pst + 1;
+  }
+  __device__ __forceinline__ void prologue(const WideCtx& x) {
+#pragma unroll
+    for (int j = 0; j < C::AHEAD; j++)
+      if (p_flat < x.total_slabs) produce_one(x);
+  }
+  __device__ __forceinline__ void produce(const WideCtx& x) {  // top of a consumer iteration
+    if (p_flat < x.total_slabs) {
+      // the stage was last read two iterations ago: wait for its release (completed long ago)
+      if (p_flat >= C::STAGES) mbar_wait(x.empty_u32 + 8 * pst, ((p_flat / C::STAGES) + 1) & 1);
+      produce_one(x);
+    }
+  }
+};
+
+// End of a tile for the warp that owns orders [lo(RANGE), hi(RANGE)) of tile `t` of the CTA: acc[s - S0][e] is C^(s) of
+// element (row, col + e), row = row_base + lane / 4, col = col_base + 2 * (lane % 4).  Writes the order planes (debug /
+// parity) and / or the renormalised limb planes.  EVERY thread of the CTA must call it (block-wide barriers when R > 1).
+template <class C, int RANGE>
+__device__ __forceinline__ void wide_epilogue(const WideCtx& x, const double (&acc)[C::hi(RANGE) - C::lo(RANGE)][2], int t,
+                                              int row_base, int col_base, int lane) {
+  constexpr int S0 = C::lo(RANGE), S1 = C::hi(RANGE), L = C::L, R = C::R;
+  const int row = row_base + (lane >> 2), col = col_base + 2 * (lane & 3);
+  const bool inside = row < x.m && col < x.n, two = col + 1 < x.n;
+  const size_t planeC = (size_t)x.m * x.n, at = (size_t)row * x.n + col;
+  const bool vec_ok = (x.n % 2 == 0) && (((uintptr_t)x.C_planes | (uintptr_t)x.order_planes) % 16 == 0);
+  if (x.order_planes && inside) {
+#pragma unroll
+    for (int s = S0; s < S1; s++) {
+      if (vec_ok) {
+        *reinterpret_cast<double2*>(x.order_planes + s * planeC + at) = make_double2(acc[s - S0][0], acc[s - S0][1]);
+      } else {
+        x.order_planes[s * planeC + at] = acc[s - S0][0];
+        if (two) x.order_planes[s * planeC + at + 1] = acc[s - S0][1];
+      }
+    }
+  }
+  if (!x.C_planes) return;  // uniform over the CTA
+  double out[2][L];
+  // Recombination (R9): orders are added from the smallest (s = S-1) to the largest (s = 0)
+  // into an (L+1)-term accumulator; with R ranges the accumulator travels range R-1 -> ... -> range 0.
+#pragma unroll
+  for (int rr = R - 1; rr >= 0; rr--) {
+    if (rr == RANGE) {
+#pragma unroll
+      for (int e = 0; e < 2; e++) {
+        double r[L + 1];
+        double* slot = x.xchg + (size_t)((t * 2 + e) * (L + 1)) * 32 + lane;
+#pragma unroll
+        for (int l = 0; l <= L; l++) r[l] = (RANGE == R - 1) ? 0.0 : slot[l * 32];
+#pragma unroll
+        for (int s = S1 - 1; s >= S0; s--) renorm_add<L>(r, acc[s - S0][e]);
+        if (RANGE > 0) {
+#pragma unroll
+          for (int l = 0; l <= L; l++) slot[l * 32] = r[l];
+        } else {
+          renorm_finish<L>(r, out[e]);
+        }
+      }
+    }
+    if (R > 1) __syncthreads();  // hand-over to the next range; the last one keeps the next tile's writers behind the readers
+  }
+  if (RANGE == 0 && inside) {
+#pragma unroll
+    for (int l = 0; l < L; l++) {
+      if (vec_ok) {
+        *reinterpret_cast<double2*>(x.C_planes + l * planeC + at) = make_double2(out[0][l], out[1][l]);
+      } else {
+        x.C_planes[l * planeC + at] = out[0][l];
+        if (two) x.C_planes[l * planeC + at + 1] = out[1][l];
+      }
+    }
+  }
+}
+
+// The whole life of one warp: consume the CTA's slab sequence for its (tile, order range), with thread 0 also running
+// the producer cursor.  Segment ends: a whole tile goes straight to the epilogue; a stream-K part adds its partial
+// order sums into the tile's scratch with fp64 red.add (exact, see the header) and the CTA that completes the slab
+// count finishes the tile.
+template <class C, int RANGE>
+__device__ __forceinline__ void wide_consume(const WideCtx& x, int t, int lane, int tid) {
+  constexpr int S0 = C::lo(RANGE), S1 = C::hi(RANGE), W = S1 - S0, STAGES = C::STAGES;
+  constexpr int STAGE_DOUBLES = C::A_CHUNK + C::B_CHUNK;
+  const int ti = t / C::TN, tj = t % C::TN;
+  const int a_off = ti * 32 + lane, b_off = C::A_CHUNK + tj * 32 + lane;
+
+  WideProducer<C> prod;
+  if (tid == 0) prod.prologue(x);
+
+  double acc[W][2];
+#pragma unroll
+  for (int s = 0; s < W; s++) acc[s][0] = acc[s][1] = 0.0;
+
+  int c_seg = 0, c_tile, c_s0, c_s1;
+  x.segment(0, c_tile, c_s0, c_s1);
+  int c_left = c_s1 - c_s0;
+  int st = 0;
+  uint32_t phase = 0;
+  for (int it = 0; it < x.total_slabs; it++) {
+    if (tid == 0) prod.produce(x);
+    mbar_wait(x.full_u32 + 8 * st, phase);
+    const double* stage = x.stages + (size_t)st * STAGE_DOUBLES;
+    k_step_range<C::Q, S0, S1, C::TM * 32, C::TN * 32>(acc, stage + a_off, stage + b_off);
+    __syncwarp();
+    if (lane == 0) mbar_arrive(x.empty_u32 + 8 * st);  // this warp is done reading the stage
+    if (++st == STAGES) {
+      st = 0;
+      phase ^= 1;
+    }
+    if (--c_left == 0) {
+      int tm, tn;
+      raster_tile(c_tile, x.plan.tiles_m, x.plan.tiles_n, tm, tn);
+      const int row_base = tm * C::BM + ti * 8, col_base = tn * C::BN + tj * 8;
+      if (c_s1 - c_s0 == x.KS) {  // whole tile in registers
+        wide_epilogue<C, RANGE>(x, acc, t, row_base, col_base, lane);
+      } else {                    // partial sums of a stream-K tile
+        const int r = c_tile - x.plan.dp_waves * x.G;
+        double* sc = x.sk_scratch + (size_t)r * (C::S * C::BM * C::BN) + (size_t)t * 64 + lane * 2;
+#pragma unroll
+        for (int s = S0; s < S1; s++) {
+          atomicAdd(sc + (size_t)s * (C::TILES * 64), acc[s - S0][0]);
+          atomicAdd(sc + (size_t)s * (C::TILES * 64) + 1, acc[s - S0][1]);
+        }
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) {
+          const unsigned int mine = (unsigned int)(c_s1 - c_s0);
+          *x.last_flag = (atomicAdd(&x.sk_counters[r], mine) + mine == (unsigned int)x.KS);
+        }
+        __syncthreads();
+        if (*x.last_flag) {  // every slab of the tile has been added: read the totals back and finish the tile
+          __threadfence();
+#pragma unroll
+          for (int s = S0; s < S1; s++) {
+            const double2 v = __ldcg(reinterpret_cast<const double2*>(sc + (size_t)s * (C::TILES * 64)));
+            acc[s - S0][0] = v.x;
+            acc[s - S0][1] = v.y;
+          }
+          wide_epilogue<C, RANGE>(x, acc, t, row_base, col_base, lane);
+        }
+      }
+#pragma unroll
+      for (int s = 0; s < W; s++) acc[s][0] = acc[s][1] = 0.0;
+      if (++c_seg < x.n_seg) {
+        x.segment(c_seg, c_tile, c_s0, c_s1);
+        c_left = c_s1 - c_s0;
+      }
+    }
+  }
+}
+
+template <class C>
+__global__ void __launch_bounds__(C::THREADS, 1)
+qgemm_wide_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, const double* __restrict__ Bp,
+                  double* __restrict__ order_planes, double* __restrict__ C_planes, double* __restrict__ sk_scratch,
+                  unsigned int* __restrict__ sk_counters) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  constexpr int STAGES = C::STAGES;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+
+  WideCtx x;
+  x.m = m, x.n = n, x.G = gridDim.x, x.cta = blockIdx.x, x.KS = plan.KS, x.plan = plan;
+  x.Ap = Ap, x.Bp = Bp, x.order_planes = order_planes, x.C_planes = C_planes;
+  x.sk_scratch = sk_scratch, x.sk_counters = sk_counters;
+  x.stages = reinterpret_cast<double*>(smem_raw);
+  uint64_t* const full = reinterpret_cast<uint64_t*>(smem_raw + STAGES * C::STAGE_BYTES);
+  x.stages_u32 = smem_u32(x.stages);
+  x.full_u32 = smem_u32(full);
+  x.empty_u32 = x.full_u32 + 8 * STAGES;
+  x.last_flag = reinterpret_cast<volatile int*>(smem_raw + STAGES * C::STAGE_BYTES + C::BAR_BYTES - 8);
+  x.xchg = reinterpret_cast<double*>(smem_raw + STAGES * C::STAGE_BYTES + C::BAR_BYTES);
+
+  // this CTA's segment list: its share of the stream-K slabs first, then whole tiles cta, cta + G, ...
+  const int sk_total = plan.sk_tiles * plan.KS;
+  x.g0 = min(x.cta * plan.sk_iters_per_cta, sk_total);
+  x.g1 = min(x.g0 + plan.sk_iters_per_cta, sk_total);
+  x.n_sk = x.g1 > x.g0 ? (x.g1 - 1) / plan.KS - x.g0 / plan.KS + 1 : 0;
+  x.n_seg = x.n_sk + plan.dp_waves;
+  x.total_slabs = (x.g1 - x.g0) + plan.dp_waves * plan.KS;
+
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < STAGES; s++) {
+      mbar_init(x.full_u32 + 8 * s, 1);
+      mbar_init(x.empty_u32 + 8 * s, C::WARPS);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (x.total_slabs == 0) return;
+
+  const int t = C::tile_of(warp);
+  if constexpr (C::R == 1) {
+    wide_consume<C, 0>(x, t, lane, tid);
+  } else {
+    switch (C::range_of(warp)) {  // warp-uniform
+      case 0: wide_consume<C, 0>(x, t, lane, tid); break;
+      case 1: wide_consume<C, 1>(x, t, lane, tid); break;
+      case 2: wide_consume<C, 2>(x, t, lane, tid); break;
+      default: wide_consume<C, 3>(x, t, lane, tid); break;
+    }
+  }
+}
+
+template <class C>
+cudaError_t launch_wide_cfg(int m, int n, int k, const double* Ap, const double* Bp, double* order_planes,
+                            double* C_planes, void* sk_ws, cudaStream_t stream) {
+  static_assert(C::BM == pack_bx(C::L, 0) && C::BN == pack_bx(C::L, 1) && C::BK == pack_bk(C::L),
+                "tile shape must match the packed layout");
+  const int tiles_m = (m + C::BM - 1) / C::BM, tiles_n = (n + C::BN - 1) / C::BN;
+  if ((long long)tiles_m * tiles_n > 0x7fffffffLL) return cudaErrorInvalidValue;
+  const int G = sk_grid();
+  if (G <= 0) return cudaErrorInvalidDevice;
+  const SkPlan plan = make_sk_plan(tiles_m, tiles_n, (k + C::BK - 1) / C::BK, G);
+  unsigned int* counters = static_cast<unsigned int*>(sk_ws);
+  double* scratch = reinterpret_cast<double*>(static_cast<char*>(sk_ws) + SK_COUNTER_BYTES);
+  cudaError_t err;
+  if (plan.sk_tiles > 0) {  // counters and the scratch tiles in use start at zero (one contiguous region)
+    err = cudaMemsetAsync(sk_ws, 0, SK_COUNTER_BYTES + sizeof(double) * (size_t)plan.sk_tiles * C::S * C::BM * C::BN, stream);
+    if (err != cudaSuccess) return err;
+  }
+  auto kern = qgemm_wide_kernel<C>;
+  err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+  if (err != cudaSuccess) return err;
+  kern<<<G, C::THREADS, C::SMEM_BYTES, stream>>>(m, n, plan, Ap, Bp, order_planes, C_planes, scratch, counters);
+  return cudaGetLastError();
+}
+
+using WCfgOD = WCfg<32, 8, 4, 2, 1>;   // octo double: 32 x 16 CTA tile, 8 tiles x 1 range
+using WCfgHD = WCfg<64, 16, 2, 1, 4>;  // hexa double: 16 x 8 CTA tile, 2 tiles x 4 ranges
+
+}  // namespace
+
+bool qgemm_wide_supported(int limbs, int quarters) {
+  return (limbs == 8 && quarters == 32) || (limbs == 16 && quarters == 64);
+}
+
+cudaError_t launch_qgemm_wide(int m, int n, int k, int limbs, int quarters, const double* Ap, const double* Bp,
+                              double* order_planes, double* C_planes, void* sk_ws, cudaStream_t stream,
+                              uint64_t* launches) {
+  cudaError_t err = cudaErrorInvalidValue;
+  if (limbs == 8 && quarters == 32) err = launch_wide_cfg<WCfgOD>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
+  if (limbs == 16 && quarters == 64) err = launch_wide_cfg<WCfgHD>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
+  if (err == cudaSuccess) *launches += 1;
+  return err;
+}
+
+}  // namespace md

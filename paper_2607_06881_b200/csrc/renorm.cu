@@ -7,15 +7,25 @@
 namespace md {
 namespace {
 
-template <int L, int S>
-__global__ void __launch_bounds__(256) renorm_kernel(size_t total, const double* __restrict__ order_planes,
+template <int L>
+__global__ void __launch_bounds__(256) renorm_kernel(size_t total, int S, const double* __restrict__ order_planes,
                                                      double* __restrict__ C_planes) {
   const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= total) return;
-  double c[S], out[L];
+  double r[L + 1], out[L];
 #pragma unroll
-  for (int s = 0; s < S; s++) c[s] = order_planes[(size_t)s * total + idx];
-  renorm_orders<L, S>(c, out);
+  for (int l = 0; l <= L; l++) r[l] = 0.0;
+  // smallest order first (R9); 4 loads in flight per thread
+  int s = S - 1;
+  for (; s >= 3; s -= 4) {
+    double x[4];
+#pragma unroll
+    for (int u = 0; u < 4; u++) x[u] = order_planes[(size_t)(s - u) * total + idx];
+#pragma unroll
+    for (int u = 0; u < 4; u++) renorm_add<L>(r, x[u]);
+  }
+  for (; s >= 0; s--) renorm_add<L>(r, order_planes[(size_t)s * total + idx]);
+  renorm_finish<L>(r, out);
 #pragma unroll
   for (int l = 0; l < L; l++) C_planes[(size_t)l * total + idx] = out[l];
 }
@@ -23,14 +33,7 @@ __global__ void __launch_bounds__(256) renorm_kernel(size_t total, const double*
 template <int L>
 cudaError_t dispatch_orders(int S, size_t total, const double* in, double* out, cudaStream_t stream) {
   const unsigned blocks = (unsigned)((total + 255) / 256);
-  switch (S) {
-#define MD_CASE(S_) case S_: renorm_kernel<L, S_><<<blocks, 256, 0, stream>>>(total, in, out); break;
-    MD_CASE(1) MD_CASE(2) MD_CASE(3) MD_CASE(4) MD_CASE(5) MD_CASE(6) MD_CASE(7) MD_CASE(8) MD_CASE(9) MD_CASE(10)
-    MD_CASE(11) MD_CASE(12) MD_CASE(13) MD_CASE(14) MD_CASE(15) MD_CASE(16) MD_CASE(17) MD_CASE(18) MD_CASE(19)
-    MD_CASE(20) MD_CASE(21) MD_CASE(22) MD_CASE(23) MD_CASE(24)
-#undef MD_CASE
-    default: return cudaErrorInvalidValue;
-  }
+  renorm_kernel<L><<<blocks, 256, 0, stream>>>(total, S, in, out);
   return cudaGetLastError();
 }
 
@@ -44,6 +47,8 @@ cudaError_t launch_renorm(int m, int n, int limbs, int orders, const double* ord
     case 1: err = dispatch_orders<1>(orders, total, order_planes, C_planes, stream); break;
     case 2: err = dispatch_orders<2>(orders, total, order_planes, C_planes, stream); break;
     case 4: err = dispatch_orders<4>(orders, total, order_planes, C_planes, stream); break;
+    case 8: err = dispatch_orders<8>(orders, total, order_planes, C_planes, stream); break;
+    case 16: err = dispatch_orders<16>(orders, total, order_planes, C_planes, stream); break;
     default: return cudaErrorInvalidValue;
   }
   if (err == cudaSuccess) *launches += 1;

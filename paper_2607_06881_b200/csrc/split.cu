@@ -12,20 +12,20 @@ namespace {
 __device__ __forceinline__ uint32_t abs_hi32(double x) { return (uint32_t)(__double_as_longlong(x) >> 32) & 0x7fffffffu; }
 
 // hi32 of the group maximum -> E = ilogb(max)+1 (0 for a zero group); flags out-of-range / non-finite maxima.
-__device__ __forceinline__ int exponent_from_hi32(uint32_t hi, uint32_t* flags) {
+__device__ __forceinline__ int exponent_from_hi32(uint32_t hi, uint32_t* flags, int exp_lo) {
   const int biased = (int)(hi >> 20);
   if (biased == 0) return 0;  // zero group (subnormal maxima are outside the documented range and count as zero)
   const int E = biased - 1022;
   if (flags) {
     if (biased == 0x7ff) atomicOr(flags, FLAG_NONFINITE);
-    else if (E < -EXP_LIMIT || E > EXP_LIMIT) atomicOr(flags, FLAG_EXP_RANGE);
+    else if (E < exp_lo || E > EXP_LIMIT) atomicOr(flags, FLAG_EXP_RANGE);
   }
   return E;
 }
 
 // axis 0: one block per row of the leading limb plane.
 __global__ void __launch_bounds__(256) row_exponent_kernel(int rows, int cols, const double* __restrict__ lead,
-                                                           int32_t* __restrict__ exps, uint32_t* flags) {
+                                                           int32_t* __restrict__ exps, uint32_t* flags, int exp_lo) {
   __shared__ uint32_t warp_max[8];
   for (int row = blockIdx.x; row < rows; row += gridDim.x) {
     const double* p = lead + (size_t)row * cols;
@@ -38,7 +38,7 @@ __global__ void __launch_bounds__(256) row_exponent_kernel(int rows, int cols, c
       uint32_t v = warp_max[0];
 #pragma unroll
       for (int w = 1; w < 8; w++) v = max(v, warp_max[w]);
-      exps[row] = exponent_from_hi32(v, flags);
+      exps[row] = exponent_from_hi32(v, flags, exp_lo);
     }
     __syncthreads();
   }
@@ -56,9 +56,9 @@ __global__ void __launch_bounds__(256) col_max_kernel(int rows, int cols, int ro
   for (int r = r0; r < r1; r++) mx = max(mx, abs_hi32(lead[(size_t)r * cols + col]));
   if (mx) atomicMax(reinterpret_cast<unsigned int*>(exps) + col, mx);
 }
-__global__ void col_exponent_finalize_kernel(int cols, int32_t* exps, uint32_t* flags) {
+__global__ void col_exponent_finalize_kernel(int cols, int32_t* exps, uint32_t* flags, int exp_lo) {
   const int col = blockIdx.x * blockDim.x + threadIdx.x;
-  if (col < cols) exps[col] = exponent_from_hi32((uint32_t)exps[col], flags);
+  if (col < cols) exps[col] = exponent_from_hi32((uint32_t)exps[col], flags, exp_lo);
 }
 
 // Algorithm S, step S1 (DESIGN.md section 3 R4): digit q of the element whose remainder limbs are r[0..L-1], group exponent E:
@@ -142,7 +142,7 @@ __device__ __forceinline__ void stg_256(double* p, double a, double b, double c,
 // contraction indices k = 4*k4g .. 4*k4g+3, i.e. 32 contiguous output bytes per quarter; the 32 lanes of a warp take 32
 // consecutive x, so a warp writes 1 KB contiguous per quarter (and, for B, reads 256 contiguous bytes per row).
 template <int L, int AXIS>
-__global__ void __launch_bounds__(256) split_packed_kernel(int rows, int cols, int Q, int bx, int x_blocks, int KS,
+__global__ void __launch_bounds__(256) split_packed_kernel(int rows, int cols, int Q, int bx, int bk, int x_blocks, int KS,
                                                            const double* __restrict__ planes,
                                                            double* __restrict__ packed,
                                                            const int32_t* __restrict__ exps, uint32_t* flags) {
@@ -150,7 +150,7 @@ __global__ void __launch_bounds__(256) split_packed_kernel(int rows, int cols, i
   const int x = (blockIdx.x % x_blocks) * 32 + (threadIdx.x & 31);
   const int k4g = (blockIdx.x / x_blocks) * 8 + (threadIdx.x >> 5);  // group of four k
   const int XP = (X + bx - 1) / bx * bx;                             // padded to whole tiles
-  if (k4g >= KS * (PACK_BK / 4) || x >= XP) return;
+  if (k4g >= KS * (bk / 4) || x >= XP) return;
   const int k0 = k4g * 4;
   const size_t plane = (size_t)rows * cols;
 
@@ -183,8 +183,8 @@ __global__ void __launch_bounds__(256) split_packed_kernel(int rows, int cols, i
   if (bad && flags) atomicOr(flags, FLAG_NONFINITE);
 
   // element (x, k0) of quarter 0; quarter q is q * (BK/4) * (bx/8) fragments further
-  double* dst = packed + packed_offset(x, k0, 0, bx, Q, KS);
-  const size_t q_stride = (size_t)(PACK_BK / 4) * (bx / 8) * 32;
+  double* dst = packed + packed_offset(x, k0, 0, bx, bk, Q, KS);
+  const size_t q_stride = (size_t)(bk / 4) * (bx / 8) * 32;
   for (int q = 0; q < Q; q++) {
     double d[4];
 #pragma unroll
@@ -195,10 +195,18 @@ __global__ void __launch_bounds__(256) split_packed_kernel(int rows, int cols, i
 
 }  // namespace
 
-cudaError_t launch_exponents(int rows, int cols, int axis, const double* lead, int32_t* exps, uint32_t* flags,
-                             cudaStream_t stream, uint64_t* launches) {
+// Lowest group exponent at which every kept quarter product 2^(E_i + F_j - 13(s+2)), s < quarters, is still a normal
+// double when both groups sit at the bound; -EXP_LIMIT for the paper's dd / qd quarter counts.
+int exponent_floor(int quarters) {
+  const int lo = -(1022 - 13 * (quarters + 1)) / 2;
+  return quarters <= 24 || lo < -EXP_LIMIT ? -EXP_LIMIT : lo;
+}
+
+cudaError_t launch_exponents(int rows, int cols, int axis, int quarters, const double* lead, int32_t* exps,
+                             uint32_t* flags, cudaStream_t stream, uint64_t* launches) {
+  const int exp_lo = exponent_floor(quarters);
   if (axis == 0) {
-    row_exponent_kernel<<<min(rows, 148 * 64), 256, 0, stream>>>(rows, cols, lead, exps, flags);
+    row_exponent_kernel<<<min(rows, 148 * 64), 256, 0, stream>>>(rows, cols, lead, exps, flags, exp_lo);
     *launches += 1;
     return cudaGetLastError();
   }
@@ -212,7 +220,7 @@ cudaError_t launch_exponents(int rows, int cols, int axis, const double* lead, i
   chunks = (rows + rows_per_block - 1) / rows_per_block;
   col_max_kernel<<<dim3(col_blocks, chunks), 256, 0, stream>>>(rows, cols, rows_per_block, lead, exps);
   if ((err = cudaGetLastError()) != cudaSuccess) return err;
-  col_exponent_finalize_kernel<<<col_blocks, 256, 0, stream>>>(cols, exps, flags);
+  col_exponent_finalize_kernel<<<col_blocks, 256, 0, stream>>>(cols, exps, flags, exp_lo);
   *launches += 2;
   return cudaGetLastError();
 }
@@ -231,6 +239,8 @@ cudaError_t launch_split(int rows, int cols, int limbs, int quarters, int axis, 
     case 1: MD_SPLIT(1) break;
     case 2: MD_SPLIT(2) break;
     case 4: MD_SPLIT(4) break;
+    case 8: MD_SPLIT(8) break;
+    case 16: MD_SPLIT(16) break;
     default: return cudaErrorInvalidValue;
   }
 #undef MD_SPLIT
@@ -243,18 +253,23 @@ cudaError_t launch_split_packed(int rows, int cols, int limbs, int quarters, int
                                 uint64_t* launches) {
   const int X = axis == 0 ? rows : cols, K = axis == 0 ? cols : rows;
   const int bx = pack_bx(limbs, axis);
-  const int KS = (K + PACK_BK - 1) / PACK_BK;
+  const int bk = pack_bk(limbs);
+  const int KS = (K + bk - 1) / bk;
   const int x_blocks = ((X + bx - 1) / bx * bx + 31) / 32;  // 32 groups per block over the padded extent
-  const long long k_blocks = ((long long)KS * (PACK_BK / 4) + 7) / 8;
+  const long long k_blocks = ((long long)KS * (bk / 4) + 7) / 8;
   const long long blocks = (long long)x_blocks * k_blocks;
   if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
 #define MD_SPLITP(L_, AX_)                                                                                           \
-  split_packed_kernel<L_, AX_><<<(unsigned)blocks, 256, 0, stream>>>(rows, cols, quarters, bx, x_blocks, KS, planes, \
+  split_packed_kernel<L_, AX_><<<(unsigned)blocks, 256, 0, stream>>>(rows, cols, quarters, bx, bk, x_blocks, KS, planes, \
                                                                      packed, exps, flags)
   if (limbs == 2 && axis == 0) MD_SPLITP(2, 0);
   else if (limbs == 2 && axis == 1) MD_SPLITP(2, 1);
   else if (limbs == 4 && axis == 0) MD_SPLITP(4, 0);
   else if (limbs == 4 && axis == 1) MD_SPLITP(4, 1);
+  else if (limbs == 8 && axis == 0) MD_SPLITP(8, 0);
+  else if (limbs == 8 && axis == 1) MD_SPLITP(8, 1);
+  else if (limbs == 16 && axis == 0) MD_SPLITP(16, 0);
+  else if (limbs == 16 && axis == 1) MD_SPLITP(16, 1);
   else return cudaErrorInvalidValue;
 #undef MD_SPLITP
   *launches += 1;

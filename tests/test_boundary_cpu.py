@@ -50,7 +50,13 @@ def test_argument_errors_need_no_gpu(lib):
     assert lib.md_gemm(1, 1, 2 ** 24, 2, fake, fake, fake, None) == md.MD_ERR_WORKSPACE  # passes the checks; no workspace
     assert lib.md_split(4, 4, 3, 8, 0, fake, fake, fake, None) == md.MD_ERR_BAD_ARG
     assert lib.md_split(4, 4, 2, 8, 2, fake, fake, fake, None) == md.MD_ERR_BAD_ARG
-    assert lib.md_split(4, 4, 2, 25, 0, fake, fake, fake, None) == md.MD_ERR_BAD_ARG
+    assert lib.md_split(4, 4, 2, 73, 0, fake, fake, fake, None) == md.MD_ERR_BAD_ARG  # at most 72 quarters
+    assert lib.md_renorm(4, 4, 2, 145, fake, fake, None) == md.MD_ERR_BAD_ARG
+    # octo / hexa double (Table 2): k budget 2^27 / 32 and 2^27 / 64; only md_gemm has kernels for them
+    assert lib.md_gemm(1, 1, 2 ** 22 + 1, 8, fake, fake, fake, None) == md.MD_ERR_K_TOO_LARGE
+    assert lib.md_gemm(1, 1, 2 ** 21 + 1, 16, fake, fake, fake, None) == md.MD_ERR_K_TOO_LARGE
+    assert lib.md_gemm(1, 1, 2 ** 21, 16, fake, fake, fake, None) == md.MD_ERR_WORKSPACE
+    assert lib.md_qgemm(4, 4, 4, 8, 32, 32, fake, fake, fake, fake, None) == md.MD_ERR_UNSUPPORTED
     assert lib.md_renorm(4, 4, 2, 0, fake, fake, None) == md.MD_ERR_BAD_ARG
     assert lib.md_qgemm(4, 4, 4, 2, 8, 7, fake, fake, fake, fake, None) == md.MD_ERR_UNSUPPORTED
     assert lib.md_qgemm(4, 4, 4, 2, 12, 12, fake, fake, fake, fake, None) == md.MD_ERR_UNSUPPORTED
@@ -70,6 +76,9 @@ def test_options_and_workspace_sizes(lib):
     assert lib.md_workspace_bytes(64, 64, 64, 2) >= 2 * 9 * 64 * 64 * 8
     assert lib.md_set_option(md.MD_OPT_QUARTERS, 0) == 0
     assert lib.md_workspace_bytes(64, 64, 64, 4) >= 2 * 16 * 64 * 64 * 8  # quad double: 16 times
+    # octo double 32 times, hexa double 64 times (4 quarters per limb)
+    assert lib.md_workspace_bytes(64, 64, 64, 8) >= 2 * 32 * 64 * 64 * 8
+    assert lib.md_workspace_bytes(64, 64, 64, 16) >= 2 * 64 * 64 * 64 * 8
     assert lib.md_workspace_bytes(0, 64, 64, 2) == 0 and lib.md_workspace_bytes(64, 64, 64, 3) == 0
     assert lib.md_host_scratch_bytes(64, 64, 64, 2) >= base + 3 * 2 * 64 * 64 * 8
     assert lib.md_set_option(99, 1) == md.MD_ERR_BAD_ARG and lib.md_set_option(md.MD_OPT_QUARTERS, 99) == md.MD_ERR_BAD_ARG
