@@ -15,6 +15,7 @@
 // rational arithmetic in Python, closed forms, hand-derived special cases, the paper's constants):
 //   O1  oracle_exact_*      exact product  C = A*B of multiple-double matrices (plain definition)
 //   O2  oracle_split        Algorithm S: exponent vectors + 13-bit quarters
+//       oracle_*_w          the same with the slice width as a parameter (R13; 13 = the paper's quarter)
 //   O3  oracle_orders_*     order matrices C^(s) = sum_{p+q=s} A_p B_q  (eq. 3-4)
 //   O4  oracle_renorm       sum of the S order values -> L non-overlapping limbs
 //   O5  oracle_classic_gemm classical multiple-double GEMM on "regular cores", cross-check
@@ -222,8 +223,10 @@ extern "C" {
 //   remainder       [limbs][rows][cols] or NULL: what is left after the last quarter (sum of quarters + remainder
 //                   == element, exactly)
 // =====================================================================================================
-void oracle_split(int rows, int cols, int limbs, int quarters, int axis, const double* planes,
-                  double* quarter_planes, int32_t* exps, double* remainder) {
+//   oracle_split_w: the same procedure with `bits` in place of 13 (R13: a slice of `bits` bits per part,
+//   unit u_q = 2^(E_g - bits*(q+1)); the paper's quarter is bits = 13 = 52/4).
+void oracle_split_w(int rows, int cols, int limbs, int quarters, int bits, int axis, const double* planes,
+                    double* quarter_planes, int32_t* exps, double* remainder) {
   const size_t plane = (size_t)rows * cols;
   const int groups = axis == 0 ? rows : cols;
   // S0: the exponent of each scale group, from the leading limb only.
@@ -246,7 +249,7 @@ void oracle_split(int rows, int cols, int limbs, int quarters, int axis, const d
       const int E = exps[axis == 0 ? i : j];
       for (int l = 0; l < limbs; l++) r[l] = planes[l * plane + at];
       for (int q = 0; q < quarters; q++) {
-        const double u = std::ldexp(1.0, E - 13 * (q + 1));  // the unit of quarter q
+        const double u = std::ldexp(1.0, E - bits * (q + 1));  // the unit of quarter q
         const double c = 6755399441055744.0 * u;            // 3 * 2^51 * u: ulp(c) == u, so r0 + c rounds r0 to a multiple of u
         const double t = r[0] + c;
         const double d = t - c;   // exact; the quarter
@@ -260,6 +263,11 @@ void oracle_split(int rows, int cols, int limbs, int quarters, int axis, const d
   }
 }
 
+void oracle_split(int rows, int cols, int limbs, int quarters, int axis, const double* planes,
+                  double* quarter_planes, int32_t* exps, double* remainder) {
+  oracle_split_w(rows, cols, limbs, quarters, 13, axis, planes, quarter_planes, exps, remainder);  // 13 bits
+}
+
 // =====================================================================================================
 // O3 -- order matrices C^(s)[i,j] = sum_k sum_{p+q=s} A_p[i,k] * B_q[k,j], s = 0..orders-1 (the paper's C_{s+1}).
 //   PAPER.md:66-71 eq. (3): "the convolutions with the sum of the last two indices ... equal to the index of the
@@ -269,18 +277,19 @@ void oracle_split(int rows, int cols, int limbs, int quarters, int axis, const d
 //   * oracle_orders_fp64: the same sums in plain fp64, k innermost, products in the order p = 0..s.
 //   Aq [quarters][m][k], Bq [quarters][k][n], order_planes [orders][m][n] (true values).
 // =====================================================================================================
-void oracle_orders_int(int m, int n, int k, int quarters, int orders, const double* Aq, const int32_t* expA,
-                       const double* Bq, const int32_t* expB, double* order_planes, int64_t* raw_sums) {
+//   The _w variants take the slice width `bits` (13 in the paper): unit of order s = 2^(E_i + F_j - bits*(s+2)).
+void oracle_orders_int_w(int m, int n, int k, int quarters, int orders, int bits, const double* Aq, const int32_t* expA,
+                         const double* Bq, const int32_t* expB, double* order_planes, int64_t* raw_sums) {
   const size_t pa = (size_t)m * k, pb = (size_t)k * n, pc = (size_t)m * n;
   // integer digits
   std::vector<int32_t> DA((size_t)quarters * pa), DB((size_t)quarters * pb);
   for (int q = 0; q < quarters; q++) {
     for (int i = 0; i < m; i++)
       for (int t = 0; t < k; t++)
-        DA[q * pa + (size_t)i * k + t] = (int32_t)std::ldexp(Aq[q * pa + (size_t)i * k + t], -(expA[i] - 13 * (q + 1)));
+        DA[q * pa + (size_t)i * k + t] = (int32_t)std::ldexp(Aq[q * pa + (size_t)i * k + t], -(expA[i] - bits * (q + 1)));
     for (int t = 0; t < k; t++)
       for (int j = 0; j < n; j++)
-        DB[q * pb + (size_t)t * n + j] = (int32_t)std::ldexp(Bq[q * pb + (size_t)t * n + j], -(expB[j] - 13 * (q + 1)));
+        DB[q * pb + (size_t)t * n + j] = (int32_t)std::ldexp(Bq[q * pb + (size_t)t * n + j], -(expB[j] - bits * (q + 1)));
   }
 #pragma omp parallel for schedule(static)
   for (int i = 0; i < m; i++)
@@ -295,14 +304,19 @@ void oracle_orders_int(int m, int n, int k, int quarters, int orders, const doub
         }
         if (raw_sums) raw_sums[s * pc + (size_t)i * n + j] = acc;
         // |acc| < 2^53 under the k-budget (R6), so the conversion and the scaling are exact.
-        order_planes[s * pc + (size_t)i * n + j] = std::ldexp((double)acc, expA[i] + expB[j] - 13 * (s + 2));
+        order_planes[s * pc + (size_t)i * n + j] = std::ldexp((double)acc, expA[i] + expB[j] - bits * (s + 2));
       }
 }
 
+void oracle_orders_int(int m, int n, int k, int quarters, int orders, const double* Aq, const int32_t* expA,
+                       const double* Bq, const int32_t* expB, double* order_planes, int64_t* raw_sums) {
+  oracle_orders_int_w(m, n, k, quarters, orders, 13, Aq, expA, Bq, expB, order_planes, raw_sums);
+}
+
 // The same integer route at sampled output positions only (for full-size matrices): out[t*orders + s] = C^(s)[si[t], sj[t]].
-void oracle_orders_int_samples(int m, int n, int k, int quarters, int orders, const double* Aq, const int32_t* expA,
-                               const double* Bq, const int32_t* expB, int64_t nsamples, const int64_t* si,
-                               const int64_t* sj, double* out) {
+void oracle_orders_int_samples_w(int m, int n, int k, int quarters, int orders, int bits, const double* Aq,
+                                 const int32_t* expA, const double* Bq, const int32_t* expB, int64_t nsamples,
+                                 const int64_t* si, const int64_t* sj, double* out) {
   const size_t pa = (size_t)m * k, pb = (size_t)k * n;
 #pragma omp parallel for schedule(dynamic, 16)
   for (int64_t t = 0; t < nsamples; t++) {
@@ -313,14 +327,20 @@ void oracle_orders_int_samples(int m, int n, int k, int quarters, int orders, co
         const int q = s - p;
         if (p >= quarters || q >= quarters) continue;
         for (int kk = 0; kk < k; kk++) {
-          const int64_t da = (int64_t)std::ldexp(Aq[p * pa + (size_t)i * k + kk], -(expA[i] - 13 * (p + 1)));
-          const int64_t db = (int64_t)std::ldexp(Bq[q * pb + (size_t)kk * n + j], -(expB[j] - 13 * (q + 1)));
+          const int64_t da = (int64_t)std::ldexp(Aq[p * pa + (size_t)i * k + kk], -(expA[i] - bits * (p + 1)));
+          const int64_t db = (int64_t)std::ldexp(Bq[q * pb + (size_t)kk * n + j], -(expB[j] - bits * (q + 1)));
           acc += da * db;
         }
       }
-      out[t * orders + s] = std::ldexp((double)acc, expA[i] + expB[j] - 13 * (s + 2));
+      out[t * orders + s] = std::ldexp((double)acc, expA[i] + expB[j] - bits * (s + 2));
     }
   }
+}
+
+void oracle_orders_int_samples(int m, int n, int k, int quarters, int orders, const double* Aq, const int32_t* expA,
+                               const double* Bq, const int32_t* expB, int64_t nsamples, const int64_t* si,
+                               const int64_t* sj, double* out) {
+  oracle_orders_int_samples_w(m, n, k, quarters, orders, 13, Aq, expA, Bq, expB, nsamples, si, sj, out);
 }
 
 void oracle_orders_fp64(int m, int n, int k, int quarters, int orders, const double* Aq, const double* Bq,
@@ -485,18 +505,23 @@ void oracle_classic_gemm(int m, int n, int k, int limbs, const double* A, const 
 // parts.  Steps 2 and 4 are index bookkeeping only (Abar/Bbar are never stored).  Computes rows [row0,row1) of C
 // into C_rows [limbs][row1-row0][n]; B's quarters are computed for the whole of B every call.
 // =====================================================================================================
-void oracle_md_gemm_rows(int m, int n, int k, int limbs, int quarters, int orders, const double* A, const double* B,
-                         int row0, int row1, double* C_rows) {
+void oracle_md_gemm_rows_w(int m, int n, int k, int limbs, int quarters, int orders, int bits, const double* A,
+                           const double* B, int row0, int row1, double* C_rows) {
   const int mr = row1 - row0;
   std::vector<double> Arows((size_t)limbs * mr * k);
   for (int l = 0; l < limbs; l++)
     std::memcpy(&Arows[(size_t)l * mr * k], &A[(size_t)l * m * k + (size_t)row0 * k], sizeof(double) * (size_t)mr * k);
   std::vector<double> Aq((size_t)quarters * mr * k), Bq((size_t)quarters * k * n), ord((size_t)orders * mr * n);
   std::vector<int32_t> eA(mr), eB(n);
-  oracle_split(mr, k, limbs, quarters, 0, Arows.data(), Aq.data(), eA.data(), nullptr);
-  oracle_split(k, n, limbs, quarters, 1, B, Bq.data(), eB.data(), nullptr);
+  oracle_split_w(mr, k, limbs, quarters, bits, 0, Arows.data(), Aq.data(), eA.data(), nullptr);
+  oracle_split_w(k, n, limbs, quarters, bits, 1, B, Bq.data(), eB.data(), nullptr);
   oracle_orders_fp64(mr, n, k, quarters, orders, Aq.data(), Bq.data(), ord.data());
   oracle_renorm(mr, n, limbs, orders, ord.data(), C_rows);
+}
+
+void oracle_md_gemm_rows(int m, int n, int k, int limbs, int quarters, int orders, const double* A, const double* B,
+                         int row0, int row1, double* C_rows) {
+  oracle_md_gemm_rows_w(m, n, k, limbs, quarters, orders, 13, A, B, row0, row1, C_rows);
 }
 
 int oracle_num_threads(void) {

@@ -44,19 +44,20 @@ def num_threads() -> int:
     return int(lib().oracle_num_threads())
 
 
-def split(planes: np.ndarray, axis: int, quarters: int | None = None, want_remainder: bool = False):
-    """O2.  planes [limbs, rows, cols] -> (quarter_planes [Q, rows, cols], exps int32, remainder or None)."""
+def split(planes: np.ndarray, axis: int, quarters: int | None = None, want_remainder: bool = False, bits: int = 13):
+    """O2.  planes [limbs, rows, cols] -> (quarter_planes [Q, rows, cols], exps int32, remainder or None).
+    bits = slice width (13 = the paper's quarter; other widths: DESIGN.md R13)."""
     planes = _f64(planes)
     limbs, rows, cols = planes.shape
     Q = 4 * limbs if quarters is None else quarters
     qp = np.empty((Q, rows, cols), dtype=np.float64)
     exps = np.empty(rows if axis == 0 else cols, dtype=np.int32)
     rem = np.empty_like(planes) if want_remainder else None
-    lib().oracle_split(rows, cols, limbs, Q, axis, _d(planes), _d(qp), exps.ctypes.data_as(_ip), _d(rem))
+    lib().oracle_split_w(rows, cols, limbs, Q, bits, axis, _d(planes), _d(qp), exps.ctypes.data_as(_ip), _d(rem))
     return qp, exps, rem
 
 
-def orders_int(Aq, expA, Bq, expB, orders: int | None = None, want_raw: bool = False):
+def orders_int(Aq, expA, Bq, expB, orders: int | None = None, want_raw: bool = False, bits: int = 13):
     """O3, int64 digit route.  Aq [Q, m, k], Bq [Q, k, n] -> order planes [S, m, n] (and raw int64 sums)."""
     Aq, Bq = _f64(Aq), _f64(Bq)
     Q, m, k = Aq.shape
@@ -66,12 +67,12 @@ def orders_int(Aq, expA, Bq, expB, orders: int | None = None, want_raw: bool = F
     raw = np.empty((S, m, n), dtype=np.int64) if want_raw else None
     expA = np.ascontiguousarray(expA, dtype=np.int32)
     expB = np.ascontiguousarray(expB, dtype=np.int32)
-    lib().oracle_orders_int(m, n, k, Q, S, _d(Aq), expA.ctypes.data_as(_ip), _d(Bq), expB.ctypes.data_as(_ip),
-                            _d(out), None if raw is None else raw.ctypes.data_as(_lp))
+    lib().oracle_orders_int_w(m, n, k, Q, S, bits, _d(Aq), expA.ctypes.data_as(_ip), _d(Bq), expB.ctypes.data_as(_ip),
+                              _d(out), None if raw is None else raw.ctypes.data_as(_lp))
     return (out, raw) if want_raw else out
 
 
-def orders_int_samples(Aq, expA, Bq, expB, si, sj, orders: int | None = None):
+def orders_int_samples(Aq, expA, Bq, expB, si, sj, orders: int | None = None, bits: int = 13):
     """O3, int64 digit route at sampled positions: returns [nsamples, S]."""
     Aq, Bq = _f64(Aq), _f64(Bq)
     Q, m, k = Aq.shape
@@ -82,8 +83,9 @@ def orders_int_samples(Aq, expA, Bq, expB, si, sj, orders: int | None = None):
     out = np.empty((si.size, S), dtype=np.float64)
     expA = np.ascontiguousarray(expA, dtype=np.int32)
     expB = np.ascontiguousarray(expB, dtype=np.int32)
-    lib().oracle_orders_int_samples(m, n, k, Q, S, _d(Aq), expA.ctypes.data_as(_ip), _d(Bq), expB.ctypes.data_as(_ip),
-                                    ctypes.c_int64(si.size), si.ctypes.data_as(_lp), sj.ctypes.data_as(_lp), _d(out))
+    lib().oracle_orders_int_samples_w(m, n, k, Q, S, bits, _d(Aq), expA.ctypes.data_as(_ip), _d(Bq),
+                                      expB.ctypes.data_as(_ip), ctypes.c_int64(si.size), si.ctypes.data_as(_lp),
+                                      sj.ctypes.data_as(_lp), _d(out))
     return out
 
 
@@ -159,7 +161,7 @@ def classic_gemm(A, B):
 
 
 def md_gemm_rows(A, B, row0: int = 0, row1: int | None = None, quarters: int | None = None,
-                 orders: int | None = None):
+                 orders: int | None = None, bits: int = 13):
     """The paper's five steps through the oracle: rows [row0,row1) of C = A*B."""
     A, B = _f64(A), _f64(B)
     limbs, m, k = A.shape
@@ -168,5 +170,5 @@ def md_gemm_rows(A, B, row0: int = 0, row1: int | None = None, quarters: int | N
     Q = 4 * limbs if quarters is None else quarters
     S = Q if orders is None else orders
     C = np.empty((limbs, row1 - row0, n))
-    lib().oracle_md_gemm_rows(m, n, k, limbs, Q, S, _d(A), _d(B), row0, row1, _d(C))
+    lib().oracle_md_gemm_rows_w(m, n, k, limbs, Q, S, bits, _d(A), _d(B), row0, row1, _d(C))
     return C

@@ -36,12 +36,12 @@ def round_half_even(q: Fraction) -> int:
     return round(q)  # Python's round() on a Fraction rounds half to even
 
 
-def nearest_digits(value: Fraction, E: int, Q: int):
+def nearest_digits(value: Fraction, E: int, Q: int, bits: int = 13):
     """Signed-digit expansion by exact nearest rounding: D_q = RN(R_q / u_q), R_{q+1} = R_q - D_q u_q.
     Also returns min over q of the distance of R_q/u_q from a tie (x.5)."""
     digits, R, margin = [], value, Fraction(1)
     for q in range(Q):
-        u = Fraction(2) ** (E - 13 * (q + 1))
+        u = Fraction(2) ** (E - bits * (q + 1))
         t = R / u
         margin = min(margin, abs(abs(t - math.floor(t)) - Fraction(1, 2)))
         D = round_half_even(t)
