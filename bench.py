@@ -56,6 +56,9 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (default 2: the headline)")
+    ap.add_argument("--slices", default="paper", choices=["paper", "adaptive"],
+                    help="paper: 13-bit quarters, 4 per limb (the headline).  adaptive: the (bits, count) md_plan_slices "
+                         "picks for this k -- wider, fewer slices (DESIGN.md R13; NOT the paper's quarters)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -139,7 +142,7 @@ def cpu_oracle_sample(cfg, rows: int, cols: int | None = None):
     B = np.ascontiguousarray(inputs.generate(cfg, "B", 0, None, 0, cols))
     threads = min(orc.num_threads(), rows)
     t0 = time.perf_counter()
-    orc.md_gemm_rows(A, B, quarters=cfg.quarters)
+    orc.md_gemm_rows(A, B, quarters=cfg.quarters, bits=cfg.bits)
     dt = time.perf_counter() - t0
     return 2.0 * rows * cols * cfg.k / dt / 1e9, dt, threads
 
@@ -199,9 +202,11 @@ def run_ours(args):
 
     base = inputs.CONFIGS[args.config]
     # weak scaling: the global A has world * m rows, rank r owns one block of m rows (no collective on the data path)
+    if args.slices == "adaptive":
+        base = base.with_slices(*md.md_plan_slices(base.k, base.limbs))
     cfg = base.with_shape(m=base.m * world)
     row0, row1 = shard.row_block(cfg.m, world, rank)
-    m, n, k, L, Q = row1 - row0, cfg.n, cfg.k, cfg.limbs, cfg.quarters
+    m, n, k, L, Q, W = row1 - row0, cfg.n, cfg.k, cfg.limbs, cfg.quarters, cfg.bits
     A_host = torch.from_numpy(inputs.generate(cfg, "A", row0, row1)).pin_memory()
     B_host = torch.from_numpy(inputs.generate(cfg, "B")).pin_memory()
     C_host = torch.empty((L, m, n), dtype=torch.float64).pin_memory()
@@ -222,7 +227,7 @@ def run_ours(args):
         return float(t.item())
 
     sampler = ClockSampler(local_rank)
-    with md.Workspace(m, n, k, L, Q):
+    with md.Workspace(m, n, k, L, Q, bits=W):
         for _ in range(args.warmup):
             md.md_gemm(A, B, C)
         barrier()
@@ -246,10 +251,39 @@ def run_ours(args):
     dmma_probe_tflops = measure_dmma_peak(md, torch)
     probe_launches = md.md_launch_count() - probe_launches0
 
+    # beside the headline (the paper's quarters): the same problem with the k-adaptive slices, outside the timed region
+    adaptive = None
+    if args.slices == "paper" and world == 1:
+        aW, aQ = md.md_plan_slices(k, L)
+        if (aW, aQ) != (W, Q):
+            C2 = torch.empty_like(C)
+            with md.Workspace(m, n, k, L, aQ, bits=aW):
+                md.md_gemm(A, B, C2)
+                md.md_profile_enable(3)
+                torch.cuda.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                for _ in range(3):
+                    md.md_gemm(A, B, C2)
+                e1.record(stream)
+                torch.cuda.synchronize()
+                _, a_gemm_ms = md.md_profile_read(3)
+                md.md_profile_enable(0)
+            a_ms = e0.elapsed_time(e1) / 3
+            aT = aQ * (aQ + 1) // 2
+            adaptive = {"slice_bits": aW, "slices": aQ, "products": aT, "ms_per_step": a_ms,
+                        "value": base.md_flops / (a_ms * 1e-3) / 1e9, "unit": UNIT,
+                        "kernel_frac_of_fp64_tensor_peak": aT * base.md_flops / (sum(a_gemm_ms) / 3 * 1e-3) / 1e12 / FP64_TENSOR_PEAK_TFLOPS,
+                        "max_abs_diff_vs_paper_quarters": float((C2 - C).abs().sum(dim=0).max()),
+                        "note": "md_plan_slices: wider, fewer slices on the same kernels (DESIGN.md R13); not the paper's "
+                                "13-bit quarters, so not the headline; 3 steps after 1 warm-up, CUDA events"}
+            del C2
+
     # end to end: pinned host buffers through md_gemm_host (H2D A, B + the whole path + D2H C, synchronous)
     e2e = None
     if not args.no_e2e:
         md.md_set_option(md.MD_OPT_QUARTERS, 0 if Q == 4 * L else Q)  # before sizing the scratch: it depends on Q
+        md.md_set_option(md.MD_OPT_SLICE_BITS, 0 if W == 13 else W)
         scratch = torch.empty(md.md_host_scratch_bytes(m, n, k, L), dtype=torch.uint8, device="cuda")
         for _ in range(min(args.warmup, 2)):
             md.md_gemm_host(A_host, B_host, C_host, scratch)
@@ -264,6 +298,7 @@ def run_ours(args):
         e2e_ms = max_over_ranks(e0.elapsed_time(e1))
         wall_ms = max_over_ranks((time.perf_counter() - t0) * 1e3)
         md.md_set_option(md.MD_OPT_QUARTERS, 0)
+        md.md_set_option(md.MD_OPT_SLICE_BITS, 0)
         e2e = {"value": world * base.md_flops * args.steps / (max(e2e_ms, wall_ms) * 1e-3) / 1e9, "unit": UNIT,
                "h2d_bytes_per_step": A_host.numel() * 8 + B_host.numel() * 8, "d2h_bytes_per_step": C_host.numel() * 8,
                "ms_per_step": max(e2e_ms, wall_ms) / args.steps, "launches": md.md_launch_count() - launches_e2e0,
@@ -316,7 +351,8 @@ def run_ours(args):
         "dtype": "f64", "data": "synthetic",
         "config": {
             "workload": f"BASELINE.json configs[{base.index}] {base.name}: m={base.m} n={base.n} k={base.k} per GPU, "
-                        f"limbs={L}, quarters={Q} (T={base.products} quarter products), seed {base.seed}",
+                        f"limbs={L}, quarters={Q} of {W} bits (T={base.products} quarter products), seed {base.seed}",
+            "slices": args.slices,
             "parallelism": "single GPU" if world == 1 else f"rows of A sharded over {world} GPUs, B replicated, no collective",
             "l2": "inputs (%.0f MiB) and quarter planes (%.0f MiB) exceed the 126 MB L2; no explicit flush" % (
                 (A.numel() + B.numel()) * 8 / 2 ** 20, 8.0 * Q * (m * k + k * n) / 2 ** 20),
@@ -325,6 +361,7 @@ def run_ours(args):
         "fp64_tflops_issued": world * base.fp64_flops / (ms_per_step * 1e-3) / 1e12,
         "pct_of_fp64_tensor_peak": 100.0 * base.fp64_flops / (ms_per_step * 1e-3) / 1e12 / FP64_TENSOR_PEAK_TFLOPS,
         "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": launches,
+        "adaptive_slices": adaptive,
         "clocks": clocks, "status_flags": flags,
     }
     print(json.dumps(line))

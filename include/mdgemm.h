@@ -56,11 +56,24 @@ enum {
   MD_OPT_QUARTERS = 1,  /* quarters per element used by md_gemm / md_gemm_orders / md_gemm_host.  Default 4*limbs, the
                            paper's count (8 for double double, 16 for quad double).  Supported:
                            limbs=2: 8, 9, 10; limbs=4: 16, 17, 18 (R5). */
-  MD_OPT_ORDERS = 2     /* kept product orders S (the paper's C_1..C_S).  Default = quarters.  Must equal
+  MD_OPT_ORDERS = 2,    /* kept product orders S (the paper's C_1..C_S).  Default = quarters.  Must equal
                            quarters in this version. */
+  MD_OPT_SLICE_BITS = 3 /* width W of a slice in bits, used by md_split and the md_gemm family.  Default 13: the paper's
+                           quarter ("4 parts ... each of 13 bits").  Other widths (4..24) are the k-adaptive
+                           variant of DESIGN.md R13 / SURVEY.md 8(f) NEXT-3 -- NOT the paper's quarters: a slice of W
+                           bits sits on the unit 2^(E_g - W(q+1)), |D| <= 2^W (q = 0), 2^(W-1) (q > 0), and the
+                           exactness budget becomes k * orders * 2^(2W) <= 2^53.  With wider slices fewer are needed:
+                           set MD_OPT_QUARTERS to the slice count (limbs=2: 6, 7; limbs=4: 11, 12; limbs=8: 22), or
+                           take both from md_plan_slices. */
 };
 md_status md_set_option(int key, int value);
 int md_get_option(int key); /* current value (0 = default), or -1 for an unknown key */
+
+/* Host-only helper for MD_OPT_SLICE_BITS: the fewest slices with a kernel for `limbs`, at the widest width W whose
+ * exactness budget k * Q * 2^(2W) <= 2^53 holds (eq. 5 generalised), such that the window W * Q is at least
+ * the paper's 13 * 4 * limbs bits.  Stores W in *bits_out and Q in *quarters_out (host pointers); (13, 4*limbs), the paper's
+ * own split, when nothing wider qualifies.  Launches nothing and changes no option. */
+md_status md_plan_slices(int k, int limbs, int* bits_out, int* quarters_out);
 
 /* ---------------------------------------------------------------------------------------------------------------------
  * md_split -- steps a1 + a2: exponent vectors ("balancing") and quarter planes.

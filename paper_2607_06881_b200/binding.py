@@ -16,13 +16,14 @@ LIB_PATH = os.path.join(_HERE, "libmdgemm.so")
 
 MD_OK = 0
 MD_ERR_BAD_ARG, MD_ERR_K_TOO_LARGE, MD_ERR_WORKSPACE, MD_ERR_CUDA, MD_ERR_UNSUPPORTED = -1, -2, -3, -4, -5
-MD_OPT_QUARTERS, MD_OPT_ORDERS = 1, 2
+MD_OPT_QUARTERS, MD_OPT_ORDERS, MD_OPT_SLICE_BITS = 1, 2, 3
 
 # every symbol include/mdgemm.h declares: name -> (restype, argtypes)
 _c = ctypes
 _SIGNATURES = {
     "md_set_option": (_c.c_int, [_c.c_int, _c.c_int]),
     "md_get_option": (_c.c_int, [_c.c_int]),
+    "md_plan_slices": (_c.c_int, [_c.c_int, _c.c_int, _c.c_void_p, _c.c_void_p]),
     "md_split": (_c.c_int, [_c.c_int] * 5 + [_c.c_void_p] * 4),
     "md_qgemm": (_c.c_int, [_c.c_int] * 6 + [_c.c_void_p] * 5),
     "md_renorm": (_c.c_int, [_c.c_int] * 4 + [_c.c_void_p] * 3),
@@ -87,6 +88,13 @@ def md_set_option(key: int, value: int):
 
 def md_get_option(key: int) -> int:
     return lib().md_get_option(key)
+
+
+def md_plan_slices(k: int, limbs: int):
+    """(slice bits W, slice count Q) of the k-adaptive split for contraction length k (include/mdgemm.h)."""
+    bits, quarters = ctypes.c_int(0), ctypes.c_int(0)
+    _check(lib().md_plan_slices(k, limbs, ctypes.addressof(bits), ctypes.addressof(quarters)), "md_plan_slices")
+    return bits.value, quarters.value
 
 
 def md_workspace_bytes(m, n, k, limbs) -> int:
@@ -203,8 +211,9 @@ def md_launch_count() -> int:
 class Workspace:
     """Allocates and registers the md_gemm workspace for one problem shape (context manager)."""
 
-    def __init__(self, m, n, k, limbs, quarters: int = 0, device="cuda"):
+    def __init__(self, m, n, k, limbs, quarters: int = 0, device="cuda", bits: int = 0):
         md_set_option(MD_OPT_QUARTERS, 0 if quarters == 4 * limbs else quarters)
+        md_set_option(MD_OPT_SLICE_BITS, 0 if bits == 13 else bits)
         nbytes = md_workspace_bytes(m, n, k, limbs)
         if nbytes == 0:
             raise ValueError("bad shape for workspace")
@@ -214,6 +223,7 @@ class Workspace:
     def close(self):
         md_set_workspace(None)
         md_set_option(MD_OPT_QUARTERS, 0)
+        md_set_option(MD_OPT_SLICE_BITS, 0)
         self.buffer = None
 
     def __enter__(self):

@@ -14,6 +14,7 @@ namespace {
 struct State {
   int opt_quarters = 0;  // 0 = default (4 * limbs)
   int opt_orders = 0;    // 0 = default (= quarters)
+  int opt_bits = 0;      // 0 = default (13, the paper's quarter)
   void* ws = nullptr;
   size_t ws_bytes = 0;
 };
@@ -33,6 +34,12 @@ inline size_t round_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 inline int quarters_for(int limbs) { return g_state.opt_quarters ? g_state.opt_quarters : 4 * limbs; }
 inline int orders_for(int limbs) { return g_state.opt_orders ? g_state.opt_orders : quarters_for(limbs); }
+inline int slice_bits() { return g_state.opt_bits ? g_state.opt_bits : 13; }
+constexpr int MD_MIN_BITS = 4, MD_MAX_BITS = 24;
+// Exactness budget (eq. 5 generalised; R6, R13): order s adds (s+1) <= S products per k, each an
+// integer of at most 2^(2W) units, so every partial sum is exactly representable while k * S * 2^(2W) <= 2^53.
+// W = 13: k * S <= 2^27.
+inline bool k_budget_ok(long long k, int S, int bits) { return k * S <= (1ll << (53 - 2 * bits)); }
 
 // Workspace layout: [status word | expA int32[m] | expB int32[n] | Aq | Bq], Aq / Bq = the packed quarter planes of A / B
 // (md_packed.cuh: zero padded to whole CTA tiles and k-slabs), then the stream-K scratch of the fused GEMM
@@ -73,26 +80,24 @@ md_status check_gemm_args(int m, int n, int k, int limbs, const void* A, const v
   if (limbs != 2 && limbs != 4 && limbs != 8 && limbs != 16) return MD_ERR_BAD_ARG;
   const int Q = quarters_for(limbs), S = orders_for(limbs);
   if (S != Q || !(md::qgemm_supported(limbs, Q) || md::qgemm_wide_supported(limbs, Q))) return MD_ERR_UNSUPPORTED;
-  // exactness budget: every partial sum of an order is below k * S * 2^26 units, which must not exceed 2^53
-  // (eq. 5 generalised to S products per k; R6)
-  if ((long long)k * S > (1ll << 27)) return MD_ERR_K_TOO_LARGE;
+  if (!k_budget_ok(k, S, slice_bits())) return MD_ERR_K_TOO_LARGE;
   return MD_OK;
 }
 
 // split A (rows) and B (columns) into the packed quarter planes of the carved workspace, then the fused quarter GEMM.
 md_status gemm_impl(int m, int n, int k, int limbs, const double* A, const double* B, double* C_planes,
                     double* order_planes, void* ws, size_t ws_bytes, cudaStream_t stream) {
-  const int Q = quarters_for(limbs);
+  const int Q = quarters_for(limbs), W = slice_bits();
   if (!ws) return MD_ERR_WORKSPACE;
   const Carve c = carve(ws, m, n, k, limbs, Q);
   if (c.total > ws_bytes) return MD_ERR_WORKSPACE;
   uint64_t launches = 0;
   cudaEvent_t* ev = (g_prof.count < g_prof.capacity) ? &g_prof.ev[3 * (size_t)g_prof.count] : nullptr;
   if (ev) cudaEventRecord(ev[0], stream);
-  cudaError_t err = md::launch_exponents(m, k, 0, Q, A, c.expA, c.flags, stream, &launches);
-  if (err == cudaSuccess) err = md::launch_exponents(k, n, 1, Q, B, c.expB, c.flags, stream, &launches);
-  if (err == cudaSuccess) err = md::launch_split_packed(m, k, limbs, Q, 0, A, c.Aq, c.expA, c.flags, stream, &launches);
-  if (err == cudaSuccess) err = md::launch_split_packed(k, n, limbs, Q, 1, B, c.Bq, c.expB, c.flags, stream, &launches);
+  cudaError_t err = md::launch_exponents(m, k, 0, Q, W, A, c.expA, c.flags, stream, &launches);
+  if (err == cudaSuccess) err = md::launch_exponents(k, n, 1, Q, W, B, c.expB, c.flags, stream, &launches);
+  if (err == cudaSuccess) err = md::launch_split_packed(m, k, limbs, Q, W, 0, A, c.Aq, c.expA, c.flags, stream, &launches);
+  if (err == cudaSuccess) err = md::launch_split_packed(k, n, limbs, Q, W, 1, B, c.Bq, c.expB, c.flags, stream, &launches);
   if (ev) cudaEventRecord(ev[1], stream);
   if (err == cudaSuccess)
     err = limbs <= 4 ? md::launch_qgemm_packed(m, n, k, limbs, Q, c.Aq, c.Bq, order_planes, C_planes, c.sk, stream, &launches)
@@ -112,6 +117,10 @@ extern "C" {
 md_status md_set_option(int key, int value) {
   if (value < 0 || value > MD_MAX_QUARTERS) return MD_ERR_BAD_ARG;
   switch (key) {
+    case MD_OPT_SLICE_BITS:
+      if (value != 0 && (value < MD_MIN_BITS || value > MD_MAX_BITS)) return MD_ERR_BAD_ARG;
+      g_state.opt_bits = value;
+      return MD_OK;
     case MD_OPT_QUARTERS: g_state.opt_quarters = value; return MD_OK;
     case MD_OPT_ORDERS: g_state.opt_orders = value; return MD_OK;
     default: return MD_ERR_BAD_ARG;
@@ -122,6 +131,7 @@ int md_get_option(int key) {
   switch (key) {
     case MD_OPT_QUARTERS: return g_state.opt_quarters;
     case MD_OPT_ORDERS: return g_state.opt_orders;
+    case MD_OPT_SLICE_BITS: return g_state.opt_bits;
     default: return -1;
   }
 }
@@ -135,9 +145,10 @@ md_status md_split(int rows, int cols, int limbs, int quarters, int axis, const 
   uint32_t* flags = g_state.ws ? static_cast<uint32_t*>(g_state.ws) : nullptr;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   uint64_t launches = 0;
-  cudaError_t err = md::launch_exponents(rows, cols, axis, quarters, planes, exps, flags, st, &launches);
+  const int W = slice_bits();
+  cudaError_t err = md::launch_exponents(rows, cols, axis, quarters, W, planes, exps, flags, st, &launches);
   if (err == cudaSuccess)
-    err = md::launch_split(rows, cols, limbs, quarters, axis, planes, quarter_planes, exps, flags, st, &launches);
+    err = md::launch_split(rows, cols, limbs, quarters, W, axis, planes, quarter_planes, exps, flags, st, &launches);
   g_launches += launches;
   return err == cudaSuccess ? MD_OK : MD_ERR_CUDA;
 }
@@ -149,7 +160,7 @@ md_status md_qgemm(int m, int n, int k, int limbs, int quarters, int orders, con
   if (limbs != 2 && limbs != 4 && limbs != 8 && limbs != 16) return MD_ERR_BAD_ARG;
   // plain-layout quarter planes: double / quad double only (octo / hexa double go through md_gemm's packed operands)
   if (orders != quarters || !md::qgemm_supported(limbs, quarters)) return MD_ERR_UNSUPPORTED;
-  if ((long long)k * orders > (1ll << 27)) return MD_ERR_K_TOO_LARGE;
+  if (!k_budget_ok(k, orders, slice_bits())) return MD_ERR_K_TOO_LARGE;
   uint64_t launches = 0;
   cudaError_t err = md::launch_qgemm(m, n, k, limbs, quarters, Aq, Bq, order_planes, C_planes,
                                      static_cast<cudaStream_t>(stream), &launches);
@@ -205,6 +216,27 @@ md_status md_gemm_orders(int m, int n, int k, int limbs, const double* A_planes,
   if (st != MD_OK) return st;
   return gemm_impl(m, n, k, limbs, A_planes, B_planes, nullptr, order_planes, g_state.ws, g_state.ws_bytes,
                    static_cast<cudaStream_t>(stream));
+}
+
+md_status md_plan_slices(int k, int limbs, int* bits_out, int* quarters_out) {
+  if (k <= 0 || !bits_out || !quarters_out) return MD_ERR_BAD_ARG;
+  if (limbs != 2 && limbs != 4 && limbs != 8 && limbs != 16) return MD_ERR_BAD_ARG;
+  // the fewest slices Q with a kernel, at the widest W the exactness budget allows for (k, Q), whose window W * Q covers
+  // the paper's 13 * 4 * limbs bits; the paper's own (13, 4 * limbs) when nothing better qualifies
+  for (int Q = 1; Q < 4 * limbs; Q++) {
+    if (!(md::qgemm_supported(limbs, Q) || md::qgemm_wide_supported(limbs, Q))) continue;
+    int W = MD_MAX_BITS;
+    while (W >= MD_MIN_BITS && !k_budget_ok(k, Q, W)) W--;
+    if (W >= MD_MIN_BITS && W * Q >= 52 * limbs) {
+      *bits_out = W;
+      *quarters_out = Q;
+      return MD_OK;
+    }
+  }
+  if (!k_budget_ok(k, 4 * limbs, 13)) return MD_ERR_K_TOO_LARGE;
+  *bits_out = 13;
+  *quarters_out = 4 * limbs;
+  return MD_OK;
 }
 
 size_t md_host_scratch_bytes(int m, int n, int k, int limbs) {
@@ -285,7 +317,7 @@ const char* md_status_string(md_status status) {
   switch (status) {
     case MD_OK: return "MD_OK";
     case MD_ERR_BAD_ARG: return "MD_ERR_BAD_ARG: null/misaligned pointer, bad dimension, or unsupported limbs/quarters/orders value";
-    case MD_ERR_K_TOO_LARGE: return "MD_ERR_K_TOO_LARGE: k * orders exceeds 2^27, fp64 accumulation would not be exact";
+    case MD_ERR_K_TOO_LARGE: return "MD_ERR_K_TOO_LARGE: k * orders * 2^(2 * slice bits) exceeds 2^53 (k * orders > 2^27 for 13-bit quarters), fp64 accumulation would not be exact";
     case MD_ERR_WORKSPACE: return "MD_ERR_WORKSPACE: workspace missing or too small (md_workspace_bytes / md_host_scratch_bytes)";
     case MD_ERR_CUDA: return "MD_ERR_CUDA: a CUDA call failed (see cudaGetLastError)";
     case MD_ERR_UNSUPPORTED: return "MD_ERR_UNSUPPORTED: no kernel for this (limbs, quarters, orders)";

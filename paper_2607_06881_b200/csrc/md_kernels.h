@@ -6,11 +6,12 @@
 
 namespace md {
 
-// `quarters` only sets the lower bound of the exponent range that is flagged (exponent_floor)
-cudaError_t launch_exponents(int rows, int cols, int axis, int quarters, const double* lead_plane, int32_t* exps,
-                             uint32_t* flags, cudaStream_t stream, uint64_t* launches);
-int exponent_floor(int quarters);
-cudaError_t launch_split(int rows, int cols, int limbs, int quarters, int axis, const double* planes,
+// `bits` = slice width W (13 = the paper's quarter; R13).  In launch_exponents `quarters` and `bits` only set
+// the lower bound of the exponent range that is flagged (exponent_floor).
+cudaError_t launch_exponents(int rows, int cols, int axis, int quarters, int bits, const double* lead_plane,
+                             int32_t* exps, uint32_t* flags, cudaStream_t stream, uint64_t* launches);
+int exponent_floor(int quarters, int bits);
+cudaError_t launch_split(int rows, int cols, int limbs, int quarters, int bits, int axis, const double* planes,
                          double* quarter_planes, const int32_t* exps, uint32_t* flags, cudaStream_t stream,
                          uint64_t* launches);
 cudaError_t launch_renorm(int m, int n, int limbs, int orders, const double* order_planes, double* C_planes,
@@ -21,7 +22,7 @@ cudaError_t launch_qgemm(int m, int n, int k, int limbs, int quarters, const dou
 bool qgemm_supported(int limbs, int quarters);
 // md_gemm's internal pair: splitter writing the fragment-major packed layout (md_packed.cuh) and the bulk-copy /
 // mbarrier pipelined fused GEMM reading it.  Same (limbs, quarters) support as launch_qgemm.
-cudaError_t launch_split_packed(int rows, int cols, int limbs, int quarters, int axis, const double* planes,
+cudaError_t launch_split_packed(int rows, int cols, int limbs, int quarters, int bits, int axis, const double* planes,
                                 double* packed, const int32_t* exps, uint32_t* flags, cudaStream_t stream,
                                 uint64_t* launches);
 // sk_ws: sk_workspace_bytes(limbs, quarters) bytes of device scratch for the stream-K tail (slab counters + one

@@ -179,17 +179,22 @@ template <int Q> using CfgQD = Cfg<Q, 4, 32, 16, 8, 4, 2>;
 }  // namespace
 
 bool qgemm_supported(int limbs, int quarters) {
-  return (limbs == 2 && quarters >= 8 && quarters <= 10) || (limbs == 4 && quarters >= 16 && quarters <= 18);
+  // 8-10 / 16-18: the paper's 13-bit quarters (R5); 6, 7 / 11, 12: wider slices (MD_OPT_SLICE_BITS, R13)
+  return (limbs == 2 && quarters >= 6 && quarters <= 10) || (limbs == 4 && ((quarters >= 16 && quarters <= 18) || quarters == 11 || quarters == 12));
 }
 
 cudaError_t launch_qgemm(int m, int n, int k, int limbs, int quarters, const double* Aq, const double* Bq,
                          double* order_planes, double* C_planes, cudaStream_t stream, uint64_t* launches) {
   cudaError_t err = cudaErrorInvalidValue;
   if (limbs == 2) {
+    if (quarters == 6) err = launch_cfg<CfgDD<6>>(m, n, k, Aq, Bq, order_planes, C_planes, stream);
+    if (quarters == 7) err = launch_cfg<CfgDD<7>>(m, n, k, Aq, Bq, order_planes, C_planes, stream);
     if (quarters == 8) err = launch_cfg<CfgDD<8>>(m, n, k, Aq, Bq, order_planes, C_planes, stream);
     if (quarters == 9) err = launch_cfg<CfgDD<9>>(m, n, k, Aq, Bq, order_planes, C_planes, stream);
     if (quarters == 10) err = launch_cfg<CfgDD<10>>(m, n, k, Aq, Bq, order_planes, C_planes, stream);
   } else if (limbs == 4) {
+    if (quarters == 11) err = launch_cfg<CfgQD<11>>(m, n, k, Aq, Bq, order_planes, C_planes, stream);
+    if (quarters == 12) err = launch_cfg<CfgQD<12>>(m, n, k, Aq, Bq, order_planes, C_planes, stream);
     if (quarters == 16) err = launch_cfg<CfgQD<16>>(m, n, k, Aq, Bq, order_planes, C_planes, stream);
     if (quarters == 17) err = launch_cfg<CfgQD<17>>(m, n, k, Aq, Bq, order_planes, C_planes, stream);
     if (quarters == 18) err = launch_cfg<CfgQD<18>>(m, n, k, Aq, Bq, order_planes, C_planes, stream);

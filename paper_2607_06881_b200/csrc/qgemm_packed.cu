@@ -334,10 +334,14 @@ cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, co
                                 uint64_t* launches) {
   cudaError_t err = cudaErrorInvalidValue;
   if (limbs == 2) {
+    if (quarters == 6) err = launch_cfg<PCfgDD<6>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
+    if (quarters == 7) err = launch_cfg<PCfgDD<7>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
     if (quarters == 8) err = launch_cfg<PCfgDD<8>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
     if (quarters == 9) err = launch_cfg<PCfgDD<9>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
     if (quarters == 10) err = launch_cfg<PCfgDD<10>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
   } else if (limbs == 4) {
+    if (quarters == 11) err = launch_cfg<PCfgQD<11>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
+    if (quarters == 12) err = launch_cfg<PCfgQD<12>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
     if (quarters == 16) err = launch_cfg<PCfgQD<16>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
     if (quarters == 17) err = launch_cfg<PCfgQD<17>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
     if (quarters == 18) err = launch_cfg<PCfgQD<18>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);

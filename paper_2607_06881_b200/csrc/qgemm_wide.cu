@@ -365,12 +365,13 @@ cudaError_t launch_wide_cfg(int m, int n, int k, const double* Ap, const double*
 }
 
 using WCfgOD = WCfg<32, 8, 4, 2, 1>;   // octo double: 32 x 16 CTA tile, 8 tiles x 1 range
+using WCfgOD22 = WCfg<22, 8, 4, 2, 1>; // octo double in 22 slices of 19 bits (MD_OPT_SLICE_BITS; R13)
 using WCfgHD = WCfg<64, 16, 2, 1, 4>;  // hexa double: 16 x 8 CTA tile, 2 tiles x 4 ranges
 
 }  // namespace
 
 bool qgemm_wide_supported(int limbs, int quarters) {
-  return (limbs == 8 && quarters == 32) || (limbs == 16 && quarters == 64);
+  return (limbs == 8 && (quarters == 32 || quarters == 22)) || (limbs == 16 && quarters == 64);
 }
 
 cudaError_t launch_qgemm_wide(int m, int n, int k, int limbs, int quarters, const double* Ap, const double* Bp,
@@ -378,6 +379,7 @@ cudaError_t launch_qgemm_wide(int m, int n, int k, int limbs, int quarters, cons
                               uint64_t* launches) {
   cudaError_t err = cudaErrorInvalidValue;
   if (limbs == 8 && quarters == 32) err = launch_wide_cfg<WCfgOD>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
+  if (limbs == 8 && quarters == 22) err = launch_wide_cfg<WCfgOD22>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
   if (limbs == 16 && quarters == 64) err = launch_wide_cfg<WCfgHD>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
   if (err == cudaSuccess) *launches += 1;
   return err;

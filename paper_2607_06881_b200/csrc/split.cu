@@ -62,12 +62,13 @@ __global__ void col_exponent_finalize_kernel(int cols, int32_t* exps, uint32_t* 
 }
 
 // Algorithm S, step S1 (DESIGN.md section 3 R4): digit q of the element whose remainder limbs are r[0..L-1], group exponent E:
-//   c = 3*2^51 * u_q (so that ulp(c) = u_q = 2^(E - 13(q+1)));  d_q = (r_0 + c) - c;  r_0 -= d_q;  carry r through the limbs.
-// Every operation is exact except r_0 + c, whose rounding IS the digit selection.
+//   c = 3*2^51 * u_q (so that ulp(c) = u_q = 2^(E - W(q+1)));  d_q = (r_0 + c) - c;  r_0 -= d_q;  carry r through the limbs.
+// Every operation is exact except r_0 + c, whose rounding IS the digit selection.  W = `bits`, the slice width: 13 for the
+// paper's quarters, other widths under MD_OPT_SLICE_BITS (R13).
 template <int L>
-__device__ __forceinline__ double extract_digit(double (&r)[L], int E, int q) {
-  // c = 1.5 * 2^(E - 13(q+1) + 52): exponent field + the top mantissa bit
-  const long long cbits = ((long long)(E - 13 * (q + 1) + 52 + 1023) << 52) | (1ll << 51);
+__device__ __forceinline__ double extract_digit(double (&r)[L], int E, int q, int bits) {
+  // c = 1.5 * 2^(E - W(q+1) + 52): exponent field + the top mantissa bit
+  const long long cbits = ((long long)(E - bits * (q + 1) + 52 + 1023) << 52) | (1ll << 51);
   const double c = __longlong_as_double(cbits);
   const double t = __dadd_rn(r[0], c);
   const double d = __dsub_rn(t, c);
@@ -87,7 +88,7 @@ __device__ __forceinline__ bool any_nonfinite(const double (&r)[L]) {
 
 // md_split: plain [quarters][rows][cols] output.  VEC elements per thread.
 template <int L, int VEC>
-__global__ void __launch_bounds__(256) split_kernel(size_t rows, size_t cols, int Q, int axis,
+__global__ void __launch_bounds__(256) split_kernel(size_t rows, size_t cols, int Q, int bits, int axis,
                                                     const double* __restrict__ planes, double* __restrict__ qplanes,
                                                     const int32_t* __restrict__ exps, uint32_t* flags) {
   const size_t plane = rows * cols;
@@ -119,7 +120,7 @@ __global__ void __launch_bounds__(256) split_kernel(size_t rows, size_t cols, in
   for (int q = 0; q < Q; q++) {
     double d[VEC];
 #pragma unroll
-    for (int v = 0; v < VEC; v++) d[v] = extract_digit<L>(r[v], E[v], q);
+    for (int v = 0; v < VEC; v++) d[v] = extract_digit<L>(r[v], E[v], q, bits);
     if (VEC == 2)
       *reinterpret_cast<double2*>(qplanes + (size_t)q * plane + idx) = make_double2(d[0], d[VEC - 1]);
     else
@@ -142,7 +143,7 @@ __device__ __forceinline__ void stg_256(double* p, double a, double b, double c,
 // contraction indices k = 4*k4g .. 4*k4g+3, i.e. 32 contiguous output bytes per quarter; the 32 lanes of a warp take 32
 // consecutive x, so a warp writes 1 KB contiguous per quarter (and, for B, reads 256 contiguous bytes per row).
 template <int L, int AXIS>
-__global__ void __launch_bounds__(256) split_packed_kernel(int rows, int cols, int Q, int bx, int bk, int x_blocks, int KS,
+__global__ void __launch_bounds__(256) split_packed_kernel(int rows, int cols, int Q, int bits, int bx, int bk, int x_blocks, int KS,
                                                            const double* __restrict__ planes,
                                                            double* __restrict__ packed,
                                                            const int32_t* __restrict__ exps, uint32_t* flags) {
@@ -188,23 +189,23 @@ __global__ void __launch_bounds__(256) split_packed_kernel(int rows, int cols, i
   for (int q = 0; q < Q; q++) {
     double d[4];
 #pragma unroll
-    for (int t = 0; t < 4; t++) d[t] = extract_digit<L>(r[t], E, q);
+    for (int t = 0; t < 4; t++) d[t] = extract_digit<L>(r[t], E, q, bits);
     stg_256(dst + q * q_stride, d[0], d[1], d[2], d[3]);  // a fragment row; the warp writes 1 KB contiguous
   }
 }
 
 }  // namespace
 
-// Lowest group exponent at which every kept quarter product 2^(E_i + F_j - 13(s+2)), s < quarters, is still a normal
+// Lowest group exponent at which every kept quarter product 2^(E_i + F_j - W(s+2)), s < quarters, is still a normal
 // double when both groups sit at the bound; -EXP_LIMIT for the paper's dd / qd quarter counts.
-int exponent_floor(int quarters) {
-  const int lo = -(1022 - 13 * (quarters + 1)) / 2;
-  return quarters <= 24 || lo < -EXP_LIMIT ? -EXP_LIMIT : lo;
+int exponent_floor(int quarters, int bits) {
+  const int lo = -(1022 - bits * (quarters + 1)) / 2;
+  return bits * quarters <= 13 * 24 || lo < -EXP_LIMIT ? -EXP_LIMIT : lo;
 }
 
-cudaError_t launch_exponents(int rows, int cols, int axis, int quarters, const double* lead, int32_t* exps,
+cudaError_t launch_exponents(int rows, int cols, int axis, int quarters, int bits, const double* lead, int32_t* exps,
                              uint32_t* flags, cudaStream_t stream, uint64_t* launches) {
-  const int exp_lo = exponent_floor(quarters);
+  const int exp_lo = exponent_floor(quarters, bits);
   if (axis == 0) {
     row_exponent_kernel<<<min(rows, 148 * 64), 256, 0, stream>>>(rows, cols, lead, exps, flags, exp_lo);
     *launches += 1;
@@ -225,7 +226,7 @@ cudaError_t launch_exponents(int rows, int cols, int axis, int quarters, const d
   return cudaGetLastError();
 }
 
-cudaError_t launch_split(int rows, int cols, int limbs, int quarters, int axis, const double* planes,
+cudaError_t launch_split(int rows, int cols, int limbs, int quarters, int bits, int axis, const double* planes,
                          double* qplanes, const int32_t* exps, uint32_t* flags, cudaStream_t stream,
                          uint64_t* launches) {
   const size_t total = (size_t)rows * cols;
@@ -233,8 +234,8 @@ cudaError_t launch_split(int rows, int cols, int limbs, int quarters, int axis, 
   const size_t threads = vec ? total / 2 : total;
   const unsigned blocks = (unsigned)((threads + 255) / 256);
 #define MD_SPLIT(L_)                                                                                              \
-  if (vec) split_kernel<L_, 2><<<blocks, 256, 0, stream>>>(rows, cols, quarters, axis, planes, qplanes, exps, flags); \
-  else split_kernel<L_, 1><<<blocks, 256, 0, stream>>>(rows, cols, quarters, axis, planes, qplanes, exps, flags);
+  if (vec) split_kernel<L_, 2><<<blocks, 256, 0, stream>>>(rows, cols, quarters, bits, axis, planes, qplanes, exps, flags); \
+  else split_kernel<L_, 1><<<blocks, 256, 0, stream>>>(rows, cols, quarters, bits, axis, planes, qplanes, exps, flags);
   switch (limbs) {
     case 1: MD_SPLIT(1) break;
     case 2: MD_SPLIT(2) break;
@@ -248,7 +249,7 @@ cudaError_t launch_split(int rows, int cols, int limbs, int quarters, int axis, 
   return cudaGetLastError();
 }
 
-cudaError_t launch_split_packed(int rows, int cols, int limbs, int quarters, int axis, const double* planes,
+cudaError_t launch_split_packed(int rows, int cols, int limbs, int quarters, int bits, int axis, const double* planes,
                                 double* packed, const int32_t* exps, uint32_t* flags, cudaStream_t stream,
                                 uint64_t* launches) {
   const int X = axis == 0 ? rows : cols, K = axis == 0 ? cols : rows;
@@ -260,7 +261,7 @@ cudaError_t launch_split_packed(int rows, int cols, int limbs, int quarters, int
   const long long blocks = (long long)x_blocks * k_blocks;
   if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
 #define MD_SPLITP(L_, AX_)                                                                                           \
-  split_packed_kernel<L_, AX_><<<(unsigned)blocks, 256, 0, stream>>>(rows, cols, quarters, bx, bk, x_blocks, KS, planes, \
+  split_packed_kernel<L_, AX_><<<(unsigned)blocks, 256, 0, stream>>>(rows, cols, quarters, bits, bx, bk, x_blocks, KS, planes, \
                                                                      packed, exps, flags)
   if (limbs == 2 && axis == 0) MD_SPLITP(2, 0);
   else if (limbs == 2 && axis == 1) MD_SPLITP(2, 1);

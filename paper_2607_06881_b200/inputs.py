@@ -36,6 +36,9 @@ class Config:
     # (PAPER.md:73, :80); config 3 "stresses balancing/quarter count" (BASELINE.json) and is run with 9, see
     # DESIGN.md reading R5.  This is a parameter handed to md_set_option, not part of the input data.
     quarters: int = 0
+    # Slice width in bits: 13 = the paper's quarter.  Other widths are the k-adaptive variant (DESIGN.md
+    # R13), again a parameter handed to md_set_option, not part of the input data.
+    bits: int = 13
 
     def __post_init__(self):
         if self.quarters == 0:
@@ -55,6 +58,9 @@ class Config:
     def md_flops(self) -> int:
         """2mnk multiple-double flops (BASELINE.json `metric`)."""
         return 2 * self.m * self.n * self.k
+
+    def with_slices(self, bits: int, quarters: int) -> "Config":
+        return dataclasses.replace(self, bits=bits, quarters=quarters)
 
     def with_shape(self, m=None, n=None, k=None) -> "Config":
         return dataclasses.replace(self, m=m or self.m, n=n or self.n, k=k or self.k)

@@ -84,3 +84,44 @@ def test_options_and_workspace_sizes(lib):
     assert lib.md_set_option(99, 1) == md.MD_ERR_BAD_ARG and lib.md_set_option(md.MD_OPT_QUARTERS, 99) == md.MD_ERR_BAD_ARG
     assert lib.md_set_workspace(None, 16) == md.MD_ERR_BAD_ARG
     assert lib.md_set_workspace(None, 0) == 0
+
+
+def test_plan_slices_matches_a_brute_force_search(lib):
+    """md_plan_slices (host only; R13): fewest slices Q that has a kernel, at the widest W with
+    k * Q * 2^(2W) <= 2^53 (eq. 5 generalised), such that W * Q >= 13 * 4 * limbs (the paper's window,
+    PAPER.md:47, :73); else the paper's (13, 4 * limbs).  Restated here as a plain search over all (Q, W)."""
+    have = {2: (6, 7, 8, 9, 10), 4: (11, 12, 16, 17, 18), 8: (22, 32), 16: (64,)}
+    for limbs in (2, 4, 8, 16):
+        for k in (1, 64, 512, 1024, 2048, 4096, 5461, 5462, 8192, 2 ** 15, 2 ** 18, 2 ** 20):
+            best = None
+            for Q in have[limbs]:
+                if Q >= 4 * limbs:
+                    continue
+                ok = [W for W in range(4, 25) if k * Q * 2 ** (2 * W) <= 2 ** 53 and W * Q >= 52 * limbs]
+                if ok:
+                    best = (max(ok), Q)
+                    break
+            want = best or (13, 4 * limbs)
+            assert md.md_plan_slices(k, limbs) == want, (limbs, k)
+    assert md.md_plan_slices(4096, 2) == (19, 6) and md.md_plan_slices(2048, 4) == (19, 11)
+    assert md.md_plan_slices(1024, 8) == (19, 22) and md.md_plan_slices(512, 16) == (13, 64)
+    fake_int = ctypes.c_int(0)
+    assert lib.md_plan_slices(0, 2, ctypes.addressof(fake_int), ctypes.addressof(fake_int)) == md.MD_ERR_BAD_ARG
+    assert lib.md_plan_slices(8, 3, ctypes.addressof(fake_int), ctypes.addressof(fake_int)) == md.MD_ERR_BAD_ARG
+
+
+def test_slice_bits_option_and_its_k_budget(lib):
+    fake = ctypes.c_void_p(4096)
+    assert lib.md_set_option(md.MD_OPT_SLICE_BITS, 3) == md.MD_ERR_BAD_ARG
+    assert lib.md_set_option(md.MD_OPT_SLICE_BITS, 25) == md.MD_ERR_BAD_ARG
+    try:
+        assert lib.md_set_option(md.MD_OPT_SLICE_BITS, 19) == md.MD_OK and lib.md_get_option(md.MD_OPT_SLICE_BITS) == 19
+        assert lib.md_set_option(md.MD_OPT_QUARTERS, 6) == md.MD_OK
+        # k * 6 * 2^38 <= 2^53  <=>  k <= 5461
+        assert lib.md_gemm(1, 1, 5462, 2, fake, fake, fake, None) == md.MD_ERR_K_TOO_LARGE
+        assert lib.md_gemm(1, 1, 5461, 2, fake, fake, fake, None) == md.MD_ERR_WORKSPACE
+        assert lib.md_set_option(md.MD_OPT_QUARTERS, 5) == md.MD_OK
+        assert lib.md_gemm(1, 1, 64, 2, fake, fake, fake, None) == md.MD_ERR_UNSUPPORTED
+    finally:
+        lib.md_set_option(md.MD_OPT_SLICE_BITS, 0)
+        lib.md_set_option(md.MD_OPT_QUARTERS, 0)
