@@ -58,13 +58,16 @@ enum {
                            limbs=2: 8, 9, 10; limbs=4: 16, 17, 18 (R5). */
   MD_OPT_ORDERS = 2,    /* kept product orders S (the paper's C_1..C_S).  Default = quarters.  Must equal
                            quarters in this version. */
-  MD_OPT_SLICE_BITS = 3 /* width W of a slice in bits, used by md_split and the md_gemm family.  Default 13: the paper's
+  MD_OPT_SLICE_BITS = 3, /* width W of a slice in bits, used by md_split and the md_gemm family.  Default 13: the paper's
                            quarter ("4 parts ... each of 13 bits").  Other widths (4..24) are the k-adaptive
                            variant of DESIGN.md R13 / SURVEY.md 8(f) NEXT-3 -- NOT the paper's quarters: a slice of W
                            bits sits on the unit 2^(E_g - W(q+1)), |D| <= 2^W (q = 0), 2^(W-1) (q > 0), and the
                            exactness budget becomes k * orders * 2^(2W) <= 2^53.  With wider slices fewer are needed:
                            set MD_OPT_QUARTERS to the slice count (limbs=2: 6, 7; limbs=4: 11, 12; limbs=8: 22), or
                            take both from md_plan_slices. */
+  MD_OPT_HOST_BLOCKS = 4 /* md_gemm_host only: number of blocks C is cut into for overlapping copies and kernels.
+                            Default 0 = automatic (about one wave of CTA tiles per block, at most 32); 1 = no overlap;
+                            PR * 256 + PC = explicit numbers of row panels and column panels (each <= 64). */
 };
 md_status md_set_option(int key, int value);
 int md_get_option(int key); /* current value (0 = default), or -1 for an unknown key */
@@ -148,10 +151,13 @@ md_status md_read_flags(uint32_t* flags_host, md_stream stream);
 
 /* ---------------------------------------------------------------------------------------------------------------------
  * md_gemm_host -- md_gemm on HOST buffers (end-to-end path).  A_host, B_host, C_host are HOST pointers (pinned memory
- *   makes the copies asynchronous and fast; pageable works).  dev_scratch is DEVICE memory of at least
+ *   makes the copies asynchronous and fast; pageable works, without overlap).  dev_scratch is DEVICE memory of at least
  *   md_host_scratch_bytes(m,n,k,limbs) bytes, 256-byte aligned, owned by the caller; it receives the device copies of
- *   A, B, C and the workspace.  Copies A and B to the device, runs md_gemm, copies C back, all on `stream`, then
- *   SYNCHRONISES the stream: C_host is complete on return.
+ *   A, B, C and the workspace.  C is cut into blocks (row panels of A x column panels of B; a row's / column's exponent
+ *   depends on that row / column only, so each block is an independent md_gemm with bit-identical results) and the
+ *   copies in, the kernels and the copies out of successive blocks overlap: kernels run on `stream`, the copies on two
+ *   streams the library creates on first use and keeps (the only resources it ever creates).  Work already enqueued on
+ *   `stream` is waited for first; the call SYNCHRONISES `stream` before returning: C_host is complete on return.
  * ------------------------------------------------------------------------------------------------------------------ */
 size_t md_host_scratch_bytes(int m, int n, int k, int limbs);
 md_status md_gemm_host(int m, int n, int k, int limbs, const double* A_host, const double* B_host, double* C_host,

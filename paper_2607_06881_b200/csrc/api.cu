@@ -15,6 +15,7 @@ struct State {
   int opt_quarters = 0;  // 0 = default (4 * limbs)
   int opt_orders = 0;    // 0 = default (= quarters)
   int opt_bits = 0;      // 0 = default (13, the paper's quarter)
+  int opt_host_blocks = 0;  // md_gemm_host: 0 = automatic panel plan, else the number of blocks of C (1 = no pipelining)
   void* ws = nullptr;
   size_t ws_bytes = 0;
 };
@@ -110,11 +111,65 @@ md_status gemm_impl(int m, int n, int k, int limbs, const double* A, const doubl
   return err == cudaSuccess ? MD_OK : MD_ERR_CUDA;
 }
 
+
+// ---- md_gemm_host: panel plan and the library's two copy streams ------------------------------------------------------
+struct HostPanels {
+  int PR, PC;  // row panels of A / C, column panels of B / C
+  int mp, np;  // rows / columns per panel (multiples of the CTA tile; the last panel takes what is left)
+};
+// About one wave of CTA tiles per block, at most 32 blocks (the stream-K tail keeps a short block efficient; measured on
+// dd 4096^3: 8 x 4 blocks 138.4 ms, 4 x 2 140.0 ms, 1 block 150.2 ms against 135.1 ms of kernels alone); four column
+// panels from 16 blocks up, two from 4, so that the first kernel waits for a fraction of B only.
+HostPanels plan_host_panels(int m, int n, int limbs) {
+  const int bxA = md::pack_bx(limbs, 0), bxB = md::pack_bx(limbs, 1);
+  const long long tm = (m + bxA - 1) / bxA, tn = (n + bxB - 1) / bxB;
+  int G = md::sk_grid();
+  if (G <= 0) G = 148;
+  long long blocks = (tm * tn + G - 1) / G;
+  if (g_state.opt_host_blocks > 0) blocks = g_state.opt_host_blocks;
+  blocks = blocks < 1 ? 1 : blocks > 32 ? 32 : blocks;
+  HostPanels hp;
+  hp.PC = blocks >= 16 ? 4 : blocks >= 4 ? 2 : 1;
+  hp.PR = (int)(blocks / hp.PC);
+  if (g_state.opt_host_blocks >= 256) hp.PR = g_state.opt_host_blocks >> 8, hp.PC = g_state.opt_host_blocks & 255;  // PR * 256 + PC
+  if (hp.PR < 1) hp.PR = 1;
+  if (hp.PC < 1) hp.PC = 1;
+  if (hp.PC > tn) hp.PC = (int)tn;
+  if (hp.PR > tm) hp.PR = (int)tm;
+  hp.mp = (int)((tm + hp.PR - 1) / hp.PR) * bxA;
+  hp.np = (int)((tn + hp.PC - 1) / hp.PC) * bxB;
+  hp.PR = (m + hp.mp - 1) / hp.mp;
+  hp.PC = (n + hp.np - 1) / hp.np;
+  return hp;
+}
+
+struct HostPipeline {
+  cudaStream_t in = nullptr, out = nullptr;
+  std::vector<cudaEvent_t> ev;
+};
+HostPipeline g_host;
+// streams and events are created on first use and kept (no device memory is allocated)
+bool host_pipeline_ready(int events) {
+  if (!g_host.in && cudaStreamCreateWithFlags(&g_host.in, cudaStreamNonBlocking) != cudaSuccess) return false;
+  if (!g_host.out && cudaStreamCreateWithFlags(&g_host.out, cudaStreamNonBlocking) != cudaSuccess) return false;
+  while ((int)g_host.ev.size() < events) {
+    cudaEvent_t e;
+    if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) return false;
+    g_host.ev.push_back(e);
+  }
+  return true;
+}
+
 }  // namespace
 
 extern "C" {
 
 md_status md_set_option(int key, int value) {
+  if (key == MD_OPT_HOST_BLOCKS) {  // 0 = automatic, 1..32 blocks, or PR * 256 + PC (explicit panel counts, each <= 64)
+    if (value < 0 || (value > 32 && (value < 256 || (value >> 8) > 64 || (value & 255) > 64))) return MD_ERR_BAD_ARG;
+    g_state.opt_host_blocks = value;
+    return MD_OK;
+  }
   if (value < 0 || value > MD_MAX_QUARTERS) return MD_ERR_BAD_ARG;
   switch (key) {
     case MD_OPT_SLICE_BITS:
@@ -132,6 +187,7 @@ int md_get_option(int key) {
     case MD_OPT_QUARTERS: return g_state.opt_quarters;
     case MD_OPT_ORDERS: return g_state.opt_orders;
     case MD_OPT_SLICE_BITS: return g_state.opt_bits;
+    case MD_OPT_HOST_BLOCKS: return g_state.opt_host_blocks;
     default: return -1;
   }
 }
@@ -253,6 +309,7 @@ md_status md_gemm_host(int m, int n, int k, int limbs, const double* A_host, con
   if (!dev_scratch || reinterpret_cast<uintptr_t>(dev_scratch) % ALIGN) return MD_ERR_BAD_ARG;
   if (scratch_bytes < md_host_scratch_bytes(m, n, k, limbs)) return MD_ERR_WORKSPACE;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const int Q = quarters_for(limbs), W = slice_bits();
   const size_t a_bytes = sizeof(double) * (size_t)limbs * m * k, b_bytes = sizeof(double) * (size_t)limbs * k * n,
                c_bytes = sizeof(double) * (size_t)limbs * m * n;
   char* p = static_cast<char*>(dev_scratch);
@@ -260,14 +317,102 @@ md_status md_gemm_host(int m, int n, int k, int limbs, const double* A_host, con
   double* dB = reinterpret_cast<double*>(p + round_up(a_bytes));
   double* dC = reinterpret_cast<double*>(p + round_up(a_bytes) + round_up(b_bytes));
   char* ws = p + round_up(a_bytes) + round_up(b_bytes) + round_up(c_bytes);
-  const size_t ws_bytes = scratch_bytes - (size_t)(ws - p);
-  if (cudaMemsetAsync(ws, 0, ALIGN, st) != cudaSuccess) return MD_ERR_CUDA;
-  if (cudaMemcpyAsync(dA, A_host, a_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return MD_ERR_CUDA;
-  if (cudaMemcpyAsync(dB, B_host, b_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return MD_ERR_CUDA;
-  const md_status run = gemm_impl(m, n, k, limbs, dA, dB, dC, nullptr, ws, ws_bytes, st);
-  if (run != MD_OK) return run;
-  if (cudaMemcpyAsync(C_host, dC, c_bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return MD_ERR_CUDA;
-  return cudaStreamSynchronize(st) == cudaSuccess ? MD_OK : MD_ERR_CUDA;
+  const Carve c = carve(ws, m, n, k, limbs, Q);
+
+  // Panels: C is cut into PR x PC blocks (rows of A x columns of B).  A row's exponent and quarters depend on that row of A
+  // only, a column's on that column of B only, so every block is an independent md_gemm on COMPACT
+  // device copies of its operands: panel i of A is [limbs][mi][k] at dA + limbs * row0 * k, panel j of B is [limbs][k][nj]
+  // at dB + limbs * k * col0, block (i, j) of C is [limbs][mi][nj].  Three streams: copies in (in order of first use),
+  // the kernels (the caller's stream), copies out; the first kernel starts after A_0 and B_0 have arrived and the last
+  // copy out is one block of C, instead of the whole of A, B before and the whole of C after.
+  const HostPanels hp = plan_host_panels(m, n, limbs);
+  if (!host_pipeline_ready(hp.PR + hp.PC + hp.PR * hp.PC + 2)) return MD_ERR_CUDA;
+  cudaStream_t s_in = g_host.in, s_out = g_host.out;
+  cudaEvent_t* ev = g_host.ev.data();
+  cudaEvent_t ev_start = ev[0], ev_done = ev[1];
+  cudaEvent_t* ev_A = ev + 2;
+  cudaEvent_t* ev_B = ev_A + hp.PR;
+  cudaEvent_t* ev_C = ev_B + hp.PC;
+#define MD_TRY(call) \
+  if ((call) != cudaSuccess) return MD_ERR_CUDA
+  MD_TRY(cudaMemsetAsync(ws, 0, ALIGN, st));  // the status word
+  MD_TRY(cudaEventRecord(ev_start, st));
+  MD_TRY(cudaStreamWaitEvent(s_in, ev_start, 0));
+  MD_TRY(cudaStreamWaitEvent(s_out, ev_start, 0));
+  auto rows_of = [&](int i, int& r0, int& mi) { r0 = i * hp.mp, mi = (r0 + hp.mp <= m ? hp.mp : m - r0); };
+  auto cols_of = [&](int j, int& c0, int& nj) { c0 = j * hp.np, nj = (c0 + hp.np <= n ? hp.np : n - c0); };
+  auto copy_in_A = [&](int i) -> cudaError_t {
+    int r0, mi;
+    rows_of(i, r0, mi);
+    double* dst = dA + (size_t)limbs * r0 * k;
+    for (int l = 0; l < limbs; l++) {
+      cudaError_t e = cudaMemcpyAsync(dst + (size_t)l * mi * k, A_host + (size_t)l * m * k + (size_t)r0 * k,
+                                      sizeof(double) * (size_t)mi * k, cudaMemcpyHostToDevice, s_in);
+      if (e != cudaSuccess) return e;
+    }
+    return cudaEventRecord(ev_A[i], s_in);
+  };
+  auto copy_in_B = [&](int j) -> cudaError_t {
+    int c0, nj;
+    cols_of(j, c0, nj);
+    double* dst = dB + (size_t)limbs * k * c0;
+    // all limb planes at once: limbs * k rows of nj doubles out of rows of n
+    cudaError_t e = cudaMemcpy2DAsync(dst, sizeof(double) * (size_t)nj, B_host + c0, sizeof(double) * (size_t)n,
+                                      sizeof(double) * (size_t)nj, (size_t)limbs * k, cudaMemcpyHostToDevice, s_in);
+    if (e != cudaSuccess) return e;
+    return cudaEventRecord(ev_B[j], s_in);
+  };
+  // copies in, in the order the blocks (column panel outer, row panel inner) first touch them
+  MD_TRY(copy_in_A(0));
+  MD_TRY(copy_in_B(0));
+  for (int i = 1; i < hp.PR; i++) MD_TRY(copy_in_A(i));
+  for (int j = 1; j < hp.PC; j++) MD_TRY(copy_in_B(j));
+
+  const int bxA = md::pack_bx(limbs, 0), bxB = md::pack_bx(limbs, 1), bk = md::pack_bk(limbs);
+  const size_t KS = ((size_t)k + bk - 1) / bk;
+  const size_t chunkA = (size_t)Q * bk * bxA, chunkB = (size_t)Q * bk * bxB;  // doubles per (tile, k slab)
+  uint64_t launches = 0;
+  cudaError_t err = cudaSuccess;
+  for (int j = 0; j < hp.PC && err == cudaSuccess; j++) {
+    int c0, nj;
+    cols_of(j, c0, nj);
+    const double* Bj = dB + (size_t)limbs * k * c0;
+    double* Bq = c.Bq + (size_t)(c0 / bxB) * KS * chunkB;  // panel boundaries are multiples of the CTA tile
+    MD_TRY(cudaStreamWaitEvent(st, ev_B[j], 0));
+    err = md::launch_exponents(k, nj, 1, Q, W, Bj, c.expB + c0, c.flags, st, &launches);
+    if (err == cudaSuccess) err = md::launch_split_packed(k, nj, limbs, Q, W, 1, Bj, Bq, c.expB + c0, c.flags, st, &launches);
+    for (int i = 0; i < hp.PR && err == cudaSuccess; i++) {
+      int r0, mi;
+      rows_of(i, r0, mi);
+      const double* Ai = dA + (size_t)limbs * r0 * k;
+      double* Aq = c.Aq + (size_t)(r0 / bxA) * KS * chunkA;
+      if (j == 0) {
+        MD_TRY(cudaStreamWaitEvent(st, ev_A[i], 0));
+        err = md::launch_exponents(mi, k, 0, Q, W, Ai, c.expA + r0, c.flags, st, &launches);
+        if (err == cudaSuccess) err = md::launch_split_packed(mi, k, limbs, Q, W, 0, Ai, Aq, c.expA + r0, c.flags, st, &launches);
+        if (err != cudaSuccess) break;
+      }
+      // block (i, j): compact [limbs][mi][nj] at the position its elements have in a row-panel-major walk of C
+      double* Cb = dC + (size_t)limbs * ((size_t)r0 * n + (size_t)mi * c0);
+      err = limbs <= 4 ? md::launch_qgemm_packed(mi, nj, k, limbs, Q, Aq, Bq, nullptr, Cb, c.sk, st, &launches)
+                       : md::launch_qgemm_wide(mi, nj, k, limbs, Q, Aq, Bq, nullptr, Cb, c.sk, st, &launches);
+      if (err != cudaSuccess) break;
+      cudaEvent_t done = ev_C[j * hp.PR + i];
+      MD_TRY(cudaEventRecord(done, st));
+      MD_TRY(cudaStreamWaitEvent(s_out, done, 0));
+      for (int l = 0; l < limbs; l++)
+        MD_TRY(cudaMemcpy2DAsync(C_host + (size_t)l * m * n + (size_t)r0 * n + c0, sizeof(double) * (size_t)n,
+                                 Cb + (size_t)l * mi * nj, sizeof(double) * (size_t)nj, sizeof(double) * (size_t)nj,
+                                 (size_t)mi, cudaMemcpyDeviceToHost, s_out));
+    }
+  }
+  g_launches += launches;
+  // join: the caller's stream waits for the last copy out (and, on an error path, for whatever was enqueued)
+  MD_TRY(cudaEventRecord(ev_done, s_out));
+  MD_TRY(cudaStreamWaitEvent(st, ev_done, 0));
+#undef MD_TRY
+  if (cudaStreamSynchronize(st) != cudaSuccess || err != cudaSuccess) return MD_ERR_CUDA;
+  return MD_OK;
 }
 
 md_status md_profile_enable(int capacity) {

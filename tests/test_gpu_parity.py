@@ -211,6 +211,27 @@ def test_host_entry_point_matches_device_entry_point():
     assert bits_equal(Ch.numpy(), C)
 
 
+@pytest.mark.parametrize("cfg_idx,shape,blocks", [(1, (300, 200, 100), 6), (3, (129, 31, 130), 16), (4, (100, 90, 40), 8),
+                                                  (2, (640, 96, 24), 3), (5, (70, 50, 20), 4)])
+def test_host_entry_point_pipelined_over_blocks_is_bit_identical(cfg_idx, shape, blocks):
+    """md_gemm_host cuts C into row-panel x column-panel blocks and overlaps copies with kernels (include/mdgemm.h): a
+    row's / column's exponent depends on that row / column only, so the blocks reproduce md_gemm bit for bit."""
+    cfg, A, B = gen(cfg_idx, *shape)
+    L = cfg.limbs
+    with md.Workspace(cfg.m, cfg.n, cfg.k, L, cfg.quarters):
+        C = host(md.md_gemm(dev(A), dev(B)))
+        Ah, Bh = torch.from_numpy(A).pin_memory(), torch.from_numpy(B).pin_memory()
+        Ch = torch.full((L, cfg.m, cfg.n), float("nan"), dtype=torch.float64).pin_memory()
+        scratch = torch.empty(md.md_host_scratch_bytes(cfg.m, cfg.n, cfg.k, L), dtype=torch.uint8, device="cuda")
+        md.md_set_option(md.MD_OPT_HOST_BLOCKS, blocks)
+        try:
+            md.md_gemm_host(Ah, Bh, Ch, scratch)
+            md.md_gemm_host(Ah, Bh, Ch, scratch)  # a second call reuses the library's streams and events
+        finally:
+            md.md_set_option(md.MD_OPT_HOST_BLOCKS, 0)
+    assert bits_equal(Ch.numpy(), C)
+
+
 def test_flags_and_runtime_errors():
     cfg, A, B = gen(0, 16, 16, 16)
     A[0, 3, 4] = np.inf
