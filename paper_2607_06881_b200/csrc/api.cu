@@ -64,9 +64,9 @@ Carve carve(void* base, int m, int n, int k, int limbs, int quarters) {
   c.expB = reinterpret_cast<int32_t*>(p + off);
   off += round_up(sizeof(int32_t) * (size_t)n);
   c.Aq = reinterpret_cast<double*>(p + off);
-  off += round_up(sizeof(double) * md::packed_doubles(m, k, md::pack_bx(limbs, 0), md::pack_bk(limbs), quarters));
+  off += round_up(sizeof(double) * md::packed_doubles(m, k, md::pack_bx(limbs, quarters, 0), md::pack_bk(limbs), quarters));
   c.Bq = reinterpret_cast<double*>(p + off);
-  off += round_up(sizeof(double) * md::packed_doubles(n, k, md::pack_bx(limbs, 1), md::pack_bk(limbs), quarters));
+  off += round_up(sizeof(double) * md::packed_doubles(n, k, md::pack_bx(limbs, quarters, 1), md::pack_bk(limbs), quarters));
   c.sk = p + off;
   off += round_up(md::sk_workspace_bytes(limbs, quarters));
   c.total = off;
@@ -120,8 +120,8 @@ struct HostPanels {
 // About one wave of CTA tiles per block, at most 32 blocks (the stream-K tail keeps a short block efficient; measured on
 // dd 4096^3: 8 x 4 blocks 138.4 ms, 4 x 2 140.0 ms, 1 block 150.2 ms against 135.1 ms of kernels alone); four column
 // panels from 16 blocks up, two from 4, so that the first kernel waits for a fraction of B only.
-HostPanels plan_host_panels(int m, int n, int limbs) {
-  const int bxA = md::pack_bx(limbs, 0), bxB = md::pack_bx(limbs, 1);
+HostPanels plan_host_panels(int m, int n, int limbs, int quarters) {
+  const int bxA = md::pack_bx(limbs, quarters, 0), bxB = md::pack_bx(limbs, quarters, 1);
   const long long tm = (m + bxA - 1) / bxA, tn = (n + bxB - 1) / bxB;
   int G = md::sk_grid();
   if (G <= 0) G = 148;
@@ -325,7 +325,7 @@ md_status md_gemm_host(int m, int n, int k, int limbs, const double* A_host, con
   // at dB + limbs * k * col0, block (i, j) of C is [limbs][mi][nj].  Three streams: copies in (in order of first use),
   // the kernels (the caller's stream), copies out; the first kernel starts after A_0 and B_0 have arrived and the last
   // copy out is one block of C, instead of the whole of A, B before and the whole of C after.
-  const HostPanels hp = plan_host_panels(m, n, limbs);
+  const HostPanels hp = plan_host_panels(m, n, limbs, Q);
   if (!host_pipeline_ready(hp.PR + hp.PC + hp.PR * hp.PC + 2)) return MD_ERR_CUDA;
   cudaStream_t s_in = g_host.in, s_out = g_host.out;
   cudaEvent_t* ev = g_host.ev.data();
@@ -368,7 +368,7 @@ md_status md_gemm_host(int m, int n, int k, int limbs, const double* A_host, con
   for (int i = 1; i < hp.PR; i++) MD_TRY(copy_in_A(i));
   for (int j = 1; j < hp.PC; j++) MD_TRY(copy_in_B(j));
 
-  const int bxA = md::pack_bx(limbs, 0), bxB = md::pack_bx(limbs, 1), bk = md::pack_bk(limbs);
+  const int bxA = md::pack_bx(limbs, Q, 0), bxB = md::pack_bx(limbs, Q, 1), bk = md::pack_bk(limbs);
   const size_t KS = ((size_t)k + bk - 1) / bk;
   const size_t chunkA = (size_t)Q * bk * bxA, chunkB = (size_t)Q * bk * bxB;  // doubles per (tile, k slab)
   uint64_t launches = 0;

@@ -279,7 +279,7 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
 template <class C>
 cudaError_t launch_cfg(int m, int n, int k, const double* Ap, const double* Bp, double* order_planes, double* C_planes,
                        void* sk_ws, cudaStream_t stream) {
-  static_assert(C::BM == pack_bx(C::L, 0) && C::BN == pack_bx(C::L, 1), "tile shape must match the packed layout");
+  static_assert(C::BM == pack_bx(C::L, C::Q, 0) && C::BN == pack_bx(C::L, C::Q, 1), "tile shape must match the packed layout");
   const int tiles_m = (m + C::BM - 1) / C::BM, tiles_n = (n + C::BN - 1) / C::BN;
   const long long tiles = (long long)tiles_m * tiles_n;
   if (tiles > 0x7fffffffLL) return cudaErrorInvalidValue;
@@ -310,6 +310,9 @@ cudaError_t launch_cfg(int m, int n, int k, const double* Ap, const double* Bp, 
 // (16 orders x 2 registers per 8x8 tile).
 template <int Q> using PCfgDD = PCfg<Q, 2, 4, 2, 2, 2>;
 template <int Q> using PCfgQD = PCfg<Q, 4, 4, 2, 1, 1>;
+// quad double in 11 / 12 wide slices (MD_OPT_SLICE_BITS): 22 / 24 accumulator registers per 8x8 tile leave room for the
+// double-double warp tile (16 x 16), which halves the LDS and L2 traffic per DMMA and doubles the DMMAs per slab
+template <int Q> using PCfgQDW = PCfg<Q, 4, 4, 2, 2, 2>;
 
 }  // namespace
 
@@ -326,7 +329,7 @@ int sk_grid() {
 }
 
 size_t sk_workspace_bytes(int limbs, int quarters) {
-  return SK_COUNTER_BYTES + sizeof(double) * (size_t)SK_MAX_TILES * quarters * pack_bx(limbs, 0) * pack_bx(limbs, 1);
+  return SK_COUNTER_BYTES + sizeof(double) * (size_t)SK_MAX_TILES * quarters * pack_bx(limbs, quarters, 0) * pack_bx(limbs, quarters, 1);
 }
 
 cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, const double* Ap, const double* Bp,
@@ -340,8 +343,8 @@ cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, co
     if (quarters == 9) err = launch_cfg<PCfgDD<9>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
     if (quarters == 10) err = launch_cfg<PCfgDD<10>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
   } else if (limbs == 4) {
-    if (quarters == 11) err = launch_cfg<PCfgQD<11>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
-    if (quarters == 12) err = launch_cfg<PCfgQD<12>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
+    if (quarters == 11) err = launch_cfg<PCfgQDW<11>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
+    if (quarters == 12) err = launch_cfg<PCfgQDW<12>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
     if (quarters == 16) err = launch_cfg<PCfgQD<16>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
     if (quarters == 17) err = launch_cfg<PCfgQD<17>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
     if (quarters == 18) err = launch_cfg<PCfgQD<18>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);

@@ -343,7 +343,7 @@ qgemm_wide_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, cons
 template <class C>
 cudaError_t launch_wide_cfg(int m, int n, int k, const double* Ap, const double* Bp, double* order_planes,
                             double* C_planes, void* sk_ws, cudaStream_t stream) {
-  static_assert(C::BM == pack_bx(C::L, 0) && C::BN == pack_bx(C::L, 1) && C::BK == pack_bk(C::L),
+  static_assert(C::BM == pack_bx(C::L, C::Q, 0) && C::BN == pack_bx(C::L, C::Q, 1) && C::BK == pack_bk(C::L),
                 "tile shape must match the packed layout");
   const int tiles_m = (m + C::BM - 1) / C::BM, tiles_n = (n + C::BN - 1) / C::BN;
   if ((long long)tiles_m * tiles_n > 0x7fffffffLL) return cudaErrorInvalidValue;

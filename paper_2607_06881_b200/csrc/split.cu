@@ -253,7 +253,7 @@ cudaError_t launch_split_packed(int rows, int cols, int limbs, int quarters, int
                                 double* packed, const int32_t* exps, uint32_t* flags, cudaStream_t stream,
                                 uint64_t* launches) {
   const int X = axis == 0 ? rows : cols, K = axis == 0 ? cols : rows;
-  const int bx = pack_bx(limbs, axis);
+  const int bx = pack_bx(limbs, quarters, axis);
   const int bk = pack_bk(limbs);
   const int KS = (K + bk - 1) / bk;
   const int x_blocks = ((X + bx - 1) / bx * bx + 31) / 32;  // 32 groups per block over the padded extent
