@@ -58,7 +58,7 @@ def parse_args():
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (default 2: the headline)")
     ap.add_argument("--slices", default="paper", choices=["paper", "adaptive"],
                     help="paper: 13-bit quarters, 4 per limb (the headline).  adaptive: the (bits, count) md_plan_slices "
-                         "picks for this k -- wider, fewer slices (DESIGN.md R13; NOT the paper's quarters)")
+                         "picks for this k -- wider, fewer slices (DESIGN.md R14; NOT the paper's quarters)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -275,7 +275,7 @@ def run_ours(args):
                         "value": base.md_flops / (a_ms * 1e-3) / 1e9, "unit": UNIT,
                         "kernel_frac_of_fp64_tensor_peak": aT * base.md_flops / (sum(a_gemm_ms) / 3 * 1e-3) / 1e12 / FP64_TENSOR_PEAK_TFLOPS,
                         "max_abs_diff_vs_paper_quarters": float((C2 - C).abs().sum(dim=0).max()),
-                        "note": "md_plan_slices: wider, fewer slices on the same kernels (DESIGN.md R13); not the paper's "
+                        "note": "md_plan_slices: wider, fewer slices on the same kernels (DESIGN.md R14); not the paper's "
                                 "13-bit quarters, so not the headline; 3 steps after 1 warm-up, CUDA events"}
             del C2
 

@@ -60,7 +60,7 @@ enum {
                            quarters in this version. */
   MD_OPT_SLICE_BITS = 3, /* width W of a slice in bits, used by md_split and the md_gemm family.  Default 13: the paper's
                            quarter ("4 parts ... each of 13 bits").  Other widths (4..24) are the k-adaptive
-                           variant of DESIGN.md R13 / SURVEY.md 8(f) NEXT-3 -- NOT the paper's quarters: a slice of W
+                           variant of DESIGN.md R14 / SURVEY.md 8(f) NEXT-3 -- NOT the paper's quarters: a slice of W
                            bits sits on the unit 2^(E_g - W(q+1)), |D| <= 2^W (q = 0), 2^(W-1) (q > 0), and the
                            exactness budget becomes k * orders * 2^(2W) <= 2^53.  With wider slices fewer are needed:
                            set MD_OPT_QUARTERS to the slice count (limbs=2: 6, 7; limbs=4: 11, 12; limbs=8: 22), or

@@ -15,7 +15,7 @@
 // rational arithmetic in Python, closed forms, hand-derived special cases, the paper's constants):
 //   O1  oracle_exact_*      exact product  C = A*B of multiple-double matrices (plain definition)
 //   O2  oracle_split        Algorithm S: exponent vectors + 13-bit quarters
-//       oracle_*_w          the same with the slice width as a parameter (R13; 13 = the paper's quarter)
+//       oracle_*_w          the same with the slice width as a parameter (R14; 13 = the paper's quarter)
 //   O3  oracle_orders_*     order matrices C^(s) = sum_{p+q=s} A_p B_q  (eq. 3-4)
 //   O4  oracle_renorm       sum of the S order values -> L non-overlapping limbs
 //   O5  oracle_classic_gemm classical multiple-double GEMM on "regular cores", cross-check
@@ -223,7 +223,7 @@ extern "C" {
 //   remainder       [limbs][rows][cols] or NULL: what is left after the last quarter (sum of quarters + remainder
 //                   == element, exactly)
 // =====================================================================================================
-//   oracle_split_w: the same procedure with `bits` in place of 13 (R13: a slice of `bits` bits per part,
+//   oracle_split_w: the same procedure with `bits` in place of 13 (R14: a slice of `bits` bits per part,
 //   unit u_q = 2^(E_g - bits*(q+1)); the paper's quarter is bits = 13 = 52/4).
 void oracle_split_w(int rows, int cols, int limbs, int quarters, int bits, int axis, const double* planes,
                     double* quarter_planes, int32_t* exps, double* remainder) {

@@ -46,7 +46,7 @@ def num_threads() -> int:
 
 def split(planes: np.ndarray, axis: int, quarters: int | None = None, want_remainder: bool = False, bits: int = 13):
     """O2.  planes [limbs, rows, cols] -> (quarter_planes [Q, rows, cols], exps int32, remainder or None).
-    bits = slice width (13 = the paper's quarter; other widths: DESIGN.md R13)."""
+    bits = slice width (13 = the paper's quarter; other widths: DESIGN.md R14)."""
     planes = _f64(planes)
     limbs, rows, cols = planes.shape
     Q = 4 * limbs if quarters is None else quarters

@@ -37,7 +37,7 @@ inline int quarters_for(int limbs) { return g_state.opt_quarters ? g_state.opt_q
 inline int orders_for(int limbs) { return g_state.opt_orders ? g_state.opt_orders : quarters_for(limbs); }
 inline int slice_bits() { return g_state.opt_bits ? g_state.opt_bits : 13; }
 constexpr int MD_MIN_BITS = 4, MD_MAX_BITS = 24;
-// Exactness budget (eq. 5 generalised; R6, R13): order s adds (s+1) <= S products per k, each an
+// Exactness budget (eq. 5 generalised; R6, R14): order s adds (s+1) <= S products per k, each an
 // integer of at most 2^(2W) units, so every partial sum is exactly representable while k * S * 2^(2W) <= 2^53.
 // W = 13: k * S <= 2^27.
 inline bool k_budget_ok(long long k, int S, int bits) { return k * S <= (1ll << (53 - 2 * bits)); }

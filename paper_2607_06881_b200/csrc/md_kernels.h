@@ -6,7 +6,7 @@
 
 namespace md {
 
-// `bits` = slice width W (13 = the paper's quarter; R13).  In launch_exponents `quarters` and `bits` only set
+// `bits` = slice width W (13 = the paper's quarter; R14).  In launch_exponents `quarters` and `bits` only set
 // the lower bound of the exponent range that is flagged (exponent_floor).
 cudaError_t launch_exponents(int rows, int cols, int axis, int quarters, int bits, const double* lead_plane,
                              int32_t* exps, uint32_t* flags, cudaStream_t stream, uint64_t* launches);

@@ -179,7 +179,7 @@ template <int Q> using CfgQD = Cfg<Q, 4, 32, 16, 8, 4, 2>;
 }  // namespace
 
 bool qgemm_supported(int limbs, int quarters) {
-  // 8-10 / 16-18: the paper's 13-bit quarters (R5); 6, 7 / 11, 12: wider slices (MD_OPT_SLICE_BITS, R13)
+  // 8-10 / 16-18: the paper's 13-bit quarters (R5); 6, 7 / 11, 12: wider slices (MD_OPT_SLICE_BITS, R14)
   return (limbs == 2 && quarters >= 6 && quarters <= 10) || (limbs == 4 && ((quarters >= 16 && quarters <= 18) || quarters == 11 || quarters == 12));
 }
 

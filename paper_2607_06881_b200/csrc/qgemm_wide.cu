@@ -365,7 +365,7 @@ cudaError_t launch_wide_cfg(int m, int n, int k, const double* Ap, const double*
 }
 
 using WCfgOD = WCfg<32, 8, 4, 2, 1>;   // octo double: 32 x 16 CTA tile, 8 tiles x 1 range
-using WCfgOD22 = WCfg<22, 8, 4, 2, 1>; // octo double in 22 slices of 19 bits (MD_OPT_SLICE_BITS; R13)
+using WCfgOD22 = WCfg<22, 8, 4, 2, 1>; // octo double in 22 slices of 19 bits (MD_OPT_SLICE_BITS; R14)
 using WCfgHD = WCfg<64, 16, 2, 1, 4>;  // hexa double: 16 x 8 CTA tile, 2 tiles x 4 ranges
 
 }  // namespace

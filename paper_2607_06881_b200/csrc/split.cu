@@ -64,7 +64,7 @@ __global__ void col_exponent_finalize_kernel(int cols, int32_t* exps, uint32_t* 
 // Algorithm S, step S1 (DESIGN.md section 3 R4): digit q of the element whose remainder limbs are r[0..L-1], group exponent E:
 //   c = 3*2^51 * u_q (so that ulp(c) = u_q = 2^(E - W(q+1)));  d_q = (r_0 + c) - c;  r_0 -= d_q;  carry r through the limbs.
 // Every operation is exact except r_0 + c, whose rounding IS the digit selection.  W = `bits`, the slice width: 13 for the
-// paper's quarters, other widths under MD_OPT_SLICE_BITS (R13).
+// paper's quarters, other widths under MD_OPT_SLICE_BITS (R14).
 template <int L>
 __device__ __forceinline__ double extract_digit(double (&r)[L], int E, int q, int bits) {
   // c = 1.5 * 2^(E - W(q+1) + 52): exponent field + the top mantissa bit

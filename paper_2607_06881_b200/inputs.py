@@ -37,7 +37,7 @@ class Config:
     # DESIGN.md reading R5.  This is a parameter handed to md_set_option, not part of the input data.
     quarters: int = 0
     # Slice width in bits: 13 = the paper's quarter.  Other widths are the k-adaptive variant (DESIGN.md
-    # R13), again a parameter handed to md_set_option, not part of the input data.
+    # R14), again a parameter handed to md_set_option, not part of the input data.
     bits: int = 13
 
     def __post_init__(self):

@@ -87,7 +87,7 @@ def test_options_and_workspace_sizes(lib):
 
 
 def test_plan_slices_matches_a_brute_force_search(lib):
-    """md_plan_slices (host only; R13): fewest slices Q that has a kernel, at the widest W with
+    """md_plan_slices (host only; R14): fewest slices Q that has a kernel, at the widest W with
     k * Q * 2^(2W) <= 2^53 (eq. 5 generalised), such that W * Q >= 13 * 4 * limbs (the paper's window,
     PAPER.md:47, :73); else the paper's (13, 4 * limbs).  Restated here as a plain search over all (Q, W)."""
     have = {2: (6, 7, 8, 9, 10), 4: (11, 12, 16, 17, 18), 8: (22, 32), 16: (64,)}

@@ -1,4 +1,4 @@
-"""GPU parity of the k-adaptive slice variant (MD_OPT_SLICE_BITS; R13): slices of W != 13
+"""GPU parity of the k-adaptive slice variant (MD_OPT_SLICE_BITS; R14): slices of W != 13
 bits, fewer of them.  Same bars as the paper's quarters: split and order matrices BIT-EXACT against the oracle's
 oracle_*_w functions, final C within 1e-28 / 1e-58 (|A||B|)_ij of the exact product.  Small cases span several CTA tiles
 with ragged tails; the full-size cases run BASELINE.json's shapes with the (W, Q) md_plan_slices picks, checked on samples."""
@@ -66,7 +66,7 @@ def test_orders_bit_exact_and_C_within_tolerance(cfg_idx, bits, Q, shape):
 
 
 def test_k_budget_follows_the_slice_width():
-    """k * S * 2^(2W) <= 2^53 (R13): W = 19, S = 6 allows k <= 5461."""
+    """k * S * 2^(2W) <= 2^53 (R14): W = 19, S = 6 allows k <= 5461."""
     A = torch.zeros((2, 8, 5462), dtype=torch.float64, device="cuda")
     B = torch.zeros((2, 5462, 8), dtype=torch.float64, device="cuda")
     with md.Workspace(8, 8, 5462, 2, 6, bits=19):

@@ -1,4 +1,4 @@
-"""Pins for the oracle's slice-width parameter (oracle_*_w; R13): Algorithm S with `bits` in place of the
+"""Pins for the oracle's slice-width parameter (oracle_*_w; R14): Algorithm S with `bits` in place of the
 paper's 13 ("4 parts ... each of 13 bits" = 52/4), the order matrices on the unit 2^(E_i+F_j-bits(s+2)),
 and the k-budget that generalises PAPER.md:95-99 eq. 5.
 
@@ -105,7 +105,7 @@ def test_order_routes_agree_and_match_rational_brute_force(bits, Q):
 def test_k_budget_generalises_eq5():
     """PAPER.md:95-99 eq. 5: N (2^26 - 1) <= 2^52 -> N <= 67 108 865 for products of two 13-bit parts.  With slices of
     `bits` bits (|D| <= 2^bits) and S products per k in an order, every partial sum stays an exactly representable
-    integer while k S 2^(2 bits) <= 2^53 (R6 / R13).  Worst-case digits at the bound still accumulate exactly."""
+    integer while k S 2^(2 bits) <= 2^53 (R6 / R14).  Worst-case digits at the bound still accumulate exactly."""
     assert (2 ** 52) // (2 ** 26 - 1) == PAPER["exact_sum_bound_N"][0]
     for bits, S in ((13, 8), (19, 6), (20, 4)):
         k = 2 ** 53 // (S * 2 ** (2 * bits))
