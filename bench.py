@@ -59,6 +59,9 @@ def parse_args():
     ap.add_argument("--slices", default="paper", choices=["paper", "adaptive"],
                     help="paper: 13-bit quarters, 4 per limb (the headline).  adaptive: the (bits, count) md_plan_slices "
                          "picks for this k -- wider, fewer slices (DESIGN.md R14; NOT the paper's quarters)")
+    ap.add_argument("--paper-paths", action="store_true",
+                    help="also time the paper's own two paths on this GPU (libmdcompare: materialised top-down product "
+                         "through cuBLAS DGEMM, CUDA-core classical GEMM; SURVEY.md 8(f) NEXT-2), outside the timed region")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -279,6 +282,49 @@ def run_ours(args):
                                 "13-bit quarters, so not the headline; 3 steps after 1 warm-up, CUDA events"}
             del C2
 
+    # the paper's own two paths on the same inputs (context; outside the timed region; N = 1, dd / qd only)
+    paper_paths = None
+    if args.paper_paths and world == 1 and L <= 4:
+        from paper_2607_06881_b200 import compare as mdc
+        PQ = 4 * L
+        ws = torch.empty(mdc.mdc_topdown_workspace_bytes(m, n, k, L, PQ), dtype=torch.uint8, device="cuda")
+        C_td, _, _ = mdc.mdc_topdown_gemm(A, B, ws=ws)  # warm-up (cuBLAS handle, heuristics)
+        stage = [0.0] * 4
+        torch.cuda.synchronize()
+        t_e0, t_e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t_e0.record(stream)
+        reps = 3
+        for _ in range(reps):
+            C_td, _, times = mdc.mdc_topdown_gemm(A, B, ws=ws, want_times=True)
+            stage = [a + b / reps for a, b in zip(stage, times)]
+        t_e1.record(stream)
+        torch.cuda.synchronize()
+        td_ms = t_e0.elapsed_time(t_e1) / reps
+        del ws
+        C_cl = mdc.mdc_classic_gemm(A, B)
+        torch.cuda.synchronize()
+        t_e0.record(stream)
+        C_cl = mdc.mdc_classic_gemm(A, B)
+        t_e1.record(stream)
+        torch.cuda.synchronize()
+        cl_ms = t_e0.elapsed_time(t_e1)
+        same_as_fused = bool((C_td == C).all()) if (Q, W) == (PQ, 13) else None
+        paper_paths = {
+            "topdown_materialised_cublas_dgemm": {
+                "ms_per_step": td_ms, "value": base.md_flops / (td_ms * 1e-3) / 1e9, "unit": UNIT,
+                "stage_ms": {"split": stage[0], "construct_Atil": stage[1], "dgemm": stage[2], "recombine": stage[3]},
+                "dgemm_fp64_tflops": 2.0 * (PQ * m) * n * (PQ * k) / (stage[2] * 1e-3) / 1e12,
+                "block_products": PQ * PQ, "bit_identical_to_fused_md_gemm": same_as_fused,
+                "what": "PAPER.md:73-89 eq. 4, :192-207 Table 2: Atil (A convoluted, %d x %d doubles) * Bstk (B stacked) "
+                        "through ONE cublasDgemm, then md_renorm; the paper's t_TC" % (PQ * m, PQ * k)},
+            "cuda_core_classical": {
+                "ms_per_step": cl_ms, "value": base.md_flops / (cl_ms * 1e-3) / 1e9, "unit": UNIT,
+                "max_abs_diff_vs_fused": float((C_cl - C).abs().sum(dim=0).max()),
+                "what": "PAPER.md:166: one thread per inner product, TwoSum / TwoProd on the regular FP64 cores; the paper's t_CUDA"},
+            "note": "comparison paths (libmdcompare), measured after the timed region: 3 / 1 steps after 1 warm-up, CUDA events",
+        }
+        del C_td, C_cl
+
     # end to end: pinned host buffers through md_gemm_host (H2D A, B + the whole path + D2H C, synchronous)
     e2e = None
     if not args.no_e2e:
@@ -361,7 +407,7 @@ def run_ours(args):
         "fp64_tflops_issued": world * base.fp64_flops / (ms_per_step * 1e-3) / 1e12,
         "pct_of_fp64_tensor_peak": 100.0 * base.fp64_flops / (ms_per_step * 1e-3) / 1e12 / FP64_TENSOR_PEAK_TFLOPS,
         "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": launches,
-        "adaptive_slices": adaptive,
+        "adaptive_slices": adaptive, "paper_paths": paper_paths,
         "clocks": clocks, "status_flags": flags,
     }
     print(json.dumps(line))

@@ -55,7 +55,8 @@ typedef void* md_stream;    /* a cudaStream_t */
 enum {
   MD_OPT_QUARTERS = 1,  /* quarters per element used by md_gemm / md_gemm_orders / md_gemm_host.  Default 4*limbs, the
                            paper's count (8 for double double, 16 for quad double).  Supported:
-                           limbs=2: 8, 9, 10; limbs=4: 16, 17, 18 (R5). */
+                           limbs=2: 8, 9, 10; limbs=4: 16, 17, 18 (R5); limbs=8: 32; limbs=16: 64 (octo / hexa double,
+                           PAPER.md:196-205 Table 2, R13); fewer with MD_OPT_SLICE_BITS (below). */
   MD_OPT_ORDERS = 2,    /* kept product orders S (the paper's C_1..C_S).  Default = quarters.  Must equal
                            quarters in this version. */
   MD_OPT_SLICE_BITS = 3, /* width W of a slice in bits, used by md_split and the md_gemm family.  Default 13: the paper's
@@ -93,7 +94,8 @@ md_status md_plan_slices(int k, int limbs, int* bits_out, int* quarters_out);
  *   planes          in   [limbs][rows][cols]
  *   quarter_planes  out  [quarters][rows][cols]  true-valued quarters (not the integers D)
  *   exps            out  int32[rows] (axis 0) / int32[cols] (axis 1)
- *   limbs in {1, 2, 4}; 1 <= quarters <= 24; rows, cols >= 1.  Bit-exact against the oracle's Algorithm S.
+ *   limbs in {1, 2, 4, 8, 16}; 1 <= quarters <= 72; rows, cols >= 1.  Bit-exact against the oracle's Algorithm S.
+ *   With MD_OPT_SLICE_BITS = W the 13 above reads W (R14).
  * ------------------------------------------------------------------------------------------------------------------ */
 md_status md_split(int rows, int cols, int limbs, int quarters, int axis, const double* planes,
                    double* quarter_planes, int32_t* exps, md_stream stream);
@@ -108,7 +110,8 @@ md_status md_split(int rows, int cols, int limbs, int quarters, int axis, const 
  *   order_planes  out  [orders][m][n] fp64, C^(s) true-valued; may be NULL
  *   C_planes      out  [limbs][m][n]: the orders summed error-free into `limbs` limbs in the kernel's epilogue
  *                      (same arithmetic as md_renorm); may be NULL.  Not both NULL.
- *   Needs orders == quarters, (limbs, quarters) as listed at MD_OPT_QUARTERS, k * orders <= 2^27.
+ *   Needs orders == quarters, limbs in {2, 4} with (limbs, quarters) as listed at MD_OPT_QUARTERS and MD_OPT_SLICE_BITS
+ *   (octo / hexa double go through md_gemm's packed operands only), k * orders * 2^(2W) <= 2^53 (W = 13: k * orders <= 2^27).
  * ------------------------------------------------------------------------------------------------------------------ */
 md_status md_qgemm(int m, int n, int k, int limbs, int quarters, int orders, const double* Aq, const double* Bq,
                    double* order_planes, double* C_planes, md_stream stream);
@@ -119,7 +122,7 @@ md_status md_qgemm(int m, int n, int k, int limbs, int quarters, int orders, con
  *   order_planes  in   [orders][m][n]
  *   C_planes      out  [limbs][m][n]:  sum_s C^(s) as `limbs` non-overlapping doubles (|limb_{l+1}| <= ulp(limb_l)/2),
  *                      within 2^-(53*limbs - 3) * sum_s |C^(s)| of the exact sum (R9).
- *   limbs in {1, 2, 4}; 1 <= orders <= 24.
+ *   limbs in {1, 2, 4, 8, 16}; 1 <= orders <= 144.
  * ------------------------------------------------------------------------------------------------------------------ */
 md_status md_renorm(int m, int n, int limbs, int orders, const double* order_planes, double* C_planes,
                     md_stream stream);
@@ -127,7 +130,8 @@ md_status md_renorm(int m, int n, int limbs, int orders, const double* order_pla
 /* ---------------------------------------------------------------------------------------------------------------------
  * md_gemm -- the whole hot path: C = A * B (all five steps), A: m x k, B: k x n, C: m x n, each with
  *   `limbs` limb planes.  Splits A by rows and B by columns into the registered workspace, then one fused kernel does
- *   the quarter products and writes the renormalised C once.  limbs in {2, 4}.
+ *   the quarter products and writes the renormalised C once.  limbs in {2, 4, 8, 16} (double double, quad double, and the
+ *   octo / hexa double of PAPER.md:196-205 Table 2).
  *   Accuracy: |C - A*B|_ij <= k (Q+1) 2^(E_i + F_j - 13Q - 2) + 2^-(53*limbs - 3) |C|_ij for any input (Q = quarters; E, F
  *   the exponent vectors of A's rows and B's columns); on the BASELINE.json workloads this is within 1e-28 (|A||B|)_ij
  *   (double double) and 1e-58 (|A||B|)_ij (quad double).

@@ -15,6 +15,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmdgemm.so")
+COMPARE_LIB = os.path.join(HERE, "libmdcompare.so")
 SOURCES = ["api.cu", "split.cu", "renorm.cu", "qgemm.cu", "qgemm_packed.cu", "qgemm_wide.cu", "probe.cu"]
 HEADERS = [os.path.join(CSRC, "md_common.cuh"), os.path.join(CSRC, "md_kernels.h"), os.path.join(CSRC, "md_packed.cuh"),
            os.path.join(CSRC, "qgemm_common.cuh"), os.path.join(CSRC, "qgemm_pipeline.cuh"),
@@ -56,7 +57,26 @@ def build(force: bool = False, verbose: bool = False) -> str:
                     raise RuntimeError("nvcc failed: " + " ".join(cmd))
     if jobs or force or _stale(LIB, objs):
         subprocess.check_call([nvcc, "-shared", "-o", LIB] + objs)
+    build_compare(nvcc, force, verbose)
     return LIB
+
+
+def build_compare(nvcc: str, force: bool = False, verbose: bool = False) -> str:
+    """libmdcompare.so (include/mdcompare.h): the paper's own two paths as comparison beside the product -- links cuBLAS
+    (the plain DGEMM of the top-down path) and libmdgemm.so (md_split / md_renorm through the C-ABI)."""
+    src = os.path.join(CSRC, "compare", "compare.cu")
+    deps = [src, LIB, os.path.join(os.path.dirname(HERE), "include", "mdcompare.h"),
+            os.path.join(os.path.dirname(HERE), "include", "mdgemm.h")]
+    if force or _stale(COMPARE_LIB, deps):
+        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + [
+            "-shared", src, "-o", COMPARE_LIB, "-L" + HERE, "-l:libmdgemm.so", "-lcublas",
+            "-Xlinker", "-rpath=$ORIGIN"]
+        res = subprocess.run(cmd, capture_output=True, text=True)
+        if verbose or res.returncode:
+            sys.stderr.write(" ".join(cmd) + "\n" + res.stdout + res.stderr)
+        if res.returncode:
+            raise RuntimeError("nvcc failed: " + " ".join(cmd))
+    return COMPARE_LIB
 
 
 if __name__ == "__main__":

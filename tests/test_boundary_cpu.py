@@ -125,3 +125,15 @@ def test_slice_bits_option_and_its_k_budget(lib):
     finally:
         lib.md_set_option(md.MD_OPT_SLICE_BITS, 0)
         lib.md_set_option(md.MD_OPT_QUARTERS, 0)
+
+
+def test_compare_library_exports_its_header(lib):
+    """libmdcompare.so (include/mdcompare.h, the paper's own two paths as comparison): every declared symbol exported."""
+    from paper_2607_06881_b200 import compare as mdc
+    text = open(os.path.join(ROOT, "include", "mdcompare.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    declared = sorted(set(re.findall(r"\b(mdc_[a-z_]+)\s*\(", text)))
+    assert declared == sorted(mdc.EXPORTED_SYMBOLS) and len(declared) == 3
+    for name in declared:
+        assert hasattr(mdc.lib(), name)
+    assert mdc.lib().mdc_topdown_workspace_bytes(0, 4, 4, 2, 8) == 0
