@@ -64,7 +64,7 @@ enum {
                            variant of DESIGN.md R14 / SURVEY.md 8(f) NEXT-3 -- NOT the paper's quarters: a slice of W
                            bits sits on the unit 2^(E_g - W(q+1)), |D| <= 2^W (q = 0), 2^(W-1) (q > 0), and the
                            exactness budget becomes k * orders * 2^(2W) <= 2^53.  With wider slices fewer are needed:
-                           set MD_OPT_QUARTERS to the slice count (limbs=2: 6, 7; limbs=4: 11, 12; limbs=8: 22), or
+                           set MD_OPT_QUARTERS to the slice count (limbs=2: 6, 7; limbs=4: 11, 12; limbs=8: 22; limbs=16: 44), or
                            take both from md_plan_slices. */
   MD_OPT_HOST_BLOCKS = 4 /* md_gemm_host only: number of blocks C is cut into for overlapping copies and kernels.
                             Default 0 = automatic (about one wave of CTA tiles per block, at most 32); 1 = no overlap;

@@ -44,17 +44,23 @@ struct WCfg {
   static constexpr int AHEAD = STAGES - 2;
   static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + XCHG_BYTES;
   static_assert(WARPS == 8, "8 warps per CTA (2 per SM sub-partition)");
-  static_assert(R == 1 || R == 4, "order ranges: 1 (octo double) or 4 (hexa double)");
+  static_assert(R == 1 || (R == 4 && Q == 64) || (R == 2 && Q == 44), "order ranges: 1 (octo double), 4 / 2 (hexa double)");
   static_assert(STAGES >= 3, "the non-blocking refill needs at least 3 stages");
   static_assert(2 * STAGES * 8 <= BAR_BYTES - 8, "barrier area (its last 8 bytes hold the stream-K flag)");
   static_assert(STAGE_BYTES % 128 == 0 && XCHG_BYTES % 128 == 0, "alignment");
-  // order range r = [lo(r), hi(r))
-  __host__ __device__ static constexpr int lo(int r) { return R == 1 ? 0 : (r == 0 ? 0 : r == 1 ? 32 : r == 2 ? 45 : 55); }
-  __host__ __device__ static constexpr int hi(int r) { return R == 1 ? S : (r == 0 ? 32 : r == 1 ? 45 : r == 2 ? 55 : 64); }
-  // warp -> (tile, range).  Warps w and w + 4 share an SM sub-partition: pair ranges (0,1) and (2,3) there.
-  __host__ __device__ static constexpr int tile_of(int w) { return R == 1 ? w : w / 4; }
+  // order range r = [lo(r), hi(r)): boundaries that balance the product counts sum_{s in range} (s + 1) --
+  //   Q = 64, R = 4: 0 | 32 | 45 | 55 | 64 -> 528 / 507 / 505 / 540;   Q = 44, R = 2: 0 | 31 | 44 -> 496 / 494
+  __host__ __device__ static constexpr int bound(int r) {
+    return R == 1 ? (r == 0 ? 0 : S) : R == 2 ? (r == 0 ? 0 : r == 1 ? 31 : 44) : (r == 0 ? 0 : r == 1 ? 32 : r == 2 ? 45 : r == 3 ? 55 : 64);
+  }
+  __host__ __device__ static constexpr int lo(int r) { return bound(r); }
+  __host__ __device__ static constexpr int hi(int r) { return bound(r + 1); }
+  // warp -> (tile, range).  Warps w and w + 4 share an SM sub-partition: R = 4 pairs ranges (0,1) and (2,3) there (1035 /
+  // 1045 DMMAs per k-step), R = 2 the two ranges of one tile (990).
+  __host__ __device__ static constexpr int tile_of(int w) { return R == 1 ? w : R == 2 ? w % 4 : w / 4; }
   __host__ __device__ static constexpr int range_of(int w) {
-    return R == 1 ? 0 : (w < 4 ? (w == 0 ? 0 : w == 1 ? 2 : w == 2 ? 1 : 3) : (w == 4 ? 1 : w == 5 ? 3 : w == 6 ? 0 : 2));
+    return R == 1 ? 0 : R == 2 ? w / 4
+                      : (w < 4 ? (w == 0 ? 0 : w == 1 ? 2 : w == 2 ? 1 : 3) : (w == 4 ? 1 : w == 5 ? 3 : w == 6 ? 0 : 2));
   }
 };
 
@@ -331,11 +337,16 @@ qgemm_wide_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, cons
   if constexpr (C::R == 1) {
     wide_consume<C, 0>(x, t, lane, tid);
   } else {
-    switch (C::range_of(warp)) {  // warp-uniform
-      case 0: wide_consume<C, 0>(x, t, lane, tid); break;
-      case 1: wide_consume<C, 1>(x, t, lane, tid); break;
-      case 2: wide_consume<C, 2>(x, t, lane, tid); break;
-      default: wide_consume<C, 3>(x, t, lane, tid); break;
+    if constexpr (C::R == 2) {
+      if (C::range_of(warp) == 0) wide_consume<C, 0>(x, t, lane, tid);  // warp-uniform
+      else wide_consume<C, 1>(x, t, lane, tid);
+    } else {
+      switch (C::range_of(warp)) {  // warp-uniform
+        case 0: wide_consume<C, 0>(x, t, lane, tid); break;
+        case 1: wide_consume<C, 1>(x, t, lane, tid); break;
+        case 2: wide_consume<C, 2>(x, t, lane, tid); break;
+        default: wide_consume<C, 3>(x, t, lane, tid); break;
+      }
     }
   }
 }
@@ -367,11 +378,12 @@ cudaError_t launch_wide_cfg(int m, int n, int k, const double* Ap, const double*
 using WCfgOD = WCfg<32, 8, 4, 2, 1>;   // octo double: 32 x 16 CTA tile, 8 tiles x 1 range
 using WCfgOD22 = WCfg<22, 8, 4, 2, 1>; // octo double in 22 slices of 19 bits (MD_OPT_SLICE_BITS; R14)
 using WCfgHD = WCfg<64, 16, 2, 1, 4>;  // hexa double: 16 x 8 CTA tile, 2 tiles x 4 ranges
+using WCfgHD44 = WCfg<44, 16, 2, 2, 2>;  // hexa double in 44 slices of 19 bits: 16 x 16 CTA tile, 4 tiles x 2 ranges
 
 }  // namespace
 
 bool qgemm_wide_supported(int limbs, int quarters) {
-  return (limbs == 8 && (quarters == 32 || quarters == 22)) || (limbs == 16 && quarters == 64);
+  return (limbs == 8 && (quarters == 32 || quarters == 22)) || (limbs == 16 && (quarters == 64 || quarters == 44));
 }
 
 cudaError_t launch_qgemm_wide(int m, int n, int k, int limbs, int quarters, const double* Ap, const double* Bp,
@@ -380,6 +392,7 @@ cudaError_t launch_qgemm_wide(int m, int n, int k, int limbs, int quarters, cons
   cudaError_t err = cudaErrorInvalidValue;
   if (limbs == 8 && quarters == 32) err = launch_wide_cfg<WCfgOD>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
   if (limbs == 8 && quarters == 22) err = launch_wide_cfg<WCfgOD22>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
+  if (limbs == 16 && quarters == 44) err = launch_wide_cfg<WCfgHD44>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
   if (limbs == 16 && quarters == 64) err = launch_wide_cfg<WCfgHD>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
   if (err == cudaSuccess) *launches += 1;
   return err;

@@ -90,7 +90,7 @@ def test_plan_slices_matches_a_brute_force_search(lib):
     """md_plan_slices (host only; R14): fewest slices Q that has a kernel, at the widest W with
     k * Q * 2^(2W) <= 2^53 (eq. 5 generalised), such that W * Q >= 13 * 4 * limbs (the paper's window,
     PAPER.md:47, :73); else the paper's (13, 4 * limbs).  Restated here as a plain search over all (Q, W)."""
-    have = {2: (6, 7, 8, 9, 10), 4: (11, 12, 16, 17, 18), 8: (22, 32), 16: (64,)}
+    have = {2: (6, 7, 8, 9, 10), 4: (11, 12, 16, 17, 18), 8: (22, 32), 16: (44, 64)}
     for limbs in (2, 4, 8, 16):
         for k in (1, 64, 512, 1024, 2048, 4096, 5461, 5462, 8192, 2 ** 15, 2 ** 18, 2 ** 20):
             best = None
@@ -104,7 +104,7 @@ def test_plan_slices_matches_a_brute_force_search(lib):
             want = best or (13, 4 * limbs)
             assert md.md_plan_slices(k, limbs) == want, (limbs, k)
     assert md.md_plan_slices(4096, 2) == (19, 6) and md.md_plan_slices(2048, 4) == (19, 11)
-    assert md.md_plan_slices(1024, 8) == (19, 22) and md.md_plan_slices(512, 16) == (13, 64)
+    assert md.md_plan_slices(1024, 8) == (19, 22) and md.md_plan_slices(512, 16) == (19, 44)
     fake_int = ctypes.c_int(0)
     assert lib.md_plan_slices(0, 2, ctypes.addressof(fake_int), ctypes.addressof(fake_int)) == md.MD_ERR_BAD_ARG
     assert lib.md_plan_slices(8, 3, ctypes.addressof(fake_int), ctypes.addressof(fake_int)) == md.MD_ERR_BAD_ARG

@@ -13,9 +13,9 @@ from tests.test_gpu_fullsize import sample_positions
 
 pytestmark = pytest.mark.gpu
 
-TOL = {2: 1e-28, 4: 1e-58, 8: 1e-120}
+TOL = {2: 1e-28, 4: 1e-58, 8: 1e-120, 16: 1e-245}
 # (config index, W, Q): the plans md_plan_slices gives at the BASELINE sizes, and a few others with kernels
-CASES = [(0, 19, 6), (1, 19, 6), (2, 19, 6), (3, 19, 6), (3, 16, 7), (4, 19, 11), (4, 18, 12), (5, 19, 22)]
+CASES = [(0, 19, 6), (1, 19, 6), (2, 19, 6), (3, 19, 6), (3, 16, 7), (4, 19, 11), (4, 18, 12), (5, 19, 22), (6, 19, 44)]
 SHAPES = [(64, 64, 64), (150, 70, 90), (37, 51, 77), (1, 1, 1)]
 
 
