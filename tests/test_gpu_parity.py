@@ -74,6 +74,23 @@ def test_split_hand_derived_cases_on_gpu():
                           [0, 4096, 0, 0, 0, 0, -2048, 0], [8192, 0, 0, 0, -3072, 0, 0, 0]]
 
 
+def test_split_idempotent_on_a_quarter_plane_and_powers_of_two_on_gpu():
+    """a quarter plane split again is itself in one digit; a row of equal powers of two is one digit."""
+    cfg, A, _ = gen(1, 40, 8, 36)
+    qp, exps = md.md_split(dev(A), 0, 8)
+    E = host(exps)
+    Y = np.zeros_like(A)
+    Y[0] = host(qp)[3]
+    Y[0, :, 0] = np.ldexp(0.75, E)
+    qq, e2 = md.md_split(dev(Y), 0, 8)
+    assert (host(e2) == E).all()
+    got = host(qq)
+    assert bits_equal(got[3][:, 1:], host(qp)[3][:, 1:]) and not got[[0, 1, 2, 4, 5, 6, 7]][:, :, 1:].any()
+    row = np.ldexp(1.0, -40) * np.array([[1.0, -1.0, 1.0, 1.0, -1.0]])
+    q2, e3 = md.md_split(dev(np.stack([row, np.zeros_like(row)])), 0, 8)
+    assert host(e3).tolist() == [-39] and bits_equal(host(q2)[0], row) and not host(q2)[1:].any()
+
+
 # ------------------------------------------------------------------------------------------------ a3: order matrices
 @pytest.mark.parametrize("cfg_idx", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("shape", SHAPES)

@@ -187,3 +187,30 @@ def test_values_already_on_the_grid_leave_no_remainder():
     X[1, :, 0] = 0.0
     _, exps, rem = orc.split(X, 0, want_remainder=True)
     assert (exps == 0).all() and not rem.any()
+
+
+def test_split_of_a_quarter_plane_returns_itself_in_one_digit():
+    """Idempotence: quarter plane q of a matrix, split again on the same group exponents, is a single
+    non-zero digit -- itself -- at position q (or q-1 .. when the row's maximum moved: here every row keeps an element
+    that pins E, so the position is q)."""
+    cfg = small_cfg(1, 9, 5, 11)
+    X = inputs.generate(cfg, "A")
+    qp, exps, _ = orc.split(X, 0)
+    for q in (0, 3, 7):
+        Y = np.zeros_like(X)
+        Y[0] = qp[q]
+        Y[0, :, 0] = np.ldexp(0.75, exps)  # one element per row pins the row exponent E_i (0.75 * 2^E has ilogb = E - 1)
+        qq, e2, rem = orc.split(Y, 0, want_remainder=True)
+        assert (e2 == exps).all() and not rem.any()
+        for t in range(qq.shape[0]):
+            want = qp[q][:, 1:] if t == q else np.zeros_like(qp[q][:, 1:])
+            assert (qq[t][:, 1:] == want).all()
+
+
+def test_row_of_equal_powers_of_two_is_one_digit():
+    """A row whose elements are all +-2^e: E = e + 1, and every element is the single digit +-2^12 u_0 (u_0 = 2^(E-13))."""
+    for e in (-40, 0, 17):
+        row = np.ldexp(1.0, e) * np.array([[1.0, -1.0, 1.0, 1.0, -1.0]])
+        qp, exps, rem = orc.split(np.stack([row, np.zeros_like(row)]), 0, want_remainder=True)
+        assert list(exps) == [e + 1] and not rem.any() and not qp[1:].any()
+        assert (qp[0] == row).all() and (np.abs(qp[0]) == 4096 * np.ldexp(1.0, e + 1 - W)).all()
