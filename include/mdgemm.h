@@ -142,6 +142,26 @@ md_status md_gemm(int m, int n, int k, int limbs, const double* A_planes, const 
 md_status md_gemm_orders(int m, int n, int k, int limbs, const double* A_planes, const double* B_planes,
                          double* order_planes, md_stream stream);
 
+/* ---------------------------------------------------------------------------------------------------------------------
+ * md_plan_quarters -- how many quarters THIS data needs (R15; SURVEY.md 8(f) NEXT-1 "exponent-spread-driven quarter
+ *   count").  With one exponent per row of A / column of B the error of md_gemm is bounded relative to 2^(E_i + F_j), not to
+ *   (|A||B|)_ij (see md_gemm below): |C - A*B|_ij <= k (Q+1) 2^(E_i + F_j - W Q - 2) + renormalisation, W = slice width (13).
+ *   This call measures D = max over positions with (|A_0||B_0|)_ij > 0 of E_i + F_j - ilogb((|A_0||B_0|)_ij) -- the leading
+ *   limb planes multiplied in plain fp64 on the same DMMA kernel, 1/36 of a double-double md_gemm -- and returns the
+ *   smallest Q >= ceil(52 limbs / W) with k (Q+1) 2^(D - W Q - 2) <= rel_tol: with MD_OPT_QUARTERS = Q the first term of
+ *   the bound is below rel_tol (|A||B|)_ij at EVERY position, for any input.  It is a worst-case guarantee (all dropped
+ *   digit products at their bound with one sign); measured errors are 2-3 orders of magnitude below it.
+ *   scratch        device, 256-byte aligned, md_plan_scratch_bytes(m, n, k) bytes (|A_0|, |B_0|, their product, exponents)
+ *   rel_tol        0 = the tolerance of the format: 1e-28 (limbs 2), 1e-58 (4), 1e-120 (8), 1e-245 (16), 2^-50 (1)
+ *   quarters_out   HOST: Q (not limited to the counts that have a kernel: md_gemm returns MD_ERR_UNSUPPORTED for those)
+ *   spread_out     HOST, may be NULL: D (INT32_MIN when |A||B| is zero everywhere)
+ *   SYNCHRONISES `stream`.  Launches 8 kernels.  Bit-exact against the oracle's plan up to the rounding of the fp64 sums
+ *   (D can differ by one where a sum sits on a power of two).
+ * ------------------------------------------------------------------------------------------------------------------ */
+size_t md_plan_scratch_bytes(int m, int n, int k);
+md_status md_plan_quarters(int m, int n, int k, int limbs, const double* A_planes, const double* B_planes, void* scratch,
+                           size_t scratch_bytes, double rel_tol, int* quarters_out, int* spread_out, md_stream stream);
+
 /* Workspace for md_gemm / md_gemm_orders: quarter planes of A and B, exponent vectors and the status word, for the
  * CURRENT option values.  The caller allocates (device memory, 256-byte aligned) and registers it; the library keeps
  * the pointer until it is replaced (ptr = NULL, bytes = 0 unregisters).  md_workspace_bytes returns 0 on bad arguments. */

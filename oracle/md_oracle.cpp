@@ -532,4 +532,48 @@ int oracle_num_threads(void) {
 #endif
 }
 
+
+// =====================================================================================================
+// Planning the quarter count from the data (R15; SURVEY.md 8(f) NEXT-1 "exponent-spread-driven quarter count").
+//   With one exponent per row of A / column of B (R2) the error of the path is bounded relative to
+//   2^(E_i + F_j), not to (|A||B|)_ij (R5):
+//       |C - A*B|_ij <= k (Q+1) 2^(E_i + F_j - bits*Q - 2)  +  (renormalisation, 2^-(53 limbs - 1) |C|_ij).
+//   The first term stays below rel_tol * W_ij, W = |A||B|, at every position iff
+//       k (Q+1) 2^(D - bits*Q - 2) <= rel_tol,     D >= log2 max_ij 2^(E_i + F_j) / W_ij.
+//   Plain definition, written out: W~_ij = sum_k |A_0[i,k]| |B_0[k,j]| on the leading limbs in fp64 (k innermost),
+//   D = max over positions with W~_ij > 0 of E_i + F_j - ilogb(W~_ij) (an integer upper bound of the log2 above), and
+//   Q = the smallest Q >= ceil(52 limbs / bits) that satisfies the inequality.  Positions with W~_ij = 0 have C_ij = 0
+//   exactly and need nothing.  Returns Q; *spread_out = D (INT32_MIN when W~ == 0 everywhere, then Q is the minimum).
+// =====================================================================================================
+int oracle_plan_quarters(int m, int n, int k, int limbs, int bits, const double* A, const double* B, double rel_tol,
+                         int32_t* spread_out) {
+  std::vector<int32_t> E(m), F(n);
+  for (int i = 0; i < m; i++) {
+    double M = 0.0;
+    for (int t = 0; t < k; t++) M = std::fmax(M, std::fabs(A[(size_t)i * k + t]));
+    E[i] = (M == 0.0) ? 0 : std::ilogb(M) + 1;
+  }
+  for (int j = 0; j < n; j++) {
+    double M = 0.0;
+    for (int t = 0; t < k; t++) M = std::fmax(M, std::fabs(B[(size_t)t * n + j]));
+    F[j] = (M == 0.0) ? 0 : std::ilogb(M) + 1;
+  }
+  int32_t D = INT32_MIN;
+  for (int i = 0; i < m; i++)
+    for (int j = 0; j < n; j++) {
+      double w = 0.0;
+      for (int t = 0; t < k; t++) w += std::fabs(A[(size_t)i * k + t]) * std::fabs(B[(size_t)t * n + j]);
+      if (w > 0.0) {
+        const int32_t d = E[i] + F[j] - std::ilogb(w);
+        if (d > D) D = d;
+      }
+    }
+  if (spread_out) *spread_out = D;
+  int Q = (52 * limbs + bits - 1) / bits;
+  if (D == INT32_MIN) return Q;
+  // k (Q+1) 2^(D - bits*Q - 2) <= rel_tol: the left side is exact in fp64 (an integer below 2^53 times a power of two)
+  while (Q < 4096 && std::ldexp((double)k * (Q + 1), D - bits * Q - 2) > rel_tol) Q++;
+  return Q;
+}
+
 }  // extern "C"

@@ -172,3 +172,16 @@ def md_gemm_rows(A, B, row0: int = 0, row1: int | None = None, quarters: int | N
     C = np.empty((limbs, row1 - row0, n))
     lib().oracle_md_gemm_rows_w(m, n, k, limbs, Q, S, bits, _d(A), _d(B), row0, row1, _d(C))
     return C
+
+
+def plan_quarters(A, B, rel_tol: float, bits: int = 13):
+    """DESIGN.md R15: the smallest quarter count whose error bound k (Q+1) 2^(E_i+F_j-bits Q-2) stays below
+    rel_tol (|A||B|)_ij at every position.  Returns (Q, D), D = max_ij E_i + F_j - ilogb((|A_0||B_0|)_ij)."""
+    A, B = _f64(A), _f64(B)
+    limbs, m, k = A.shape
+    n = B.shape[2]
+    D = ctypes.c_int32(0)
+    f = lib().oracle_plan_quarters
+    f.restype = ctypes.c_int
+    Q = f(m, n, k, limbs, bits, _d(A), _d(B), ctypes.c_double(rel_tol), ctypes.byref(D))
+    return int(Q), int(D.value)

@@ -24,6 +24,8 @@ _SIGNATURES = {
     "md_set_option": (_c.c_int, [_c.c_int, _c.c_int]),
     "md_get_option": (_c.c_int, [_c.c_int]),
     "md_plan_slices": (_c.c_int, [_c.c_int, _c.c_int, _c.c_void_p, _c.c_void_p]),
+    "md_plan_scratch_bytes": (_c.c_size_t, [_c.c_int] * 3),
+    "md_plan_quarters": (_c.c_int, [_c.c_int] * 4 + [_c.c_void_p] * 3 + [_c.c_size_t, _c.c_double] + [_c.c_void_p] * 3),
     "md_split": (_c.c_int, [_c.c_int] * 5 + [_c.c_void_p] * 4),
     "md_qgemm": (_c.c_int, [_c.c_int] * 6 + [_c.c_void_p] * 5),
     "md_renorm": (_c.c_int, [_c.c_int] * 4 + [_c.c_void_p] * 3),
@@ -95,6 +97,18 @@ def md_plan_slices(k: int, limbs: int):
     bits, quarters = ctypes.c_int(0), ctypes.c_int(0)
     _check(lib().md_plan_slices(k, limbs, ctypes.addressof(bits), ctypes.addressof(quarters)), "md_plan_slices")
     return bits.value, quarters.value
+
+
+def md_plan_quarters(A: torch.Tensor, B: torch.Tensor, rel_tol: float = 0.0, stream=None):
+    """(Q, D): the quarter count this data needs for rel_tol (0 = the format's tolerance) and the measured spread D
+    (include/mdgemm.h).  Synchronises."""
+    limbs, m, k = A.shape
+    n = B.shape[2]
+    scratch = torch.empty(lib().md_plan_scratch_bytes(m, n, k), dtype=torch.uint8, device=A.device)
+    q, d = ctypes.c_int(0), ctypes.c_int(0)
+    _check(lib().md_plan_quarters(m, n, k, limbs, _dev(A), _dev(B), _dev(scratch, torch.uint8), scratch.numel(),
+                                  rel_tol, ctypes.addressof(q), ctypes.addressof(d), _stream(stream)), "md_plan_quarters")
+    return q.value, d.value
 
 
 def md_workspace_bytes(m, n, k, limbs) -> int:

@@ -1,6 +1,7 @@
 // api.cu -- the C-ABI of libmdgemm (include/mdgemm.h): argument checking, options, workspace carving, and the sequence
 // of kernel launches of the hot path.  No arithmetic of the method lives here.
 #include <atomic>
+#include <cmath>
 #include <cstdint>
 #include <vector>
 
@@ -292,6 +293,53 @@ md_status md_plan_slices(int k, int limbs, int* bits_out, int* quarters_out) {
   if (!k_budget_ok(k, 4 * limbs, 13)) return MD_ERR_K_TOO_LARGE;
   *bits_out = 13;
   *quarters_out = 4 * limbs;
+  return MD_OK;
+}
+
+size_t md_plan_scratch_bytes(int m, int n, int k) {
+  if (m <= 0 || n <= 0 || k <= 0) return 0;
+  return ALIGN + round_up(sizeof(int32_t) * (size_t)m) + round_up(sizeof(int32_t) * (size_t)n) +
+         round_up(sizeof(double) * (size_t)m * k) + round_up(sizeof(double) * (size_t)k * n) +
+         round_up(sizeof(double) * (size_t)m * n);
+}
+
+md_status md_plan_quarters(int m, int n, int k, int limbs, const double* A_planes, const double* B_planes, void* scratch,
+                           size_t scratch_bytes, double rel_tol, int* quarters_out, int* spread_out, md_stream stream) {
+  if (m <= 0 || n <= 0 || k <= 0 || !A_planes || !B_planes || !scratch || !quarters_out) return MD_ERR_BAD_ARG;
+  if (limbs != 1 && limbs != 2 && limbs != 4 && limbs != 8 && limbs != 16) return MD_ERR_BAD_ARG;
+  if (!aligned8(A_planes) || !aligned8(B_planes) || reinterpret_cast<uintptr_t>(scratch) % ALIGN) return MD_ERR_BAD_ARG;
+  if (scratch_bytes < md_plan_scratch_bytes(m, n, k)) return MD_ERR_WORKSPACE;
+  if (rel_tol == 0.0) rel_tol = limbs == 1 ? 0x1p-50 : limbs == 2 ? 1e-28 : limbs == 4 ? 1e-58 : limbs == 8 ? 1e-120 : 1e-245;
+  if (!(rel_tol > 0.0)) return MD_ERR_BAD_ARG;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const int W = slice_bits();
+  char* p = static_cast<char*>(scratch);
+  int32_t* spread = reinterpret_cast<int32_t*>(p);
+  int32_t* expA = reinterpret_cast<int32_t*>(p + ALIGN);
+  int32_t* expB = reinterpret_cast<int32_t*>(p + ALIGN + round_up(sizeof(int32_t) * (size_t)m));
+  double* absA = reinterpret_cast<double*>(reinterpret_cast<char*>(expB) + round_up(sizeof(int32_t) * (size_t)n));
+  double* absB = reinterpret_cast<double*>(reinterpret_cast<char*>(absA) + round_up(sizeof(double) * (size_t)m * k));
+  double* Wt = reinterpret_cast<double*>(reinterpret_cast<char*>(absB) + round_up(sizeof(double) * (size_t)k * n));
+  const int32_t none = INT32_MIN;
+  uint64_t launches = 0;
+  cudaError_t err = cudaMemcpyAsync(spread, &none, sizeof(none), cudaMemcpyHostToDevice, st);
+  // exponent vectors of the leading limb planes, |A_0| |B_0| on the DMMA kernel, then the spread D
+  if (err == cudaSuccess) err = md::launch_exponents(m, k, 0, 4 * limbs, W, A_planes, expA, nullptr, st, &launches);
+  if (err == cudaSuccess) err = md::launch_exponents(k, n, 1, 4 * limbs, W, B_planes, expB, nullptr, st, &launches);
+  if (err == cudaSuccess) err = md::launch_abs((size_t)m * k, A_planes, absA, st, &launches);
+  if (err == cudaSuccess) err = md::launch_abs((size_t)k * n, B_planes, absB, st, &launches);
+  if (err == cudaSuccess) err = md::launch_plain_dgemm(m, n, k, absA, absB, Wt, st, &launches);
+  if (err == cudaSuccess) err = md::launch_spread(m, n, Wt, expA, expB, spread, st, &launches);
+  g_launches += launches;
+  int32_t D = 0;
+  if (err == cudaSuccess) err = cudaMemcpyAsync(&D, spread, sizeof(D), cudaMemcpyDeviceToHost, st);
+  if (err != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) return MD_ERR_CUDA;
+  if (spread_out) *spread_out = D;
+  // the smallest Q >= ceil(52 limbs / W) with k (Q+1) 2^(D - W Q - 2) <= rel_tol (R15; the left side is exact)
+  int Q = (52 * limbs + W - 1) / W;
+  if (D != INT32_MIN)
+    while (Q < 4096 && ldexp((double)k * (Q + 1), D - W * Q - 2) > rel_tol) Q++;
+  *quarters_out = Q;
   return MD_OK;
 }
 

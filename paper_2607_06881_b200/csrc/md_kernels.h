@@ -20,6 +20,13 @@ cudaError_t launch_renorm(int m, int n, int limbs, int orders, const double* ord
 cudaError_t launch_qgemm(int m, int n, int k, int limbs, int quarters, const double* Aq, const double* Bq,
                          double* order_planes, double* C_planes, cudaStream_t stream, uint64_t* launches);
 bool qgemm_supported(int limbs, int quarters);
+// md_plan_quarters (plan.cu): plain fp64 product of two non-negative matrices on the DMMA kernel of qgemm.cu; absolute
+// values of a plane; D = max over W~ > 0 of E_i + F_j - ilogb(W~_ij) folded into *spread (pre-set to INT32_MIN)
+cudaError_t launch_plain_dgemm(int m, int n, int k, const double* X, const double* Y, double* XY, cudaStream_t stream,
+                               uint64_t* launches);
+cudaError_t launch_abs(size_t count, const double* in, double* out, cudaStream_t stream, uint64_t* launches);
+cudaError_t launch_spread(int m, int n, const double* W, const int32_t* expA, const int32_t* expB, int32_t* spread,
+                          cudaStream_t stream, uint64_t* launches);
 // md_gemm's internal pair: splitter writing the fragment-major packed layout (md_packed.cuh) and the bulk-copy /
 // mbarrier pipelined fused GEMM reading it.  Same (limbs, quarters) support as launch_qgemm.
 cudaError_t launch_split_packed(int rows, int cols, int limbs, int quarters, int bits, int axis, const double* planes,

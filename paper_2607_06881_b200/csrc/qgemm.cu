@@ -183,6 +183,15 @@ bool qgemm_supported(int limbs, int quarters) {
   return (limbs == 2 && quarters >= 6 && quarters <= 10) || (limbs == 4 && ((quarters >= 16 && quarters <= 18) || quarters == 11 || quarters == 12));
 }
 
+// md_plan_quarters: W~ = X * Y for two plain fp64 matrices (|A_0|, |B_0|) on the same DMMA kernel with one "quarter" and
+// one order (no exactness needed there: all terms are non-negative, the relative error is k 2^-53).
+cudaError_t launch_plain_dgemm(int m, int n, int k, const double* X, const double* Y, double* XY, cudaStream_t stream,
+                               uint64_t* launches) {
+  const cudaError_t err = launch_cfg<CfgDD<1>>(m, n, k, X, Y, XY, nullptr, stream);
+  if (err == cudaSuccess) *launches += 1;
+  return err;
+}
+
 cudaError_t launch_qgemm(int m, int n, int k, int limbs, int quarters, const double* Aq, const double* Bq,
                          double* order_planes, double* C_planes, cudaStream_t stream, uint64_t* launches) {
   cudaError_t err = cudaErrorInvalidValue;

@@ -137,3 +137,16 @@ def test_compare_library_exports_its_header(lib):
     for name in declared:
         assert hasattr(mdc.lib(), name)
     assert mdc.lib().mdc_topdown_workspace_bytes(0, 4, 4, 2, 8) == 0
+
+
+def test_plan_quarters_argument_errors(lib):
+    fake = ctypes.c_void_p(4096)
+    q = ctypes.c_int(0)
+    assert lib.md_plan_scratch_bytes(0, 4, 4) == 0
+    need = lib.md_plan_scratch_bytes(64, 32, 16)
+    assert need >= 8 * (64 * 16 + 16 * 32 + 64 * 32) + 4 * (64 + 32)
+    args = (fake, fake, fake, need, 0.0, ctypes.addressof(q), None, None)
+    assert lib.md_plan_quarters(0, 32, 16, 2, *args) == md.MD_ERR_BAD_ARG
+    assert lib.md_plan_quarters(64, 32, 16, 3, *args) == md.MD_ERR_BAD_ARG
+    assert lib.md_plan_quarters(64, 32, 16, 2, fake, fake, fake, need - 1, 0.0, ctypes.addressof(q), None, None) == md.MD_ERR_WORKSPACE
+    assert lib.md_plan_quarters(64, 32, 16, 2, fake, fake, fake, need, -1.0, ctypes.addressof(q), None, None) == md.MD_ERR_BAD_ARG
