@@ -56,9 +56,10 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (default 2: the headline)")
-    ap.add_argument("--slices", default="paper", choices=["paper", "adaptive"],
+    ap.add_argument("--slices", default="paper", choices=["paper", "adaptive", "chunked"],
                     help="paper: 13-bit quarters, 4 per limb (the headline).  adaptive: the (bits, count) md_plan_slices "
-                         "picks for this k -- wider, fewer slices (DESIGN.md R14; NOT the paper's quarters)")
+                         "picks for this k -- wider, fewer slices (DESIGN.md R14; NOT the paper's quarters).  chunked: "
+                         "md_plan_slices_chunked(k, limbs, 256) -- still wider slices, exact per chunk of k (DESIGN.md R16)")
     ap.add_argument("--paper-paths", action="store_true",
                     help="also time the paper's own two paths on this GPU (libmdcompare: materialised top-down product "
                          "through cuBLAS DGEMM, CUDA-core classical GEMM; SURVEY.md 8(f) NEXT-2), outside the timed region")
@@ -207,6 +208,8 @@ def run_ours(args):
     # weak scaling: the global A has world * m rows, rank r owns one block of m rows (no collective on the data path)
     if args.slices == "adaptive":
         base = base.with_slices(*md.md_plan_slices(base.k, base.limbs))
+    elif args.slices == "chunked":
+        base = base.with_slices(*md.md_plan_slices_chunked(base.k, base.limbs, 256)[:2])
     cfg = base.with_shape(m=base.m * world)
     row0, row1 = shard.row_block(cfg.m, world, rank)
     m, n, k, L, Q, W = row1 - row0, cfg.n, cfg.k, cfg.limbs, cfg.quarters, cfg.bits
@@ -270,31 +273,38 @@ def run_ours(args):
 
     # beside the headline (the paper's quarters): the same problem with the k-adaptive slices, outside the timed region
     adaptive = None
+
+    def time_variant(aW, aQ, note):
+        C2 = torch.empty_like(C)
+        with md.Workspace(m, n, k, L, aQ, bits=aW):
+            md.md_gemm(A, B, C2)
+            md.md_profile_enable(3)
+            torch.cuda.synchronize()
+            v0, v1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            v0.record(stream)
+            for _ in range(3):
+                md.md_gemm(A, B, C2)
+            v1.record(stream)
+            torch.cuda.synchronize()
+            _, a_gemm_ms = md.md_profile_read(3)
+            md.md_profile_enable(0)
+        a_ms = v0.elapsed_time(v1) / 3
+        aT = aQ * (aQ + 1) // 2
+        return {"slice_bits": aW, "slices": aQ, "products": aT, "ms_per_step": a_ms,
+                "value": base.md_flops / (a_ms * 1e-3) / 1e9, "unit": UNIT,
+                "kernel_frac_of_fp64_tensor_peak": aT * base.md_flops / (sum(a_gemm_ms) / 3 * 1e-3) / 1e12 / FP64_TENSOR_PEAK_TFLOPS,
+                "max_abs_diff_vs_paper_quarters": float((C2 - C).abs().sum(dim=0).max()), "note": note}
+
     if args.slices == "paper" and world == 1:
+        cW, cQ, cK = md.md_plan_slices_chunked(k, L, 256)
         aW, aQ = md.md_plan_slices(k, L)
         if (aW, aQ) != (W, Q):
-            C2 = torch.empty_like(C)
-            with md.Workspace(m, n, k, L, aQ, bits=aW):
-                md.md_gemm(A, B, C2)
-                md.md_profile_enable(3)
-                torch.cuda.synchronize()
-                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                e0.record(stream)
-                for _ in range(3):
-                    md.md_gemm(A, B, C2)
-                e1.record(stream)
-                torch.cuda.synchronize()
-                _, a_gemm_ms = md.md_profile_read(3)
-                md.md_profile_enable(0)
-            a_ms = e0.elapsed_time(e1) / 3
-            aT = aQ * (aQ + 1) // 2
-            adaptive = {"slice_bits": aW, "slices": aQ, "products": aT, "ms_per_step": a_ms,
-                        "value": base.md_flops / (a_ms * 1e-3) / 1e9, "unit": UNIT,
-                        "kernel_frac_of_fp64_tensor_peak": aT * base.md_flops / (sum(a_gemm_ms) / 3 * 1e-3) / 1e12 / FP64_TENSOR_PEAK_TFLOPS,
-                        "max_abs_diff_vs_paper_quarters": float((C2 - C).abs().sum(dim=0).max()),
-                        "note": "md_plan_slices: wider, fewer slices on the same kernels (DESIGN.md R14); not the paper's "
-                                "13-bit quarters, so not the headline; 3 steps after 1 warm-up, CUDA events"}
-            del C2
+            adaptive = time_variant(aW, aQ, "md_plan_slices: wider, fewer slices on the same kernels (DESIGN.md R14); not the "
+                                            "paper's 13-bit quarters, so not the headline; 3 steps after 1 warm-up, CUDA events")
+            if (cW, cQ) != (aW, aQ):
+                adaptive["chunked"] = time_variant(cW, cQ, "md_plan_slices_chunked(k, limbs, 256): exactness kept per chunk of %d "
+                                                           "contraction indices (DESIGN.md R16)" % cK)
+                adaptive["chunked"]["chunk"] = cK
 
     # the paper's own two paths on the same inputs (context; outside the timed region; N = 1, dd / qd only)
     paper_paths = None

@@ -43,7 +43,8 @@ typedef int md_status;
 enum {
   MD_OK = 0,
   MD_ERR_BAD_ARG = -1,      /* null pointer, dimension <= 0, misaligned pointer, limbs/quarters/orders unsupported */
-  MD_ERR_K_TOO_LARGE = -2,  /* k exceeds the exactness budget k * orders <= 2^27 (eq. 5; R6) */
+  MD_ERR_K_TOO_LARGE = -2,  /* k exceeds the exactness budget k * orders <= 2^27 (eq. 5; R6) and the
+                               call cannot chunk the contraction (md_gemm_orders, md_qgemm, quad double and wider) */
   MD_ERR_WORKSPACE = -3,    /* no workspace registered, or it is too small (md_workspace_bytes) */
   MD_ERR_CUDA = -4,         /* a CUDA call failed */
   MD_ERR_UNSUPPORTED = -5   /* combination of (limbs, quarters, orders) that has no kernel instantiation */
@@ -66,6 +67,12 @@ enum {
                            exactness budget becomes k * orders * 2^(2W) <= 2^53.  With wider slices fewer are needed:
                            set MD_OPT_QUARTERS to the slice count (limbs=2: 6, 7; limbs=4: 11, 12; limbs=8: 22; limbs=16: 44), or
                            take both from md_plan_slices. */
+  MD_OPT_K_CHUNK = 5,    /* md_gemm / md_gemm_host, double double only (R16): length of the chunks of the
+                            contraction over which the accumulations are kept exact.  Default 0 = automatic: chunking is
+                            used only when k exceeds the exactness budget k * orders * 2^(2W) <= 2^53, with the largest
+                            chunk the budget allows; a value (a multiple of 8) forces a shorter chunk.  Within a chunk
+                            every order sum is exact; at its end the sums are added into the element's expansion by the
+                            TwoSum cascade of md_renorm.  md_gemm_orders never chunks (MD_ERR_K_TOO_LARGE as before). */
   MD_OPT_HOST_BLOCKS = 4 /* md_gemm_host only: number of blocks C is cut into for overlapping copies and kernels.
                             Default 0 = automatic (about one wave of CTA tiles per block, at most 32); 1 = no overlap;
                             PR * 256 + PC = explicit numbers of row panels and column panels (each <= 64). */
@@ -78,6 +85,11 @@ int md_get_option(int key); /* current value (0 = default), or -1 for an unknown
  * the paper's 13 * 4 * limbs bits.  Stores W in *bits_out and Q in *quarters_out (host pointers); (13, 4*limbs), the paper's
  * own split, when nothing wider qualifies.  Launches nothing and changes no option. */
 md_status md_plan_slices(int k, int limbs, int* bits_out, int* quarters_out);
+/* The same with chunked accumulation allowed (MD_OPT_K_CHUNK, R16): the budget only has to hold for a chunk of at
+ * least min_chunk (>= 8) contraction indices where a chunked kernel exists (double double: 5, 6, 8 slices), which admits
+ * wider and fewer slices: double double at k = 4096 gets 5 slices of 21 bits in chunks of 408 (15 products instead of 21).
+ * *chunk_out = the chunk md_gemm will use, 0 when this k needs none.  md_gemm_orders is not available beyond the budget. */
+md_status md_plan_slices_chunked(int k, int limbs, int min_chunk, int* bits_out, int* quarters_out, int* chunk_out);
 
 /* ---------------------------------------------------------------------------------------------------------------------
  * md_split -- steps a1 + a2: exponent vectors ("balancing") and quarter planes.

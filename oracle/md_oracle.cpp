@@ -524,6 +524,36 @@ void oracle_md_gemm_rows(int m, int n, int k, int limbs, int quarters, int order
   oracle_md_gemm_rows_w(m, n, k, limbs, quarters, orders, 13, A, B, row0, row1, C_rows);
 }
 
+// Chunked accumulation (R16): the contraction is cut into chunks of `chunk` indices; inside a chunk the order sums
+// are formed exactly as above (the budget k S 2^(2 bits) <= 2^53 now only has to hold for chunk in place of k), and the
+// parts of ALL chunks -- orders * ceil(k / chunk) doubles per element -- are added into the multiple-double result
+// (here by the exact sum of oracle_renorm).  chunk >= k is oracle_md_gemm_rows_w.
+void oracle_md_gemm_rows_chunked_w(int m, int n, int k, int limbs, int quarters, int orders, int bits, int chunk,
+                                   const double* A, const double* B, int row0, int row1, double* C_rows) {
+  const int mr = row1 - row0;
+  std::vector<double> Arows((size_t)limbs * mr * k);
+  for (int l = 0; l < limbs; l++)
+    std::memcpy(&Arows[(size_t)l * mr * k], &A[(size_t)l * m * k + (size_t)row0 * k], sizeof(double) * (size_t)mr * k);
+  std::vector<double> Aq((size_t)quarters * mr * k), Bq((size_t)quarters * k * n);
+  std::vector<int32_t> eA(mr), eB(n);
+  oracle_split_w(mr, k, limbs, quarters, bits, 0, Arows.data(), Aq.data(), eA.data(), nullptr);
+  oracle_split_w(k, n, limbs, quarters, bits, 1, B, Bq.data(), eB.data(), nullptr);
+  const int nchunks = (k + chunk - 1) / chunk;
+  std::vector<double> ord((size_t)nchunks * orders * mr * n);
+  for (int c = 0; c < nchunks; c++) {
+    const int k0 = c * chunk, kc = (k0 + chunk <= k ? chunk : k - k0);
+    // the quarter planes of this chunk: columns [k0, k0 + kc) of A's, rows [k0, k0 + kc) of B's
+    std::vector<double> Ac((size_t)quarters * mr * kc), Bc((size_t)quarters * kc * n);
+    for (int q = 0; q < quarters; q++) {
+      for (int i = 0; i < mr; i++)
+        std::memcpy(&Ac[((size_t)q * mr + i) * kc], &Aq[((size_t)q * mr + i) * k + k0], sizeof(double) * (size_t)kc);
+      std::memcpy(&Bc[(size_t)q * kc * n], &Bq[((size_t)q * k + k0) * n], sizeof(double) * (size_t)kc * n);
+    }
+    oracle_orders_fp64(mr, n, kc, quarters, orders, Ac.data(), Bc.data(), &ord[(size_t)c * orders * mr * n]);
+  }
+  oracle_renorm(mr, n, limbs, nchunks * orders, ord.data(), C_rows);
+}
+
 int oracle_num_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();

@@ -185,3 +185,14 @@ def plan_quarters(A, B, rel_tol: float, bits: int = 13):
     f.restype = ctypes.c_int
     Q = f(m, n, k, limbs, bits, _d(A), _d(B), ctypes.c_double(rel_tol), ctypes.byref(D))
     return int(Q), int(D.value)
+
+
+def md_gemm_rows_chunked(A, B, chunk: int, quarters: int, bits: int, row0: int = 0, row1: int | None = None):
+    """DESIGN.md R16: the five steps with the order sums formed exactly per chunk of the contraction."""
+    A, B = _f64(A), _f64(B)
+    limbs, m, k = A.shape
+    n = B.shape[2]
+    row1 = m if row1 is None else row1
+    C = np.empty((limbs, row1 - row0, n))
+    lib().oracle_md_gemm_rows_chunked_w(m, n, k, limbs, quarters, quarters, bits, chunk, _d(A), _d(B), row0, row1, _d(C))
+    return C

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libmdgemm.so")
 
 MD_OK = 0
 MD_ERR_BAD_ARG, MD_ERR_K_TOO_LARGE, MD_ERR_WORKSPACE, MD_ERR_CUDA, MD_ERR_UNSUPPORTED = -1, -2, -3, -4, -5
-MD_OPT_QUARTERS, MD_OPT_ORDERS, MD_OPT_SLICE_BITS, MD_OPT_HOST_BLOCKS = 1, 2, 3, 4
+MD_OPT_QUARTERS, MD_OPT_ORDERS, MD_OPT_SLICE_BITS, MD_OPT_HOST_BLOCKS, MD_OPT_K_CHUNK = 1, 2, 3, 4, 5
 
 # every symbol include/mdgemm.h declares: name -> (restype, argtypes)
 _c = ctypes
@@ -26,6 +26,7 @@ _SIGNATURES = {
     "md_plan_slices": (_c.c_int, [_c.c_int, _c.c_int, _c.c_void_p, _c.c_void_p]),
     "md_plan_scratch_bytes": (_c.c_size_t, [_c.c_int] * 3),
     "md_plan_quarters": (_c.c_int, [_c.c_int] * 4 + [_c.c_void_p] * 3 + [_c.c_size_t, _c.c_double] + [_c.c_void_p] * 3),
+    "md_plan_slices_chunked": (_c.c_int, [_c.c_int] * 3 + [_c.c_void_p] * 3),
     "md_split": (_c.c_int, [_c.c_int] * 5 + [_c.c_void_p] * 4),
     "md_qgemm": (_c.c_int, [_c.c_int] * 6 + [_c.c_void_p] * 5),
     "md_renorm": (_c.c_int, [_c.c_int] * 4 + [_c.c_void_p] * 3),
@@ -97,6 +98,14 @@ def md_plan_slices(k: int, limbs: int):
     bits, quarters = ctypes.c_int(0), ctypes.c_int(0)
     _check(lib().md_plan_slices(k, limbs, ctypes.addressof(bits), ctypes.addressof(quarters)), "md_plan_slices")
     return bits.value, quarters.value
+
+
+def md_plan_slices_chunked(k: int, limbs: int, min_chunk: int = 256):
+    """(W, Q, chunk) with chunked accumulation allowed (include/mdgemm.h, R16); chunk = 0: none needed."""
+    bits, quarters, chunk = ctypes.c_int(0), ctypes.c_int(0), ctypes.c_int(0)
+    _check(lib().md_plan_slices_chunked(k, limbs, min_chunk, ctypes.addressof(bits), ctypes.addressof(quarters),
+                                        ctypes.addressof(chunk)), "md_plan_slices_chunked")
+    return bits.value, quarters.value, chunk.value
 
 
 def md_plan_quarters(A: torch.Tensor, B: torch.Tensor, rel_tol: float = 0.0, stream=None):

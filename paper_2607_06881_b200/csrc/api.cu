@@ -16,6 +16,7 @@ struct State {
   int opt_quarters = 0;  // 0 = default (4 * limbs)
   int opt_orders = 0;    // 0 = default (= quarters)
   int opt_bits = 0;      // 0 = default (13, the paper's quarter)
+  int opt_k_chunk = 0;   // 0 = chunked accumulation only when k exceeds the exactness budget; else the chunk length to force
   int opt_host_blocks = 0;  // md_gemm_host: 0 = automatic panel plan, else the number of blocks of C (1 = no pipelining)
   void* ws = nullptr;
   size_t ws_bytes = 0;
@@ -42,6 +43,17 @@ constexpr int MD_MIN_BITS = 4, MD_MAX_BITS = 24;
 // integer of at most 2^(2W) units, so every partial sum is exactly representable while k * S * 2^(2W) <= 2^53.
 // W = 13: k * S <= 2^27.
 inline bool k_budget_ok(long long k, int S, int bits) { return k * S <= (1ll << (53 - 2 * bits)); }
+// Chunked accumulation (R16): the budget is kept per chunk of the contraction; the chunk md_gemm uses for
+// (limbs, S, W), a multiple of the k-slab depth 8, or 0 when the path stays unchunked / cannot be chunked.
+inline int chunk_for(int k, int limbs, int S, int bits) {
+  if (!md::qgemm_chunk_supported(limbs, S)) return 0;
+  long long c = (1ll << (53 - 2 * bits)) / S;
+  if (g_state.opt_k_chunk > 0 && g_state.opt_k_chunk < c) c = g_state.opt_k_chunk;
+  c = c / md::PACK_BK * md::PACK_BK;
+  if (c < md::PACK_BK) return 0;
+  const bool needed = !k_budget_ok(k, S, bits) || !md::qgemm_supported(limbs, S) || (g_state.opt_k_chunk > 0 && k > c);
+  return needed ? (int)(c > 0x40000000 ? 0x40000000 : c) : 0;
+}
 
 // Workspace layout: [status word | expA int32[m] | expB int32[n] | Aq | Bq], Aq / Bq = the packed quarter planes of A / B
 // (md_packed.cuh: zero padded to whole CTA tiles and k-slabs), then the stream-K scratch of the fused GEMM
@@ -76,14 +88,26 @@ Carve carve(void* base, int m, int n, int k, int limbs, int quarters) {
 
 inline bool aligned8(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 7) == 0; }
 
-md_status check_gemm_args(int m, int n, int k, int limbs, const void* A, const void* B, const void* C) {
+md_status check_gemm_args(int m, int n, int k, int limbs, const void* A, const void* B, const void* C,
+                          bool want_orders = false) {
   if (m <= 0 || n <= 0 || k <= 0 || !A || !B || !C) return MD_ERR_BAD_ARG;
   if (!aligned8(A) || !aligned8(B) || !aligned8(C)) return MD_ERR_BAD_ARG;
   if (limbs != 2 && limbs != 4 && limbs != 8 && limbs != 16) return MD_ERR_BAD_ARG;
   const int Q = quarters_for(limbs), S = orders_for(limbs);
-  if (S != Q || !(md::qgemm_supported(limbs, Q) || md::qgemm_wide_supported(limbs, Q))) return MD_ERR_UNSUPPORTED;
-  if (!k_budget_ok(k, S, slice_bits())) return MD_ERR_K_TOO_LARGE;
+  // order planes need the order sums of the WHOLE contraction to be exact doubles: no chunking there
+  const int chunk = want_orders ? 0 : chunk_for(k, limbs, S, slice_bits());
+  if (S != Q || !(md::qgemm_supported(limbs, Q) || md::qgemm_wide_supported(limbs, Q) || chunk > 0)) return MD_ERR_UNSUPPORTED;
+  if (chunk == 0 && !k_budget_ok(k, S, slice_bits())) return MD_ERR_K_TOO_LARGE;
   return MD_OK;
+}
+
+// the fused quarter GEMM of one (block of a) problem on packed operands: double / quad double (chunked when md_gemm asks
+// for C of a contraction beyond the exactness budget), octo / hexa double
+cudaError_t launch_fused(int m, int n, int k, int limbs, int Q, int W, const double* Aq, const double* Bq,
+                         double* order_planes, double* C_planes, void* sk, cudaStream_t stream, uint64_t* launches) {
+  if (limbs > 4) return md::launch_qgemm_wide(m, n, k, limbs, Q, Aq, Bq, order_planes, C_planes, sk, stream, launches);
+  const int chunk = order_planes ? 0 : chunk_for(k, limbs, Q, W);
+  return md::launch_qgemm_packed(m, n, k, limbs, Q, chunk, Aq, Bq, order_planes, C_planes, sk, stream, launches);
 }
 
 // split A (rows) and B (columns) into the packed quarter planes of the carved workspace, then the fused quarter GEMM.
@@ -101,9 +125,7 @@ md_status gemm_impl(int m, int n, int k, int limbs, const double* A, const doubl
   if (err == cudaSuccess) err = md::launch_split_packed(m, k, limbs, Q, W, 0, A, c.Aq, c.expA, c.flags, stream, &launches);
   if (err == cudaSuccess) err = md::launch_split_packed(k, n, limbs, Q, W, 1, B, c.Bq, c.expB, c.flags, stream, &launches);
   if (ev) cudaEventRecord(ev[1], stream);
-  if (err == cudaSuccess)
-    err = limbs <= 4 ? md::launch_qgemm_packed(m, n, k, limbs, Q, c.Aq, c.Bq, order_planes, C_planes, c.sk, stream, &launches)
-                     : md::launch_qgemm_wide(m, n, k, limbs, Q, c.Aq, c.Bq, order_planes, C_planes, c.sk, stream, &launches);
+  if (err == cudaSuccess) err = launch_fused(m, n, k, limbs, Q, W, c.Aq, c.Bq, order_planes, C_planes, c.sk, stream, &launches);
   if (ev) {
     cudaEventRecord(ev[2], stream);
     if (err == cudaSuccess) g_prof.count++;
@@ -166,6 +188,11 @@ bool host_pipeline_ready(int events) {
 extern "C" {
 
 md_status md_set_option(int key, int value) {
+  if (key == MD_OPT_K_CHUNK) {  // 0 = automatic, else a chunk length: a multiple of 8
+    if (value < 0 || value % md::PACK_BK) return MD_ERR_BAD_ARG;
+    g_state.opt_k_chunk = value;
+    return MD_OK;
+  }
   if (key == MD_OPT_HOST_BLOCKS) {  // 0 = automatic, 1..32 blocks, or PR * 256 + PC (explicit panel counts, each <= 64)
     if (value < 0 || (value > 32 && (value < 256 || (value >> 8) > 64 || (value & 255) > 64))) return MD_ERR_BAD_ARG;
     g_state.opt_host_blocks = value;
@@ -189,6 +216,7 @@ int md_get_option(int key) {
     case MD_OPT_ORDERS: return g_state.opt_orders;
     case MD_OPT_SLICE_BITS: return g_state.opt_bits;
     case MD_OPT_HOST_BLOCKS: return g_state.opt_host_blocks;
+    case MD_OPT_K_CHUNK: return g_state.opt_k_chunk;
     default: return -1;
   }
 }
@@ -269,7 +297,7 @@ md_status md_gemm(int m, int n, int k, int limbs, const double* A_planes, const 
 
 md_status md_gemm_orders(int m, int n, int k, int limbs, const double* A_planes, const double* B_planes,
                          double* order_planes, md_stream stream) {
-  const md_status st = check_gemm_args(m, n, k, limbs, A_planes, B_planes, order_planes);
+  const md_status st = check_gemm_args(m, n, k, limbs, A_planes, B_planes, order_planes, true);
   if (st != MD_OK) return st;
   return gemm_impl(m, n, k, limbs, A_planes, B_planes, nullptr, order_planes, g_state.ws, g_state.ws_bytes,
                    static_cast<cudaStream_t>(stream));
@@ -294,6 +322,31 @@ md_status md_plan_slices(int k, int limbs, int* bits_out, int* quarters_out) {
   *bits_out = 13;
   *quarters_out = 4 * limbs;
   return MD_OK;
+}
+
+md_status md_plan_slices_chunked(int k, int limbs, int min_chunk, int* bits_out, int* quarters_out, int* chunk_out) {
+  if (k <= 0 || min_chunk < md::PACK_BK || !bits_out || !quarters_out || !chunk_out) return MD_ERR_BAD_ARG;
+  if (limbs != 2 && limbs != 4 && limbs != 8 && limbs != 16) return MD_ERR_BAD_ARG;
+  // as md_plan_slices, but the budget only has to hold for a chunk of at least min_chunk contraction indices where a
+  // chunked kernel exists: the fewest slices, then the widest width
+  for (int Q = 1; Q < 4 * limbs; Q++) {
+    const bool whole = md::qgemm_supported(limbs, Q) || md::qgemm_wide_supported(limbs, Q);
+    const bool chunked = md::qgemm_chunk_supported(limbs, Q);
+    if (!whole && !chunked) continue;
+    for (int W = MD_MAX_BITS; W >= MD_MIN_BITS && W * Q >= 52 * limbs; W--) {
+      if (whole && k_budget_ok(k, Q, W)) {
+        *bits_out = W, *quarters_out = Q, *chunk_out = 0;
+        return MD_OK;
+      }
+      const long long c = (1ll << (53 - 2 * W)) / Q / md::PACK_BK * md::PACK_BK;
+      if (chunked && c >= min_chunk) {
+        *bits_out = W, *quarters_out = Q, *chunk_out = (int)(c < k ? c : 0);
+        return MD_OK;
+      }
+    }
+  }
+  *chunk_out = 0;
+  return md_plan_slices(k, limbs, bits_out, quarters_out);
 }
 
 size_t md_plan_scratch_bytes(int m, int n, int k) {
@@ -442,8 +495,7 @@ md_status md_gemm_host(int m, int n, int k, int limbs, const double* A_host, con
       }
       // block (i, j): compact [limbs][mi][nj] at the position its elements have in a row-panel-major walk of C
       double* Cb = dC + (size_t)limbs * ((size_t)r0 * n + (size_t)mi * c0);
-      err = limbs <= 4 ? md::launch_qgemm_packed(mi, nj, k, limbs, Q, Aq, Bq, nullptr, Cb, c.sk, st, &launches)
-                       : md::launch_qgemm_wide(mi, nj, k, limbs, Q, Aq, Bq, nullptr, Cb, c.sk, st, &launches);
+      err = launch_fused(mi, nj, k, limbs, Q, W, Aq, Bq, nullptr, Cb, c.sk, st, &launches);
       if (err != cudaSuccess) break;
       cudaEvent_t done = ev_C[j * hp.PR + i];
       MD_TRY(cudaEventRecord(done, st));

@@ -38,9 +38,12 @@ constexpr int SK_MAX_TILES = 256;
 constexpr size_t SK_COUNTER_BYTES = 1024;  // SK_MAX_TILES unsigned ints
 size_t sk_workspace_bytes(int limbs, int quarters);
 int sk_grid();
-cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, const double* Ap, const double* Bp,
-                                double* order_planes, double* C_planes, void* sk_ws, cudaStream_t stream,
-                                uint64_t* launches);
+// chunk = 0: exact orders over the whole k.  chunk > 0 (R16; a multiple of 8, qgemm_chunk_supported instances
+// only, C_planes only): the accumulators are folded into the elements' expansions every `chunk` contraction indices.
+bool qgemm_chunk_supported(int limbs, int quarters);
+cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, int chunk, const double* Ap,
+                                const double* Bp, double* order_planes, double* C_planes, void* sk_ws,
+                                cudaStream_t stream, uint64_t* launches);
 // octo / hexa double (qgemm_wide.cu): same packed operands (k-slab depth 4), same stream-K scratch convention
 bool qgemm_wide_supported(int limbs, int quarters);
 cudaError_t launch_qgemm_wide(int m, int n, int k, int limbs, int quarters, const double* Ap, const double* Bp,

@@ -70,6 +70,38 @@ __device__ __forceinline__ void qgemm_epilogue(const double (&acc)[S][MT][NT][2]
   }
 }
 
+// Epilogue of one warp in chunked mode (qgemm_packed.cu, R16): r[i][j][e] is the (L+1)-term expansion that has
+// received every order value of every chunk; finish it (renorm_finish) and write the L limb planes.
+template <int L, int MT, int NT>
+__device__ __forceinline__ void chunk_epilogue(double (&r)[MT][NT][2][L + 1], int m, int n, int row_base, int col_base,
+                                               int lane, double* __restrict__ C_planes) {
+  const int g = lane >> 2, t4 = lane & 3;
+  const size_t planeC = (size_t)m * n;
+  const bool vec_ok = (n % 2 == 0) && ((uintptr_t)C_planes % 16 == 0);
+#pragma unroll
+  for (int i = 0; i < MT; i++) {
+    const int row = row_base + i * 8 + g;
+#pragma unroll
+    for (int j = 0; j < NT; j++) {
+      const int col = col_base + j * 8 + 2 * t4;
+      if (row >= m || col >= n) continue;
+      const size_t at = (size_t)row * n + col;
+      double o0[L], o1[L];
+      renorm_finish<L>(r[i][j][0], o0);
+      renorm_finish<L>(r[i][j][1], o1);
+#pragma unroll
+      for (int l = 0; l < L; l++) {
+        if (vec_ok) {
+          *reinterpret_cast<double2*>(C_planes + l * planeC + at) = make_double2(o0[l], o1[l]);
+        } else {
+          C_planes[l * planeC + at] = o0[l];
+          if (col + 1 < n) C_planes[l * planeC + at + 1] = o1[l];
+        }
+      }
+    }
+  }
+}
+
 // Tile rasterisation shared by both kernels: groups of GROUP_M tile rows are swept along n, so that the ~148 CTAs in
 // flight cover a near-square patch of C and share their A / B slabs through L2.
 __device__ __forceinline__ void raster_tile(int bid, int tiles_m, int tiles_n, int& tm, int& tn) {

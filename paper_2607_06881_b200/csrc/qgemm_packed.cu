@@ -49,7 +49,12 @@ struct PCfg {
   static_assert(STAGE_BYTES % 128 == 0, "stage alignment");
 };
 
-template <class C>
+// CHUNK (R16): the exactness budget k S 2^(2W) <= 2^53 is kept PER CHUNK of plan.flush_slabs slabs instead of
+// for the whole contraction: at the end of a chunk every order accumulator (still an exact sum) is added into the
+// element's (L+1)-term expansion by the TwoSum cascade of the recombination (renorm_add) and cleared.  The expansion
+// carries over the chunks; the epilogue only finishes it.  No stream-K in this mode (partial expansions cannot be
+// combined by an exact atomic add) and no order planes (the order sums of the whole k are no longer doubles).
+template <class C, bool CHUNK>
 __global__ void __launch_bounds__(C::THREADS, 1)
 qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, const double* __restrict__ Bp,
                     double* __restrict__ order_planes, double* __restrict__ C_planes, double* __restrict__ sk_scratch,
@@ -68,8 +73,9 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
   const int sk_total = plan.sk_tiles * KS;
   const int g0 = min(cta * plan.sk_iters_per_cta, sk_total), g1 = min(g0 + plan.sk_iters_per_cta, sk_total);
   const int n_sk = g1 > g0 ? (g1 - 1) / KS - g0 / KS + 1 : 0;
-  const int n_seg = n_sk + plan.dp_waves;
-  const int total_slabs = (g1 - g0) + plan.dp_waves * KS;
+  const int dp_mine = plan.dp_waves - (cta >= plan.dp_tail ? 1 : 0);  // whole tiles of this CTA
+  const int n_seg = n_sk + dp_mine;
+  const int total_slabs = (g1 - g0) + dp_mine * KS;
   auto segment = [&](int i, int& tile, int& s0, int& s1) {
     if (i < n_sk) {
       const int r = g0 / KS + i;
@@ -141,6 +147,33 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
         for (int j = 0; j < NT; j++) acc[s][i][j][0] = acc[s][i][j][1] = 0.0;
   };
   zero_acc();
+  // CHUNK: the running (L+1)-term expansion of every element this thread owns
+  double rexp[CHUNK ? MT : 1][CHUNK ? NT : 1][2][L + 1];
+  auto zero_rexp = [&]() {
+#pragma unroll
+    for (int i = 0; i < (CHUNK ? MT : 1); i++)
+#pragma unroll
+      for (int j = 0; j < (CHUNK ? NT : 1); j++)
+#pragma unroll
+        for (int e = 0; e < 2; e++)
+#pragma unroll
+          for (int l = 0; l <= L; l++) rexp[i][j][e][l] = 0.0;
+  };
+  auto flush_chunk = [&]() {  // orders from the smallest to the largest, as in renorm_orders (R9)
+    if constexpr (CHUNK) {
+#pragma unroll
+      for (int i = 0; i < MT; i++)
+#pragma unroll
+        for (int j = 0; j < NT; j++)
+#pragma unroll
+          for (int e = 0; e < 2; e++)
+#pragma unroll
+            for (int s = S - 1; s >= 0; s--) renorm_add<L>(rexp[i][j][e], acc[s][i][j][e]);
+      zero_acc();
+    }
+  };
+  if constexpr (CHUNK) zero_rexp();
+  int since_flush = 0;
 
   // Operand fragments of one DMMA k-step held in registers: all Q quarters of the warp's MT row blocks of A, and the
   // quarter-0 fragments of its NT column blocks of B (the B fragments of quarters 1.. are loaded inside the step).
@@ -183,7 +216,12 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
     int tm, tn;
     raster_tile(c_tile, plan.tiles_m, plan.tiles_n, tm, tn);
     const int row_base = tm * C::BM + wm * MT * 8, col_base = tn * C::BN + wn * NT * 8;
-    if (c_s1 - c_s0 == KS) {  // whole tile in registers
+    if constexpr (CHUNK) {     // whole tiles only: fold the last chunk in, finish the expansions, write C once
+      flush_chunk();
+      since_flush = 0;
+      chunk_epilogue<L, MT, NT>(rexp, m, n, row_base, col_base, lane, C_planes);
+      zero_rexp();
+    } else if (c_s1 - c_s0 == KS) {  // whole tile in registers
       qgemm_epilogue<S, L, MT, NT>(acc, m, n, row_base, col_base, lane, order_planes, C_planes);
     } else {                  // partial sums of a stream-K tile: exact fp64 reduction through the tile's scratch
       const int r = c_tile - plan.dp_waves * G;
@@ -252,6 +290,10 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
       st = nst;
       phase = nphase;
       if (--c_left == 0) end_of_segment();
+      else if (CHUNK && ++since_flush == plan.flush_slabs) {
+        flush_chunk();
+        since_flush = 0;
+      }
     }
   } else {  // one fragment set (register budget): loads of a k-step are issued at its start
     for (int it = 0; it < total_slabs; it++) {
@@ -272,10 +314,15 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
         phase ^= 1;
       }
       if (--c_left == 0) end_of_segment();
+      else if (CHUNK && ++since_flush == plan.flush_slabs) {
+        flush_chunk();
+        since_flush = 0;
+      }
     }
   }
 }
 
+// Exact orders over the whole k, persistent stream-K.
 template <class C>
 cudaError_t launch_cfg(int m, int n, int k, const double* Ap, const double* Bp, double* order_planes, double* C_planes,
                        void* sk_ws, cudaStream_t stream) {
@@ -285,13 +332,7 @@ cudaError_t launch_cfg(int m, int n, int k, const double* Ap, const double* Bp, 
   if (tiles > 0x7fffffffLL) return cudaErrorInvalidValue;
   const int G = sk_grid();
   if (G <= 0) return cudaErrorInvalidDevice;
-  SkPlan plan;
-  plan.KS = (k + C::BK - 1) / C::BK;
-  plan.tiles_m = tiles_m;
-  plan.tiles_n = tiles_n;
-  plan.dp_waves = (int)(tiles / G);
-  plan.sk_tiles = (int)(tiles % G);
-  plan.sk_iters_per_cta = (int)(((long long)plan.sk_tiles * plan.KS + G - 1) / G);
+  const SkPlan plan = make_sk_plan(tiles_m, tiles_n, (k + C::BK - 1) / C::BK, G);
   unsigned int* counters = static_cast<unsigned int*>(sk_ws);
   double* scratch = reinterpret_cast<double*>(static_cast<char*>(sk_ws) + SK_COUNTER_BYTES);
   cudaError_t err;
@@ -299,10 +340,34 @@ cudaError_t launch_cfg(int m, int n, int k, const double* Ap, const double* Bp, 
     err = cudaMemsetAsync(sk_ws, 0, SK_COUNTER_BYTES + sizeof(double) * (size_t)plan.sk_tiles * C::S * C::BM * C::BN, stream);
     if (err != cudaSuccess) return err;
   }
-  auto kern = qgemm_packed_kernel<C>;
+  auto kern = qgemm_packed_kernel<C, false>;
   err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
   if (err != cudaSuccess) return err;
   kern<<<G, C::THREADS, C::SMEM_BYTES, stream>>>(m, n, plan, Ap, Bp, order_planes, C_planes, scratch, counters);
+  return cudaGetLastError();
+}
+
+// Chunked accumulation (chunk = contraction indices per chunk, a multiple of BK): whole tiles only, wave after wave on the
+// persistent grid, the last wave possibly partial.
+template <class C>
+cudaError_t launch_chunked(int m, int n, int k, int chunk, const double* Ap, const double* Bp, double* C_planes,
+                           cudaStream_t stream) {
+  static_assert(C::BM == pack_bx(C::L, C::Q, 0) && C::BN == pack_bx(C::L, C::Q, 1), "tile shape must match the packed layout");
+  const int tiles_m = (m + C::BM - 1) / C::BM, tiles_n = (n + C::BN - 1) / C::BN;
+  const long long tiles = (long long)tiles_m * tiles_n;
+  if (tiles > 0x7fffffffLL || !C_planes || chunk <= 0 || chunk % C::BK) return cudaErrorInvalidValue;
+  const int G = sk_grid();
+  if (G <= 0) return cudaErrorInvalidDevice;
+  SkPlan plan = make_sk_plan(tiles_m, tiles_n, (k + C::BK - 1) / C::BK, G);
+  plan.dp_waves = (int)((tiles + G - 1) / G);
+  plan.dp_tail = tiles % G ? (int)(tiles % G) : G;
+  plan.sk_tiles = 0;
+  plan.sk_iters_per_cta = 0;
+  plan.flush_slabs = chunk / C::BK;
+  auto kern = qgemm_packed_kernel<C, true>;
+  cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+  if (err != cudaSuccess) return err;
+  kern<<<G, C::THREADS, C::SMEM_BYTES, stream>>>(m, n, plan, Ap, Bp, nullptr, C_planes, nullptr, nullptr);
   return cudaGetLastError();
 }
 
@@ -332,23 +397,31 @@ size_t sk_workspace_bytes(int limbs, int quarters) {
   return SK_COUNTER_BYTES + sizeof(double) * (size_t)SK_MAX_TILES * quarters * pack_bx(limbs, quarters, 0) * pack_bx(limbs, quarters, 1);
 }
 
-cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, const double* Ap, const double* Bp,
+bool qgemm_chunk_supported(int limbs, int quarters) { return limbs == 2 && (quarters == 5 || quarters == 6 || quarters == 8); }
+
+cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, int chunk, const double* Ap, const double* Bp,
                                 double* order_planes, double* C_planes, void* sk_ws, cudaStream_t stream,
                                 uint64_t* launches) {
   cudaError_t err = cudaErrorInvalidValue;
-  if (limbs == 2) {
-    if (quarters == 6) err = launch_cfg<PCfgDD<6>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
-    if (quarters == 7) err = launch_cfg<PCfgDD<7>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
-    if (quarters == 8) err = launch_cfg<PCfgDD<8>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
-    if (quarters == 9) err = launch_cfg<PCfgDD<9>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
-    if (quarters == 10) err = launch_cfg<PCfgDD<10>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
+#define MD_Q(CFG) err = launch_cfg<CFG>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream)
+  if (chunk > 0) {  // only the instances of qgemm_chunk_supported are compiled with the chunked kernel
+    if (limbs == 2 && quarters == 5) err = launch_chunked<PCfgDD<5>>(m, n, k, chunk, Ap, Bp, C_planes, stream);
+    if (limbs == 2 && quarters == 6) err = launch_chunked<PCfgDD<6>>(m, n, k, chunk, Ap, Bp, C_planes, stream);
+    if (limbs == 2 && quarters == 8) err = launch_chunked<PCfgDD<8>>(m, n, k, chunk, Ap, Bp, C_planes, stream);
+  } else if (limbs == 2) {
+    if (quarters == 6) MD_Q(PCfgDD<6>);
+    if (quarters == 7) MD_Q(PCfgDD<7>);
+    if (quarters == 8) MD_Q(PCfgDD<8>);
+    if (quarters == 9) MD_Q(PCfgDD<9>);
+    if (quarters == 10) MD_Q(PCfgDD<10>);
   } else if (limbs == 4) {
-    if (quarters == 11) err = launch_cfg<PCfgQDW<11>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
-    if (quarters == 12) err = launch_cfg<PCfgQDW<12>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
-    if (quarters == 16) err = launch_cfg<PCfgQD<16>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
-    if (quarters == 17) err = launch_cfg<PCfgQD<17>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
-    if (quarters == 18) err = launch_cfg<PCfgQD<18>>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
+    if (quarters == 11) MD_Q(PCfgQDW<11>);
+    if (quarters == 12) MD_Q(PCfgQDW<12>);
+    if (quarters == 16) MD_Q(PCfgQD<16>);
+    if (quarters == 17) MD_Q(PCfgQD<17>);
+    if (quarters == 18) MD_Q(PCfgQD<18>);
   }
+#undef MD_Q
   if (err == cudaSuccess) *launches += 1;
   return err;
 }

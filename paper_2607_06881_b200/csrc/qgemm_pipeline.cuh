@@ -56,6 +56,8 @@ struct SkPlan {
   int dp_waves;          // whole tiles per CTA
   int sk_tiles;          // tiles dp_waves*G .. dp_waves*G + sk_tiles - 1 are processed stream-K
   int sk_iters_per_cta;  // ipc
+  int dp_tail;           // CTAs 0 .. dp_tail-1 own a tile in the LAST of the dp_waves (all G of them unless chunked, below)
+  int flush_slabs;       // chunked accumulation (qgemm_packed.cu, R16): slabs between two flushes; 0 = never
 };
 
 // Plan for `tiles` output tiles of KS slabs each on a grid of G persistent CTAs.
@@ -68,6 +70,8 @@ inline SkPlan make_sk_plan(int tiles_m, int tiles_n, int KS, int G) {
   plan.dp_waves = (int)(tiles / G);
   plan.sk_tiles = (int)(tiles % G);
   plan.sk_iters_per_cta = (int)(((long long)plan.sk_tiles * KS + G - 1) / G);
+  plan.dp_tail = G;
+  plan.flush_slabs = 0;
   return plan;
 }
 

@@ -45,7 +45,9 @@ def test_argument_errors_need_no_gpu(lib):
     assert lib.md_gemm(4, 4, 4, 2, None, fake, fake, None) == md.MD_ERR_BAD_ARG
     assert lib.md_gemm(4, 4, 4, 2, ctypes.c_void_p(4100), fake, fake, None) == md.MD_ERR_BAD_ARG  # misaligned
     # k budget: k * S <= 2^27 (eq. 5 generalised, R6): 2^24 passes the check, 2^24 + 1 does not
-    assert lib.md_gemm(1, 1, 2 ** 24 + 1, 2, fake, fake, fake, None) == md.MD_ERR_K_TOO_LARGE
+    # (md_gemm on double double chunks the contraction beyond it, R16; md_gemm_orders and quad double cannot)
+    assert lib.md_gemm_orders(1, 1, 2 ** 24 + 1, 2, fake, fake, fake, None) == md.MD_ERR_K_TOO_LARGE
+    assert lib.md_gemm(1, 1, 2 ** 24 + 1, 2, fake, fake, fake, None) == md.MD_ERR_WORKSPACE
     assert lib.md_gemm(1, 1, 2 ** 23 + 1, 4, fake, fake, fake, None) == md.MD_ERR_K_TOO_LARGE
     assert lib.md_gemm(1, 1, 2 ** 24, 2, fake, fake, fake, None) == md.MD_ERR_WORKSPACE  # passes the checks; no workspace
     assert lib.md_split(4, 4, 3, 8, 0, fake, fake, fake, None) == md.MD_ERR_BAD_ARG
@@ -118,9 +120,13 @@ def test_slice_bits_option_and_its_k_budget(lib):
         assert lib.md_set_option(md.MD_OPT_SLICE_BITS, 19) == md.MD_OK and lib.md_get_option(md.MD_OPT_SLICE_BITS) == 19
         assert lib.md_set_option(md.MD_OPT_QUARTERS, 6) == md.MD_OK
         # k * 6 * 2^38 <= 2^53  <=>  k <= 5461
-        assert lib.md_gemm(1, 1, 5462, 2, fake, fake, fake, None) == md.MD_ERR_K_TOO_LARGE
-        assert lib.md_gemm(1, 1, 5461, 2, fake, fake, fake, None) == md.MD_ERR_WORKSPACE
-        assert lib.md_set_option(md.MD_OPT_QUARTERS, 5) == md.MD_OK
+        assert lib.md_gemm_orders(1, 1, 5462, 2, fake, fake, fake, None) == md.MD_ERR_K_TOO_LARGE
+        assert lib.md_gemm_orders(1, 1, 5461, 2, fake, fake, fake, None) == md.MD_ERR_WORKSPACE
+        assert lib.md_gemm(1, 1, 5462, 2, fake, fake, fake, None) == md.MD_ERR_WORKSPACE  # chunked (R16)
+        assert lib.md_set_option(md.MD_OPT_QUARTERS, 5) == md.MD_OK    # 5 slices: the chunked kernel only
+        assert lib.md_gemm(1, 1, 64, 2, fake, fake, fake, None) == md.MD_ERR_WORKSPACE
+        assert lib.md_gemm_orders(1, 1, 64, 2, fake, fake, fake, None) == md.MD_ERR_UNSUPPORTED
+        assert lib.md_set_option(md.MD_OPT_QUARTERS, 4) == md.MD_OK
         assert lib.md_gemm(1, 1, 64, 2, fake, fake, fake, None) == md.MD_ERR_UNSUPPORTED
     finally:
         lib.md_set_option(md.MD_OPT_SLICE_BITS, 0)
@@ -150,3 +156,17 @@ def test_plan_quarters_argument_errors(lib):
     assert lib.md_plan_quarters(64, 32, 16, 3, *args) == md.MD_ERR_BAD_ARG
     assert lib.md_plan_quarters(64, 32, 16, 2, fake, fake, fake, need - 1, 0.0, ctypes.addressof(q), None, None) == md.MD_ERR_WORKSPACE
     assert lib.md_plan_quarters(64, 32, 16, 2, fake, fake, fake, need, -1.0, ctypes.addressof(q), None, None) == md.MD_ERR_BAD_ARG
+
+
+def test_chunk_option_and_chunked_plan(lib):
+    assert lib.md_set_option(md.MD_OPT_K_CHUNK, 12) == md.MD_ERR_BAD_ARG  # a multiple of the k-slab depth 8
+    assert lib.md_set_option(md.MD_OPT_K_CHUNK, 64) == md.MD_OK and lib.md_get_option(md.MD_OPT_K_CHUNK) == 64
+    assert lib.md_set_option(md.MD_OPT_K_CHUNK, 0) == md.MD_OK
+    # double double, k = 4096, chunks of at least 256: 5 slices of 21 bits (105 >= 104 bits), 2^53 / (5 * 2^42) = 409 -> 408
+    assert md.md_plan_slices_chunked(4096, 2, 256) == (21, 5, 408)
+    assert md.md_plan_slices_chunked(300, 2, 256) == (21, 5, 0)       # fits one chunk
+    assert md.md_plan_slices_chunked(4096, 2, 1024) == (20, 6, 1360)  # no 5-slice chunk that long: 6 slices, one bit wider than unchunked
+    assert md.md_plan_slices(4096, 2) == (19, 6)
+    assert md.md_plan_slices_chunked(2048, 4, 256) == md.md_plan_slices(2048, 4) + (0,)    # quad double has no chunked kernel
+    for W, Q, c in (md.md_plan_slices_chunked(4096, 2, 256), md.md_plan_slices_chunked(65536, 2, 64)):
+        assert c % 8 == 0 and c * Q * 2 ** (2 * W) <= 2 ** 53 and W * Q >= 104

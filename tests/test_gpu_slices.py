@@ -71,9 +71,10 @@ def test_k_budget_follows_the_slice_width():
     B = torch.zeros((2, 5462, 8), dtype=torch.float64, device="cuda")
     with md.Workspace(8, 8, 5462, 2, 6, bits=19):
         with pytest.raises(md.MdError) as e:
-            md.md_gemm(A, B)
+            md.md_gemm_orders(A, B)
         assert e.value.status == md.MD_ERR_K_TOO_LARGE
-        md.md_gemm(A[:, :, :5461].contiguous(), B[:, :5461].contiguous())
+        md.md_gemm_orders(A[:, :, :5461].contiguous(), B[:, :5461].contiguous())
+        md.md_gemm(A, B)  # md_gemm chunks the contraction instead (R16)
 
 
 @pytest.mark.parametrize("cfg_idx", [2, 3, 4])
@@ -102,3 +103,64 @@ def test_full_size_with_planned_slices(cfg_idx):
     ratio = r["err"] / (TOL[L] * r["W"])
     print(f"cfg{cfg_idx} W={bits} Q={Q}: max err/(tol*W) = {ratio.max():.3g} over {si.size} samples")
     assert (ratio <= 1.0).all()
+
+
+# ---------------------------------------------------------------------------------------------- chunked accumulation (R16)
+def last_limb_close(C, Co, L):
+    """all but the last limb bit-identical, the last within the renormalisation bound of DESIGN.md R9"""
+    return bool((C[: L - 1] == Co[: L - 1]).all()) and bool((np.abs(C[L - 1] - Co[L - 1]) <= 2.0 ** -(53 * L - 3) * np.abs(Co[0]) * 64).all())
+
+
+@pytest.mark.parametrize("cfg_idx,shape", [(0, (64, 64, 1000)), (1, (150, 70, 900)), (2, (37, 51, 1700)), (2, (200, 100, 40))])
+def test_chunked_accumulation_with_planned_wide_slices(cfg_idx, shape):
+    """5 slices of 21 bits, chunks of 408 (md_plan_slices_chunked): C within 1e-28 (|A||B|)_ij of the exact product and equal
+    to the oracle's chunked pipeline up to the last limb's rounding."""
+    cfg = inputs.CONFIGS[cfg_idx].with_shape(*shape)
+    A, B = inputs.generate(cfg, "A"), inputs.generate(cfg, "B")
+    W, Q, chunk = md.md_plan_slices_chunked(4096, 2, 256)
+    assert (W, Q, chunk) == (21, 5, 408)
+    with md.Workspace(cfg.m, cfg.n, cfg.k, 2, Q, bits=W):
+        C = md.md_gemm(dev(A), dev(B)).cpu().numpy()
+        assert md.md_read_flags() == 0
+    r = orc.exact_all(A, B, C)
+    assert (r["err"] <= 1e-28 * r["W"]).all()
+    assert last_limb_close(C, orc.md_gemm_rows_chunked(A, B, 408, Q, W), 2)
+
+
+@pytest.mark.parametrize("Q,W", [(8, 13), (6, 19)])
+def test_forced_short_chunks_agree_with_the_unchunked_path(Q, W):
+    """MD_OPT_K_CHUNK = 64 on a contraction of 300 (5 chunks, the last one ragged), the paper's quarters and the 19-bit
+    slices: same result as the exact-order path up to the last limb, host entry point included."""
+    cfg = inputs.CONFIGS[1].with_shape(130, 66, 300)
+    A, B = inputs.generate(cfg, "A"), inputs.generate(cfg, "B")
+    with md.Workspace(cfg.m, cfg.n, cfg.k, 2, Q, bits=W):
+        C0 = md.md_gemm(dev(A), dev(B)).cpu().numpy()
+        md.md_set_option(md.MD_OPT_K_CHUNK, 64)
+        try:
+            C1 = md.md_gemm(dev(A), dev(B)).cpu().numpy()
+            Ch = torch.empty((2, cfg.m, cfg.n), dtype=torch.float64).pin_memory()
+            scratch = torch.empty(md.md_host_scratch_bytes(cfg.m, cfg.n, cfg.k, 2), dtype=torch.uint8, device="cuda")
+            md.md_gemm_host(torch.from_numpy(A).pin_memory(), torch.from_numpy(B).pin_memory(), Ch, scratch)
+        finally:
+            md.md_set_option(md.MD_OPT_K_CHUNK, 0)
+    assert last_limb_close(C1, C0, 2) and bool((Ch.numpy() == C1).all())
+    assert last_limb_close(C1, orc.md_gemm_rows_chunked(A, B, 64, Q, W), 2)
+    r = orc.exact_all(A, B, C1)
+    assert (r["err"] <= 1e-28 * r["W"]).all()
+
+
+def test_full_size_chunked_dd_4096():
+    """BASELINE.json configs[2] with the chunked plan (5 slices of 21 bits, chunks of 408), on samples."""
+    cfg = inputs.CONFIGS[2]
+    W, Q, chunk = md.md_plan_slices_chunked(cfg.k, 2, 256)
+    A, B = inputs.generate(cfg, "A"), inputs.generate(cfg, "B")
+    dA, dB = torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda()
+    si, sj = sample_positions(cfg, dA, dB, 512, 64)
+    with md.Workspace(cfg.m, cfg.n, cfg.k, 2, Q, bits=W):
+        Ch = md.md_gemm(dA, dB).cpu().numpy()
+        assert md.md_read_flags() == 0
+    r = orc.exact_samples(A, B, si, sj, Ch)
+    ratio = r["err"] / (1e-28 * r["W"])
+    print(f"cfg2 chunked W={W} Q={Q} chunk={chunk}: max err/(tol*W) = {ratio.max():.3g} over {si.size} samples")
+    assert (ratio <= 1.0).all()
+    assert (np.abs(Ch[1]) <= np.spacing(np.abs(Ch[0])) / 2).all()

@@ -130,3 +130,29 @@ def test_wide_slice_pipeline_reaches_the_north_star_tolerance(cfg_idx, bits, Q, 
     C = orc.md_gemm_rows(A, B, quarters=Q, bits=bits)
     r = orc.exact_all(A, B, C)
     assert (r["err"] <= tol * r["W"]).all()
+
+
+# ---------------------------------------------------------------------------------------------- chunked accumulation (R16)
+def test_chunked_pipeline_with_one_chunk_is_the_plain_pipeline():
+    cfg = small(1, 9, 7, 40)
+    A, B = inputs.generate(cfg, "A"), inputs.generate(cfg, "B")
+    for chunk in (40, 64):
+        assert (orc.md_gemm_rows_chunked(A, B, chunk, 6, 19) == orc.md_gemm_rows(A, B, quarters=6, bits=19)).all()
+
+
+@pytest.mark.parametrize("cfg_idx", [0, 1, 2])
+def test_chunked_pipeline_reaches_the_tolerance_beyond_the_whole_k_budget(cfg_idx):
+    """5 slices of 21 bits (105 bits >= the paper's 104): the budget k S 2^(2W) <= 2^53 allows 409 indices, so k = 1000 is
+    cut into chunks of 408; every chunk's order sums are exact (int64 route == fp64 route), and the result is within
+    1e-28 (|A||B|)_ij of the exact product O1."""
+    cfg = inputs.CONFIGS[cfg_idx].with_shape(6, 5, 1000)
+    A, B = inputs.generate(cfg, "A"), inputs.generate(cfg, "B")
+    assert 408 * 5 * 2 ** 42 <= 2 ** 53 < 1000 * 5 * 2 ** 42
+    C = orc.md_gemm_rows_chunked(A, B, 408, 5, 21)
+    r = orc.exact_all(A, B, C)
+    assert (r["err"] <= 1e-28 * r["W"]).all()
+    Aq, eA, _ = orc.split(A, 0, quarters=5, bits=21)
+    Bq, eB, _ = orc.split(B, 1, quarters=5, bits=21)
+    for k0 in (0, 408, 816):
+        a, b = np.ascontiguousarray(Aq[:, :, k0:k0 + 408]), np.ascontiguousarray(Bq[:, k0:k0 + 408])
+        assert (orc.orders_int(a, eA, b, eB, bits=21) == orc.orders_fp64(a, b)).all()
