@@ -81,7 +81,7 @@ Carve carve(void* base, int m, int n, int k, int limbs, int quarters) {
   c.Bq = reinterpret_cast<double*>(p + off);
   off += round_up(sizeof(double) * md::packed_doubles(n, k, md::pack_bx(limbs, quarters, 1), md::pack_bk(limbs), quarters));
   c.sk = p + off;
-  off += round_up(md::sk_workspace_bytes(limbs, quarters));
+  off += round_up(md::sk_workspace_bytes(limbs, quarters, k, chunk_for(k, limbs, quarters, slice_bits())));
   c.total = off;
   return c;
 }

@@ -36,7 +36,13 @@ cudaError_t launch_split_packed(int rows, int cols, int limbs, int quarters, int
 // order-plane tile per stream-K tile); zeroed by the launcher (a memset node on `stream`) as far as it is used.
 constexpr int SK_MAX_TILES = 256;
 constexpr size_t SK_COUNTER_BYTES = 1024;  // SK_MAX_TILES unsigned ints
-size_t sk_workspace_bytes(int limbs, int quarters);
+// chunk > 0: the chunked kernel's stream-K tail keeps one slot per (tile, chunk of the contraction) while that fits
+// SK_CHUNK_CAP_BYTES; beyond, the chunked kernel runs whole tiles only
+constexpr size_t SK_CHUNK_CAP_BYTES = (size_t)512 << 20;
+inline bool sk_chunk_scratch_fits(size_t nchunks, int S, int BM, int BN) {
+  return sizeof(double) * (size_t)SK_MAX_TILES * nchunks * S * BM * BN <= SK_CHUNK_CAP_BYTES;
+}
+size_t sk_workspace_bytes(int limbs, int quarters, int k, int chunk);
 int sk_grid();
 // chunk = 0: exact orders over the whole k.  chunk > 0 (R16; a multiple of 8, qgemm_chunk_supported instances
 // only, C_planes only): the accumulators are folded into the elements' expansions every `chunk` contraction indices.

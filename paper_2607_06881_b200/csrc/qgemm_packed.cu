@@ -50,10 +50,13 @@ struct PCfg {
 };
 
 // CHUNK (R16): the exactness budget k S 2^(2W) <= 2^53 is kept PER CHUNK of plan.flush_slabs slabs instead of
-// for the whole contraction: at the end of a chunk every order accumulator (still an exact sum) is added into the
-// element's (L+1)-term expansion by the TwoSum cascade of the recombination (renorm_add) and cleared.  The expansion
-// carries over the chunks; the epilogue only finishes it.  No stream-K in this mode (partial expansions cannot be
-// combined by an exact atomic add) and no order planes (the order sums of the whole k are no longer doubles).
+// for the whole contraction.  Chunks are the slab ranges [c * flush_slabs, (c+1) * flush_slabs) of a tile.  Whole tile: at
+// the end of a chunk every order accumulator (still an exact sum) is added into the element's (L+1)-term expansion by
+// the TwoSum cascade of the recombination (renorm_add) and cleared; the expansion carries over the chunks and the
+// epilogue only finishes it.  Stream-K part of a tile: the sums of each chunk are added into THAT CHUNK's slot of the
+// tile's scratch (exact, like the unchunked stream-K: the total of a chunk is within the budget whoever contributes), and
+// the CTA that completes the slab count runs the same renorm_add sequence over the chunks' totals -- so the result is
+// bit-identical to a whole-tile run whatever the split.  No order planes (the order sums of the whole k are not doubles).
 template <class C, bool CHUNK>
 __global__ void __launch_bounds__(C::THREADS, 1)
 qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, const double* __restrict__ Bp,
@@ -172,8 +175,28 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
       zero_acc();
     }
   };
+  // CHUNK, stream-K: chunk c of stream-K tile r has its own S * BM * BN slot in the scratch
+  auto chunk_slot = [&](int r, int c) -> double* {
+    const int nchunks = (KS + plan.flush_slabs - 1) / plan.flush_slabs;
+    return sk_scratch + ((size_t)r * nchunks + c) * (S * C::BM * C::BN) + (size_t)warp * (S * MT * NT * 64) + lane * 2;
+  };
+  auto flush_partial = [&](int r, int c) {  // exact fp64 red.add of this run's share of chunk c, then clear
+    if constexpr (CHUNK) {
+      double* sc = chunk_slot(r, c);
+#pragma unroll
+      for (int s = 0; s < S; s++)
+#pragma unroll
+        for (int i = 0; i < MT; i++)
+#pragma unroll
+          for (int j = 0; j < NT; j++) {
+            atomicAdd(sc + ((s * MT + i) * NT + j) * 64, acc[s][i][j][0]);
+            atomicAdd(sc + ((s * MT + i) * NT + j) * 64 + 1, acc[s][i][j][1]);
+          }
+      zero_acc();
+    }
+  };
   if constexpr (CHUNK) zero_rexp();
-  int since_flush = 0;
+  int c_chunk = 0, to_flush = 0;  // CHUNK: the chunk the slab being consumed belongs to; slabs left in that chunk
 
   // Operand fragments of one DMMA k-step held in registers: all Q quarters of the warp's MT row blocks of A, and the
   // quarter-0 fragments of its NT column blocks of B (the B fragments of quarters 1.. are loaded inside the step).
@@ -212,15 +235,50 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
   int c_seg = 0, c_tile, c_s0, c_s1;
   segment(0, c_tile, c_s0, c_s1);
   int c_left = c_s1 - c_s0;
+  if constexpr (CHUNK) {
+    c_chunk = c_s0 / plan.flush_slabs;
+    to_flush = plan.flush_slabs - c_s0 % plan.flush_slabs;
+  }
   auto end_of_segment = [&]() {
     int tm, tn;
     raster_tile(c_tile, plan.tiles_m, plan.tiles_n, tm, tn);
     const int row_base = tm * C::BM + wm * MT * 8, col_base = tn * C::BN + wn * NT * 8;
-    if constexpr (CHUNK) {     // whole tiles only: fold the last chunk in, finish the expansions, write C once
-      flush_chunk();
-      since_flush = 0;
-      chunk_epilogue<L, MT, NT>(rexp, m, n, row_base, col_base, lane, C_planes);
-      zero_rexp();
+    if constexpr (CHUNK) {
+      if (c_s1 - c_s0 == KS) {  // whole tile: fold the last chunk in, finish the expansions, write C once
+        flush_chunk();
+        chunk_epilogue<L, MT, NT>(rexp, m, n, row_base, col_base, lane, C_planes);
+        zero_rexp();
+      } else {                  // stream-K part: the last (possibly partial) chunk of this run, then the hand-over
+        const int r = c_tile - plan.dp_waves * G;
+        flush_partial(r, c_chunk);
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) {
+          const unsigned int mine = (unsigned int)(c_s1 - c_s0);
+          *last_flag = (atomicAdd(&sk_counters[r], mine) + mine == (unsigned int)KS);
+        }
+        __syncthreads();
+        if (*last_flag) {  // every slab of the tile is in the scratch: the chunk totals in order, as a whole-tile run would
+          __threadfence();
+          const int nchunks = (KS + plan.flush_slabs - 1) / plan.flush_slabs;
+          for (int c = 0; c < nchunks; c++) {
+            const double* sc = chunk_slot(r, c);
+#pragma unroll
+            for (int s = 0; s < S; s++)
+#pragma unroll
+              for (int i = 0; i < MT; i++)
+#pragma unroll
+                for (int j = 0; j < NT; j++) {
+                  const double2 v = __ldcg(reinterpret_cast<const double2*>(sc + ((s * MT + i) * NT + j) * 64));
+                  acc[s][i][j][0] = v.x;
+                  acc[s][i][j][1] = v.y;
+                }
+            flush_chunk();
+          }
+          chunk_epilogue<L, MT, NT>(rexp, m, n, row_base, col_base, lane, C_planes);
+          zero_rexp();
+        }
+      }
     } else if (c_s1 - c_s0 == KS) {  // whole tile in registers
       qgemm_epilogue<S, L, MT, NT>(acc, m, n, row_base, col_base, lane, order_planes, C_planes);
     } else {                  // partial sums of a stream-K tile: exact fp64 reduction through the tile's scratch
@@ -261,6 +319,21 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
     if (++c_seg < n_seg) {
       segment(c_seg, c_tile, c_s0, c_s1);
       c_left = c_s1 - c_s0;
+      if constexpr (CHUNK) {
+        c_chunk = c_s0 / plan.flush_slabs;
+        to_flush = plan.flush_slabs - c_s0 % plan.flush_slabs;
+      }
+    }
+  };
+  // CHUNK: after a slab of the current segment -- at a chunk boundary inside the segment fold the chunk away
+  auto after_slab = [&]() {
+    if constexpr (CHUNK) {
+      if (--to_flush == 0 && c_left > 0) {
+        if (c_s1 - c_s0 == KS) flush_chunk();
+        else flush_partial(c_tile - plan.dp_waves * G, c_chunk);
+        c_chunk++;
+        to_flush = plan.flush_slabs;
+      }
     }
   };
 
@@ -289,11 +362,9 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
       if (lane == 0) mbar_arrive(empty_u32 + 8 * st);  // this warp is done reading the stage
       st = nst;
       phase = nphase;
-      if (--c_left == 0) end_of_segment();
-      else if (CHUNK && ++since_flush == plan.flush_slabs) {
-        flush_chunk();
-        since_flush = 0;
-      }
+      --c_left;
+      after_slab();
+      if (c_left == 0) end_of_segment();
     }
   } else {  // one fragment set (register budget): loads of a k-step are issued at its start
     for (int it = 0; it < total_slabs; it++) {
@@ -313,11 +384,9 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
         st = 0;
         phase ^= 1;
       }
-      if (--c_left == 0) end_of_segment();
-      else if (CHUNK && ++since_flush == plan.flush_slabs) {
-        flush_chunk();
-        since_flush = 0;
-      }
+      --c_left;
+      after_slab();
+      if (c_left == 0) end_of_segment();
     }
   }
 }
@@ -351,7 +420,7 @@ cudaError_t launch_cfg(int m, int n, int k, const double* Ap, const double* Bp, 
 // persistent grid, the last wave possibly partial.
 template <class C>
 cudaError_t launch_chunked(int m, int n, int k, int chunk, const double* Ap, const double* Bp, double* C_planes,
-                           cudaStream_t stream) {
+                           void* sk_ws, cudaStream_t stream) {
   static_assert(C::BM == pack_bx(C::L, C::Q, 0) && C::BN == pack_bx(C::L, C::Q, 1), "tile shape must match the packed layout");
   const int tiles_m = (m + C::BM - 1) / C::BM, tiles_n = (n + C::BN - 1) / C::BN;
   const long long tiles = (long long)tiles_m * tiles_n;
@@ -359,15 +428,26 @@ cudaError_t launch_chunked(int m, int n, int k, int chunk, const double* Ap, con
   const int G = sk_grid();
   if (G <= 0) return cudaErrorInvalidDevice;
   SkPlan plan = make_sk_plan(tiles_m, tiles_n, (k + C::BK - 1) / C::BK, G);
-  plan.dp_waves = (int)((tiles + G - 1) / G);
-  plan.dp_tail = tiles % G ? (int)(tiles % G) : G;
-  plan.sk_tiles = 0;
-  plan.sk_iters_per_cta = 0;
   plan.flush_slabs = chunk / C::BK;
+  const size_t nchunks = ((size_t)plan.KS + plan.flush_slabs - 1) / plan.flush_slabs;
+  unsigned int* counters = static_cast<unsigned int*>(sk_ws);
+  double* scratch = reinterpret_cast<double*>(static_cast<char*>(sk_ws) + SK_COUNTER_BYTES);
+  cudaError_t err;
+  if (sk_chunk_scratch_fits(nchunks, C::S, C::BM, C::BN)) {  // stream-K tail, one scratch slot per (tile, chunk)
+    if (plan.sk_tiles > 0) {
+      err = cudaMemsetAsync(sk_ws, 0, SK_COUNTER_BYTES + sizeof(double) * plan.sk_tiles * nchunks * C::S * C::BM * C::BN, stream);
+      if (err != cudaSuccess) return err;
+    }
+  } else {  // too many chunks for the scratch (a very long contraction): whole tiles only, the last wave partial
+    plan.dp_waves = (int)((tiles + G - 1) / G);
+    plan.dp_tail = tiles % G ? (int)(tiles % G) : G;
+    plan.sk_tiles = 0;
+    plan.sk_iters_per_cta = 0;
+  }
   auto kern = qgemm_packed_kernel<C, true>;
-  cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+  err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
   if (err != cudaSuccess) return err;
-  kern<<<G, C::THREADS, C::SMEM_BYTES, stream>>>(m, n, plan, Ap, Bp, nullptr, C_planes, nullptr, nullptr);
+  kern<<<G, C::THREADS, C::SMEM_BYTES, stream>>>(m, n, plan, Ap, Bp, nullptr, C_planes, scratch, counters);
   return cudaGetLastError();
 }
 
@@ -393,8 +473,15 @@ int sk_grid() {
   return sms < SK_MAX_TILES ? sms : SK_MAX_TILES;
 }
 
-size_t sk_workspace_bytes(int limbs, int quarters) {
-  return SK_COUNTER_BYTES + sizeof(double) * (size_t)SK_MAX_TILES * quarters * pack_bx(limbs, quarters, 0) * pack_bx(limbs, quarters, 1);
+// chunk > 0 (chunked accumulation): one slot per (stream-K tile, chunk) as long as that stays below SK_CHUNK_CAP_BYTES
+size_t sk_workspace_bytes(int limbs, int quarters, int k, int chunk) {
+  const size_t tile = sizeof(double) * (size_t)quarters * pack_bx(limbs, quarters, 0) * pack_bx(limbs, quarters, 1);
+  size_t slots = SK_MAX_TILES;
+  if (chunk > 0) {
+    const size_t nchunks = ((size_t)k + chunk - 1) / chunk;
+    if (sk_chunk_scratch_fits(nchunks, quarters, pack_bx(limbs, quarters, 0), pack_bx(limbs, quarters, 1))) slots *= nchunks;
+  }
+  return SK_COUNTER_BYTES + tile * slots;
 }
 
 bool qgemm_chunk_supported(int limbs, int quarters) { return limbs == 2 && (quarters == 5 || quarters == 6 || quarters == 8); }
@@ -405,9 +492,9 @@ cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, in
   cudaError_t err = cudaErrorInvalidValue;
 #define MD_Q(CFG) err = launch_cfg<CFG>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream)
   if (chunk > 0) {  // only the instances of qgemm_chunk_supported are compiled with the chunked kernel
-    if (limbs == 2 && quarters == 5) err = launch_chunked<PCfgDD<5>>(m, n, k, chunk, Ap, Bp, C_planes, stream);
-    if (limbs == 2 && quarters == 6) err = launch_chunked<PCfgDD<6>>(m, n, k, chunk, Ap, Bp, C_planes, stream);
-    if (limbs == 2 && quarters == 8) err = launch_chunked<PCfgDD<8>>(m, n, k, chunk, Ap, Bp, C_planes, stream);
+    if (limbs == 2 && quarters == 5) err = launch_chunked<PCfgDD<5>>(m, n, k, chunk, Ap, Bp, C_planes, sk_ws, stream);
+    if (limbs == 2 && quarters == 6) err = launch_chunked<PCfgDD<6>>(m, n, k, chunk, Ap, Bp, C_planes, sk_ws, stream);
+    if (limbs == 2 && quarters == 8) err = launch_chunked<PCfgDD<8>>(m, n, k, chunk, Ap, Bp, C_planes, sk_ws, stream);
   } else if (limbs == 2) {
     if (quarters == 6) MD_Q(PCfgDD<6>);
     if (quarters == 7) MD_Q(PCfgDD<7>);

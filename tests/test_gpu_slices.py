@@ -135,14 +135,15 @@ def test_forced_short_chunks_agree_with_the_unchunked_path(Q, W):
     A, B = inputs.generate(cfg, "A"), inputs.generate(cfg, "B")
     with md.Workspace(cfg.m, cfg.n, cfg.k, 2, Q, bits=W):
         C0 = md.md_gemm(dev(A), dev(B)).cpu().numpy()
-        md.md_set_option(md.MD_OPT_K_CHUNK, 64)
-        try:
+    md.md_set_option(md.MD_OPT_K_CHUNK, 64)  # before the workspace is sized: the chunked stream-K scratch depends on it
+    try:
+        with md.Workspace(cfg.m, cfg.n, cfg.k, 2, Q, bits=W):
             C1 = md.md_gemm(dev(A), dev(B)).cpu().numpy()
             Ch = torch.empty((2, cfg.m, cfg.n), dtype=torch.float64).pin_memory()
             scratch = torch.empty(md.md_host_scratch_bytes(cfg.m, cfg.n, cfg.k, 2), dtype=torch.uint8, device="cuda")
             md.md_gemm_host(torch.from_numpy(A).pin_memory(), torch.from_numpy(B).pin_memory(), Ch, scratch)
-        finally:
-            md.md_set_option(md.MD_OPT_K_CHUNK, 0)
+    finally:
+        md.md_set_option(md.MD_OPT_K_CHUNK, 0)
     assert last_limb_close(C1, C0, 2) and bool((Ch.numpy() == C1).all())
     assert last_limb_close(C1, orc.md_gemm_rows_chunked(A, B, 64, Q, W), 2)
     r = orc.exact_all(A, B, C1)
@@ -164,3 +165,23 @@ def test_full_size_chunked_dd_4096():
     print(f"cfg2 chunked W={W} Q={Q} chunk={chunk}: max err/(tol*W) = {ratio.max():.3g} over {si.size} samples")
     assert (ratio <= 1.0).all()
     assert (np.abs(Ch[1]) <= np.spacing(np.abs(Ch[0])) / 2).all()
+
+
+def test_chunked_stream_k_tail_is_bit_identical_to_whole_tiles():
+    """The chunked kernel's stream-K tail adds each chunk's exact sums into that chunk's scratch slot and the finishing CTA
+    replays the renorm_add sequence, so cutting tiles along k must not change a bit: a 600 x 600 problem (190 tiles on 148
+    CTAs: 42 tiles are cut) against the same rows computed as part of a problem whose tiles are all whole-wave (a 64 x 32
+    block = 1 tile, processed whole)."""
+    cfg = inputs.CONFIGS[2].with_shape(600, 600, 1000)
+    A, B = inputs.generate(cfg, "A"), inputs.generate(cfg, "B")
+    W, Q = 21, 5
+    with md.Workspace(cfg.m, cfg.n, cfg.k, 2, Q, bits=W):
+        C = md.md_gemm(dev(A), dev(B)).cpu().numpy()
+    for (r0, c0) in ((0, 0), (512, 576), (320, 96)):  # single-tile problems: never cut along k
+        Ab, Bb = np.ascontiguousarray(A[:, r0:r0 + 64]), np.ascontiguousarray(B[:, :, c0:c0 + 32])
+        mb, nb = Ab.shape[1], Bb.shape[2]
+        with md.Workspace(mb, nb, cfg.k, 2, Q, bits=W):
+            Cb = md.md_gemm(dev(Ab), dev(Bb)).cpu().numpy()
+        assert bool((C[:, r0:r0 + mb, c0:c0 + nb] == Cb).all())
+    r = orc.exact_samples(A, B, *inputs.sample_indices(cfg, 256), C)
+    assert (r["err"] <= 1e-28 * r["W"]).all()
