@@ -56,7 +56,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
                 if res.returncode:
                     raise RuntimeError("nvcc failed: " + " ".join(cmd))
     if jobs or force or _stale(LIB, objs):
-        subprocess.check_call([nvcc, "-shared", "-o", LIB] + objs)
+        subprocess.check_call([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs)
     build_compare(nvcc, force, verbose)
     return LIB
 
