@@ -20,7 +20,10 @@
 //   O4  oracle_renorm       sum of the S order values -> L non-overlapping limbs
 //   O5  oracle_classic_gemm classical multiple-double GEMM on "regular cores", cross-check
 //   --  oracle_md_gemm      O2 -> O3 (fp64 route) -> O4, the paper's 5-step algorithm
-// Parity status: every function above has an independent pin; none is "parity unpinned".
+//   --  oracle_md_gemm_rows_chunked_w   the same with the order sums formed exactly per chunk of k (R16)
+//   --  oracle_plan_quarters            the quarter count a given input needs for a tolerance (R15)
+// Parity status: every function above has an independent pin (tests/test_oracle_*.py: accumulator, split, orders,
+// renorm_exact, wide, slices, plan); none is "parity unpinned".
 
 #include <cmath>
 #include <cstdint>
