@@ -59,7 +59,7 @@ def parse_args():
     ap.add_argument("--slices", default="paper", choices=["paper", "adaptive", "chunked"],
                     help="paper: 13-bit quarters, 4 per limb (the headline).  adaptive: the (bits, count) md_plan_slices "
                          "picks for this k -- wider, fewer slices (DESIGN.md R14; NOT the paper's quarters).  chunked: "
-                         "md_plan_slices_chunked(k, limbs, 256) -- still wider slices, exact per chunk of k (DESIGN.md R16)")
+                         "md_plan_slices_chunked(k, limbs, 128) -- still wider slices, exact per chunk of k (DESIGN.md R16)")
     ap.add_argument("--paper-paths", action="store_true",
                     help="also time the paper's own two paths on this GPU (libmdcompare: materialised top-down product "
                          "through cuBLAS DGEMM, CUDA-core classical GEMM; SURVEY.md 8(f) NEXT-2), outside the timed region")
@@ -209,7 +209,7 @@ def run_ours(args):
     if args.slices == "adaptive":
         base = base.with_slices(*md.md_plan_slices(base.k, base.limbs))
     elif args.slices == "chunked":
-        base = base.with_slices(*md.md_plan_slices_chunked(base.k, base.limbs, 256)[:2])
+        base = base.with_slices(*md.md_plan_slices_chunked(base.k, base.limbs, 128)[:2])
     cfg = base.with_shape(m=base.m * world)
     row0, row1 = shard.row_block(cfg.m, world, rank)
     m, n, k, L, Q, W = row1 - row0, cfg.n, cfg.k, cfg.limbs, cfg.quarters, cfg.bits
@@ -296,13 +296,13 @@ def run_ours(args):
                 "max_abs_diff_vs_paper_quarters": float((C2 - C).abs().sum(dim=0).max()), "note": note}
 
     if args.slices == "paper" and world == 1:
-        cW, cQ, cK = md.md_plan_slices_chunked(k, L, 256)
+        cW, cQ, cK = md.md_plan_slices_chunked(k, L, 128)
         aW, aQ = md.md_plan_slices(k, L)
         if (aW, aQ) != (W, Q):
             adaptive = time_variant(aW, aQ, "md_plan_slices: wider, fewer slices on the same kernels (DESIGN.md R14); not the "
                                             "paper's 13-bit quarters, so not the headline; 3 steps after 1 warm-up, CUDA events")
             if (cW, cQ) != (aW, aQ):
-                adaptive["chunked"] = time_variant(cW, cQ, "md_plan_slices_chunked(k, limbs, 256): exactness kept per chunk of %d "
+                adaptive["chunked"] = time_variant(cW, cQ, "md_plan_slices_chunked(k, limbs, 128): exactness kept per chunk of %d "
                                                            "contraction indices (DESIGN.md R16)" % cK)
                 adaptive["chunked"]["chunk"] = cK
 

@@ -67,7 +67,7 @@ enum {
                            exactness budget becomes k * orders * 2^(2W) <= 2^53.  With wider slices fewer are needed:
                            set MD_OPT_QUARTERS to the slice count (limbs=2: 6, 7; limbs=4: 11, 12; limbs=8: 22; limbs=16: 44), or
                            take both from md_plan_slices. */
-  MD_OPT_K_CHUNK = 5,    /* md_gemm / md_gemm_host, double double only (R16): length of the chunks of the
+  MD_OPT_K_CHUNK = 5,    /* md_gemm / md_gemm_host, double double (5, 6, 8 slices) and quad double (10 slices) (R16): length of the chunks of the
                             contraction over which the accumulations are kept exact.  Default 0 = automatic: chunking is
                             used only when k exceeds the exactness budget k * orders * 2^(2W) <= 2^53, with the largest
                             chunk the budget allows; a value (a multiple of 8) forces a shorter chunk.  Within a chunk
@@ -86,7 +86,7 @@ int md_get_option(int key); /* current value (0 = default), or -1 for an unknown
  * own split, when nothing wider qualifies.  Launches nothing and changes no option. */
 md_status md_plan_slices(int k, int limbs, int* bits_out, int* quarters_out);
 /* The same with chunked accumulation allowed (MD_OPT_K_CHUNK, R16): the budget only has to hold for a chunk of at
- * least min_chunk (>= 8) contraction indices where a chunked kernel exists (double double: 5, 6, 8 slices), which admits
+ * least min_chunk (>= 8) contraction indices where a chunked kernel exists (double double: 5, 6, 8 slices; quad double: 10), which admits
  * wider and fewer slices: double double at k = 4096 gets 5 slices of 21 bits in chunks of 408 (15 products instead of 21).
  * *chunk_out = the chunk md_gemm will use, 0 when this k needs none.  md_gemm_orders is not available beyond the budget. */
 md_status md_plan_slices_chunked(int k, int limbs, int min_chunk, int* bits_out, int* quarters_out, int* chunk_out);

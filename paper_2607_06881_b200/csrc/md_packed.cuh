@@ -26,7 +26,8 @@ __host__ __device__ constexpr int pack_bk(int limbs) { return limbs <= 4 ? PACK_
 // (dd 64 x 32, qd 32 x 16 -- 64 x 32 with the 11 / 12 wide slices of MD_OPT_SLICE_BITS, whose accumulators leave room for
 // four 8x8 tiles per warp: qgemm_packed.cu; od 32 x 16, hd 16 x 8 -- 16 x 16 in 44 wide slices: qgemm_wide.cu).
 __host__ __device__ constexpr int pack_bx(int limbs, int quarters, int axis) {
-  return (limbs == 2 || (limbs == 4 && quarters <= 12)) ? (axis == 0 ? 64 : 32)
+  return (limbs == 4 && quarters <= 10) ? (axis == 0 ? 64 : 16)  // quad double, chunked accumulation: 16 x 8 warp tile
+         : (limbs == 2 || (limbs == 4 && quarters <= 12)) ? (axis == 0 ? 64 : 32)
          : limbs == 16 ? (axis == 0 ? 16 : (quarters <= 44 ? 16 : 8)) : (axis == 0 ? 32 : 16);
 }
 

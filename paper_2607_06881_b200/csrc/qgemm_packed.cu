@@ -458,6 +458,9 @@ template <int Q> using PCfgQD = PCfg<Q, 4, 4, 2, 1, 1>;
 // quad double in 11 / 12 wide slices (MD_OPT_SLICE_BITS): 22 / 24 accumulator registers per 8x8 tile leave room for the
 // double-double warp tile (16 x 16), which halves the LDS and L2 traffic per DMMA and doubles the DMMAs per slab
 template <int Q> using PCfgQDW = PCfg<Q, 4, 4, 2, 2, 2>;
+// quad double with chunked accumulation (10 slices): the expansions of the elements (5 terms each) live in registers
+// beside the accumulators, so the warp tile is 16 x 8 (64 x 16 CTA tile)
+template <int Q> using PCfgQDC = PCfg<Q, 4, 4, 2, 2, 1>;
 
 }  // namespace
 
@@ -484,7 +487,9 @@ size_t sk_workspace_bytes(int limbs, int quarters, int k, int chunk) {
   return SK_COUNTER_BYTES + tile * slots;
 }
 
-bool qgemm_chunk_supported(int limbs, int quarters) { return limbs == 2 && (quarters == 5 || quarters == 6 || quarters == 8); }
+bool qgemm_chunk_supported(int limbs, int quarters) {
+  return (limbs == 2 && (quarters == 5 || quarters == 6 || quarters == 8)) || (limbs == 4 && quarters == 10);
+}
 
 cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, int chunk, const double* Ap, const double* Bp,
                                 double* order_planes, double* C_planes, void* sk_ws, cudaStream_t stream,
@@ -495,6 +500,7 @@ cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, in
     if (limbs == 2 && quarters == 5) err = launch_chunked<PCfgDD<5>>(m, n, k, chunk, Ap, Bp, C_planes, sk_ws, stream);
     if (limbs == 2 && quarters == 6) err = launch_chunked<PCfgDD<6>>(m, n, k, chunk, Ap, Bp, C_planes, sk_ws, stream);
     if (limbs == 2 && quarters == 8) err = launch_chunked<PCfgDD<8>>(m, n, k, chunk, Ap, Bp, C_planes, sk_ws, stream);
+    if (limbs == 4 && quarters == 10) err = launch_chunked<PCfgQDC<10>>(m, n, k, chunk, Ap, Bp, C_planes, sk_ws, stream);
   } else if (limbs == 2) {
     if (quarters == 6) MD_Q(PCfgDD<6>);
     if (quarters == 7) MD_Q(PCfgDD<7>);

@@ -51,7 +51,7 @@ def main():
         sj = np.concatenate([sj, flat % cfg.n]).astype(np.int64)
         pq, pd = md.md_plan_quarters(dA, dB)
         plans = [("paper's quarters", cfg.bits, cfg.quarters, 0), ("md_plan_slices",) + md.md_plan_slices(cfg.k, L) + (0,)]
-        cw, cq, ck = md.md_plan_slices_chunked(cfg.k, L, 256)
+        cw, cq, ck = md.md_plan_slices_chunked(cfg.k, L, 128)
         if (cw, cq) != plans[1][1:3]:
             plans.append(("md_plan_slices_chunked", cw, cq, ck))
         for name, W, Q, chunk in plans:

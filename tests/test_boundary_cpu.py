@@ -167,6 +167,8 @@ def test_chunk_option_and_chunked_plan(lib):
     assert md.md_plan_slices_chunked(300, 2, 256) == (21, 5, 0)       # fits one chunk
     assert md.md_plan_slices_chunked(4096, 2, 1024) == (20, 6, 1360)  # no 5-slice chunk that long: 6 slices, one bit wider than unchunked
     assert md.md_plan_slices(4096, 2) == (19, 6)
-    assert md.md_plan_slices_chunked(2048, 4, 256) == md.md_plan_slices(2048, 4) + (0,)    # quad double has no chunked kernel
+    assert md.md_plan_slices_chunked(2048, 4, 256) == md.md_plan_slices(2048, 4) + (0,)    # quad double: no chunk that long
+    assert md.md_plan_slices_chunked(2048, 4, 128) == (21, 10, 200)   # 10 slices of 21 bits (210 >= 208), 2^11 / 10 = 204 -> 200
+    assert md.md_plan_slices_chunked(1024, 8, 64) == md.md_plan_slices(1024, 8) + (0,)     # octo double has no chunked kernel
     for W, Q, c in (md.md_plan_slices_chunked(4096, 2, 256), md.md_plan_slices_chunked(65536, 2, 64)):
         assert c % 8 == 0 and c * Q * 2 ** (2 * W) <= 2 ** 53 and W * Q >= 104

@@ -185,3 +185,18 @@ def test_chunked_stream_k_tail_is_bit_identical_to_whole_tiles():
         assert bool((C[:, r0:r0 + mb, c0:c0 + nb] == Cb).all())
     r = orc.exact_samples(A, B, *inputs.sample_indices(cfg, 256), C)
     assert (r["err"] <= 1e-28 * r["W"]).all()
+
+
+@pytest.mark.parametrize("shape", [(70, 45, 500), (130, 40, 90)])
+def test_chunked_accumulation_quad_double(shape):
+    """Quad double in 10 slices of 21 bits, chunks of 200 (md_plan_slices_chunked(2048, 4, 128)): C within 1e-58 (|A||B|)_ij
+    and equal to the oracle's chunked pipeline up to the last limb."""
+    assert md.md_plan_slices_chunked(2048, 4, 128) == (21, 10, 200)
+    cfg = inputs.CONFIGS[4].with_shape(*shape)
+    A, B = inputs.generate(cfg, "A"), inputs.generate(cfg, "B")
+    with md.Workspace(cfg.m, cfg.n, cfg.k, 4, 10, bits=21):
+        C = md.md_gemm(dev(A), dev(B)).cpu().numpy()
+        assert md.md_read_flags() == 0
+    r = orc.exact_all(A, B, C)
+    assert (r["err"] <= 1e-58 * r["W"]).all()
+    assert last_limb_close(C, orc.md_gemm_rows_chunked(A, B, 200, 10, 21), 4)
