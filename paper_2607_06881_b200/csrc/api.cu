@@ -16,6 +16,7 @@ struct State {
   int opt_quarters = 0;  // 0 = default (4 * limbs)
   int opt_orders = 0;    // 0 = default (= quarters)
   int opt_bits = 0;      // 0 = default (13, the paper's quarter)
+  int opt_fused_prep = 0;  // 0 = automatic (small / medium operands), 1 = always, 2 = never
   int opt_k_chunk = 0;   // 0 = chunked accumulation only when k exceeds the exactness budget; else the chunk length to force
   int opt_host_blocks = 0;  // md_gemm_host: 0 = automatic panel plan, else the number of blocks of C (1 = no pipelining)
   void* ws = nullptr;
@@ -101,6 +102,15 @@ md_status check_gemm_args(int m, int n, int k, int limbs, const void* A, const v
   return MD_OK;
 }
 
+// Fused preparation (one launch for both exponent vectors and both packed splits) where the operands are so small that the
+// latencies of five dependent launches dominate (each block owns 32 groups over the whole contraction, so the kernel has
+// little parallelism: it loses against the separate kernels from about 384^3 on)
+inline bool use_fused_prep(int m, int n, int k) {
+  if (g_state.opt_fused_prep == 1) return true;
+  if (g_state.opt_fused_prep == 2) return false;
+  return ((long long)m + n) * k <= (1ll << 17);  // measured: 43 -> 31 us at 64^3, 50 -> 38 us at 128^3, even at 256^3, slower beyond
+}
+
 // the fused quarter GEMM of one (block of a) problem on packed operands: double / quad double (chunked when md_gemm asks
 // for C of a contraction beyond the exactness budget), octo / hexa double
 cudaError_t launch_fused(int m, int n, int k, int limbs, int Q, int W, const double* Aq, const double* Bq,
@@ -120,10 +130,15 @@ md_status gemm_impl(int m, int n, int k, int limbs, const double* A, const doubl
   uint64_t launches = 0;
   cudaEvent_t* ev = (g_prof.count < g_prof.capacity) ? &g_prof.ev[3 * (size_t)g_prof.count] : nullptr;
   if (ev) cudaEventRecord(ev[0], stream);
-  cudaError_t err = md::launch_exponents(m, k, 0, Q, W, A, c.expA, c.flags, stream, &launches);
-  if (err == cudaSuccess) err = md::launch_exponents(k, n, 1, Q, W, B, c.expB, c.flags, stream, &launches);
-  if (err == cudaSuccess) err = md::launch_split_packed(m, k, limbs, Q, W, 0, A, c.Aq, c.expA, c.flags, stream, &launches);
-  if (err == cudaSuccess) err = md::launch_split_packed(k, n, limbs, Q, W, 1, B, c.Bq, c.expB, c.flags, stream, &launches);
+  cudaError_t err;
+  if (use_fused_prep(m, n, k)) {  // one launch instead of five: what matters below ~1024^3
+    err = md::launch_prep_packed(m, n, k, limbs, Q, W, A, B, c.Aq, c.Bq, c.expA, c.expB, c.flags, stream, &launches);
+  } else {
+    err = md::launch_exponents(m, k, 0, Q, W, A, c.expA, c.flags, stream, &launches);
+    if (err == cudaSuccess) err = md::launch_exponents(k, n, 1, Q, W, B, c.expB, c.flags, stream, &launches);
+    if (err == cudaSuccess) err = md::launch_split_packed(m, k, limbs, Q, W, 0, A, c.Aq, c.expA, c.flags, stream, &launches);
+    if (err == cudaSuccess) err = md::launch_split_packed(k, n, limbs, Q, W, 1, B, c.Bq, c.expB, c.flags, stream, &launches);
+  }
   if (ev) cudaEventRecord(ev[1], stream);
   if (err == cudaSuccess) err = launch_fused(m, n, k, limbs, Q, W, c.Aq, c.Bq, order_planes, C_planes, c.sk, stream, &launches);
   if (ev) {
@@ -193,6 +208,11 @@ md_status md_set_option(int key, int value) {
     g_state.opt_k_chunk = value;
     return MD_OK;
   }
+  if (key == MD_OPT_FUSED_PREP) {
+    if (value < 0 || value > 2) return MD_ERR_BAD_ARG;
+    g_state.opt_fused_prep = value;
+    return MD_OK;
+  }
   if (key == MD_OPT_HOST_BLOCKS) {  // 0 = automatic, 1..32 blocks, or PR * 256 + PC (explicit panel counts, each <= 64)
     if (value < 0 || (value > 32 && (value < 256 || (value >> 8) > 64 || (value & 255) > 64))) return MD_ERR_BAD_ARG;
     g_state.opt_host_blocks = value;
@@ -217,6 +237,7 @@ int md_get_option(int key) {
     case MD_OPT_SLICE_BITS: return g_state.opt_bits;
     case MD_OPT_HOST_BLOCKS: return g_state.opt_host_blocks;
     case MD_OPT_K_CHUNK: return g_state.opt_k_chunk;
+    case MD_OPT_FUSED_PREP: return g_state.opt_fused_prep;
     default: return -1;
   }
 }

@@ -32,6 +32,10 @@ cudaError_t launch_spread(int m, int n, const double* W, const int32_t* expA, co
 cudaError_t launch_split_packed(int rows, int cols, int limbs, int quarters, int bits, int axis, const double* planes,
                                 double* packed, const int32_t* exps, uint32_t* flags, cudaStream_t stream,
                                 uint64_t* launches);
+// exponent vectors + packed quarter planes of BOTH operands in one launch (small and medium problems: md_gemm's fused prep)
+cudaError_t launch_prep_packed(int m, int n, int k, int limbs, int quarters, int bits, const double* A, const double* B,
+                               double* Ap, double* Bp, int32_t* expA, int32_t* expB, uint32_t* flags, cudaStream_t stream,
+                               uint64_t* launches);
 // sk_ws: sk_workspace_bytes(limbs, quarters) bytes of device scratch for the stream-K tail (slab counters + one
 // order-plane tile per stream-K tile); zeroed by the launcher (a memset node on `stream`) as far as it is used.
 constexpr int SK_MAX_TILES = 256;

@@ -142,19 +142,14 @@ __device__ __forceinline__ void stg_256(double* p, double a, double b, double c,
 // tiles and k-slabs).  A thread owns one fragment row: group x (row of A, AXIS 0 / column of B, AXIS 1) and the four
 // contraction indices k = 4*k4g .. 4*k4g+3, i.e. 32 contiguous output bytes per quarter; the 32 lanes of a warp take 32
 // consecutive x, so a warp writes 1 KB contiguous per quarter (and, for B, reads 256 contiguous bytes per row).
+// One fragment row of the packed layout: group x (row of A, AXIS 0 / column of B, AXIS 1), contraction indices k0 .. k0+3,
+// all Q slices.  E = the group's exponent.  Zero padding outside the matrix.
 template <int L, int AXIS>
-__global__ void __launch_bounds__(256) split_packed_kernel(int rows, int cols, int Q, int bits, int bx, int bk, int x_blocks, int KS,
-                                                           const double* __restrict__ planes,
-                                                           double* __restrict__ packed,
-                                                           const int32_t* __restrict__ exps, uint32_t* flags) {
+__device__ __forceinline__ void split_fragment_row(int rows, int cols, int Q, int bits, int bx, int bk, int KS, int x, int k0,
+                                                   int E, const double* __restrict__ planes, double* __restrict__ packed,
+                                                   uint32_t* flags) {
   const int X = AXIS == 0 ? rows : cols, K = AXIS == 0 ? cols : rows;
-  const int x = (blockIdx.x % x_blocks) * 32 + (threadIdx.x & 31);
-  const int k4g = (blockIdx.x / x_blocks) * 8 + (threadIdx.x >> 5);  // group of four k
-  const int XP = (X + bx - 1) / bx * bx;                             // padded to whole tiles
-  if (k4g >= KS * (bk / 4) || x >= XP) return;
-  const int k0 = k4g * 4;
   const size_t plane = (size_t)rows * cols;
-
   double r[4][L];
   const bool x_ok = x < X;
   if (AXIS == 0) {
@@ -177,7 +172,6 @@ __global__ void __launch_bounds__(256) split_packed_kernel(int rows, int cols, i
       for (int t = 0; t < 4; t++)
         r[t][l] = (x_ok && k0 + t < K) ? planes[l * plane + (size_t)(k0 + t) * cols + x] : 0.0;
   }
-  const int E = x_ok ? exps[x] : 0;
   bool bad = false;
 #pragma unroll
   for (int t = 0; t < 4; t++) bad |= any_nonfinite<L>(r[t]);
@@ -191,6 +185,71 @@ __global__ void __launch_bounds__(256) split_packed_kernel(int rows, int cols, i
 #pragma unroll
     for (int t = 0; t < 4; t++) d[t] = extract_digit<L>(r[t], E, q, bits);
     stg_256(dst + q * q_stride, d[0], d[1], d[2], d[3]);  // a fragment row; the warp writes 1 KB contiguous
+  }
+}
+
+// md_gemm's splitter: same digits, written in the fragment-major packed layout of md_packed.cuh (zero padded to whole
+// tiles and k-slabs).  A thread owns one fragment row: group x and the four contraction indices k = 4*k4g .. 4*k4g+3, i.e.
+// 32 contiguous output bytes per quarter; the 32 lanes of a warp take 32 consecutive x, so a warp writes 1 KB contiguous
+// per quarter (and, for B, reads 256 contiguous bytes per row).
+template <int L, int AXIS>
+__global__ void __launch_bounds__(256) split_packed_kernel(int rows, int cols, int Q, int bits, int bx, int bk, int x_blocks, int KS,
+                                                           const double* __restrict__ planes,
+                                                           double* __restrict__ packed,
+                                                           const int32_t* __restrict__ exps, uint32_t* flags) {
+  const int X = AXIS == 0 ? rows : cols;
+  const int x = (blockIdx.x % x_blocks) * 32 + (threadIdx.x & 31);
+  const int k4g = (blockIdx.x / x_blocks) * 8 + (threadIdx.x >> 5);  // group of four k
+  const int XP = (X + bx - 1) / bx * bx;                             // padded to whole tiles
+  if (k4g >= KS * (bk / 4) || x >= XP) return;
+  split_fragment_row<L, AXIS>(rows, cols, Q, bits, bx, bk, KS, x, k4g * 4, x < X ? exps[x] : 0, planes, packed, flags);
+}
+
+// Small problems (md_gemm's fused preparation): exponent vectors AND packed quarter planes of BOTH operands in ONE launch
+// -- five dependent launches of a few microseconds each are a third of the time of a 64^3 product.  A block owns
+// 32 groups of one operand over the whole contraction (blocks 0 .. blocksA-1: rows of A, the rest: columns of B): phase 1
+// folds the maxima of the leading limb (the same hi-32-bit maximum as the separate exponent kernels), phase 2 splits --
+// the second read of the block's elements comes from L1 / L2.  Identical digits and exponents.
+template <int L>
+__global__ void __launch_bounds__(256) prep_packed_kernel(int m, int n, int k, int Q, int bits, int bxA, int bxB, int bk,
+                                                          int blocksA, const double* __restrict__ A,
+                                                          const double* __restrict__ B, double* __restrict__ Ap,
+                                                          double* __restrict__ Bp, int32_t* __restrict__ expA,
+                                                          int32_t* __restrict__ expB, uint32_t* flags, int exp_lo) {
+  __shared__ uint32_t gmax[32];
+  const bool isA = (int)blockIdx.x < blocksA;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int x = (isA ? blockIdx.x : blockIdx.x - blocksA) * 32 + lane;
+  const int X = isA ? m : n, bx = isA ? bxA : bxB;
+  const int XP = (X + bx - 1) / bx * bx;
+  const int KS = (k + bk - 1) / bk, k4_groups = KS * (bk / 4);
+  if (threadIdx.x < 32) gmax[threadIdx.x] = 0;
+  __syncthreads();
+  if (isA) {  // a warp per row, lanes along the row: coalesced
+    for (int r = warp; r < 32; r += 8) {
+      const int xr = blockIdx.x * 32 + r;
+      if (xr >= m) break;
+      const double* row = A + (size_t)xr * k;  // leading limb plane
+      uint32_t mx = 0;
+      for (int t = lane; t < k; t += 32) mx = max(mx, abs_hi32(row[t]));
+      mx = __reduce_max_sync(0xffffffffu, mx);
+      if (lane == 0) gmax[r] = mx;
+    }
+  } else if (x < X) {  // a lane per column, warps along the rows: coalesced
+    uint32_t mx = 0;
+    for (int t = warp; t < k; t += 8) mx = max(mx, abs_hi32(B[(size_t)t * n + x]));
+    if (mx) atomicMax(&gmax[lane], mx);
+  }
+  __syncthreads();
+  int E = 0;
+  if (x < X) {
+    E = exponent_from_hi32(gmax[lane], warp == 0 ? flags : nullptr, exp_lo);
+    if (warp == 0) (isA ? expA : expB)[x] = E;
+  }
+  if (x >= XP) return;
+  for (int k4g = warp; k4g < k4_groups; k4g += 8) {
+    if (isA) split_fragment_row<L, 0>(m, k, Q, bits, bxA, bk, KS, x, k4g * 4, E, A, Ap, flags);
+    else split_fragment_row<L, 1>(k, n, Q, bits, bxB, bk, KS, x, k4g * 4, E, B, Bp, flags);
   }
 }
 
@@ -245,6 +304,27 @@ cudaError_t launch_split(int rows, int cols, int limbs, int quarters, int bits, 
     default: return cudaErrorInvalidValue;
   }
 #undef MD_SPLIT
+  *launches += 1;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_prep_packed(int m, int n, int k, int limbs, int quarters, int bits, const double* A, const double* B,
+                               double* Ap, double* Bp, int32_t* expA, int32_t* expB, uint32_t* flags, cudaStream_t stream,
+                               uint64_t* launches) {
+  const int bxA = pack_bx(limbs, quarters, 0), bxB = pack_bx(limbs, quarters, 1), bk = pack_bk(limbs);
+  const int blocksA = ((m + bxA - 1) / bxA * bxA + 31) / 32, blocksB = ((n + bxB - 1) / bxB * bxB + 31) / 32;
+  const int exp_lo = exponent_floor(quarters, bits);
+#define MD_PREP(L_) \
+  prep_packed_kernel<L_><<<blocksA + blocksB, 256, 0, stream>>>(m, n, k, quarters, bits, bxA, bxB, bk, blocksA, A, B, Ap, Bp, \
+                                                              expA, expB, flags, exp_lo)
+  switch (limbs) {
+    case 2: MD_PREP(2); break;
+    case 4: MD_PREP(4); break;
+    case 8: MD_PREP(8); break;
+    case 16: MD_PREP(16); break;
+    default: return cudaErrorInvalidValue;
+  }
+#undef MD_PREP
   *launches += 1;
   return cudaGetLastError();
 }

@@ -280,3 +280,27 @@ def test_on_a_side_stream_and_in_a_cuda_graph():
             graph.replay()
         s.synchronize()
         assert bool((out == ref).all())
+
+
+@pytest.mark.parametrize("cfg_idx,shape", [(0, (64, 64, 64)), (1, (150, 70, 90)), (3, (37, 51, 77)), (4, (70, 45, 91)), (5, (40, 30, 20)),
+                                           (2, (1, 1, 1)), (6, (20, 10, 12))])
+def test_fused_preparation_is_bit_identical_to_the_separate_kernels(cfg_idx, shape):
+    """MD_OPT_FUSED_PREP: exponent vectors and packed quarter planes of both operands in one launch (2 launches per md_gemm
+    instead of 6) against the five separate launches: the order matrices and C must not differ in a bit."""
+    cfg, A, B = gen(cfg_idx, *shape)
+    out = {}
+    for mode in (1, 2):
+        md.md_set_option(md.MD_OPT_FUSED_PREP, mode)
+        try:
+            with md.Workspace(cfg.m, cfg.n, cfg.k, cfg.limbs, cfg.quarters):
+                before = md.md_launch_count()
+                C = md.md_gemm(dev(A), dev(B))
+                launches = md.md_launch_count() - before
+                out[mode] = (host(md.md_gemm_orders(dev(A), dev(B))), host(C), launches, md.md_read_flags())
+        finally:
+            md.md_set_option(md.MD_OPT_FUSED_PREP, 0)
+    assert out[1][2] == 2 and out[2][2] == 6 and out[1][3] == out[2][3] == 0
+    assert bits_equal(out[1][0], out[2][0]) and bits_equal(out[1][1], out[2][1])
+    Aq, eA, _ = orc.split(A, 0, cfg.quarters)
+    Bq, eB, _ = orc.split(B, 1, cfg.quarters)
+    assert bits_equal(out[1][0], orc.orders_int(Aq, eA, Bq, eB))
