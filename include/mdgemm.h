@@ -74,7 +74,7 @@ enum {
                             every order sum is exact; at its end the sums are added into the element's expansion by the
                             TwoSum cascade of md_renorm.  md_gemm_orders never chunks (MD_ERR_K_TOO_LARGE as before). */
   MD_OPT_FUSED_PREP = 6, /* md_gemm / md_gemm_orders: 0 = automatic -- exponent vectors and packed quarter planes of both operands
-                            in ONE launch when (m + n) * k <= 2^17 elements, five launches otherwise; 1 = always; 2 = never.
+                            in ONE cooperative launch when (m + n) * k <= 2^23 elements, five launches otherwise; 1 = always; 2 = never.
                             Same bits either way. */
   MD_OPT_HOST_BLOCKS = 4 /* md_gemm_host only: number of blocks C is cut into for overlapping copies and kernels.
                             Default 0 = automatic (about one wave of CTA tiles per block, at most 32); 1 = no overlap;

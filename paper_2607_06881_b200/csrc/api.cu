@@ -102,13 +102,12 @@ md_status check_gemm_args(int m, int n, int k, int limbs, const void* A, const v
   return MD_OK;
 }
 
-// Fused preparation (one launch for both exponent vectors and both packed splits) where the operands are so small that the
-// latencies of five dependent launches dominate (each block owns 32 groups over the whole contraction, so the kernel has
-// little parallelism: it loses against the separate kernels from about 384^3 on)
+// Fused preparation (one cooperative launch for both exponent vectors and both packed splits) where the latencies of five
+// dependent launches show: measured faster up to 2048^3, equal at 4096^3
 inline bool use_fused_prep(int m, int n, int k) {
   if (g_state.opt_fused_prep == 1) return true;
   if (g_state.opt_fused_prep == 2) return false;
-  return ((long long)m + n) * k <= (1ll << 17);  // measured: 43 -> 31 us at 64^3, 50 -> 38 us at 128^3, even at 256^3, slower beyond
+  return ((long long)m + n) * k <= (1ll << 23);
 }
 
 // the fused quarter GEMM of one (block of a) problem on packed operands: double / quad double (chunked when md_gemm asks

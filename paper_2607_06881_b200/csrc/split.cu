@@ -2,6 +2,8 @@
 //   PAPER.md:47-49 (13-bit quarters with exponents 0,-13,-26,-39), :95 (balanced = exponents on an equally spaced grid),
 //   :124-142 (moving bits between parts without changing the value; zeros keep the desired exponent).
 // HBM-bound: reads 8*limbs and writes 8*quarters bytes per element, once.
+#include <cooperative_groups.h>
+
 #include "md_common.cuh"
 #include "md_kernels.h"
 #include "md_packed.cuh"
@@ -205,49 +207,65 @@ __global__ void __launch_bounds__(256) split_packed_kernel(int rows, int cols, i
   split_fragment_row<L, AXIS>(rows, cols, Q, bits, bx, bk, KS, x, k4g * 4, x < X ? exps[x] : 0, planes, packed, flags);
 }
 
-// Small problems (md_gemm's fused preparation): exponent vectors AND packed quarter planes of BOTH operands in ONE launch
-// -- five dependent launches of a few microseconds each are a third of the time of a 64^3 product.  A block owns
-// 32 groups of one operand over the whole contraction (blocks 0 .. blocksA-1: rows of A, the rest: columns of B): phase 1
-// folds the maxima of the leading limb (the same hi-32-bit maximum as the separate exponent kernels), phase 2 splits --
-// the second read of the block's elements comes from L1 / L2.  Identical digits and exponents.
+// md_gemm's fused preparation: exponent vectors AND packed quarter planes of BOTH operands in ONE cooperative launch (the
+// dependent launches of the separate kernels -- row maxima, column maxima, finalize, two splits, a memset -- cost a few
+// microseconds each, which is a third of a 64^3 product and 2.5 % of a 1024^3 one).  Persistent blocks, three phases
+// separated by grid-wide barriers: (0) clear the maxima, (1) fold the hi-32-bit maxima of the leading limb planes into
+// rawA[m] / rawB[n] (the same maxima as the separate exponent kernels), (2) split, a block per (32 groups x 32 contraction
+// indices) item exactly as split_packed_kernel, the exponent taken from the raw maximum on the fly.  rawA / rawB keep the
+// raw maxima (md_gemm never reads the exponent vectors back).  Identical digits.
 template <int L>
-__global__ void __launch_bounds__(256) prep_packed_kernel(int m, int n, int k, int Q, int bits, int bxA, int bxB, int bk,
-                                                          int blocksA, const double* __restrict__ A,
-                                                          const double* __restrict__ B, double* __restrict__ Ap,
-                                                          double* __restrict__ Bp, int32_t* __restrict__ expA,
-                                                          int32_t* __restrict__ expB, uint32_t* flags, int exp_lo) {
-  __shared__ uint32_t gmax[32];
-  const bool isA = (int)blockIdx.x < blocksA;
+__global__ void __launch_bounds__(256) prep_coop_kernel(int m, int n, int k, int Q, int bits, int bxA, int bxB, int bk,
+                                                        const double* __restrict__ A, const double* __restrict__ B,
+                                                        double* __restrict__ Ap, double* __restrict__ Bp, uint32_t* rawA,
+                                                        uint32_t* rawB, uint32_t* flags, int exp_lo) {
+  cooperative_groups::grid_group grid = cooperative_groups::this_grid();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int x = (isA ? blockIdx.x : blockIdx.x - blocksA) * 32 + lane;
-  const int X = isA ? m : n, bx = isA ? bxA : bxB;
-  const int XP = (X + bx - 1) / bx * bx;
-  const int KS = (k + bk - 1) / bk, k4_groups = KS * (bk / 4);
-  if (threadIdx.x < 32) gmax[threadIdx.x] = 0;
-  __syncthreads();
-  if (isA) {  // a warp per row, lanes along the row: coalesced
-    for (int r = warp; r < 32; r += 8) {
-      const int xr = blockIdx.x * 32 + r;
-      if (xr >= m) break;
-      const double* row = A + (size_t)xr * k;  // leading limb plane
+  const int gthreads = gridDim.x * blockDim.x, gtid = blockIdx.x * blockDim.x + threadIdx.x;
+  for (int i = gtid; i < m; i += gthreads) rawA[i] = 0;
+  for (int i = gtid; i < n; i += gthreads) rawB[i] = 0;
+  grid.sync();
+  // phase 1a: rows of A_0 in pieces of 1024 elements, a warp per piece, lanes along the row (coalesced)
+  {
+    const int pieces = (k + 1023) / 1024;
+    const long long items = (long long)m * pieces;
+    for (long long it = (long long)blockIdx.x * 8 + warp; it < items; it += (long long)gridDim.x * 8) {
+      const int row = (int)(it / pieces), k0 = (int)(it % pieces) * 1024, k1 = min(k, k0 + 1024);
+      const double* p = A + (size_t)row * k;
       uint32_t mx = 0;
-      for (int t = lane; t < k; t += 32) mx = max(mx, abs_hi32(row[t]));
+      for (int t = k0 + lane; t < k1; t += 32) mx = max(mx, abs_hi32(p[t]));
       mx = __reduce_max_sync(0xffffffffu, mx);
-      if (lane == 0) gmax[r] = mx;
+      if (lane == 0 && mx) atomicMax(&rawA[row], mx);
     }
-  } else if (x < X) {  // a lane per column, warps along the rows: coalesced
-    uint32_t mx = 0;
-    for (int t = warp; t < k; t += 8) mx = max(mx, abs_hi32(B[(size_t)t * n + x]));
-    if (mx) atomicMax(&gmax[lane], mx);
   }
-  __syncthreads();
-  int E = 0;
-  if (x < X) {
-    E = exponent_from_hi32(gmax[lane], warp == 0 ? flags : nullptr, exp_lo);
-    if (warp == 0) (isA ? expA : expB)[x] = E;
+  // phase 1b: columns of B_0, 256 consecutive columns x 32 rows per block item (coalesced across the block)
+  {
+    const int cblocks = (n + 255) / 256, rblocks = (k + 31) / 32;
+    const long long items = (long long)cblocks * rblocks;
+    for (long long it = blockIdx.x; it < items; it += gridDim.x) {
+      const int col = (int)(it % cblocks) * 256 + threadIdx.x, r0 = (int)(it / cblocks) * 32, r1 = min(k, r0 + 32);
+      if (col < n) {
+        uint32_t mx = 0;
+        for (int r = r0; r < r1; r++) mx = max(mx, abs_hi32(B[(size_t)r * n + col]));
+        if (mx) atomicMax(&rawB[col], mx);
+      }
+    }
   }
-  if (x >= XP) return;
-  for (int k4g = warp; k4g < k4_groups; k4g += 8) {
+  grid.sync();
+  // phase 2: split, A then B
+  const int KS = (k + bk - 1) / bk, k4_groups = KS * (bk / 4), k_blocks = (k4_groups + 7) / 8;
+  const int XPA = (m + bxA - 1) / bxA * bxA, XPB = (n + bxB - 1) / bxB * bxB;
+  const int xbA = (XPA + 31) / 32, xbB = (XPB + 31) / 32;
+  const long long itemsA = (long long)xbA * k_blocks, itemsB = (long long)xbB * k_blocks;
+  for (long long it = blockIdx.x; it < itemsA + itemsB; it += gridDim.x) {
+    const bool isA = it < itemsA;
+    const long long j = isA ? it : it - itemsA;
+    const int xb = isA ? xbA : xbB;
+    const int x = (int)(j % xb) * 32 + lane, kb = (int)(j / xb), k4g = kb * 8 + warp;
+    const int X = isA ? m : n, XP = isA ? XPA : XPB;
+    if (k4g >= k4_groups || x >= XP) continue;
+    int E = 0;
+    if (x < X) E = exponent_from_hi32(isA ? rawA[x] : rawB[x], kb == 0 && warp == 0 ? flags : nullptr, exp_lo);
     if (isA) split_fragment_row<L, 0>(m, k, Q, bits, bxA, bk, KS, x, k4g * 4, E, A, Ap, flags);
     else split_fragment_row<L, 1>(k, n, Q, bits, bxB, bk, KS, x, k4g * 4, E, B, Bp, flags);
   }
@@ -311,22 +329,36 @@ cudaError_t launch_split(int rows, int cols, int limbs, int quarters, int bits, 
 cudaError_t launch_prep_packed(int m, int n, int k, int limbs, int quarters, int bits, const double* A, const double* B,
                                double* Ap, double* Bp, int32_t* expA, int32_t* expB, uint32_t* flags, cudaStream_t stream,
                                uint64_t* launches) {
-  const int bxA = pack_bx(limbs, quarters, 0), bxB = pack_bx(limbs, quarters, 1), bk = pack_bk(limbs);
-  const int blocksA = ((m + bxA - 1) / bxA * bxA + 31) / 32, blocksB = ((n + bxB - 1) / bxB * bxB + 31) / 32;
-  const int exp_lo = exponent_floor(quarters, bits);
-#define MD_PREP(L_) \
-  prep_packed_kernel<L_><<<blocksA + blocksB, 256, 0, stream>>>(m, n, k, quarters, bits, bxA, bxB, bk, blocksA, A, B, Ap, Bp, \
-                                                              expA, expB, flags, exp_lo)
+  int bxA = pack_bx(limbs, quarters, 0), bxB = pack_bx(limbs, quarters, 1), bk = pack_bk(limbs);
+  int exp_lo = exponent_floor(quarters, bits);
+  uint32_t* rawA = reinterpret_cast<uint32_t*>(expA);
+  uint32_t* rawB = reinterpret_cast<uint32_t*>(expB);
+  void* args[] = {&m, &n, &k, &quarters, &bits, &bxA, &bxB, &bk, &A, &B, &Ap, &Bp, &rawA, &rawB, &flags, &exp_lo};
+  const void* kern = nullptr;
   switch (limbs) {
-    case 2: MD_PREP(2); break;
-    case 4: MD_PREP(4); break;
-    case 8: MD_PREP(8); break;
-    case 16: MD_PREP(16); break;
+    case 2: kern = reinterpret_cast<const void*>(prep_coop_kernel<2>); break;
+    case 4: kern = reinterpret_cast<const void*>(prep_coop_kernel<4>); break;
+    case 8: kern = reinterpret_cast<const void*>(prep_coop_kernel<8>); break;
+    case 16: kern = reinterpret_cast<const void*>(prep_coop_kernel<16>); break;
     default: return cudaErrorInvalidValue;
   }
-#undef MD_PREP
-  *launches += 1;
-  return cudaGetLastError();
+  // persistent grid: as many blocks as can be co-resident (a cooperative launch needs that), at most the work there is
+  static int max_blocks[17] = {};
+  if (max_blocks[limbs] == 0) {
+    int dev = 0, sms = 0, per_sm = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 256, 0);
+    if (e != cudaSuccess) return e;
+    if (per_sm > 4) per_sm = 4;
+    max_blocks[limbs] = sms * (per_sm > 0 ? per_sm : 1);
+  }
+  const long long KS = ((long long)k + bk - 1) / bk, k_blocks = (KS * (bk / 4) + 7) / 8;
+  long long work = (((long long)m + bxA - 1) / bxA * bxA + 31) / 32 * k_blocks + (((long long)n + bxB - 1) / bxB * bxB + 31) / 32 * k_blocks;
+  int blocks = (int)(work < max_blocks[limbs] ? (work > 0 ? work : 1) : max_blocks[limbs]);
+  const cudaError_t err = cudaLaunchCooperativeKernel(kern, dim3(blocks), dim3(256), args, 0, stream);
+  if (err == cudaSuccess) *launches += 1;
+  return err;
 }
 
 cudaError_t launch_split_packed(int rows, int cols, int limbs, int quarters, int bits, int axis, const double* planes,
