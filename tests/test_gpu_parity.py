@@ -304,3 +304,26 @@ def test_fused_preparation_is_bit_identical_to_the_separate_kernels(cfg_idx, sha
     Aq, eA, _ = orc.split(A, 0, cfg.quarters)
     Bq, eB, _ = orc.split(B, 1, cfg.quarters)
     assert bits_equal(out[1][0], orc.orders_int(Aq, eA, Bq, eB))
+
+
+@pytest.mark.parametrize("shape", [(70001, 5, 3), (3, 70001, 5), (5, 3, 70001), (1, 40000, 1), (40000, 1, 1)])
+def test_extreme_aspect_ratios(shape):
+    """Tall, wide and deep degenerate shapes (one dimension 70 001, the others a handful): order matrices bit-exact, C
+    within tolerance, host entry point bit-identical, with the paper's quarters and with 7 slices of 16 bits (whose
+    whole-k budget, k <= 2^21 / 7, covers the deep shape; 19-bit slices stop at k = 5461)."""
+    cfg, A, B = gen(0, *shape)
+    for Q, W in ((8, 13), (7, 16)):
+        with md.Workspace(cfg.m, cfg.n, cfg.k, 2, Q, bits=W):
+            orders = host(md.md_gemm_orders(dev(A), dev(B)))
+            C = md.md_gemm(dev(A), dev(B))
+            assert md.md_read_flags() == 0
+            Ch = torch.empty((2, cfg.m, cfg.n), dtype=torch.float64).pin_memory()
+            scratch = torch.empty(md.md_host_scratch_bytes(cfg.m, cfg.n, cfg.k, 2), dtype=torch.uint8, device="cuda")
+            md.md_gemm_host(torch.from_numpy(A).pin_memory(), torch.from_numpy(B).pin_memory(), Ch, scratch)
+        assert bool((Ch == C.cpu()).all())
+        Aq, eA, _ = orc.split(A, 0, Q, bits=W)
+        Bq, eB, _ = orc.split(B, 1, Q, bits=W)
+        assert bits_equal(orders, orc.orders_int(Aq, eA, Bq, eB, bits=W))
+        si, sj = inputs.sample_indices(cfg, min(2000, cfg.m * cfg.n))
+        r = orc.exact_samples(A, B, si, sj, host(C))
+        assert (r["err"] <= 1e-28 * r["W"]).all()
