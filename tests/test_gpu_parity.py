@@ -327,3 +327,32 @@ def test_extreme_aspect_ratios(shape):
         si, sj = inputs.sample_indices(cfg, min(2000, cfg.m * cfg.n))
         r = orc.exact_samples(A, B, si, sj, host(C))
         assert (r["err"] <= 1e-28 * r["W"]).all()
+
+
+@pytest.mark.parametrize("fused", [1, 2])
+def test_exponent_range_flag_and_scaling_near_the_limits(fused):
+    """include/mdgemm.h data preconditions: group exponents within [-900, 900] -- beyond, bit 1 of the status word is set
+    (both preparation paths); inside, a problem scaled by 2^+-850 per operand is the same digits on a shifted grid, so C is
+    the scaled C bit for bit; a group whose maximum is subnormal counts as a zero group."""
+    cfg, A, B = gen(0, 40, 24, 32)
+    md.md_set_option(md.MD_OPT_FUSED_PREP, fused)
+    try:
+        with md.Workspace(cfg.m, cfg.n, cfg.k, 2):
+            C = host(md.md_gemm(dev(A), dev(B)))
+            assert md.md_read_flags() == 0
+            up, down = 2.0 ** 850, 2.0 ** -850
+            Cs = host(md.md_gemm(dev(A * up), dev(B * down)))   # rows of A at 2^850, columns of B at 2^-850: C unchanged
+            assert md.md_read_flags() == 0 and bits_equal(Cs, C)
+            Cu = host(md.md_gemm(dev(A * 2.0 ** 400), dev(B * 2.0 ** 400)))
+            assert md.md_read_flags() == 0 and bits_equal(Cu, C * 2.0 ** 800)
+        with md.Workspace(cfg.m, cfg.n, cfg.k, 2):
+            md.md_gemm(dev(A * 2.0 ** 950), dev(B))
+            assert md.md_read_flags() == 2          # exponent out of range (bit 1), nothing non-finite (bit 0)
+        with md.Workspace(cfg.m, cfg.n, cfg.k, 2):
+            A2 = A.copy()
+            A2[:, 3, :] = 0.0
+            A2[0, 3, 5] = 5e-320                    # a subnormal row maximum: the row counts as zero
+            C2 = host(md.md_gemm(dev(A2), dev(B)))
+            assert not C2[:, 3, :].any() and bits_equal(np.delete(C2, 3, axis=1), np.delete(C, 3, axis=1))
+    finally:
+        md.md_set_option(md.MD_OPT_FUSED_PREP, 0)
