@@ -214,3 +214,16 @@ def test_row_of_equal_powers_of_two_is_one_digit():
         qp, exps, rem = orc.split(np.stack([row, np.zeros_like(row)]), 0, want_remainder=True)
         assert list(exps) == [e + 1] and not rem.any() and not qp[1:].any()
         assert (qp[0] == row).all() and (np.abs(qp[0]) == 4096 * np.ldexp(1.0, e + 1 - W)).all()
+
+
+def test_power_of_two_scaling_shifts_the_grid_and_nothing_else():
+    """Scaling a row by 2^s moves its exponent by s and multiplies every quarter by 2^s: same integer digits (the method
+    is scale-free per group -- what a common exponent per row / column buys, R2)."""
+    cfg = small_cfg(3, 9, 5, 11)
+    X = inputs.generate(cfg, "A")
+    s = np.array([-300, -7, 0, 1, 13, 52, 200, 511, -512], dtype=np.int32)
+    Xs = X * np.ldexp(1.0, s)[None, :, None]
+    q0, e0, r0 = orc.split(X, 0, want_remainder=True)
+    q1, e1, r1 = orc.split(Xs, 0, want_remainder=True)
+    assert (e1 == e0 + s).all()
+    assert (q1 == q0 * np.ldexp(1.0, s)[None, :, None]).all() and (r1 == r0 * np.ldexp(1.0, s)[None, :, None]).all()
