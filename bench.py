@@ -258,8 +258,18 @@ def run_ours(args):
     probe_launches = md.md_launch_count() - probe_launches0
 
     # what the data needs (md_plan_quarters, R15): the any-input guarantee for this input, outside the timed region
-    quarter_plan = None
-    if world == 1:
+    # (the blocks from here to the e2e leg are context beside the headline: a failure in one of them is recorded in its
+    # place and never costs the JSON line)
+    def context_block(fn):
+        try:
+            return fn()
+        except Exception as exc:  # noqa: BLE001
+            for key in (md.MD_OPT_SLICE_BITS, md.MD_OPT_QUARTERS):
+                md.md_set_option(key, 0)
+            md.md_set_workspace(None)
+            return {"error": f"{type(exc).__name__}: {exc}"}
+
+    def plan_block():
         md.md_set_option(md.MD_OPT_SLICE_BITS, 0 if W == 13 else W)
         md.md_plan_quarters(A, B)
         torch.cuda.synchronize()
@@ -267,9 +277,11 @@ def run_ours(args):
         pq, pd = md.md_plan_quarters(A, B)
         plan_ms = (time.perf_counter() - t0) * 1e3
         md.md_set_option(md.MD_OPT_SLICE_BITS, 0)
-        quarter_plan = {"spread_D": pd, "guaranteed_quarters": pq, "run_with": Q, "slice_bits": W, "ms": plan_ms,
-                        "note": "smallest Q with k (Q+1) 2^(D - W Q - 2) <= the format's tolerance at every position "
-                                "(worst case; measured errors are 2-3 orders of magnitude below the bound)"}
+        return {"spread_D": pd, "guaranteed_quarters": pq, "run_with": Q, "slice_bits": W, "ms": plan_ms,
+                "note": "smallest Q with k (Q+1) 2^(D - W Q - 2) <= the format's tolerance at every position "
+                        "(worst case; measured errors are 2-3 orders of magnitude below the bound)"}
+
+    quarter_plan = context_block(plan_block) if world == 1 else None
 
     # beside the headline (the paper's quarters): the same problem with the k-adaptive slices, outside the timed region
     adaptive = None
@@ -295,16 +307,21 @@ def run_ours(args):
                 "kernel_frac_of_fp64_tensor_peak": aT * base.md_flops / (sum(a_gemm_ms) / 3 * 1e-3) / 1e12 / FP64_TENSOR_PEAK_TFLOPS,
                 "max_abs_diff_vs_paper_quarters": float((C2 - C).abs().sum(dim=0).max()), "note": note}
 
-    if args.slices == "paper" and world == 1:
+    def adaptive_block():
         cW, cQ, cK = md.md_plan_slices_chunked(k, L, 128)
         aW, aQ = md.md_plan_slices(k, L)
-        if (aW, aQ) != (W, Q):
-            adaptive = time_variant(aW, aQ, "md_plan_slices: wider, fewer slices on the same kernels (DESIGN.md R14); not the "
-                                            "paper's 13-bit quarters, so not the headline; 3 steps after 1 warm-up, CUDA events")
-            if (cW, cQ) != (aW, aQ):
-                adaptive["chunked"] = time_variant(cW, cQ, "md_plan_slices_chunked(k, limbs, 128): exactness kept per chunk of %d "
-                                                           "contraction indices (DESIGN.md R16)" % cK)
-                adaptive["chunked"]["chunk"] = cK
+        if (aW, aQ) == (W, Q):
+            return None
+        out = time_variant(aW, aQ, "md_plan_slices: wider, fewer slices on the same kernels (DESIGN.md R14); not the "
+                                   "paper's 13-bit quarters, so not the headline; 3 steps after 1 warm-up, CUDA events")
+        if (cW, cQ) != (aW, aQ):
+            out["chunked"] = time_variant(cW, cQ, "md_plan_slices_chunked(k, limbs, 128): exactness kept per chunk of %d "
+                                                  "contraction indices (DESIGN.md R16)" % cK)
+            out["chunked"]["chunk"] = cK
+        return out
+
+    if args.slices == "paper" and world == 1:
+        adaptive = context_block(adaptive_block)
 
     # the paper's own two paths on the same inputs (context; outside the timed region; N = 1, dd / qd only)
     paper_paths = None
@@ -352,28 +369,33 @@ def run_ours(args):
     # end to end: pinned host buffers through md_gemm_host (H2D A, B + the whole path + D2H C, synchronous)
     e2e = None
     if not args.no_e2e:
-        md.md_set_option(md.MD_OPT_QUARTERS, 0 if Q == 4 * L else Q)  # before sizing the scratch: it depends on Q
-        md.md_set_option(md.MD_OPT_SLICE_BITS, 0 if W == 13 else W)
-        scratch = torch.empty(md.md_host_scratch_bytes(m, n, k, L), dtype=torch.uint8, device="cuda")
-        for _ in range(min(args.warmup, 2)):
-            md.md_gemm_host(A_host, B_host, C_host, scratch)
-        barrier()
-        launches_e2e0 = md.md_launch_count()
-        t0 = time.perf_counter()
-        e0.record(stream)
-        for _ in range(args.steps):
-            md.md_gemm_host(A_host, B_host, C_host, scratch)
-        e1.record(stream)
-        barrier()
-        e2e_ms = max_over_ranks(e0.elapsed_time(e1))
-        wall_ms = max_over_ranks((time.perf_counter() - t0) * 1e3)
-        md.md_set_option(md.MD_OPT_QUARTERS, 0)
-        md.md_set_option(md.MD_OPT_SLICE_BITS, 0)
-        e2e = {"value": world * base.md_flops * args.steps / (max(e2e_ms, wall_ms) * 1e-3) / 1e9, "unit": UNIT,
-               "h2d_bytes_per_step": A_host.numel() * 8 + B_host.numel() * 8, "d2h_bytes_per_step": C_host.numel() * 8,
-               "ms_per_step": max(e2e_ms, wall_ms) / args.steps, "launches": md.md_launch_count() - launches_e2e0,
-               "matches_device_path": bool((C_host == C.cpu()).all())}
-        del scratch
+        try:
+            md.md_set_option(md.MD_OPT_QUARTERS, 0 if Q == 4 * L else Q)  # before sizing the scratch: it depends on Q
+            md.md_set_option(md.MD_OPT_SLICE_BITS, 0 if W == 13 else W)
+            scratch = torch.empty(md.md_host_scratch_bytes(m, n, k, L), dtype=torch.uint8, device="cuda")
+            for _ in range(min(args.warmup, 2)):
+                md.md_gemm_host(A_host, B_host, C_host, scratch)
+            barrier()
+            launches_e2e0 = md.md_launch_count()
+            t0 = time.perf_counter()
+            e0.record(stream)
+            for _ in range(args.steps):
+                md.md_gemm_host(A_host, B_host, C_host, scratch)
+            e1.record(stream)
+            barrier()
+            e2e_ms = max_over_ranks(e0.elapsed_time(e1))
+            wall_ms = max_over_ranks((time.perf_counter() - t0) * 1e3)
+            md.md_set_option(md.MD_OPT_QUARTERS, 0)
+            md.md_set_option(md.MD_OPT_SLICE_BITS, 0)
+            e2e = {"value": world * base.md_flops * args.steps / (max(e2e_ms, wall_ms) * 1e-3) / 1e9, "unit": UNIT,
+                   "h2d_bytes_per_step": A_host.numel() * 8 + B_host.numel() * 8, "d2h_bytes_per_step": C_host.numel() * 8,
+                   "ms_per_step": max(e2e_ms, wall_ms) / args.steps, "launches": md.md_launch_count() - launches_e2e0,
+                   "matches_device_path": bool((C_host == C.cpu()).all())}
+            del scratch
+        except Exception as exc:  # noqa: BLE001 -- the device-resident headline must still be reported
+            for key in (md.MD_OPT_SLICE_BITS, md.MD_OPT_QUARTERS):
+                md.md_set_option(key, 0)
+            e2e = {"error": f"{type(exc).__name__}: {exc}"}
     sampler.stop()
     clocks = sampler.summary()
     clocks["samples_in_device_loop"] = clocks_after_device_loop
@@ -408,7 +430,11 @@ def run_ours(args):
 
     cpu_baseline = None
     if world == 1 and not args.no_cpu_baseline:
-        v, dt, threads = cpu_oracle_sample(base, CPU_SAMPLE_ROWS)
+        try:
+            v, dt, threads = cpu_oracle_sample(base, CPU_SAMPLE_ROWS)
+        except Exception as exc:  # noqa: BLE001
+            v, dt, threads = None, None, 0
+            print(f"bench.py: cpu_baseline failed: {exc}", file=sys.stderr)
         cpu_baseline = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "seconds": dt,
                         "sample": f"first {CPU_SAMPLE_ROWS} rows of A ({CPU_SAMPLE_ROWS}x{base.n} outputs of the "
                                   f"{base.m}x{base.n}x{base.k} problem), all of B; oracle split + {base.products} plain "
