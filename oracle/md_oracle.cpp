@@ -67,7 +67,7 @@ struct LongAcc {
       carry = (v - lo) >> 32;  // arithmetic shift: floor division by 2^32
       w[i] = lo;
     }
-    w[NW - 1] += carry << 32;  // keep the sign in the top word
+    w[NW - 1] += carry * 4294967296LL;  // carry * 2^32 (a multiplication: << of a negative carry is undefined before C++20); keeps the sign in the top word
     pending = 0;
   }
 
