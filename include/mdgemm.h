@@ -76,6 +76,9 @@ enum {
   MD_OPT_FUSED_PREP = 6, /* md_gemm / md_gemm_orders: 0 = automatic -- exponent vectors and packed quarter planes of both operands
                             in ONE cooperative launch when (m + n) * k <= 2^23 elements, five launches otherwise; 1 = always; 2 = never.
                             Same bits either way. */
+  MD_OPT_TILE = 7,       /* md_gemm / md_gemm_orders, double double with 8 or 6 slices: 0 = automatic -- the 32 x 16 CTA tile
+                            instance of the fused kernel when the 64 x 32 tiles would number at most two thirds of the SMs
+                            (up to about 448^3), 64 x 32 otherwise; 1 = 32 x 16 wherever it exists; 2 = never.  Same bits. */
   MD_OPT_HOST_BLOCKS = 4 /* md_gemm_host only: number of blocks C is cut into for overlapping copies and kernels.
                             Default 0 = automatic (about one wave of CTA tiles per block, at most 32); 1 = no overlap;
                             PR * 256 + PC = explicit numbers of row panels and column panels (each <= 64). */

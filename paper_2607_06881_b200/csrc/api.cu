@@ -16,6 +16,7 @@ struct State {
   int opt_quarters = 0;  // 0 = default (4 * limbs)
   int opt_orders = 0;    // 0 = default (= quarters)
   int opt_bits = 0;      // 0 = default (13, the paper's quarter)
+  int opt_tile = 0;        // 0 = automatic, 1 = the 32 x 16 tile instance wherever it exists, 2 = never
   int opt_fused_prep = 0;  // 0 = automatic (small / medium operands), 1 = always, 2 = never
   int opt_k_chunk = 0;   // 0 = chunked accumulation only when k exceeds the exactness budget; else the chunk length to force
   int opt_host_blocks = 0;  // md_gemm_host: 0 = automatic panel plan, else the number of blocks of C (1 = no pipelining)
@@ -67,7 +68,7 @@ struct Carve {
   void* sk;  // stream-K scratch of the fused GEMM
   size_t total;
 };
-Carve carve(void* base, int m, int n, int k, int limbs, int quarters) {
+Carve carve(void* base, int m, int n, int k, int limbs, int quarters, bool small = false) {
   Carve c;
   size_t off = 0;
   char* p = static_cast<char*>(base);
@@ -78,9 +79,9 @@ Carve carve(void* base, int m, int n, int k, int limbs, int quarters) {
   c.expB = reinterpret_cast<int32_t*>(p + off);
   off += round_up(sizeof(int32_t) * (size_t)n);
   c.Aq = reinterpret_cast<double*>(p + off);
-  off += round_up(sizeof(double) * md::packed_doubles(m, k, md::pack_bx(limbs, quarters, 0), md::pack_bk(limbs), quarters));
+  off += round_up(sizeof(double) * md::packed_doubles(m, k, md::pack_bx(limbs, quarters, 0, small), md::pack_bk(limbs), quarters));
   c.Bq = reinterpret_cast<double*>(p + off);
-  off += round_up(sizeof(double) * md::packed_doubles(n, k, md::pack_bx(limbs, quarters, 1), md::pack_bk(limbs), quarters));
+  off += round_up(sizeof(double) * md::packed_doubles(n, k, md::pack_bx(limbs, quarters, 1, small), md::pack_bk(limbs), quarters));
   c.sk = p + off;
   off += round_up(md::sk_workspace_bytes(limbs, quarters, k, chunk_for(k, limbs, quarters, slice_bits())));
   c.total = off;
@@ -110,13 +111,24 @@ inline bool use_fused_prep(int m, int n, int k) {
   return ((long long)m + n) * k <= (1ll << 23);
 }
 
+// The 32 x 16 tile instance of the double-double kernel: where the 64 x 32 tiles would not fill the SMs (at most one tile
+// per SM), every tile would be cut along k and each CTA would flush a whole tile of partial sums through L2 atomics; four
+// times the tiles avoid most of that (measured).  Splitter and GEMM must agree on the answer.
+inline bool use_small_tiles(int m, int n, int k, int limbs, int Q, int W) {
+  if (!md::qgemm_small_supported(limbs, Q) || chunk_for(k, limbs, Q, W) > 0 || g_state.opt_tile == 2) return false;
+  if (g_state.opt_tile == 1) return true;
+  const int G = md::sk_grid();
+  const long long tiles = ((long long)m + 63) / 64 * (((long long)n + 31) / 32);
+  return G > 0 && 3 * tiles <= 2 * G;  // measured on dd n^3: faster up to n = 448 (98 tiles), slower from n = 512 (128 tiles)
+}
+
 // the fused quarter GEMM of one (block of a) problem on packed operands: double / quad double (chunked when md_gemm asks
 // for C of a contraction beyond the exactness budget), octo / hexa double
-cudaError_t launch_fused(int m, int n, int k, int limbs, int Q, int W, const double* Aq, const double* Bq,
+cudaError_t launch_fused(int m, int n, int k, int limbs, int Q, int W, bool small, const double* Aq, const double* Bq,
                          double* order_planes, double* C_planes, void* sk, cudaStream_t stream, uint64_t* launches) {
   if (limbs > 4) return md::launch_qgemm_wide(m, n, k, limbs, Q, Aq, Bq, order_planes, C_planes, sk, stream, launches);
   const int chunk = order_planes ? 0 : chunk_for(k, limbs, Q, W);
-  return md::launch_qgemm_packed(m, n, k, limbs, Q, chunk, Aq, Bq, order_planes, C_planes, sk, stream, launches);
+  return md::launch_qgemm_packed(m, n, k, limbs, Q, chunk, small, Aq, Bq, order_planes, C_planes, sk, stream, launches);
 }
 
 // split A (rows) and B (columns) into the packed quarter planes of the carved workspace, then the fused quarter GEMM.
@@ -124,22 +136,23 @@ md_status gemm_impl(int m, int n, int k, int limbs, const double* A, const doubl
                     double* order_planes, void* ws, size_t ws_bytes, cudaStream_t stream) {
   const int Q = quarters_for(limbs), W = slice_bits();
   if (!ws) return MD_ERR_WORKSPACE;
-  const Carve c = carve(ws, m, n, k, limbs, Q);
+  const bool small = use_small_tiles(m, n, k, limbs, Q, W);
+  const Carve c = carve(ws, m, n, k, limbs, Q, small);
   if (c.total > ws_bytes) return MD_ERR_WORKSPACE;
   uint64_t launches = 0;
   cudaEvent_t* ev = (g_prof.count < g_prof.capacity) ? &g_prof.ev[3 * (size_t)g_prof.count] : nullptr;
   if (ev) cudaEventRecord(ev[0], stream);
   cudaError_t err;
   if (use_fused_prep(m, n, k)) {  // one launch instead of five: what matters below ~1024^3
-    err = md::launch_prep_packed(m, n, k, limbs, Q, W, A, B, c.Aq, c.Bq, c.expA, c.expB, c.flags, stream, &launches);
+    err = md::launch_prep_packed(m, n, k, limbs, Q, W, small, A, B, c.Aq, c.Bq, c.expA, c.expB, c.flags, stream, &launches);
   } else {
     err = md::launch_exponents(m, k, 0, Q, W, A, c.expA, c.flags, stream, &launches);
     if (err == cudaSuccess) err = md::launch_exponents(k, n, 1, Q, W, B, c.expB, c.flags, stream, &launches);
-    if (err == cudaSuccess) err = md::launch_split_packed(m, k, limbs, Q, W, 0, A, c.Aq, c.expA, c.flags, stream, &launches);
-    if (err == cudaSuccess) err = md::launch_split_packed(k, n, limbs, Q, W, 1, B, c.Bq, c.expB, c.flags, stream, &launches);
+    if (err == cudaSuccess) err = md::launch_split_packed(m, k, limbs, Q, W, 0, small, A, c.Aq, c.expA, c.flags, stream, &launches);
+    if (err == cudaSuccess) err = md::launch_split_packed(k, n, limbs, Q, W, 1, small, B, c.Bq, c.expB, c.flags, stream, &launches);
   }
   if (ev) cudaEventRecord(ev[1], stream);
-  if (err == cudaSuccess) err = launch_fused(m, n, k, limbs, Q, W, c.Aq, c.Bq, order_planes, C_planes, c.sk, stream, &launches);
+  if (err == cudaSuccess) err = launch_fused(m, n, k, limbs, Q, W, small, c.Aq, c.Bq, order_planes, C_planes, c.sk, stream, &launches);
   if (ev) {
     cudaEventRecord(ev[2], stream);
     if (err == cudaSuccess) g_prof.count++;
@@ -207,6 +220,11 @@ md_status md_set_option(int key, int value) {
     g_state.opt_k_chunk = value;
     return MD_OK;
   }
+  if (key == MD_OPT_TILE) {
+    if (value < 0 || value > 2) return MD_ERR_BAD_ARG;
+    g_state.opt_tile = value;
+    return MD_OK;
+  }
   if (key == MD_OPT_FUSED_PREP) {
     if (value < 0 || value > 2) return MD_ERR_BAD_ARG;
     g_state.opt_fused_prep = value;
@@ -237,6 +255,7 @@ int md_get_option(int key) {
     case MD_OPT_HOST_BLOCKS: return g_state.opt_host_blocks;
     case MD_OPT_K_CHUNK: return g_state.opt_k_chunk;
     case MD_OPT_FUSED_PREP: return g_state.opt_fused_prep;
+    case MD_OPT_TILE: return g_state.opt_tile;
     default: return -1;
   }
 }
@@ -501,7 +520,7 @@ md_status md_gemm_host(int m, int n, int k, int limbs, const double* A_host, con
     double* Bq = c.Bq + (size_t)(c0 / bxB) * KS * chunkB;  // panel boundaries are multiples of the CTA tile
     MD_TRY(cudaStreamWaitEvent(st, ev_B[j], 0));
     err = md::launch_exponents(k, nj, 1, Q, W, Bj, c.expB + c0, c.flags, st, &launches);
-    if (err == cudaSuccess) err = md::launch_split_packed(k, nj, limbs, Q, W, 1, Bj, Bq, c.expB + c0, c.flags, st, &launches);
+    if (err == cudaSuccess) err = md::launch_split_packed(k, nj, limbs, Q, W, 1, false, Bj, Bq, c.expB + c0, c.flags, st, &launches);
     for (int i = 0; i < hp.PR && err == cudaSuccess; i++) {
       int r0, mi;
       rows_of(i, r0, mi);
@@ -510,12 +529,12 @@ md_status md_gemm_host(int m, int n, int k, int limbs, const double* A_host, con
       if (j == 0) {
         MD_TRY(cudaStreamWaitEvent(st, ev_A[i], 0));
         err = md::launch_exponents(mi, k, 0, Q, W, Ai, c.expA + r0, c.flags, st, &launches);
-        if (err == cudaSuccess) err = md::launch_split_packed(mi, k, limbs, Q, W, 0, Ai, Aq, c.expA + r0, c.flags, st, &launches);
+        if (err == cudaSuccess) err = md::launch_split_packed(mi, k, limbs, Q, W, 0, false, Ai, Aq, c.expA + r0, c.flags, st, &launches);
         if (err != cudaSuccess) break;
       }
       // block (i, j): compact [limbs][mi][nj] at the position its elements have in a row-panel-major walk of C
       double* Cb = dC + (size_t)limbs * ((size_t)r0 * n + (size_t)mi * c0);
-      err = launch_fused(mi, nj, k, limbs, Q, W, Aq, Bq, nullptr, Cb, c.sk, st, &launches);
+      err = launch_fused(mi, nj, k, limbs, Q, W, false, Aq, Bq, nullptr, Cb, c.sk, st, &launches);  // the host path keeps the 64 x 32 tiles its panels are cut to
       if (err != cudaSuccess) break;
       cudaEvent_t done = ev_C[j * hp.PR + i];
       MD_TRY(cudaEventRecord(done, st));

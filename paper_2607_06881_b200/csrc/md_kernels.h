@@ -29,13 +29,15 @@ cudaError_t launch_spread(int m, int n, const double* W, const int32_t* expA, co
                           cudaStream_t stream, uint64_t* launches);
 // md_gemm's internal pair: splitter writing the fragment-major packed layout (md_packed.cuh) and the bulk-copy /
 // mbarrier pipelined fused GEMM reading it.  Same (limbs, quarters) support as launch_qgemm.
-cudaError_t launch_split_packed(int rows, int cols, int limbs, int quarters, int bits, int axis, const double* planes,
-                                double* packed, const int32_t* exps, uint32_t* flags, cudaStream_t stream,
-                                uint64_t* launches);
+// small: the 32 x 16 tile instance of the double-double kernel (md_packed.cuh pack_bx); splitter and GEMM must agree
+cudaError_t launch_split_packed(int rows, int cols, int limbs, int quarters, int bits, int axis, bool small,
+                                const double* planes, double* packed, const int32_t* exps, uint32_t* flags,
+                                cudaStream_t stream, uint64_t* launches);
+bool qgemm_small_supported(int limbs, int quarters);
 // exponent vectors + packed quarter planes of BOTH operands in one launch (small and medium problems: md_gemm's fused prep)
-cudaError_t launch_prep_packed(int m, int n, int k, int limbs, int quarters, int bits, const double* A, const double* B,
-                               double* Ap, double* Bp, int32_t* expA, int32_t* expB, uint32_t* flags, cudaStream_t stream,
-                               uint64_t* launches);
+cudaError_t launch_prep_packed(int m, int n, int k, int limbs, int quarters, int bits, bool small, const double* A,
+                               const double* B, double* Ap, double* Bp, int32_t* expA, int32_t* expB, uint32_t* flags,
+                               cudaStream_t stream, uint64_t* launches);
 // sk_ws: sk_workspace_bytes(limbs, quarters) bytes of device scratch for the stream-K tail (slab counters + one
 // order-plane tile per stream-K tile); zeroed by the launcher (a memset node on `stream`) as far as it is used.
 constexpr int SK_MAX_TILES = 256;
@@ -51,7 +53,7 @@ int sk_grid();
 // chunk = 0: exact orders over the whole k.  chunk > 0 (R16; a multiple of 8, qgemm_chunk_supported instances
 // only, C_planes only): the accumulators are folded into the elements' expansions every `chunk` contraction indices.
 bool qgemm_chunk_supported(int limbs, int quarters);
-cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, int chunk, const double* Ap,
+cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, int chunk, bool small, const double* Ap,
                                 const double* Bp, double* order_planes, double* C_planes, void* sk_ws,
                                 cudaStream_t stream, uint64_t* launches);
 // octo / hexa double (qgemm_wide.cu): same packed operands (k-slab depth 4), same stream-K scratch convention

@@ -395,7 +395,8 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
 template <class C>
 cudaError_t launch_cfg(int m, int n, int k, const double* Ap, const double* Bp, double* order_planes, double* C_planes,
                        void* sk_ws, cudaStream_t stream) {
-  static_assert(C::BM == pack_bx(C::L, C::Q, 0) && C::BN == pack_bx(C::L, C::Q, 1), "tile shape must match the packed layout");
+  constexpr bool SMALL = C::L == 2 && C::MT == 1;
+  static_assert(C::BM == pack_bx(C::L, C::Q, 0, SMALL) && C::BN == pack_bx(C::L, C::Q, 1, SMALL), "tile shape must match the packed layout");
   const int tiles_m = (m + C::BM - 1) / C::BM, tiles_n = (n + C::BN - 1) / C::BN;
   const long long tiles = (long long)tiles_m * tiles_n;
   if (tiles > 0x7fffffffLL) return cudaErrorInvalidValue;
@@ -454,6 +455,9 @@ cudaError_t launch_chunked(int m, int n, int k, int chunk, const double* Ap, con
 // double double: 64 x 32 CTA tile, 8 warps (4 x 2), 16 x 16 warp tile.  quad double: 32 x 16 CTA tile, 8 x 8 warp tile
 // (16 orders x 2 registers per 8x8 tile).
 template <int Q> using PCfgDD = PCfg<Q, 2, 4, 2, 2, 2>;
+// double double on 32 x 16 CTA tiles (8 x 8 warp tiles): four times the tiles, for problems whose 64 x 32 tiles would not
+// fill the SMs -- every tile would be cut along k and each CTA would flush a whole tile of partial sums through L2
+template <int Q> using PCfgDDS = PCfg<Q, 2, 4, 2, 1, 1>;
 template <int Q> using PCfgQD = PCfg<Q, 4, 4, 2, 1, 1>;
 // quad double in 11 / 12 wide slices (MD_OPT_SLICE_BITS): 22 / 24 accumulator registers per 8x8 tile leave room for the
 // double-double warp tile (16 x 16), which halves the LDS and L2 traffic per DMMA and doubles the DMMAs per slab
@@ -487,16 +491,22 @@ size_t sk_workspace_bytes(int limbs, int quarters, int k, int chunk) {
   return SK_COUNTER_BYTES + tile * slots;
 }
 
+bool qgemm_small_supported(int limbs, int quarters) { return limbs == 2 && (quarters == 8 || quarters == 6); }
+
 bool qgemm_chunk_supported(int limbs, int quarters) {
   return (limbs == 2 && (quarters == 5 || quarters == 6 || quarters == 8)) || (limbs == 4 && quarters == 10);
 }
 
-cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, int chunk, const double* Ap, const double* Bp,
-                                double* order_planes, double* C_planes, void* sk_ws, cudaStream_t stream,
+cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, int chunk, bool small, const double* Ap,
+                                const double* Bp, double* order_planes, double* C_planes, void* sk_ws, cudaStream_t stream,
                                 uint64_t* launches) {
   cudaError_t err = cudaErrorInvalidValue;
 #define MD_Q(CFG) err = launch_cfg<CFG>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream)
-  if (chunk > 0) {  // only the instances of qgemm_chunk_supported are compiled with the chunked kernel
+  if (small) {
+    if (chunk > 0 || !qgemm_small_supported(limbs, quarters)) return cudaErrorInvalidValue;
+    if (quarters == 8) MD_Q(PCfgDDS<8>);
+    if (quarters == 6) MD_Q(PCfgDDS<6>);
+  } else if (chunk > 0) {  // only the instances of qgemm_chunk_supported are compiled with the chunked kernel
     if (limbs == 2 && quarters == 5) err = launch_chunked<PCfgDD<5>>(m, n, k, chunk, Ap, Bp, C_planes, sk_ws, stream);
     if (limbs == 2 && quarters == 6) err = launch_chunked<PCfgDD<6>>(m, n, k, chunk, Ap, Bp, C_planes, sk_ws, stream);
     if (limbs == 2 && quarters == 8) err = launch_chunked<PCfgDD<8>>(m, n, k, chunk, Ap, Bp, C_planes, sk_ws, stream);

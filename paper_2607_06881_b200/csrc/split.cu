@@ -326,10 +326,10 @@ cudaError_t launch_split(int rows, int cols, int limbs, int quarters, int bits, 
   return cudaGetLastError();
 }
 
-cudaError_t launch_prep_packed(int m, int n, int k, int limbs, int quarters, int bits, const double* A, const double* B,
-                               double* Ap, double* Bp, int32_t* expA, int32_t* expB, uint32_t* flags, cudaStream_t stream,
-                               uint64_t* launches) {
-  int bxA = pack_bx(limbs, quarters, 0), bxB = pack_bx(limbs, quarters, 1), bk = pack_bk(limbs);
+cudaError_t launch_prep_packed(int m, int n, int k, int limbs, int quarters, int bits, bool small, const double* A,
+                               const double* B, double* Ap, double* Bp, int32_t* expA, int32_t* expB, uint32_t* flags,
+                               cudaStream_t stream, uint64_t* launches) {
+  int bxA = pack_bx(limbs, quarters, 0, small), bxB = pack_bx(limbs, quarters, 1, small), bk = pack_bk(limbs);
   int exp_lo = exponent_floor(quarters, bits);
   uint32_t* rawA = reinterpret_cast<uint32_t*>(expA);
   uint32_t* rawB = reinterpret_cast<uint32_t*>(expB);
@@ -361,11 +361,11 @@ cudaError_t launch_prep_packed(int m, int n, int k, int limbs, int quarters, int
   return err;
 }
 
-cudaError_t launch_split_packed(int rows, int cols, int limbs, int quarters, int bits, int axis, const double* planes,
-                                double* packed, const int32_t* exps, uint32_t* flags, cudaStream_t stream,
-                                uint64_t* launches) {
+cudaError_t launch_split_packed(int rows, int cols, int limbs, int quarters, int bits, int axis, bool small,
+                                const double* planes, double* packed, const int32_t* exps, uint32_t* flags,
+                                cudaStream_t stream, uint64_t* launches) {
   const int X = axis == 0 ? rows : cols, K = axis == 0 ? cols : rows;
-  const int bx = pack_bx(limbs, quarters, axis);
+  const int bx = pack_bx(limbs, quarters, axis, small);
   const int bk = pack_bk(limbs);
   const int KS = (K + bk - 1) / bk;
   const int x_blocks = ((X + bx - 1) / bx * bx + 31) / 32;  // 32 groups per block over the padded extent

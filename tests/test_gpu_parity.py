@@ -258,9 +258,11 @@ def test_flags_and_runtime_errors():
     with pytest.raises(md.MdError) as e:  # no workspace registered
         md.md_gemm(dev(A), dev(B))
     assert e.value.status == md.MD_ERR_WORKSPACE
-    with md.Workspace(8, 8, 8, 2):  # too small for 16^3
-        with pytest.raises(md.MdError):
-            md.md_gemm(dev(A), dev(B))
+    with md.Workspace(8, 8, 8, 2):  # too small for 200 x 200 x 64
+        cfg2, A2, B2 = gen(0, 200, 200, 64)
+        with pytest.raises(md.MdError) as e2:
+            md.md_gemm(dev(A2), dev(B2))
+        assert e2.value.status == md.MD_ERR_WORKSPACE
 
 
 def test_on_a_side_stream_and_in_a_cuda_graph():
@@ -356,3 +358,29 @@ def test_exponent_range_flag_and_scaling_near_the_limits(fused):
             assert not C2[:, 3, :].any() and bits_equal(np.delete(C2, 3, axis=1), np.delete(C, 3, axis=1))
     finally:
         md.md_set_option(md.MD_OPT_FUSED_PREP, 0)
+
+
+@pytest.mark.parametrize("cfg_idx,shape,Q,W", [(0, (64, 64, 64), 8, 13), (1, (150, 70, 90), 8, 13), (3, (37, 51, 77), 8, 13),
+                                               (2, (129, 31, 130), 6, 19), (2, (1, 1, 1), 8, 13), (1, (300, 200, 100), 6, 19)])
+def test_small_tile_instance_is_bit_identical_to_the_large_one(cfg_idx, shape, Q, W):
+    """MD_OPT_TILE: the 32 x 16 CTA tile instance of the double-double kernel (picked automatically when the 64 x 32 tiles
+    would not fill the SMs) against the 64 x 32 one: order matrices and C must not differ in a bit, and both preparation
+    paths must feed it."""
+    cfg, A, B = gen(cfg_idx, *shape)
+    out = {}
+    for tile in (1, 2):
+        for fused in (1, 2):
+            md.md_set_option(md.MD_OPT_TILE, tile)
+            md.md_set_option(md.MD_OPT_FUSED_PREP, fused)
+            try:
+                with md.Workspace(cfg.m, cfg.n, cfg.k, 2, Q, bits=W):
+                    out[tile, fused] = (host(md.md_gemm_orders(dev(A), dev(B))), host(md.md_gemm(dev(A), dev(B))), md.md_read_flags())
+            finally:
+                md.md_set_option(md.MD_OPT_TILE, 0)
+                md.md_set_option(md.MD_OPT_FUSED_PREP, 0)
+    Aq, eA, _ = orc.split(A, 0, Q, bits=W)
+    Bq, eB, _ = orc.split(B, 1, Q, bits=W)
+    want = orc.orders_int(Aq, eA, Bq, eB, bits=W)
+    for key, (orders, C, flags) in out.items():
+        assert flags == 0 and bits_equal(orders, want), key
+        assert bits_equal(C, out[2, 2][1]), key
