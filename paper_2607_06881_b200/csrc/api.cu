@@ -466,6 +466,15 @@ md_status md_gemm_host(int m, int n, int k, int limbs, const double* A_host, con
   // the kernels (the caller's stream), copies out; the first kernel starts after A_0 and B_0 have arrived and the last
   // copy out is one block of C, instead of the whole of A, B before and the whole of C after.
   const HostPanels hp = plan_host_panels(m, n, limbs, Q);
+  if (hp.PR == 1 && hp.PC == 1) {  // one block: nothing to overlap -- copy in, the device path as md_gemm runs it, copy out
+    if (cudaMemsetAsync(ws, 0, ALIGN, st) != cudaSuccess) return MD_ERR_CUDA;
+    if (cudaMemcpyAsync(dA, A_host, a_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return MD_ERR_CUDA;
+    if (cudaMemcpyAsync(dB, B_host, b_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return MD_ERR_CUDA;
+    const md_status run = gemm_impl(m, n, k, limbs, dA, dB, dC, nullptr, ws, scratch_bytes - (size_t)(ws - p), st);
+    if (run != MD_OK) return run;
+    if (cudaMemcpyAsync(C_host, dC, c_bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return MD_ERR_CUDA;
+    return cudaStreamSynchronize(st) == cudaSuccess ? MD_OK : MD_ERR_CUDA;
+  }
   if (!host_pipeline_ready(hp.PR + hp.PC + hp.PR * hp.PC + 2)) return MD_ERR_CUDA;
   cudaStream_t s_in = g_host.in, s_out = g_host.out;
   cudaEvent_t* ev = g_host.ev.data();
