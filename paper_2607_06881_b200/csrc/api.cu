@@ -142,10 +142,12 @@ md_status gemm_impl(int m, int n, int k, int limbs, const double* A, const doubl
   uint64_t launches = 0;
   cudaEvent_t* ev = (g_prof.count < g_prof.capacity) ? &g_prof.ev[3 * (size_t)g_prof.count] : nullptr;
   if (ev) cudaEventRecord(ev[0], stream);
-  cudaError_t err;
-  if (use_fused_prep(m, n, k)) {  // one launch instead of five: what matters below ~1024^3
+  cudaError_t err = cudaErrorUnknown;
+  if (use_fused_prep(m, n, k)) {  // one launch instead of five: what matters below ~2048^3
     err = md::launch_prep_packed(m, n, k, limbs, Q, W, small, A, B, c.Aq, c.Bq, c.expA, c.expB, c.flags, stream, &launches);
-  } else {
+    if (err != cudaSuccess) cudaGetLastError();  // a cooperative launch the context cannot take: the separate kernels do the same
+  }
+  if (err != cudaSuccess) {
     err = md::launch_exponents(m, k, 0, Q, W, A, c.expA, c.flags, stream, &launches);
     if (err == cudaSuccess) err = md::launch_exponents(k, n, 1, Q, W, B, c.expB, c.flags, stream, &launches);
     if (err == cudaSuccess) err = md::launch_split_packed(m, k, limbs, Q, W, 0, small, A, c.Aq, c.expA, c.flags, stream, &launches);
