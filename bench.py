@@ -63,6 +63,16 @@ def parse_args():
     ap.add_argument("--paper-paths", action="store_true",
                     help="also time the paper's own two paths on this GPU (libmdcompare: materialised top-down product "
                          "through cuBLAS DGEMM, CUDA-core classical GEMM; SURVEY.md 8(f) NEXT-2), outside the timed region")
+    ap.add_argument("--shape", default=None, help="m,n,k override of the config's shape (same recipe and seed): for the "
+                                                  "small / medium size tables in profiles/")
+    ap.add_argument("--quarters", type=int, default=0, help="override the config's quarter count (MD_OPT_QUARTERS)")
+    ap.add_argument("--orders", type=int, default=0, help="kept product orders S (MD_OPT_ORDERS); default = quarters")
+    ap.add_argument("--raster-group", type=int, default=0, help="MD_OPT_RASTER_GROUP (tile rows per raster group; 0 = default)")
+    ap.add_argument("--micro", action="store_true",
+                    help="instead of the md_gemm step: time the public per-step entry points on this config's shapes -- "
+                         "md_split (axis 0 on A, axis 1 on B) and md_renorm -- and print their achieved HBM GB/s against "
+                         "MEASURED_PEAKS.json (north_star: 'achieved HBM GB/s for the split and epilogue')")
+    ap.add_argument("--lean", action="store_true", help="skip the context blocks beside the headline (quarter plan, adaptive slices)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -185,6 +195,82 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def hbm_peak_gbs():
+    """Measured HBM copy bandwidth of this pool's B200s (driver-written MEASURED_PEAKS.json), else the profiling guide's fallback."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
+    except Exception:  # noqa: BLE001
+        return 6550.0, "fallback of /opt/skills/guides/B200_PROFILING.md (MEASURED_PEAKS.json absent)"
+
+
+def apply_overrides(args, base):
+    import dataclasses
+    if args.shape:
+        m, n, k = (int(x) for x in args.shape.split(","))
+        base = base.with_shape(m, n, k)
+    if args.quarters or args.orders:
+        q = args.quarters or base.quarters
+        base = dataclasses.replace(base, quarters=q, orders=args.orders or q)
+    return base
+
+
+def run_micro(args):
+    """--micro: the public per-step entry points (md_split, md_renorm) on this config's shapes, HBM roofline."""
+    import torch
+    from paper_2607_06881_b200 import binding as md
+    from paper_2607_06881_b200 import inputs
+    torch.cuda.set_device(0)
+    cfg = apply_overrides(args, inputs.CONFIGS[args.config])
+    L, Q = cfg.limbs, cfg.quarters
+    A = torch.from_numpy(inputs.generate(cfg, "A")).cuda()
+    B = torch.from_numpy(inputs.generate(cfg, "B")).cuda()
+    peak, src = hbm_peak_gbs()
+    stream = torch.cuda.current_stream()
+
+    def timed(fn):
+        for _ in range(max(args.warmup, 3)):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(args.steps):
+            fn()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / args.steps
+
+    out = {"impl": "ours", "mode": "micro", "hbm_peak_gbs": peak, "hbm_peak_source": src, "steps": args.steps,
+           "config": {"workload": f"BASELINE.json configs[{cfg.index}] {cfg.name}: m={cfg.m} n={cfg.n} k={cfg.k}, limbs={L}, quarters={Q}"},
+           "kernels": {}}
+    for name, X, axis in (("md_split_axis0_A", A, 0), ("md_split_axis1_B", B, 1)):
+        qp = torch.empty((Q,) + tuple(X.shape[1:]), dtype=torch.float64, device="cuda")
+        ex = torch.empty(X.shape[1] if axis == 0 else X.shape[2], dtype=torch.int32, device="cuda")
+        rows, cols = X.shape[1], X.shape[2]
+
+        def call():
+            st = md.lib().md_split(rows, cols, L, Q, axis, X.data_ptr(), qp.data_ptr(), ex.data_ptr(), stream.cuda_stream)
+            assert st == 0
+        ms = timed(call)
+        # exponent pass reads the leading plane (8 B / element); the split reads 8 L and writes 8 Q bytes per element
+        nbytes = X[0].numel() * 8 * (1 + L + Q)
+        out["kernels"][name] = {"ms": ms, "algorithmic_bytes": nbytes, "gbs": nbytes / ms / 1e6, "frac_of_hbm_peak": nbytes / ms / 1e6 / peak,
+                                "launches": "exponent kernel(s) + split_kernel"}
+        del qp
+    S = args.orders or Q
+    orders = torch.randn((S, cfg.m, cfg.n), dtype=torch.float64, device="cuda") * torch.exp2(-13.0 * torch.arange(S, device="cuda", dtype=torch.float64))[:, None, None]
+    C = torch.empty((L, cfg.m, cfg.n), dtype=torch.float64, device="cuda")
+
+    def call_r():
+        st = md.lib().md_renorm(cfg.m, cfg.n, L, S, orders.data_ptr(), C.data_ptr(), stream.cuda_stream)
+        assert st == 0
+    ms = timed(call_r)
+    nbytes = cfg.m * cfg.n * 8 * (S + L)
+    out["kernels"]["md_renorm"] = {"ms": ms, "algorithmic_bytes": nbytes, "gbs": nbytes / ms / 1e6, "frac_of_hbm_peak": nbytes / ms / 1e6 / peak,
+                                   "note": "synthetic order planes of the right magnitudes (timing only)"}
+    print(json.dumps(out))
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -204,7 +290,8 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     md.lib()  # fail loudly now if the extension is missing
 
-    base = inputs.CONFIGS[args.config]
+    base = apply_overrides(args, inputs.CONFIGS[args.config])
+    md.md_set_option(md.MD_OPT_RASTER_GROUP, args.raster_group)
     # weak scaling: the global A has world * m rows, rank r owns one block of m rows (no collective on the data path)
     if args.slices == "adaptive":
         base = base.with_slices(*md.md_plan_slices(base.k, base.limbs))
@@ -212,7 +299,7 @@ def run_ours(args):
         base = base.with_slices(*md.md_plan_slices_chunked(base.k, base.limbs, 128)[:2])
     cfg = base.with_shape(m=base.m * world)
     row0, row1 = shard.row_block(cfg.m, world, rank)
-    m, n, k, L, Q, W = row1 - row0, cfg.n, cfg.k, cfg.limbs, cfg.quarters, cfg.bits
+    m, n, k, L, Q, W, S = row1 - row0, cfg.n, cfg.k, cfg.limbs, cfg.quarters, cfg.bits, cfg.orders
     A_host = torch.from_numpy(inputs.generate(cfg, "A", row0, row1)).pin_memory()
     B_host = torch.from_numpy(inputs.generate(cfg, "B")).pin_memory()
     C_host = torch.empty((L, m, n), dtype=torch.float64).pin_memory()
@@ -233,7 +320,7 @@ def run_ours(args):
         return float(t.item())
 
     sampler = ClockSampler(local_rank)
-    with md.Workspace(m, n, k, L, Q, bits=W):
+    with md.Workspace(m, n, k, L, Q, bits=W, orders=0 if S == Q else S):
         for _ in range(args.warmup):
             md.md_gemm(A, B, C)
         barrier()
@@ -281,7 +368,7 @@ def run_ours(args):
                 "note": "smallest Q with k (Q+1) 2^(D - W Q - 2) <= the format's tolerance at every position "
                         "(worst case; measured errors are 2-3 orders of magnitude below the bound)"}
 
-    quarter_plan = context_block(plan_block) if world == 1 else None
+    quarter_plan = context_block(plan_block) if world == 1 and not args.lean else None
 
     # beside the headline (the paper's quarters): the same problem with the k-adaptive slices, outside the timed region
     adaptive = None
@@ -320,7 +407,7 @@ def run_ours(args):
             out["chunked"]["chunk"] = cK
         return out
 
-    if args.slices == "paper" and world == 1:
+    if args.slices == "paper" and world == 1 and not args.lean:
         adaptive = context_block(adaptive_block)
 
     # the paper's own two paths on the same inputs (context; outside the timed region; N = 1, dd / qd only)
@@ -371,6 +458,7 @@ def run_ours(args):
     if not args.no_e2e:
         try:
             md.md_set_option(md.MD_OPT_QUARTERS, 0 if Q == 4 * L else Q)  # before sizing the scratch: it depends on Q
+            md.md_set_option(md.MD_OPT_ORDERS, 0 if S == Q else S)
             md.md_set_option(md.MD_OPT_SLICE_BITS, 0 if W == 13 else W)
             scratch = torch.empty(md.md_host_scratch_bytes(m, n, k, L), dtype=torch.uint8, device="cuda")
             for _ in range(min(args.warmup, 2)):
@@ -386,6 +474,7 @@ def run_ours(args):
             e2e_ms = max_over_ranks(e0.elapsed_time(e1))
             wall_ms = max_over_ranks((time.perf_counter() - t0) * 1e3)
             md.md_set_option(md.MD_OPT_QUARTERS, 0)
+            md.md_set_option(md.MD_OPT_ORDERS, 0)
             md.md_set_option(md.MD_OPT_SLICE_BITS, 0)
             e2e = {"value": world * base.md_flops * args.steps / (max(e2e_ms, wall_ms) * 1e-3) / 1e9, "unit": UNIT,
                    "h2d_bytes_per_step": A_host.numel() * 8 + B_host.numel() * 8, "d2h_bytes_per_step": C_host.numel() * 8,
@@ -393,7 +482,7 @@ def run_ours(args):
                    "matches_device_path": bool((C_host == C.cpu()).all())}
             del scratch
         except Exception as exc:  # noqa: BLE001 -- the device-resident headline must still be reported
-            for key in (md.MD_OPT_SLICE_BITS, md.MD_OPT_QUARTERS):
+            for key in (md.MD_OPT_SLICE_BITS, md.MD_OPT_QUARTERS, md.MD_OPT_ORDERS):
                 md.md_set_option(key, 0)
             e2e = {"error": f"{type(exc).__name__}: {exc}"}
     sampler.stop()
@@ -447,7 +536,7 @@ def run_ours(args):
         "dtype": "f64", "data": "synthetic",
         "config": {
             "workload": f"BASELINE.json configs[{base.index}] {base.name}: m={base.m} n={base.n} k={base.k} per GPU, "
-                        f"limbs={L}, quarters={Q} of {W} bits (T={base.products} quarter products), seed {base.seed}",
+                        f"limbs={L}, quarters={Q} of {W} bits, orders={S} (T={base.products} quarter products), seed {base.seed}",
             "slices": args.slices,
             "parallelism": "single GPU" if world == 1 else f"rows of A sharded over {world} GPUs, B replicated, no collective",
             "l2": "inputs (%.0f MiB) and quarter planes (%.0f MiB) exceed the 126 MB L2; no explicit flush" % (
@@ -469,6 +558,8 @@ def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.micro:
+        run_micro(args)
     else:
         run_ours(args)
 

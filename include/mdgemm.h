@@ -25,9 +25,22 @@
  *   - Return value: MD_OK (0) or a negative md_status.  Errors are detected from the ARGUMENTS only, synchronously,
  *     and nothing has been enqueued when one is returned (MD_ERR_CUDA: a launch failed; cudaGetLastError is preserved).
  *   - Data preconditions (cannot be seen without a sync, so they are not return codes): inputs finite; the leading limb
- *     is the largest in magnitude and |limb_{l+1}| <= ulp(limb_l); every group exponent (below) within [-900, 900].
- *     Violations set bits in a device status word (md_read_flags) and give unspecified values, never a fault.
- *   - Not thread-safe with respect to md_set_option / md_set_workspace (process-wide state); otherwise re-entrant.
+ *     is the largest in magnitude and |limb_{l+1}| <= ulp(limb_l); every group exponent E (below) within [-900, 900] and
+ *     E >= W * quarters - 1022 (every digit unit a normal double).  Violations set bits in a device status word
+ *     (md_read_flags) and give unspecified values, never a fault.  For a PRODUCT the conditions are pairwise: with E_i the
+ *     exponent of row i of A and F_j of column j of B, exactness needs E_i + F_j <= 1023 and E_i + F_j - W (orders + 1) >= -1022
+ *     (the smallest kept order unit a normal double).  The first shows in C itself (an overflow gives +-inf / NaN there);
+ *     the second is NOT flagged per pair: below it the lowest orders lose bits silently.  |E| <= 450 on both sides is always
+ *     safe for double and quad double.
+ *   - ACCURACY IS RELATIVE TO 2^(E_i + F_j), NOT TO (|A||B|)_ij (see md_gemm): on data whose rows / columns span many binades
+ *     the default quarter count can miss the format's tolerance relative to (|A||B|)_ij without any flag.  md_plan_quarters
+ *     measures what the data needs, md_gemm_auto runs the plan and the product in one call, and every count the plan can
+ *     return (up to 16 / 24 / 40 / 72 quarters for 2 / 4 / 8 / 16 limbs) has a kernel.
+ *   - Options (md_set_option) are process-wide; the registered workspace, the profile record and md_gemm_host's copy streams
+ *     are per DEVICE (the current device of the calling thread).  All calls of the md_gemm family that share a workspace
+ *     (including its stream-K scratch) must be serialised on ONE stream; two md_gemm_host calls on one device must not run
+ *     concurrently; md_set_option / md_set_workspace / md_profile_* must not race with anything.  Distinct devices are
+ *     independent.
  */
 #ifndef MDGEMM_H_
 #define MDGEMM_H_
@@ -55,11 +68,17 @@ typedef void* md_stream;    /* a cudaStream_t */
 /* Options (process-wide).  value 0 restores the default. */
 enum {
   MD_OPT_QUARTERS = 1,  /* quarters per element used by md_gemm / md_gemm_orders / md_gemm_host.  Default 4*limbs, the
-                           paper's count (8 for double double, 16 for quad double).  Supported:
-                           limbs=2: 8, 9, 10; limbs=4: 16, 17, 18 (R5); limbs=8: 32; limbs=16: 64 (octo / hexa double,
-                           PAPER.md:196-205 Table 2, R13); fewer with MD_OPT_SLICE_BITS (below). */
-  MD_OPT_ORDERS = 2,    /* kept product orders S (the paper's C_1..C_S).  Default = quarters.  Must equal
-                           quarters in this version. */
+                           paper's count (8 for double double, 16 for quad double).  Any count up to 16
+                           (limbs=2), 24 (4), 40 (8), 72 (16) runs.  Tuned kernels: limbs=2: 8, 9, 10; limbs=4: 16, 17, 18
+                           (R5); limbs=8: 32; limbs=16: 64 (octo / hexa double, Table 2,
+                           DESIGN.md R13); with MD_OPT_SLICE_BITS also 6, 7 / 11, 12 / 22 / 44.  Every other count runs on
+                           the generic kernel (runtime counts; slower, same bits). */
+  MD_OPT_ORDERS = 2,    /* kept product orders S: C^(s) for s = 0..S-1 (the paper's C_1..C_S).  Default = quarters
+                           (the paper keeps C_1..C_8 of 8 quarters).  1 <= S <= min(quarters + 2, 2*quarters - 1): S < quarters
+                           is a PRUNED set (fewer products, larger error), S > quarters an EXTENDED one -- order Q adds the Q - 1
+                           products p + q = Q that the paper's set drops, for less work than another quarter (R5).
+                           Tuned kernels for (8, 9), (8, 10), (16, 17), (16, 18); the generic kernel otherwise.  Error bound:
+                           see md_gemm. */
   MD_OPT_SLICE_BITS = 3, /* width W of a slice in bits, used by md_split and the md_gemm family.  Default 13: the paper's
                            quarter ("4 parts ... each of 13 bits").  Other widths (4..24) are the k-adaptive
                            variant of DESIGN.md R14 / SURVEY.md 8(f) NEXT-3 -- NOT the paper's quarters: a slice of W
@@ -79,6 +98,9 @@ enum {
   MD_OPT_TILE = 7,       /* md_gemm / md_gemm_orders, double double with 8 or 6 slices: 0 = automatic -- the 32 x 16 CTA tile
                             instance of the fused kernel when the 64 x 32 tiles would number at most two thirds of the SMs
                             (up to about 448^3), 64 x 32 otherwise; 1 = 32 x 16 wherever it exists; 2 = never.  Same bits. */
+  MD_OPT_RASTER_GROUP = 8, /* fused quarter GEMM: tile rows per raster group (the CTAs in flight cover GROUP x (SMs / GROUP) tiles of C and
+                            share their operand slabs through L2).  0 = default 8 (the best of the measured 4 / 8 / 16 / 32,
+                            profiles/).  Same bits for any value. */
   MD_OPT_HOST_BLOCKS = 4 /* md_gemm_host only: number of blocks C is cut into for overlapping copies and kernels.
                             Default 0 = automatic (about one wave of CTA tiles per block, at most 32); 1 = no overlap;
                             PR * 256 + PC = explicit numbers of row panels and column panels (each <= 64). */
@@ -128,8 +150,10 @@ md_status md_split(int rows, int cols, int limbs, int quarters, int axis, const 
  *   order_planes  out  [orders][m][n] fp64, C^(s) true-valued; may be NULL
  *   C_planes      out  [limbs][m][n]: the orders summed error-free into `limbs` limbs in the kernel's epilogue
  *                      (same arithmetic as md_renorm); may be NULL.  Not both NULL.
- *   Needs orders == quarters, limbs in {2, 4} with (limbs, quarters) as listed at MD_OPT_QUARTERS and MD_OPT_SLICE_BITS
- *   (octo / hexa double go through md_gemm's packed operands only), k * orders * 2^(2W) <= 2^53 (W = 13: k * orders <= 2^27).
+ *   k * orders * 2^(2W) <= 2^53 (W = 13: k * orders <= 2^27).  limbs in {2, 4} with orders == quarters in {6..10} / {11, 12,
+ *   16, 17, 18} run a kernel that reads the plain planes directly; every other (limbs, quarters, orders) md_gemm accepts is
+ *   repacked into the REGISTERED WORKSPACE (md_set_workspace, sized by md_workspace_bytes with MD_OPT_QUARTERS / MD_OPT_ORDERS
+ *   set to these counts) and runs the kernel md_gemm would (MD_ERR_WORKSPACE without one).
  * ------------------------------------------------------------------------------------------------------------------ */
 md_status md_qgemm(int m, int n, int k, int limbs, int quarters, int orders, const double* Aq, const double* Bq,
                    double* order_planes, double* C_planes, md_stream stream);
@@ -150,9 +174,12 @@ md_status md_renorm(int m, int n, int limbs, int orders, const double* order_pla
  *   `limbs` limb planes.  Splits A by rows and B by columns into the registered workspace, then one fused kernel does
  *   the quarter products and writes the renormalised C once.  limbs in {2, 4, 8, 16} (double double, quad double, and the
  *   octo / hexa double of PAPER.md:196-205 Table 2).
- *   Accuracy: |C - A*B|_ij <= k (Q+1) 2^(E_i + F_j - 13Q - 2) + 2^-(53*limbs - 3) |C|_ij for any input (Q = quarters; E, F
- *   the exponent vectors of A's rows and B's columns); on the BASELINE.json workloads this is within 1e-28 (|A||B|)_ij
- *   (double double) and 1e-58 (|A||B|)_ij (quad double).
+ *   Accuracy: |C - A*B|_ij <= k (Q+1) 2^(E_i + F_j - 13Q - 2) + 2^-(53*limbs - 3) |C|_ij for any input (Q = quarters = orders;
+ *   E, F the exponent vectors of A's rows and B's columns).  THE BOUND IS RELATIVE TO 2^(E_i + F_j), NOT TO (|A||B|)_ij: on the
+ *   BASELINE.json workloads it is within 1e-28 (|A||B|)_ij (double double; configs[3] with 9 quarters) and 1e-58 (quad
+ *   double), but a row such as [2^60, 1 + 2^-70] loses the low limb of its small element -- no flag is raised; use
+ *   md_plan_quarters / md_gemm_auto when the data is not known to be well scaled.  With orders S != Q the first term is
+ *   k 2^(E_i + F_j - 2) [ 2^(1 - 13Q) + (2Q - 1 - S)+ 2^(-13S) ] (remainders of the split + dropped orders S..2Q-2).
  *   md_gemm_orders is the debug/parity variant: same split, then writes the order matrices C^(s) [orders][m][n] instead.
  * ------------------------------------------------------------------------------------------------------------------ */
 md_status md_gemm(int m, int n, int k, int limbs, const double* A_planes, const double* B_planes, double* C_planes,
@@ -180,15 +207,34 @@ size_t md_plan_scratch_bytes(int m, int n, int k);
 md_status md_plan_quarters(int m, int n, int k, int limbs, const double* A_planes, const double* B_planes, void* scratch,
                            size_t scratch_bytes, double rel_tol, int* quarters_out, int* spread_out, md_stream stream);
 
+/* ---------------------------------------------------------------------------------------------------------------------
+ * md_gemm_auto -- md_plan_quarters and md_gemm in one call: measures the spread D of THIS data, takes the smallest quarter
+ *   count Q whose bound meets rel_tol (|A||B|)_ij at every position (0 = the format's tolerance), and runs the product with
+ *   Q = S = that count (the tuned kernel where one exists, the generic one otherwise), ignoring MD_OPT_QUARTERS / MD_OPT_ORDERS.
+ *   scratch        device, 256-byte aligned, caller-owned: the plan's scratch and then the workspace of the product.
+ *                  md_auto_scratch_bytes(m, n, k, limbs, quarters) sizes it for a given count (0 = 4 * limbs, the paper's);
+ *                  if the plan needs more, the call returns MD_ERR_WORKSPACE with the needed count in *quarters_used and has
+ *                  enqueued nothing but the plan: size again and repeat.
+ *   quarters_used  HOST, may be NULL: the count the product ran with (or needs)
+ *   Returns MD_ERR_UNSUPPORTED when the plan exceeds the generic maxima (16 / 24 / 40 / 72).  SYNCHRONISES `stream` (the plan
+ *   returns Q to the host, and the status word of the call is read back for md_read_flags); not capturable in a CUDA graph.
+ * ------------------------------------------------------------------------------------------------------------------ */
+size_t md_auto_scratch_bytes(int m, int n, int k, int limbs, int quarters);
+md_status md_gemm_auto(int m, int n, int k, int limbs, const double* A_planes, const double* B_planes, double* C_planes,
+                       void* scratch, size_t scratch_bytes, double rel_tol, int* quarters_used, md_stream stream);
+
 /* Workspace for md_gemm / md_gemm_orders: quarter planes of A and B, exponent vectors and the status word, for the
- * CURRENT option values.  The caller allocates (device memory, 256-byte aligned) and registers it; the library keeps
- * the pointer until it is replaced (ptr = NULL, bytes = 0 unregisters).  md_workspace_bytes returns 0 on bad arguments. */
+ * CURRENT option values.  The caller allocates (device memory, 256-byte aligned) and registers it FOR THE CURRENT DEVICE; the
+ * library keeps the pointer until it is replaced (ptr = NULL, bytes = 0 unregisters).  md_workspace_bytes returns 0 on bad
+ * arguments.  md_set_workspace clears the status word with a SYNCHRONOUS cudaMemset (it is a set-up call, not capturable). */
 size_t md_workspace_bytes(int m, int n, int k, int limbs);
 md_status md_set_workspace(void* dev_ptr, size_t bytes);
 
-/* Device status word of the registered workspace, copied to *flags_host (host pointer); SYNCHRONISES `stream`.
- * bit 0: a non-finite input was seen; bit 1: a group exponent outside [-900, 900].  The word is cleared by md_set_workspace
- * and accumulates until then. */
+/* Device status word of the registered workspace, ORed with the status words md_gemm_host / md_gemm_auto calls on this device
+ * have brought back (they run in caller scratch, not in the registered workspace), copied to *flags_host (host pointer);
+ * SYNCHRONISES `stream`.  bit 0: a non-finite input was seen; bit 1: a group exponent outside its range (see the conventions
+ * at the top).  Cleared by md_set_workspace, accumulates until then.  Without a registered workspace: the host-side record
+ * alone, MD_ERR_WORKSPACE if there is none yet. */
 md_status md_read_flags(uint32_t* flags_host, md_stream stream);
 
 /* ---------------------------------------------------------------------------------------------------------------------
@@ -206,9 +252,11 @@ md_status md_gemm_host(int m, int n, int k, int limbs, const double* A_host, con
                        void* dev_scratch, size_t scratch_bytes, md_stream stream);
 
 /* Per-call device timing of md_gemm / md_gemm_orders / md_gemm_host, for roofline accounting (bench.py).
- * md_profile_enable(capacity > 0): each following call records CUDA events on its stream before its first kernel, before
- * the fused quarter-GEMM kernel and after it, for up to `capacity` calls (further calls are not recorded); calling it again
- * restarts the record; capacity = 0 disables and frees the events.  Do not enable while capturing a CUDA graph.
+ * md_profile_enable(capacity > 0): each following call on this device records CUDA events on its stream before its first
+ * kernel, before the fused quarter-GEMM kernel and after it, for up to `capacity` calls (further calls are not recorded);
+ * calling it again restarts the record; capacity = 0 disables and frees the events.  Do not enable while capturing a CUDA
+ * graph (the timing events would become graph nodes).  md_gemm_host is recorded only when it runs as ONE block (small
+ * problems); its multi-panel pipeline interleaves splits and products and records nothing.
  * md_profile_read synchronises the recorded events and returns how many calls were recorded (<= capacity, or a negative
  * md_status); for call i it stores the split time (exponent + split kernels) in split_ms_host[i] and the fused GEMM
  * kernel time in gemm_ms_host[i] (HOST arrays of at least `capacity` floats; either may be NULL). */

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libmdgemm.so")
 
 MD_OK = 0
 MD_ERR_BAD_ARG, MD_ERR_K_TOO_LARGE, MD_ERR_WORKSPACE, MD_ERR_CUDA, MD_ERR_UNSUPPORTED = -1, -2, -3, -4, -5
-MD_OPT_QUARTERS, MD_OPT_ORDERS, MD_OPT_SLICE_BITS, MD_OPT_HOST_BLOCKS, MD_OPT_K_CHUNK, MD_OPT_FUSED_PREP, MD_OPT_TILE = 1, 2, 3, 4, 5, 6, 7
+MD_OPT_QUARTERS, MD_OPT_ORDERS, MD_OPT_SLICE_BITS, MD_OPT_HOST_BLOCKS, MD_OPT_K_CHUNK, MD_OPT_FUSED_PREP, MD_OPT_TILE, MD_OPT_RASTER_GROUP = 1, 2, 3, 4, 5, 6, 7, 8
 
 # every symbol include/mdgemm.h declares: name -> (restype, argtypes)
 _c = ctypes
@@ -26,6 +26,8 @@ _SIGNATURES = {
     "md_plan_slices": (_c.c_int, [_c.c_int, _c.c_int, _c.c_void_p, _c.c_void_p]),
     "md_plan_scratch_bytes": (_c.c_size_t, [_c.c_int] * 3),
     "md_plan_quarters": (_c.c_int, [_c.c_int] * 4 + [_c.c_void_p] * 3 + [_c.c_size_t, _c.c_double] + [_c.c_void_p] * 3),
+    "md_auto_scratch_bytes": (_c.c_size_t, [_c.c_int] * 5),
+    "md_gemm_auto": (_c.c_int, [_c.c_int] * 4 + [_c.c_void_p] * 4 + [_c.c_size_t, _c.c_double, _c.c_void_p, _c.c_void_p]),
     "md_plan_slices_chunked": (_c.c_int, [_c.c_int] * 3 + [_c.c_void_p] * 3),
     "md_split": (_c.c_int, [_c.c_int] * 5 + [_c.c_void_p] * 4),
     "md_qgemm": (_c.c_int, [_c.c_int] * 6 + [_c.c_void_p] * 5),
@@ -150,14 +152,15 @@ def md_split(planes: torch.Tensor, axis: int, quarters: int | None = None, strea
 
 
 def md_qgemm(Aq: torch.Tensor, Bq: torch.Tensor, limbs: int, want_orders: bool = False, want_C: bool = True,
-             stream=None):
-    """Aq [Q, m, k], Bq [Q, k, n] -> (order_planes [Q, m, n] or None, C_planes [limbs, m, n] or None)."""
+             stream=None, orders_kept: int | None = None):
+    """Aq [Q, m, k], Bq [Q, k, n] -> (order_planes [S, m, n] or None, C_planes [limbs, m, n] or None); S = orders_kept or Q."""
     Q, m, k = Aq.shape
     n = Bq.shape[2]
+    S = Q if orders_kept is None else orders_kept
     assert Bq.shape[0] == Q and Bq.shape[1] == k
-    orders = torch.empty((Q, m, n), dtype=torch.float64, device=Aq.device) if want_orders else None
+    orders = torch.empty((S, m, n), dtype=torch.float64, device=Aq.device) if want_orders else None
     C = torch.empty((limbs, m, n), dtype=torch.float64, device=Aq.device) if want_C else None
-    _check(lib().md_qgemm(m, n, k, limbs, Q, Q, _dev(Aq), _dev(Bq), None if orders is None else _dev(orders),
+    _check(lib().md_qgemm(m, n, k, limbs, Q, S, _dev(Aq), _dev(Bq), None if orders is None else _dev(orders),
                           None if C is None else _dev(C), _stream(stream)), "md_qgemm")
     return orders, C
 
@@ -178,6 +181,26 @@ def md_gemm(A: torch.Tensor, B: torch.Tensor, C: torch.Tensor | None = None, str
         C = torch.empty((limbs, m, n), dtype=torch.float64, device=A.device)
     _check(lib().md_gemm(m, n, k, limbs, _dev(A), _dev(B), _dev(C), _stream(stream)), "md_gemm")
     return C
+
+
+def md_gemm_auto(A: torch.Tensor, B: torch.Tensor, C: torch.Tensor | None = None, rel_tol: float = 0.0, stream=None):
+    """md_plan_quarters + md_gemm in one call (include/mdgemm.h).  Returns (C, quarters used).  Allocates the scratch for the
+    paper's count first and again if the plan asks for more.  Synchronises."""
+    limbs, m, k = A.shape
+    n = B.shape[2]
+    if C is None:
+        C = torch.empty((limbs, m, n), dtype=torch.float64, device=A.device)
+    q = ctypes.c_int(0)
+    want = 0
+    for _ in range(2):
+        scratch = torch.empty(lib().md_auto_scratch_bytes(m, n, k, limbs, want), dtype=torch.uint8, device=A.device)
+        st = lib().md_gemm_auto(m, n, k, limbs, _dev(A), _dev(B), _dev(C), _dev(scratch, torch.uint8), scratch.numel(), rel_tol,
+                                ctypes.addressof(q), _stream(stream))
+        if st != MD_ERR_WORKSPACE or q.value == want or q.value == 0:
+            break
+        want = q.value
+    _check(st, "md_gemm_auto")
+    return C, q.value
 
 
 def md_gemm_orders(A: torch.Tensor, B: torch.Tensor, stream=None) -> torch.Tensor:
@@ -234,8 +257,9 @@ def md_launch_count() -> int:
 class Workspace:
     """Allocates and registers the md_gemm workspace for one problem shape (context manager)."""
 
-    def __init__(self, m, n, k, limbs, quarters: int = 0, device="cuda", bits: int = 0):
+    def __init__(self, m, n, k, limbs, quarters: int = 0, device="cuda", bits: int = 0, orders: int = 0):
         md_set_option(MD_OPT_QUARTERS, 0 if quarters == 4 * limbs else quarters)
+        md_set_option(MD_OPT_ORDERS, orders)
         md_set_option(MD_OPT_SLICE_BITS, 0 if bits == 13 else bits)
         nbytes = md_workspace_bytes(m, n, k, limbs)
         if nbytes == 0:
@@ -246,6 +270,7 @@ class Workspace:
     def close(self):
         md_set_workspace(None)
         md_set_option(MD_OPT_QUARTERS, 0)
+        md_set_option(MD_OPT_ORDERS, 0)
         md_set_option(MD_OPT_SLICE_BITS, 0)
         self.buffer = None
 

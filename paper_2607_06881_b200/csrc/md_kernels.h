@@ -29,13 +29,17 @@ cudaError_t launch_spread(int m, int n, const double* W, const int32_t* expA, co
                           cudaStream_t stream, uint64_t* launches);
 // md_gemm's internal pair: splitter writing the fragment-major packed layout (md_packed.cuh) and the bulk-copy /
 // mbarrier pipelined fused GEMM reading it.  Same (limbs, quarters) support as launch_qgemm.
-// small: the 32 x 16 tile instance of the double-double kernel (md_packed.cuh pack_bx); splitter and GEMM must agree
-cudaError_t launch_split_packed(int rows, int cols, int limbs, int quarters, int bits, int axis, bool small,
+// bx, bk: the CTA tile extent along the group index and the k-slab depth of the fused kernel that will read the planes
+// (md_packed.cuh pack_bx / pack_bx_generic; api.cu pick_kernel): splitter and GEMM must agree
+cudaError_t launch_split_packed(int rows, int cols, int limbs, int quarters, int bits, int axis, int bx, int bk,
                                 const double* planes, double* packed, const int32_t* exps, uint32_t* flags,
                                 cudaStream_t stream, uint64_t* launches);
-bool qgemm_small_supported(int limbs, int quarters);
+// plain [quarters][rows][cols] planes -> the packed layout (no arithmetic): md_qgemm for counts without a plain-layout kernel
+cudaError_t launch_pack_planes(int rows, int cols, int quarters, int axis, int bx, int bk, const double* planes, double* packed,
+                               cudaStream_t stream, uint64_t* launches);
+bool qgemm_small_supported(int limbs, int quarters, int orders);
 // exponent vectors + packed quarter planes of BOTH operands in one launch (small and medium problems: md_gemm's fused prep)
-cudaError_t launch_prep_packed(int m, int n, int k, int limbs, int quarters, int bits, bool small, const double* A,
+cudaError_t launch_prep_packed(int m, int n, int k, int limbs, int quarters, int bits, int bxA, int bxB, int bk, const double* A,
                                const double* B, double* Ap, double* Bp, int32_t* expA, int32_t* expB, uint32_t* flags,
                                cudaStream_t stream, uint64_t* launches);
 // sk_ws: sk_workspace_bytes(limbs, quarters) bytes of device scratch for the stream-K tail (slab counters + one
@@ -48,12 +52,13 @@ constexpr size_t SK_CHUNK_CAP_BYTES = (size_t)512 << 20;
 inline bool sk_chunk_scratch_fits(size_t nchunks, int S, int BM, int BN) {
   return sizeof(double) * (size_t)SK_MAX_TILES * nchunks * S * BM * BN <= SK_CHUNK_CAP_BYTES;
 }
-size_t sk_workspace_bytes(int limbs, int quarters, int k, int chunk);
+size_t sk_workspace_bytes(int orders, int bxA, int bxB, int k, int chunk);
 int sk_grid();
 // chunk = 0: exact orders over the whole k.  chunk > 0 (R16; a multiple of 8, qgemm_chunk_supported instances
 // only, C_planes only): the accumulators are folded into the elements' expansions every `chunk` contraction indices.
 bool qgemm_chunk_supported(int limbs, int quarters);
-cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, int chunk, bool small, const double* Ap,
+bool qgemm_packed_supported(int limbs, int quarters, int orders);
+cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, int orders, int chunk, bool small, const double* Ap,
                                 const double* Bp, double* order_planes, double* C_planes, void* sk_ws,
                                 cudaStream_t stream, uint64_t* launches);
 // octo / hexa double (qgemm_wide.cu): same packed operands (k-slab depth 4), same stream-K scratch convention
@@ -61,6 +66,17 @@ bool qgemm_wide_supported(int limbs, int quarters);
 cudaError_t launch_qgemm_wide(int m, int n, int k, int limbs, int quarters, const double* Ap, const double* Bp,
                               double* order_planes, double* C_planes, void* sk_ws, cudaStream_t stream,
                               uint64_t* launches);
+// GENERIC instances of the same kernel (qgemm_wide.cu): quarter and order counts are runtime values up to these maxima, orders
+// <= quarters + 2 (and <= 2 quarters - 1); packed operands with the tile shape of pack_bx_generic and k-slab depth 4
+constexpr int GENERIC_QMAX_DD = 16, GENERIC_QMAX_QD = 24, GENERIC_QMAX_OD = 40, GENERIC_QMAX_HD = 72;
+int qgemm_generic_max_quarters(int limbs);
+bool qgemm_generic_supported(int limbs, int quarters, int orders);
+cudaError_t launch_qgemm_generic(int m, int n, int k, int limbs, int quarters, int orders, const double* Ap, const double* Bp,
+                                 double* order_planes, double* C_planes, void* sk_ws, cudaStream_t stream, uint64_t* launches);
+// per-device bookkeeping shared by the launchers (api.cu): the current device (-1 on error) and its SM count
+constexpr int MD_MAX_DEVICES = 64;
+int current_device();
+int sm_count();
 // calibration (probe.cu): register-only DMMA loop; *flops receives the FP64 flops the launch issues
 cudaError_t launch_dmma_probe(int blocks, int warps_per_block, int iters, double* sink, cudaStream_t stream,
                               uint64_t* launches, uint64_t* flops);

@@ -34,6 +34,13 @@ __host__ __device__ constexpr int pack_bx(int limbs, int quarters, int axis, boo
          : limbs == 16 ? (axis == 0 ? 16 : (quarters <= 44 ? 16 : 8)) : (axis == 0 ? 32 : 16);
 }
 
+// The GENERIC-Q instances of qgemm_wide.cu (runtime quarter / order counts, any (limbs, quarters, orders) md_gemm accepts
+// that has no tuned kernel): 32 x 16 CTA tiles for double and quad double, 16 x 16 for octo double (two order ranges per
+// tile), 16 x 8 for hexa double (four); k-slab depth 4.
+__host__ __device__ constexpr int pack_bx_generic(int limbs, int axis) {
+  return limbs == 16 ? (axis == 0 ? 16 : 8) : limbs == 8 ? 16 : (axis == 0 ? 32 : 16);
+}
+
 // doubles in the packed image of an operand with X groups and K contraction indices
 __host__ __device__ inline size_t packed_doubles(int X, int K, int bx, int bk, int quarters) {
   const size_t xt = ((size_t)X + bx - 1) / bx, ks = ((size_t)K + bk - 1) / bk;

@@ -36,14 +36,16 @@ __global__ void __launch_bounds__(256) spread_kernel(int m, int n, const double*
 
 cudaError_t launch_abs(size_t count, const double* in, double* out, cudaStream_t stream, uint64_t* launches) {
   const size_t want = (count + 255) / 256;
-  abs_kernel<<<(unsigned)(want < 148 * 32 ? want : 148 * 32), 256, 0, stream>>>(count, in, out);
+  const int cap = (sm_count() > 0 ? sm_count() : 1) * 32;
+  abs_kernel<<<(unsigned)(want < (size_t)cap ? want : (size_t)cap), 256, 0, stream>>>(count, in, out);
   *launches += 1;
   return cudaGetLastError();
 }
 
 cudaError_t launch_spread(int m, int n, const double* W, const int32_t* expA, const int32_t* expB, int32_t* spread,
                           cudaStream_t stream, uint64_t* launches) {
-  spread_kernel<<<m < 148 * 16 ? m : 148 * 16, 256, 0, stream>>>(m, n, W, expA, expB, spread);
+  const int cap = (sm_count() > 0 ? sm_count() : 1) * 16;
+  spread_kernel<<<m < cap ? m : cap, 256, 0, stream>>>(m, n, W, expA, expB, spread);
   *launches += 1;
   return cudaGetLastError();
 }

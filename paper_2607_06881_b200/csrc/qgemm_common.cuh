@@ -104,8 +104,7 @@ __device__ __forceinline__ void chunk_epilogue(double (&r)[MT][NT][2][L + 1], in
 
 // Tile rasterisation shared by both kernels: groups of GROUP_M tile rows are swept along n, so that the ~148 CTAs in
 // flight cover a near-square patch of C and share their A / B slabs through L2.
-__device__ __forceinline__ void raster_tile(int bid, int tiles_m, int tiles_n, int& tm, int& tn) {
-  constexpr int GROUP_M = 8;
+__device__ __forceinline__ void raster_tile(int bid, int tiles_m, int tiles_n, int& tm, int& tn, int GROUP_M = 8) {
   const int per_group = GROUP_M * tiles_n;
   const int first_m = (bid / per_group) * GROUP_M;
   const int gsize = min(tiles_m - first_m, GROUP_M);

@@ -29,10 +29,11 @@
 namespace md {
 namespace {
 
-// A warp owns an (8*MT) x (8*NT) block of C and Q (= S) accumulator sets for it; WM x WN warps tile the CTA block.
-template <int Q_, int L_, int WM_, int WN_, int MT_, int NT_>
+// A warp owns an (8*MT) x (8*NT) block of C and S accumulator sets for it (S = Q, the paper's C_1..C_Q, unless MD_OPT_ORDERS
+// asks for a pruned or extended order set); WM x WN warps tile the CTA block.
+template <int Q_, int L_, int WM_, int WN_, int MT_, int NT_, int S_ = Q_>
 struct PCfg {
-  static constexpr int Q = Q_, S = Q_, L = L_, WM = WM_, WN = WN_, MT = MT_, NT = NT_;
+  static constexpr int Q = Q_, S = S_, L = L_, WM = WM_, WN = WN_, MT = MT_, NT = NT_;
   static constexpr int BM = WM * MT * 8, BN = WN * NT * 8, BK = PACK_BK;
   static constexpr int WARPS = WM * WN, THREADS = WARPS * 32;
   static constexpr int K4 = BK / 4, R8 = BM / 8, N8 = BN / 8;
@@ -112,7 +113,7 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
     if (p_left == 0) {
       int tile, s0, s1, tm, tn;
       segment(++p_seg, tile, s0, s1);
-      raster_tile(tile, plan.tiles_m, plan.tiles_n, tm, tn);
+      raster_tile(tile, plan.tiles_m, plan.tiles_n, tm, tn, plan.group_m);
       p_A = Ap + ((size_t)tm * KS + s0) * C::A_CHUNK;
       p_B = Bp + ((size_t)tn * KS + s0) * C::B_CHUNK;
       p_left = s1 - s0;
@@ -221,7 +222,7 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
 #pragma unroll
       for (int j = 0; j < NT; j++) b[j] = q == 0 ? f.b0[j] : Bs[((q * C::K4 + k4) * C::N8 + j) * 32];
 #pragma unroll
-      for (int p = 0; p + q < S; p++)  // product (p, q) goes to order s = p + q: consecutive DMMAs hit different accumulators
+      for (int p = 0; p + q < S && p < Q; p++)  // product (p, q) goes to order s = p + q: consecutive DMMAs hit different accumulators
 #pragma unroll
         for (int i = 0; i < MT; i++)
 #pragma unroll
@@ -241,7 +242,7 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
   }
   auto end_of_segment = [&]() {
     int tm, tn;
-    raster_tile(c_tile, plan.tiles_m, plan.tiles_n, tm, tn);
+    raster_tile(c_tile, plan.tiles_m, plan.tiles_n, tm, tn, plan.group_m);
     const int row_base = tm * C::BM + wm * MT * 8, col_base = tn * C::BN + wn * NT * 8;
     if constexpr (CHUNK) {
       if (c_s1 - c_s0 == KS) {  // whole tile: fold the last chunk in, finish the expansions, write C once
@@ -411,8 +412,13 @@ cudaError_t launch_cfg(int m, int n, int k, const double* Ap, const double* Bp, 
     if (err != cudaSuccess) return err;
   }
   auto kern = qgemm_packed_kernel<C, false>;
-  err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
-  if (err != cudaSuccess) return err;
+  static bool attr_done[MD_MAX_DEVICES] = {};  // the shared-memory opt-in is per function and device: once, not per launch
+  const int dev = current_device();
+  if (dev < 0 || dev >= MD_MAX_DEVICES || !attr_done[dev]) {
+    err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+    if (err != cudaSuccess) return err;
+    if (dev >= 0 && dev < MD_MAX_DEVICES) attr_done[dev] = true;
+  }
   kern<<<G, C::THREADS, C::SMEM_BYTES, stream>>>(m, n, plan, Ap, Bp, order_planes, C_planes, scratch, counters);
   return cudaGetLastError();
 }
@@ -446,19 +452,24 @@ cudaError_t launch_chunked(int m, int n, int k, int chunk, const double* Ap, con
     plan.sk_iters_per_cta = 0;
   }
   auto kern = qgemm_packed_kernel<C, true>;
-  err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
-  if (err != cudaSuccess) return err;
+  static bool attr_done[MD_MAX_DEVICES] = {};  // the shared-memory opt-in is per function and device: once, not per launch
+  const int dev = current_device();
+  if (dev < 0 || dev >= MD_MAX_DEVICES || !attr_done[dev]) {
+    err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+    if (err != cudaSuccess) return err;
+    if (dev >= 0 && dev < MD_MAX_DEVICES) attr_done[dev] = true;
+  }
   kern<<<G, C::THREADS, C::SMEM_BYTES, stream>>>(m, n, plan, Ap, Bp, nullptr, C_planes, scratch, counters);
   return cudaGetLastError();
 }
 
 // double double: 64 x 32 CTA tile, 8 warps (4 x 2), 16 x 16 warp tile.  quad double: 32 x 16 CTA tile, 8 x 8 warp tile
 // (16 orders x 2 registers per 8x8 tile).
-template <int Q> using PCfgDD = PCfg<Q, 2, 4, 2, 2, 2>;
+template <int Q, int S = Q> using PCfgDD = PCfg<Q, 2, 4, 2, 2, 2, S>;
 // double double on 32 x 16 CTA tiles (8 x 8 warp tiles): four times the tiles, for problems whose 64 x 32 tiles would not
 // fill the SMs -- every tile would be cut along k and each CTA would flush a whole tile of partial sums through L2
 template <int Q> using PCfgDDS = PCfg<Q, 2, 4, 2, 1, 1>;
-template <int Q> using PCfgQD = PCfg<Q, 4, 4, 2, 1, 1>;
+template <int Q, int S = Q> using PCfgQD = PCfg<Q, 4, 4, 2, 1, 1, S>;
 // quad double in 11 / 12 wide slices (MD_OPT_SLICE_BITS): 22 / 24 accumulator registers per 8x8 tile leave room for the
 // double-double warp tile (16 x 16), which halves the LDS and L2 traffic per DMMA and doubles the DMMAs per slab
 template <int Q> using PCfgQDW = PCfg<Q, 4, 4, 2, 2, 2>;
@@ -468,49 +479,58 @@ template <int Q> using PCfgQDC = PCfg<Q, 4, 4, 2, 2, 1>;
 
 }  // namespace
 
-// CTAs of the persistent grid: one per SM, at most SK_MAX_TILES (the scratch holds one tile per stream-K tile, < grid)
+// CTAs of the persistent grid: one per SM of the current device, at most SK_MAX_TILES (the scratch holds one tile per stream-K
+// tile, < grid)
 int sk_grid() {
-  static int sms = 0;
-  if (sms == 0) {
-    int dev = 0, v = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
-      return -1;
-    sms = v;
-  }
+  const int sms = sm_count();
+  if (sms <= 0) return -1;
   return sms < SK_MAX_TILES ? sms : SK_MAX_TILES;
 }
 
 // chunk > 0 (chunked accumulation): one slot per (stream-K tile, chunk) as long as that stays below SK_CHUNK_CAP_BYTES
-size_t sk_workspace_bytes(int limbs, int quarters, int k, int chunk) {
-  const size_t tile = sizeof(double) * (size_t)quarters * pack_bx(limbs, quarters, 0) * pack_bx(limbs, quarters, 1);
+size_t sk_workspace_bytes(int orders, int bxA, int bxB, int k, int chunk) {
+  const size_t tile = sizeof(double) * (size_t)orders * bxA * bxB;
   size_t slots = SK_MAX_TILES;
   if (chunk > 0) {
     const size_t nchunks = ((size_t)k + chunk - 1) / chunk;
-    if (sk_chunk_scratch_fits(nchunks, quarters, pack_bx(limbs, quarters, 0), pack_bx(limbs, quarters, 1))) slots *= nchunks;
+    if (sk_chunk_scratch_fits(nchunks, orders, bxA, bxB)) slots *= nchunks;
   }
   return SK_COUNTER_BYTES + tile * slots;
 }
 
-bool qgemm_small_supported(int limbs, int quarters) { return limbs == 2 && (quarters == 8 || quarters == 6); }
+bool qgemm_small_supported(int limbs, int quarters, int orders) { return limbs == 2 && orders == quarters && (quarters == 8 || quarters == 6); }
 
 bool qgemm_chunk_supported(int limbs, int quarters) {
   return (limbs == 2 && (quarters == 5 || quarters == 6 || quarters == 8)) || (limbs == 4 && quarters == 10);
 }
 
-cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, int chunk, bool small, const double* Ap,
+// tuned instances: orders == quarters for the counts of qgemm_supported, plus the extended order sets the cfg3-like cases use
+// (S = Q + 1, Q + 2 at the paper's quarter counts); everything else runs on the generic kernel (qgemm_wide.cu)
+bool qgemm_packed_supported(int limbs, int quarters, int orders) {
+  if (orders == quarters) return qgemm_supported(limbs, quarters);
+  return (limbs == 2 && quarters == 8 && (orders == 9 || orders == 10)) || (limbs == 4 && quarters == 16 && (orders == 17 || orders == 18));
+}
+
+cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, int orders, int chunk, bool small, const double* Ap,
                                 const double* Bp, double* order_planes, double* C_planes, void* sk_ws, cudaStream_t stream,
                                 uint64_t* launches) {
   cudaError_t err = cudaErrorInvalidValue;
-#define MD_Q(CFG) err = launch_cfg<CFG>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream)
+#define MD_Q(...) err = launch_cfg<__VA_ARGS__>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream)
   if (small) {
-    if (chunk > 0 || !qgemm_small_supported(limbs, quarters)) return cudaErrorInvalidValue;
+    if (chunk > 0 || !qgemm_small_supported(limbs, quarters, orders)) return cudaErrorInvalidValue;
     if (quarters == 8) MD_Q(PCfgDDS<8>);
     if (quarters == 6) MD_Q(PCfgDDS<6>);
   } else if (chunk > 0) {  // only the instances of qgemm_chunk_supported are compiled with the chunked kernel
+    if (orders != quarters) return cudaErrorInvalidValue;
     if (limbs == 2 && quarters == 5) err = launch_chunked<PCfgDD<5>>(m, n, k, chunk, Ap, Bp, C_planes, sk_ws, stream);
     if (limbs == 2 && quarters == 6) err = launch_chunked<PCfgDD<6>>(m, n, k, chunk, Ap, Bp, C_planes, sk_ws, stream);
     if (limbs == 2 && quarters == 8) err = launch_chunked<PCfgDD<8>>(m, n, k, chunk, Ap, Bp, C_planes, sk_ws, stream);
     if (limbs == 4 && quarters == 10) err = launch_chunked<PCfgQDC<10>>(m, n, k, chunk, Ap, Bp, C_planes, sk_ws, stream);
+  } else if (orders != quarters) {
+    if (limbs == 2 && quarters == 8 && orders == 9) MD_Q(PCfgDD<8, 9>);
+    if (limbs == 2 && quarters == 8 && orders == 10) MD_Q(PCfgDD<8, 10>);
+    if (limbs == 4 && quarters == 16 && orders == 17) MD_Q(PCfgQD<16, 17>);
+    if (limbs == 4 && quarters == 16 && orders == 18) MD_Q(PCfgQD<16, 18>);
   } else if (limbs == 2) {
     if (quarters == 6) MD_Q(PCfgDD<6>);
     if (quarters == 7) MD_Q(PCfgDD<7>);

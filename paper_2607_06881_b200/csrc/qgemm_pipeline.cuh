@@ -58,9 +58,11 @@ struct SkPlan {
   int sk_iters_per_cta;  // ipc
   int dp_tail;           // CTAs 0 .. dp_tail-1 own a tile in the LAST of the dp_waves (all G of them unless chunked, below)
   int flush_slabs;       // chunked accumulation (qgemm_packed.cu, R16): slabs between two flushes; 0 = never
+  int group_m;           // tile rows per raster group (raster_tile; MD_OPT_RASTER_GROUP, default 8)
 };
 
 // Plan for `tiles` output tiles of KS slabs each on a grid of G persistent CTAs.
+int raster_group();  // api.cu: MD_OPT_RASTER_GROUP (default 8)
 inline SkPlan make_sk_plan(int tiles_m, int tiles_n, int KS, int G) {
   const long long tiles = (long long)tiles_m * tiles_n;
   SkPlan plan;
@@ -72,6 +74,7 @@ inline SkPlan make_sk_plan(int tiles_m, int tiles_n, int KS, int G) {
   plan.sk_iters_per_cta = (int)(((long long)plan.sk_tiles * KS + G - 1) / G);
   plan.dp_tail = G;
   plan.flush_slabs = 0;
+  plan.group_m = raster_group();
   return plan;
 }
 

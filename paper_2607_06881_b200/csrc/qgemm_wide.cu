@@ -18,6 +18,13 @@
 //     renorm_add (md_common.cuh) goes from the warp with the smallest orders to the warp with the largest through a
 //     lane-private slot of shared memory, which performs exactly the operation sequence of the standalone md_renorm.
 //
+// GENERIC instances (WCfg<..., GENERIC = true>): the same kernel with the quarter count Q and the order count S as RUNTIME
+// values below compile-time maxima (double double Q <= 16, quad 24, octo 40, hexa 72; S <= Q + 2, so the pruned and
+// extended order sets of MD_OPT_ORDERS run here too).  Every DMMA site of the maximal triangular set stays in the code
+// behind a warp-uniform predicate; the order ranges are those of the maximal set, so a smaller problem leaves the upper
+// ranges short of work.  Slower than a tuned instance (one 8x8 tile per warp, predicates, k-slab depth 4), but every
+// (limbs, quarters, orders) that md_plan_quarters can ask for has a kernel (R5, R15).
+//
 // Exactness as in qgemm_packed.cu: k * S <= 2^27 keeps every partial sum an integer below 2^53 units (PAPER.md:95-99
 // eq. 5; R6), so the result does not depend on the order in which warps, slabs or the hardware add things.
 #include "md_kernels.h"
@@ -28,13 +35,16 @@
 namespace md {
 namespace {
 
-// TM x TN 8x8 tiles per CTA, R order ranges per tile: TM * TN * R = 8 warps.
-template <int Q_, int L_, int TM_, int TN_, int R_>
+// TM x TN 8x8 tiles per CTA, R order ranges per tile: TM * TN * R = 8 warps.  Q_, S_: the quarter / order counts of a tuned
+// instance, or their MAXIMA for a GENERIC one (runtime counts in WideCtx).
+template <int Q_, int L_, int TM_, int TN_, int R_, int S_ = Q_, bool GENERIC_ = false>
 struct WCfg {
-  static constexpr int Q = Q_, S = Q_, L = L_, TM = TM_, TN = TN_, R = R_;
+  static constexpr int Q = Q_, S = S_, L = L_, TM = TM_, TN = TN_, R = R_;
+  static constexpr bool GENERIC = GENERIC_;
   static constexpr int BM = TM * 8, BN = TN * 8, BK = PACK_BK_WIDE;
   static constexpr int TILES = TM * TN, WARPS = TILES * R, THREADS = WARPS * 32;
-  static constexpr int A_CHUNK = Q * BK * BM, B_CHUNK = Q * BK * BN;  // doubles per k-slab
+  static constexpr int A_CHUNK = Q * BK * BM, B_CHUNK = Q * BK * BN;  // doubles per k-slab (GENERIC: at most)
+  static constexpr int AQ = BK * BM, BQ = BK * BN;                    // doubles per quarter inside a chunk
   static constexpr int STAGE_BYTES = (A_CHUNK + B_CHUNK) * 8;
   static constexpr int BAR_BYTES = 128;
   // hand-over slots of the recombination chain: per tile, per lane, two elements of L+1 terms
@@ -44,14 +54,19 @@ struct WCfg {
   static constexpr int AHEAD = STAGES - 2;
   static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + XCHG_BYTES;
   static_assert(WARPS == 8, "8 warps per CTA (2 per SM sub-partition)");
-  static_assert(R == 1 || (R == 4 && Q == 64) || (R == 2 && Q == 44), "order ranges: 1 (octo double), 4 / 2 (hexa double)");
+  static_assert(R == 1 || (R == 4 && (Q == 64 || Q == 72)) || (R == 2 && (Q == 44 || Q == 40)), "order ranges with a boundary table");
   static_assert(STAGES >= 3, "the non-blocking refill needs at least 3 stages");
   static_assert(2 * STAGES * 8 <= BAR_BYTES - 8, "barrier area (its last 8 bytes hold the stream-K flag)");
   static_assert(STAGE_BYTES % 128 == 0 && XCHG_BYTES % 128 == 0, "alignment");
-  // order range r = [lo(r), hi(r)): boundaries that balance the product counts sum_{s in range} (s + 1) --
-  //   Q = 64, R = 4: 0 | 32 | 45 | 55 | 64 -> 528 / 507 / 505 / 540;   Q = 44, R = 2: 0 | 31 | 44 -> 496 / 494
+  // order range r = [lo(r), hi(r)): boundaries that balance the product counts sum_{s in range} #{(p, q): p + q = s} --
+  //   Q = 64, R = 4: 0 | 32 | 45 | 55 | 64 -> 528 / 507 / 505 / 540;   Q = 44, R = 2: 0 | 31 | 44 -> 496 / 494;
+  //   generic hexa double (Q <= 72, S <= 74), R = 4: 0 | 34 | 50 | 63 | 74 -> 595 / 680 / 741 / 753 (the first range is kept
+  //   at 34 orders: 37 would balance better but spills);  generic octo double (Q <= 40, S <= 42), R = 2: 0 | 30 | 42 -> 465 / 432
   __host__ __device__ static constexpr int bound(int r) {
-    return R == 1 ? (r == 0 ? 0 : S) : R == 2 ? (r == 0 ? 0 : r == 1 ? 31 : 44) : (r == 0 ? 0 : r == 1 ? 32 : r == 2 ? 45 : r == 3 ? 55 : 64);
+    return R == 1   ? (r == 0 ? 0 : S)
+           : R == 2 ? (Q == 40 ? (r == 0 ? 0 : r == 1 ? 30 : 42) : (r == 0 ? 0 : r == 1 ? 31 : 44))
+           : Q == 72 ? (r == 0 ? 0 : r == 1 ? 34 : r == 2 ? 50 : r == 3 ? 63 : 74)
+                     : (r == 0 ? 0 : r == 1 ? 32 : r == 2 ? 45 : r == 3 ? 55 : 64);
   }
   __host__ __device__ static constexpr int lo(int r) { return bound(r); }
   __host__ __device__ static constexpr int hi(int r) { return bound(r + 1); }
@@ -67,6 +82,8 @@ struct WCfg {
 // What a warp needs to know about the CTA's pipeline and work list (built once in the kernel).
 struct WideCtx {
   int m, n, G, cta, KS;
+  int Q, S;              // quarter / order counts of this launch (GENERIC instances; the tuned ones use C::Q, C::S)
+  int a_chunk, b_chunk;  // doubles of A / B per k-slab = Q * BK * BM, Q * BK * BN
   SkPlan plan;
   int g0, g1, n_sk, n_seg, total_slabs;  // this CTA's segment list (see qgemm_pipeline.cuh)
   const double *Ap, *Bp;
@@ -119,6 +136,38 @@ __device__ __forceinline__ void k_step_range(double (&acc)[S1 - S0][2], const do
   }
 }
 
+// The same for a GENERIC instance: QMAX, [S0, S1) are the compile-time maxima, Qr <= QMAX and Sr the counts of this launch
+// (warp-uniform).  Every site of the maximal set is predicated; for a given q the live products are a prefix
+// p = lo .. min(hi, Qr - 1, Sr - 1 - q) of the compile-time range.
+template <int QMAX, int S0, int S1, int AQ, int BQ>
+__device__ __forceinline__ void k_step_range_rt(double (&acc)[S1 - S0][2], const double* __restrict__ As,
+                                                const double* __restrict__ Bs, int Qr, int Sr) {
+  constexpr int W = S1 - S0;
+  constexpr int RW = S0 == 0 ? W : W + 1;
+  constexpr int QTOP = S1 - 1 < QMAX - 1 ? S1 - 1 : QMAX - 1;
+  if (S0 >= Sr) return;  // nothing of this range is kept
+  double a[RW];
+#pragma unroll
+  for (int p = S0; p <= QTOP; p++) a[p % RW] = p < Qr ? As[p * AQ] : 0.0;
+  double b = Bs[0];
+#pragma unroll
+  for (int q = 0; q <= QTOP; q++) {
+    if (q >= Qr) break;
+    double b_next = 0.0;
+    if (q + 1 <= QTOP && q + 1 < Qr) {
+      b_next = Bs[(q + 1) * BQ];
+      if (S0 - (q + 1) >= 0 && S0 - (q + 1) < Qr) a[(S0 - (q + 1)) % RW] = As[(S0 - (q + 1)) * AQ];
+    }
+    const int lo = S0 - q > 0 ? S0 - q : 0;
+    const int hi = S1 - 1 - q < QMAX - 1 ? S1 - 1 - q : QMAX - 1;
+    const int pmax = min(Qr - 1, Sr - 1 - q);
+#pragma unroll
+    for (int p = lo; p <= hi; p++)
+      if (p <= pmax) dmma_8x8x4(acc[p + q - S0], a[p % RW], b);
+    b = b_next;
+  }
+}
+
 // Producer cursor (thread 0 only): walks the CTA's flat slab sequence AHEAD slabs in front of the consumers.
 template <class C>
 struct WideProducer {
@@ -128,17 +177,19 @@ struct WideProducer {
     if (p_left == 0) {
       int tile, s0, s1, tm, tn;
       x.segment(++p_seg, tile, s0, s1);
-      raster_tile(tile, x.plan.tiles_m, x.plan.tiles_n, tm, tn);
-      p_A = x.Ap + ((size_t)tm * x.KS + s0) * C::A_CHUNK;
-      p_B = x.Bp + ((size_t)tn * x.KS + s0) * C::B_CHUNK;
+      raster_tile(tile, x.plan.tiles_m, x.plan.tiles_n, tm, tn, x.plan.group_m);
+      p_A = x.Ap + ((size_t)tm * x.KS + s0) * (C::GENERIC ? x.a_chunk : C::A_CHUNK);
+      p_B = x.Bp + ((size_t)tn * x.KS + s0) * (C::GENERIC ? x.b_chunk : C::B_CHUNK);
       p_left = s1 - s0;
     }
+    // GENERIC: a stage keeps its compile-time size and the B part its compile-time offset; only Q quarters of each arrive
+    const int a_chunk = C::GENERIC ? x.a_chunk : C::A_CHUNK, b_chunk = C::GENERIC ? x.b_chunk : C::B_CHUNK;
     const uint32_t dst = x.stages_u32 + pst * C::STAGE_BYTES, bar = x.full_u32 + 8 * pst;
-    mbar_expect_tx(bar, C::STAGE_BYTES);
-    bulk_g2s(dst, p_A, C::A_CHUNK * 8, bar);
-    bulk_g2s(dst + C::A_CHUNK * 8, p_B, C::B_CHUNK * 8, bar);
-    p_A += C::A_CHUNK;
-    p_B += C::B_CHUNK;
+    mbar_expect_tx(bar, (a_chunk + b_chunk) * 8);
+    bulk_g2s(dst, p_A, a_chunk * 8, bar);
+    bulk_g2s(dst + C::A_CHUNK * 8, p_B, b_chunk * 8, bar);
+    p_A += a_chunk;
+    p_B += b_chunk;
     p_left--;
     p_flat++;
     pst = (pst + 1 == C::STAGES) ? 0 : pst + 1;
@@ -168,9 +219,11 @@ __device__ __forceinline__ void wide_epilogue(const WideCtx& x, const double (&a
   const bool inside = row < x.m && col < x.n, two = col + 1 < x.n;
   const size_t planeC = (size_t)x.m * x.n, at = (size_t)row * x.n + col;
   const bool vec_ok = (x.n % 2 == 0) && (((uintptr_t)x.C_planes | (uintptr_t)x.order_planes) % 16 == 0);
+  const int Sr = C::GENERIC ? x.S : C::S;  // orders kept by this launch
   if (x.order_planes && inside) {
 #pragma unroll
     for (int s = S0; s < S1; s++) {
+      if (C::GENERIC && s >= Sr) break;
       if (vec_ok) {
         *reinterpret_cast<double2*>(x.order_planes + s * planeC + at) = make_double2(acc[s - S0][0], acc[s - S0][1]);
       } else {
@@ -193,7 +246,8 @@ __device__ __forceinline__ void wide_epilogue(const WideCtx& x, const double (&a
 #pragma unroll
         for (int l = 0; l <= L; l++) r[l] = (RANGE == R - 1) ? 0.0 : slot[l * 32];
 #pragma unroll
-        for (int s = S1 - 1; s >= S0; s--) renorm_add<L>(r, acc[s - S0][e]);
+        for (int s = S1 - 1; s >= S0; s--)
+          if (!C::GENERIC || s < Sr) renorm_add<L>(r, acc[s - S0][e]);
         if (RANGE > 0) {
 #pragma unroll
           for (int l = 0; l <= L; l++) slot[l * 32] = r[l];
@@ -244,7 +298,8 @@ __device__ __forceinline__ void wide_consume(const WideCtx& x, int t, int lane, 
     if (tid == 0) prod.produce(x);
     mbar_wait(x.full_u32 + 8 * st, phase);
     const double* stage = x.stages + (size_t)st * STAGE_DOUBLES;
-    k_step_range<C::Q, S0, S1, C::TM * 32, C::TN * 32>(acc, stage + a_off, stage + b_off);
+    if constexpr (C::GENERIC) k_step_range_rt<C::Q, S0, S1, C::AQ, C::BQ>(acc, stage + a_off, stage + b_off, x.Q, x.S);
+    else k_step_range<C::Q, S0, S1, C::AQ, C::BQ>(acc, stage + a_off, stage + b_off);
     __syncwarp();
     if (lane == 0) mbar_arrive(x.empty_u32 + 8 * st);  // this warp is done reading the stage
     if (++st == STAGES) {
@@ -253,15 +308,17 @@ __device__ __forceinline__ void wide_consume(const WideCtx& x, int t, int lane, 
     }
     if (--c_left == 0) {
       int tm, tn;
-      raster_tile(c_tile, x.plan.tiles_m, x.plan.tiles_n, tm, tn);
+      raster_tile(c_tile, x.plan.tiles_m, x.plan.tiles_n, tm, tn, x.plan.group_m);
       const int row_base = tm * C::BM + ti * 8, col_base = tn * C::BN + tj * 8;
       if (c_s1 - c_s0 == x.KS) {  // whole tile in registers
         wide_epilogue<C, RANGE>(x, acc, t, row_base, col_base, lane);
       } else {                    // partial sums of a stream-K tile
         const int r = c_tile - x.plan.dp_waves * x.G;
-        double* sc = x.sk_scratch + (size_t)r * (C::S * C::BM * C::BN) + (size_t)t * 64 + lane * 2;
+        const int Sr = C::GENERIC ? x.S : C::S;
+        double* sc = x.sk_scratch + (size_t)r * (Sr * C::BM * C::BN) + (size_t)t * 64 + lane * 2;
 #pragma unroll
         for (int s = S0; s < S1; s++) {
+          if (C::GENERIC && s >= Sr) break;
           atomicAdd(sc + (size_t)s * (C::TILES * 64), acc[s - S0][0]);
           atomicAdd(sc + (size_t)s * (C::TILES * 64) + 1, acc[s - S0][1]);
         }
@@ -276,6 +333,7 @@ __device__ __forceinline__ void wide_consume(const WideCtx& x, int t, int lane, 
           __threadfence();
 #pragma unroll
           for (int s = S0; s < S1; s++) {
+            if (C::GENERIC && s >= Sr) break;
             const double2 v = __ldcg(reinterpret_cast<const double2*>(sc + (size_t)s * (C::TILES * 64)));
             acc[s - S0][0] = v.x;
             acc[s - S0][1] = v.y;
@@ -295,7 +353,7 @@ __device__ __forceinline__ void wide_consume(const WideCtx& x, int t, int lane, 
 
 template <class C>
 __global__ void __launch_bounds__(C::THREADS, 1)
-qgemm_wide_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, const double* __restrict__ Bp,
+qgemm_wide_kernel(int m, int n, int Qr, int Sr, SkPlan plan, const double* __restrict__ Ap, const double* __restrict__ Bp,
                   double* __restrict__ order_planes, double* __restrict__ C_planes, double* __restrict__ sk_scratch,
                   unsigned int* __restrict__ sk_counters) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -304,6 +362,8 @@ qgemm_wide_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, cons
 
   WideCtx x;
   x.m = m, x.n = n, x.G = gridDim.x, x.cta = blockIdx.x, x.KS = plan.KS, x.plan = plan;
+  x.Q = C::GENERIC ? Qr : C::Q, x.S = C::GENERIC ? Sr : C::S;
+  x.a_chunk = x.Q * C::AQ, x.b_chunk = x.Q * C::BQ;
   x.Ap = Ap, x.Bp = Bp, x.order_planes = order_planes, x.C_planes = C_planes;
   x.sk_scratch = sk_scratch, x.sk_counters = sk_counters;
   x.stages = reinterpret_cast<double*>(smem_raw);
@@ -352,10 +412,13 @@ qgemm_wide_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, cons
 }
 
 template <class C>
-cudaError_t launch_wide_cfg(int m, int n, int k, const double* Ap, const double* Bp, double* order_planes,
+cudaError_t launch_wide_cfg(int m, int n, int k, int Q, int S, const double* Ap, const double* Bp, double* order_planes,
                             double* C_planes, void* sk_ws, cudaStream_t stream) {
-  static_assert(C::BM == pack_bx(C::L, C::Q, 0) && C::BN == pack_bx(C::L, C::Q, 1) && C::BK == pack_bk(C::L),
+  static_assert(C::GENERIC || (C::BM == pack_bx(C::L, C::Q, 0) && C::BN == pack_bx(C::L, C::Q, 1) && C::BK == pack_bk(C::L)),
                 "tile shape must match the packed layout");
+  static_assert(!C::GENERIC || (C::BM == pack_bx_generic(C::L, 0) && C::BN == pack_bx_generic(C::L, 1)),
+                "tile shape must match the packed layout of the generic instances");
+  if (C::GENERIC ? (Q < 1 || Q > C::Q || S < 1 || S > C::S || S > 2 * Q - 1) : (Q != C::Q || S != C::S)) return cudaErrorInvalidValue;
   const int tiles_m = (m + C::BM - 1) / C::BM, tiles_n = (n + C::BN - 1) / C::BN;
   if ((long long)tiles_m * tiles_n > 0x7fffffffLL) return cudaErrorInvalidValue;
   const int G = sk_grid();
@@ -365,13 +428,18 @@ cudaError_t launch_wide_cfg(int m, int n, int k, const double* Ap, const double*
   double* scratch = reinterpret_cast<double*>(static_cast<char*>(sk_ws) + SK_COUNTER_BYTES);
   cudaError_t err;
   if (plan.sk_tiles > 0) {  // counters and the scratch tiles in use start at zero (one contiguous region)
-    err = cudaMemsetAsync(sk_ws, 0, SK_COUNTER_BYTES + sizeof(double) * (size_t)plan.sk_tiles * C::S * C::BM * C::BN, stream);
+    err = cudaMemsetAsync(sk_ws, 0, SK_COUNTER_BYTES + sizeof(double) * (size_t)plan.sk_tiles * S * C::BM * C::BN, stream);
     if (err != cudaSuccess) return err;
   }
   auto kern = qgemm_wide_kernel<C>;
-  err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
-  if (err != cudaSuccess) return err;
-  kern<<<G, C::THREADS, C::SMEM_BYTES, stream>>>(m, n, plan, Ap, Bp, order_planes, C_planes, scratch, counters);
+  static bool attr_done[MD_MAX_DEVICES] = {};  // the shared-memory opt-in is per function and device: once, not per launch
+  const int dev = current_device();
+  if (dev < 0 || dev >= MD_MAX_DEVICES || !attr_done[dev]) {
+    err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+    if (err != cudaSuccess) return err;
+    if (dev >= 0 && dev < MD_MAX_DEVICES) attr_done[dev] = true;
+  }
+  kern<<<G, C::THREADS, C::SMEM_BYTES, stream>>>(m, n, Q, S, plan, Ap, Bp, order_planes, C_planes, scratch, counters);
   return cudaGetLastError();
 }
 
@@ -379,6 +447,11 @@ using WCfgOD = WCfg<32, 8, 4, 2, 1>;   // octo double: 32 x 16 CTA tile, 8 tiles
 using WCfgOD22 = WCfg<22, 8, 4, 2, 1>; // octo double in 22 slices of 19 bits (MD_OPT_SLICE_BITS; R14)
 using WCfgHD = WCfg<64, 16, 2, 1, 4>;  // hexa double: 16 x 8 CTA tile, 2 tiles x 4 ranges
 using WCfgHD44 = WCfg<44, 16, 2, 2, 2>;  // hexa double in 44 slices of 19 bits: 16 x 16 CTA tile, 4 tiles x 2 ranges
+// GENERIC instances: runtime (Q, S) up to these maxima
+using WCfgGenDD = WCfg<GENERIC_QMAX_DD, 2, 4, 2, 1, GENERIC_QMAX_DD + 2, true>;
+using WCfgGenQD = WCfg<GENERIC_QMAX_QD, 4, 4, 2, 1, GENERIC_QMAX_QD + 2, true>;
+using WCfgGenOD = WCfg<GENERIC_QMAX_OD, 8, 2, 2, 2, GENERIC_QMAX_OD + 2, true>;
+using WCfgGenHD = WCfg<GENERIC_QMAX_HD, 16, 2, 1, 4, GENERIC_QMAX_HD + 2, true>;
 
 }  // namespace
 
@@ -386,14 +459,35 @@ bool qgemm_wide_supported(int limbs, int quarters) {
   return (limbs == 8 && (quarters == 32 || quarters == 22)) || (limbs == 16 && (quarters == 64 || quarters == 44));
 }
 
+int qgemm_generic_max_quarters(int limbs) {
+  return limbs == 2 ? GENERIC_QMAX_DD : limbs == 4 ? GENERIC_QMAX_QD : limbs == 8 ? GENERIC_QMAX_OD : limbs == 16 ? GENERIC_QMAX_HD : 0;
+}
+bool qgemm_generic_supported(int limbs, int quarters, int orders) {
+  const int qmax = qgemm_generic_max_quarters(limbs);
+  return qmax > 0 && quarters >= 1 && quarters <= qmax && orders >= 1 && orders <= quarters + 2 && orders <= 2 * quarters - 1;
+}
+
 cudaError_t launch_qgemm_wide(int m, int n, int k, int limbs, int quarters, const double* Ap, const double* Bp,
                               double* order_planes, double* C_planes, void* sk_ws, cudaStream_t stream,
                               uint64_t* launches) {
   cudaError_t err = cudaErrorInvalidValue;
-  if (limbs == 8 && quarters == 32) err = launch_wide_cfg<WCfgOD>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
-  if (limbs == 8 && quarters == 22) err = launch_wide_cfg<WCfgOD22>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
-  if (limbs == 16 && quarters == 44) err = launch_wide_cfg<WCfgHD44>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
-  if (limbs == 16 && quarters == 64) err = launch_wide_cfg<WCfgHD>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
+  const int Q = quarters;
+  if (limbs == 8 && quarters == 32) err = launch_wide_cfg<WCfgOD>(m, n, k, Q, Q, Ap, Bp, order_planes, C_planes, sk_ws, stream);
+  if (limbs == 8 && quarters == 22) err = launch_wide_cfg<WCfgOD22>(m, n, k, Q, Q, Ap, Bp, order_planes, C_planes, sk_ws, stream);
+  if (limbs == 16 && quarters == 44) err = launch_wide_cfg<WCfgHD44>(m, n, k, Q, Q, Ap, Bp, order_planes, C_planes, sk_ws, stream);
+  if (limbs == 16 && quarters == 64) err = launch_wide_cfg<WCfgHD>(m, n, k, Q, Q, Ap, Bp, order_planes, C_planes, sk_ws, stream);
+  if (err == cudaSuccess) *launches += 1;
+  return err;
+}
+
+cudaError_t launch_qgemm_generic(int m, int n, int k, int limbs, int quarters, int orders, const double* Ap, const double* Bp,
+                                 double* order_planes, double* C_planes, void* sk_ws, cudaStream_t stream, uint64_t* launches) {
+  cudaError_t err = cudaErrorInvalidValue;
+  if (!qgemm_generic_supported(limbs, quarters, orders)) return err;
+  if (limbs == 2) err = launch_wide_cfg<WCfgGenDD>(m, n, k, quarters, orders, Ap, Bp, order_planes, C_planes, sk_ws, stream);
+  if (limbs == 4) err = launch_wide_cfg<WCfgGenQD>(m, n, k, quarters, orders, Ap, Bp, order_planes, C_planes, sk_ws, stream);
+  if (limbs == 8) err = launch_wide_cfg<WCfgGenOD>(m, n, k, quarters, orders, Ap, Bp, order_planes, C_planes, sk_ws, stream);
+  if (limbs == 16) err = launch_wide_cfg<WCfgGenHD>(m, n, k, quarters, orders, Ap, Bp, order_planes, C_planes, sk_ws, stream);
   if (err == cudaSuccess) *launches += 1;
   return err;
 }

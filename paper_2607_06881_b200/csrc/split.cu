@@ -70,8 +70,10 @@ __global__ void col_exponent_finalize_kernel(int cols, int32_t* exps, uint32_t* 
 template <int L>
 __device__ __forceinline__ double extract_digit(double (&r)[L], int E, int q, int bits) {
   // c = 1.5 * 2^(E - W(q+1) + 52): exponent field + the top mantissa bit
-  const long long cbits = ((long long)(E - bits * (q + 1) + 52 + 1023) << 52) | (1ll << 51);
-  const double c = __longlong_as_double(cbits);
+  // (a group exponent below the documented floor would make the field non-positive: clamped, the digit is then garbage
+  // but finite and the violation is flagged by the exponent kernel)
+  const long long field = max(E - bits * (q + 1) + 52 + 1023, 1);
+  const double c = __longlong_as_double((field << 52) | (1ll << 51));
   const double t = __dadd_rn(r[0], c);
   const double d = __dsub_rn(t, c);
   r[0] = __dsub_rn(r[0], d);
@@ -207,6 +209,31 @@ __global__ void __launch_bounds__(256) split_packed_kernel(int rows, int cols, i
   split_fragment_row<L, AXIS>(rows, cols, Q, bits, bx, bk, KS, x, k4g * 4, x < X ? exps[x] : 0, planes, packed, flags);
 }
 
+// md_qgemm's repacking (quarter / order counts without a plain-layout kernel): plain [Q][rows][cols] quarter planes -> the packed
+// layout, zero padded.  Same thread mapping as split_packed_kernel; no arithmetic.
+template <int AXIS>
+__global__ void __launch_bounds__(256) pack_planes_kernel(int rows, int cols, int Q, int bx, int bk, int x_blocks, int KS,
+                                                          const double* __restrict__ planes, double* __restrict__ packed) {
+  const int X = AXIS == 0 ? rows : cols, K = AXIS == 0 ? cols : rows;
+  const int x = (blockIdx.x % x_blocks) * 32 + (threadIdx.x & 31);
+  const int k4g = (blockIdx.x / x_blocks) * 8 + (threadIdx.x >> 5);
+  const int XP = (X + bx - 1) / bx * bx;
+  if (k4g >= KS * (bk / 4) || x >= XP) return;
+  const int k0 = k4g * 4;
+  const size_t plane = (size_t)rows * cols;
+  double* dst = packed + packed_offset(x, k0, 0, bx, bk, Q, KS);
+  const size_t q_stride = (size_t)(bk / 4) * (bx / 8) * 32;
+  for (int q = 0; q < Q; q++) {
+    double d[4];
+#pragma unroll
+    for (int t = 0; t < 4; t++) {
+      const bool ok = x < X && k0 + t < K;
+      d[t] = !ok ? 0.0 : AXIS == 0 ? planes[q * plane + (size_t)x * cols + k0 + t] : planes[q * plane + (size_t)(k0 + t) * cols + x];
+    }
+    stg_256(dst + q * q_stride, d[0], d[1], d[2], d[3]);
+  }
+}
+
 // md_gemm's fused preparation: exponent vectors AND packed quarter planes of BOTH operands in ONE cooperative launch (the
 // dependent launches of the separate kernels -- row maxima, column maxima, finalize, two splits, a memset -- cost a few
 // microseconds each, which is a third of a 64^3 product and 2.5 % of a 1024^3 one).  Persistent blocks, three phases
@@ -277,14 +304,18 @@ __global__ void __launch_bounds__(256) prep_coop_kernel(int m, int n, int k, int
 // double when both groups sit at the bound; -EXP_LIMIT for the paper's dd / qd quarter counts.
 int exponent_floor(int quarters, int bits) {
   const int lo = -(1022 - bits * (quarters + 1)) / 2;
-  return bits * quarters <= 13 * 24 || lo < -EXP_LIMIT ? -EXP_LIMIT : lo;
+  const int pair = bits * quarters <= 13 * 24 || lo < -EXP_LIMIT ? -EXP_LIMIT : lo;
+  // and every digit unit 2^(E - W (q+1)), q < quarters, must itself be a normal double (the splitter's constant c needs it)
+  const int own = bits * quarters - 1022;
+  return pair > own ? pair : own;
 }
 
 cudaError_t launch_exponents(int rows, int cols, int axis, int quarters, int bits, const double* lead, int32_t* exps,
                              uint32_t* flags, cudaStream_t stream, uint64_t* launches) {
   const int exp_lo = exponent_floor(quarters, bits);
   if (axis == 0) {
-    row_exponent_kernel<<<min(rows, 148 * 64), 256, 0, stream>>>(rows, cols, lead, exps, flags, exp_lo);
+    const int sms = max(sm_count(), 1);
+    row_exponent_kernel<<<min(rows, sms * 64), 256, 0, stream>>>(rows, cols, lead, exps, flags, exp_lo);
     *launches += 1;
     return cudaGetLastError();
   }
@@ -292,7 +323,7 @@ cudaError_t launch_exponents(int rows, int cols, int axis, int quarters, int bit
   if (err != cudaSuccess) return err;
   const int col_blocks = (cols + 255) / 256;
   // enough row chunks to fill the machine, at least 16 rows each
-  int chunks = max(1, min((rows + 15) / 16, (148 * 8 + col_blocks - 1) / col_blocks));
+  int chunks = max(1, min((rows + 15) / 16, (max(sm_count(), 1) * 8 + col_blocks - 1) / col_blocks));
   chunks = min(chunks, 65535);
   const int rows_per_block = (rows + chunks - 1) / chunks;
   chunks = (rows + rows_per_block - 1) / rows_per_block;
@@ -326,10 +357,9 @@ cudaError_t launch_split(int rows, int cols, int limbs, int quarters, int bits, 
   return cudaGetLastError();
 }
 
-cudaError_t launch_prep_packed(int m, int n, int k, int limbs, int quarters, int bits, bool small, const double* A,
+cudaError_t launch_prep_packed(int m, int n, int k, int limbs, int quarters, int bits, int bxA, int bxB, int bk, const double* A,
                                const double* B, double* Ap, double* Bp, int32_t* expA, int32_t* expB, uint32_t* flags,
                                cudaStream_t stream, uint64_t* launches) {
-  int bxA = pack_bx(limbs, quarters, 0, small), bxB = pack_bx(limbs, quarters, 1, small), bk = pack_bk(limbs);
   int exp_lo = exponent_floor(quarters, bits);
   uint32_t* rawA = reinterpret_cast<uint32_t*>(expA);
   uint32_t* rawB = reinterpret_cast<uint32_t*>(expB);
@@ -343,12 +373,14 @@ cudaError_t launch_prep_packed(int m, int n, int k, int limbs, int quarters, int
     default: return cudaErrorInvalidValue;
   }
   // persistent grid: as many blocks as can be co-resident (a cooperative launch needs that), at most the work there is
-  static int max_blocks[17] = {};
+  static int max_blocks_dev[MD_MAX_DEVICES][17] = {};  // per device: a process may drive several
+  const int dev = current_device();
+  if (dev < 0 || dev >= MD_MAX_DEVICES) return cudaErrorInvalidDevice;
+  int* max_blocks = max_blocks_dev[dev];
   if (max_blocks[limbs] == 0) {
-    int dev = 0, sms = 0, per_sm = 0;
-    cudaError_t e = cudaGetDevice(&dev);
-    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 256, 0);
+    int per_sm = 0;
+    const int sms = sm_count();
+    cudaError_t e = sms > 0 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 256, 0) : cudaErrorInvalidDevice;
     if (e != cudaSuccess) return e;
     if (per_sm > 4) per_sm = 4;
     max_blocks[limbs] = sms * (per_sm > 0 ? per_sm : 1);
@@ -361,12 +393,23 @@ cudaError_t launch_prep_packed(int m, int n, int k, int limbs, int quarters, int
   return err;
 }
 
-cudaError_t launch_split_packed(int rows, int cols, int limbs, int quarters, int bits, int axis, bool small,
+cudaError_t launch_pack_planes(int rows, int cols, int quarters, int axis, int bx, int bk, const double* planes, double* packed,
+                               cudaStream_t stream, uint64_t* launches) {
+  const int X = axis == 0 ? rows : cols, K = axis == 0 ? cols : rows;
+  const int KS = (K + bk - 1) / bk;
+  const int x_blocks = ((X + bx - 1) / bx * bx + 31) / 32;
+  const long long blocks = (long long)x_blocks * (((long long)KS * (bk / 4) + 7) / 8);
+  if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
+  if (axis == 0) pack_planes_kernel<0><<<(unsigned)blocks, 256, 0, stream>>>(rows, cols, quarters, bx, bk, x_blocks, KS, planes, packed);
+  else pack_planes_kernel<1><<<(unsigned)blocks, 256, 0, stream>>>(rows, cols, quarters, bx, bk, x_blocks, KS, planes, packed);
+  *launches += 1;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_split_packed(int rows, int cols, int limbs, int quarters, int bits, int axis, int bx, int bk,
                                 const double* planes, double* packed, const int32_t* exps, uint32_t* flags,
                                 cudaStream_t stream, uint64_t* launches) {
   const int X = axis == 0 ? rows : cols, K = axis == 0 ? cols : rows;
-  const int bx = pack_bx(limbs, quarters, axis, small);
-  const int bk = pack_bk(limbs);
   const int KS = (K + bk - 1) / bk;
   const int x_blocks = ((X + bx - 1) / bx * bx + 31) / 32;  // 32 groups per block over the padded extent
   const long long k_blocks = ((long long)KS * (bk / 4) + 7) / 8;

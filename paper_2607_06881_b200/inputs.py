@@ -39,15 +39,21 @@ class Config:
     # Slice width in bits: 13 = the paper's quarter.  Other widths are the k-adaptive variant (DESIGN.md
     # R14), again a parameter handed to md_set_option, not part of the input data.
     bits: int = 13
+    # Kept product orders S (MD_OPT_ORDERS; the paper's C_1..C_S).  0 = quarters, the paper's set.
+    orders: int = 0
 
     def __post_init__(self):
         if self.quarters == 0:
             object.__setattr__(self, "quarters", 4 * self.limbs)
+        if self.orders == 0:
+            object.__setattr__(self, "orders", self.quarters)
 
     @property
     def products(self) -> int:
-        """T = number of quarter products in the triangular set, orders s = 0..quarters-1 (eq. 4)."""
-        return self.quarters * (self.quarters + 1) // 2
+        """T = number of quarter products issued: pairs (p, q), p, q < quarters, p + q < orders (PAPER.md:75-78 eq. 4;
+        quarters (quarters + 1) / 2 for the paper's set orders = quarters)."""
+        Q, S = self.quarters, self.orders
+        return sum(min(s + 1, Q, 2 * Q - 1 - s) for s in range(S))
 
     @property
     def fp64_flops(self) -> int:
@@ -59,8 +65,8 @@ class Config:
         """2mnk multiple-double flops (BASELINE.json `metric`)."""
         return 2 * self.m * self.n * self.k
 
-    def with_slices(self, bits: int, quarters: int) -> "Config":
-        return dataclasses.replace(self, bits=bits, quarters=quarters)
+    def with_slices(self, bits: int, quarters: int, orders: int = 0) -> "Config":
+        return dataclasses.replace(self, bits=bits, quarters=quarters, orders=orders or quarters)
 
     def with_shape(self, m=None, n=None, k=None) -> "Config":
         return dataclasses.replace(self, m=m or self.m, n=n or self.n, k=k or self.k)

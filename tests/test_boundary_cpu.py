@@ -58,11 +58,33 @@ def test_argument_errors_need_no_gpu(lib):
     assert lib.md_gemm(1, 1, 2 ** 22 + 1, 8, fake, fake, fake, None) == md.MD_ERR_K_TOO_LARGE
     assert lib.md_gemm(1, 1, 2 ** 21 + 1, 16, fake, fake, fake, None) == md.MD_ERR_K_TOO_LARGE
     assert lib.md_gemm(1, 1, 2 ** 21, 16, fake, fake, fake, None) == md.MD_ERR_WORKSPACE
-    assert lib.md_qgemm(4, 4, 4, 8, 32, 32, fake, fake, fake, fake, None) == md.MD_ERR_UNSUPPORTED
     assert lib.md_renorm(4, 4, 2, 0, fake, fake, None) == md.MD_ERR_BAD_ARG
-    assert lib.md_qgemm(4, 4, 4, 2, 8, 7, fake, fake, fake, fake, None) == md.MD_ERR_UNSUPPORTED
-    assert lib.md_qgemm(4, 4, 4, 2, 12, 12, fake, fake, fake, fake, None) == md.MD_ERR_UNSUPPORTED
+    # md_qgemm: counts without a plain-layout kernel are repacked into the registered workspace and run on the kernel md_gemm
+    # would pick (the generic one if need be); beyond the generic maxima nothing exists
+    assert lib.md_qgemm(4, 4, 4, 8, 32, 32, fake, fake, fake, fake, None) == md.MD_ERR_WORKSPACE
+    assert lib.md_qgemm(4, 4, 4, 2, 8, 7, fake, fake, fake, fake, None) == md.MD_ERR_WORKSPACE
+    assert lib.md_qgemm(4, 4, 4, 2, 12, 12, fake, fake, fake, fake, None) == md.MD_ERR_WORKSPACE
+    assert lib.md_qgemm(4, 4, 4, 2, 17, 17, fake, fake, fake, fake, None) == md.MD_ERR_UNSUPPORTED   # dd: at most 16 quarters
+    assert lib.md_qgemm(4, 4, 4, 2, 8, 11, fake, fake, fake, fake, None) == md.MD_ERR_UNSUPPORTED    # orders <= quarters + 2
+    assert lib.md_qgemm(4, 4, 4, 4, 25, 25, fake, fake, fake, fake, None) == md.MD_ERR_UNSUPPORTED   # qd: at most 24
     assert lib.md_qgemm(4, 4, 4, 2, 8, 8, fake, fake, None, None, None) == md.MD_ERR_BAD_ARG
+    # every quarter count md_plan_quarters may return within the generic maxima has a kernel (R5, R15):
+    # dd 1..16, qd 1..24, od 1..40, hd 1..72, and MD_OPT_ORDERS in [Q - 2, Q + 2]
+    try:
+        for limbs, qmax in ((2, 16), (4, 24), (8, 40), (16, 72)):
+            for Q in range(3, qmax + 1):
+                assert lib.md_set_option(md.MD_OPT_QUARTERS, Q) == md.MD_OK
+                for S in (0, Q - 2, Q - 1, Q + 1, Q + 2):
+                    assert lib.md_set_option(md.MD_OPT_ORDERS, S) == md.MD_OK
+                    assert lib.md_gemm(8, 8, 8, limbs, fake, fake, fake, None) == md.MD_ERR_WORKSPACE, (limbs, Q, S)
+                    assert lib.md_workspace_bytes(8, 8, 8, limbs) > 0
+            assert lib.md_set_option(md.MD_OPT_ORDERS, 0) == md.MD_OK
+            if qmax < 72:  # (72 is also the largest value MD_OPT_QUARTERS takes)
+                assert lib.md_set_option(md.MD_OPT_QUARTERS, qmax + 1) == md.MD_OK
+                assert lib.md_gemm(8, 8, 8, limbs, fake, fake, fake, None) == md.MD_ERR_UNSUPPORTED
+    finally:
+        lib.md_set_option(md.MD_OPT_QUARTERS, 0)
+        lib.md_set_option(md.MD_OPT_ORDERS, 0)
 
 
 def test_options_and_workspace_sizes(lib):
@@ -123,10 +145,10 @@ def test_slice_bits_option_and_its_k_budget(lib):
         assert lib.md_gemm_orders(1, 1, 5462, 2, fake, fake, fake, None) == md.MD_ERR_K_TOO_LARGE
         assert lib.md_gemm_orders(1, 1, 5461, 2, fake, fake, fake, None) == md.MD_ERR_WORKSPACE
         assert lib.md_gemm(1, 1, 5462, 2, fake, fake, fake, None) == md.MD_ERR_WORKSPACE  # chunked (R16)
-        assert lib.md_set_option(md.MD_OPT_QUARTERS, 5) == md.MD_OK    # 5 slices: the chunked kernel only
+        assert lib.md_set_option(md.MD_OPT_QUARTERS, 5) == md.MD_OK    # 5 slices: the chunked kernel for md_gemm, the generic one for the orders
         assert lib.md_gemm(1, 1, 64, 2, fake, fake, fake, None) == md.MD_ERR_WORKSPACE
-        assert lib.md_gemm_orders(1, 1, 64, 2, fake, fake, fake, None) == md.MD_ERR_UNSUPPORTED
-        assert lib.md_set_option(md.MD_OPT_QUARTERS, 4) == md.MD_OK
+        assert lib.md_gemm_orders(1, 1, 64, 2, fake, fake, fake, None) == md.MD_ERR_WORKSPACE
+        assert lib.md_set_option(md.MD_OPT_QUARTERS, 17) == md.MD_OK   # beyond the generic maximum of double double
         assert lib.md_gemm(1, 1, 64, 2, fake, fake, fake, None) == md.MD_ERR_UNSUPPORTED
     finally:
         lib.md_set_option(md.MD_OPT_SLICE_BITS, 0)

@@ -1,6 +1,7 @@
-"""Extended full-size parity run (not collected by pytest; run by hand on a B200):
+"""Extended full-size parity: collected by pytest with a reduced sample count (`-m gpu`), and runnable by hand on a B200 for
+the tables in profiles/:
 
-    python tests/extended_parity.py [--samples 20000] [--risky 1024] > profiles/<name>.md
+    python tests/test_gpu_extended_parity.py [--samples 20000] [--risky 1024] [--configs 1,2,3,4,5,6] [--quarters 3:8] > profiles/<name>.md
 
 For every BASELINE.json config at its full size and every slice plan (the paper's quarters, md_plan_slices,
 md_plan_slices_chunked) it runs md_gemm through the C-ABI and evaluates |C - C_exact| / (tol * (|A||B|)_ij) with the
@@ -13,6 +14,7 @@ import sys
 import time
 
 import numpy as np
+import pytest
 import torch
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
@@ -24,21 +26,33 @@ from paper_2607_06881_b200 import inputs  # noqa: E402
 TOL = {2: 1e-28, 4: 1e-58, 8: 1e-120, 16: 1e-245}
 
 
-def main():
+def main(argv=None, out=None):
+    """Returns the list of (config index, plan name, Q, max uniform ratio, max riskiest ratio, orders bit-exact) rows."""
+    import dataclasses
+    import functools
+    import builtins
+    emit = functools.partial(builtins.print, file=out) if out is not None else builtins.print
     ap = argparse.ArgumentParser()
     ap.add_argument("--samples", type=int, default=20000)
     ap.add_argument("--risky", type=int, default=1024)
     ap.add_argument("--configs", default="1,2,3,4,5,6")
-    args = ap.parse_args()
-    print("# Extended full-size parity: md_gemm against the exact product at many sampled positions\n")
-    print(f"Command: `python tests/extended_parity.py --samples {args.samples} --risky {args.risky} --configs {args.configs}` "
+    ap.add_argument("--quarters", default="", help="cfg:Q[,cfg:Q] -- run a config with another quarter count (e.g. 3:8 = cfg3 "
+                                                   "with the paper's 8 quarters instead of the 9 it is configured with, DESIGN.md R5)")
+    ap.add_argument("--paper-only", action="store_true", help="only the plan with the config's 13-bit quarters")
+    args = ap.parse_args(argv)
+    q_override = {int(a.split(":")[0]): int(a.split(":")[1]) for a in args.quarters.split(",") if a}
+    rows = []
+    emit("# Extended full-size parity: md_gemm against the exact product at many sampled positions\n")
+    emit(f"Command: `python tests/test_gpu_extended_parity.py --samples {args.samples} --risky {args.risky} --configs {args.configs}{' --quarters ' + args.quarters if args.quarters else ''}{' --paper-only' if args.paper_only else ''}` "
           "(one B200).  err = |C - C_exact|_ij evaluated in the oracle's long accumulator, W = (|A||B|)_ij; a ratio <= 1 "
           "meets the north_star tolerance (1e-28 dd, 1e-58 qd; DESIGN.md R13 for od / hd).\n")
-    print("| cfg | workload | plan | Q x W (chunk) | positions | max err/(tol W), uniform | max err/(tol W), riskiest | "
+    emit("| cfg | workload | plan | Q x W (chunk) | positions | max err/(tol W), uniform | max err/(tol W), riskiest | "
           "median | order matrices bit-exact (positions) | planned Q for this data (D) | seconds (oracle) |")
-    print("|---|---|---|---|---|---|---|---|---|---|---|")
+    emit("|---|---|---|---|---|---|---|---|---|---|---|")
     for ci in [int(x) for x in args.configs.split(",")]:
         cfg = inputs.CONFIGS[ci]
+        if ci in q_override:
+            cfg = dataclasses.replace(cfg, quarters=q_override[ci])
         L = cfg.limbs
         A, B = inputs.generate(cfg, "A"), inputs.generate(cfg, "B")
         dA, dB = torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda()
@@ -54,6 +68,8 @@ def main():
         cw, cq, ck = md.md_plan_slices_chunked(cfg.k, L, 128)
         if (cw, cq) != plans[1][1:3]:
             plans.append(("md_plan_slices_chunked", cw, cq, ck))
+        if args.paper_only:
+            plans = plans[:1]
         for name, W, Q, chunk in plans:
             with md.Workspace(cfg.m, cfg.n, cfg.k, L, Q, bits=W):
                 C = md.md_gemm(dA, dB)
@@ -76,10 +92,25 @@ def main():
             dt = time.perf_counter() - t0
             ratio = r["err"] / (TOL[L] * r["W"])
             nu = args.samples
-            print(f"| {ci} | {cfg.name} | {name} | {Q} x {W}{' (%d)' % chunk if chunk else ''} | {si.size} | {ratio[:nu].max():.3g} | "
+            emit(f"| {ci} | {cfg.name} | {name} | {Q} x {W}{' (%d)' % chunk if chunk else ''} | {si.size} | {ratio[:nu].max():.3g} | "
                   f"{ratio[nu:].max():.3g} | {np.median(ratio):.3g} | {exact_orders} | {pq} ({pd}) | {dt:.0f} |", flush=True)
+            rows.append((ci, name, Q, float(ratio[:nu].max()), float(ratio[nu:].max()), exact_orders))
         del dA, dB
         torch.cuda.empty_cache()
+    return rows
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("ci", [1, 3])
+def test_extended_parity_reduced(ci):
+    """The extended run with a reduced sample count, so that the driver's `-m gpu` pass covers it: every plan of the config
+    meets the north_star tolerance on 1 500 uniform + 256 riskiest positions and the order matrices are bit-exact."""
+    import io
+    rows = main(["--samples", "1500", "--risky", "256", "--configs", str(ci)], out=io.StringIO())
+    assert rows
+    for _, name, _, uni, risky, exact_orders in rows:
+        assert uni <= 1.0 and risky <= 1.0, (name, uni, risky)
+        assert exact_orders.startswith(("True", "n/a")), (name, exact_orders)
 
 
 if __name__ == "__main__":
