@@ -22,9 +22,12 @@
 //   --  oracle_md_gemm      O2 -> O3 (fp64 route) -> O4, the paper's 5-step algorithm
 //   --  oracle_md_gemm_rows_chunked_w   the same with the order sums formed exactly per chunk of k (R16)
 //   --  oracle_plan_quarters            the quarter count a given input needs for a tolerance (R15)
+//   O6  oracle_split_literal, oracle_md_gemm_literal   the paper's own section-3 balancing, element by element: eq. 7, eq. 8,
+//                                       exponent classes A_0..A_12, sign groups of eq. 6 (R17-R22)
 // Parity status: every function above has an independent pin (tests/test_oracle_*.py: accumulator, split, orders,
 // renorm_exact, wide, slices, plan); none is "parity unpinned".
 
+#include <algorithm>
 #include <cmath>
 #include <cstdint>
 #include <cstdlib>
@@ -555,6 +558,221 @@ void oracle_md_gemm_rows_chunked_w(int m, int n, int k, int limbs, int quarters,
     oracle_orders_fp64(mr, n, kc, quarters, orders, Ac.data(), Bc.data(), &ord[(size_t)c * orders * mr * n]);
   }
   oracle_renorm(mr, n, limbs, nchunks * orders, ord.data(), C_rows);
+}
+
+// =====================================================================================================
+// O6 -- the paper's OWN balancing, element by element (section 3; R17-R22).
+//   The path of O2 gives a row of A / a column of B a common exponent (BASELINE.json north_star).  Section 3 of the paper
+//   instead works on single numbers and on the whole matrix:
+//     * PAPER.md:47-49   each double is cut into 4 parts of 13 bits relative to ITS OWN exponent          (R17)
+//     * PAPER.md:124-131 eq. (7): hi and lo of opposite sign -> take one ulp from hi and give it to lo     (R18)
+//     * PAPER.md:133-140 eq. (8): a part with leading zeros borrows half a unit of the part above it       (R19)
+//     * PAPER.md:142     a zero part keeps "the desired exponent": do nothing                              (R19)
+//     * PAPER.md:120-122 A = A_0 + ... + A_12 by the exponent of the leading quarter (mod 13), "execute many
+//                        matrix multiplications"                                                           (R20)
+//     * PAPER.md:107-118 eq. (6): A = A_+ + A_-, four sign-pair products                                   (R21)
+//   Everything below follows those passages step by step; every move is value invariant (pinned in exact rationals).
+// =====================================================================================================
+
+// R17: x = +-2^e (1.f0 f1 f2 f3), four fields of 13 bits; quarters x_0 = +-2^e (1 + f0 2^-13),
+// x_t = +-f_t 2^(e - 13 (t+1)), t = 1, 2, 3 -- "exponents 0, -13, -26, -39".  Plain bit fields; x_0 + x_1 + x_2 + x_3 == x.
+void oracle_quarter_double(double x, double* out4) {
+  out4[0] = out4[1] = out4[2] = out4[3] = 0.0;
+  if (x == 0.0) return;
+  int ex;
+  const double mant = std::frexp(std::fabs(x), &ex);      // |x| = mant 2^ex, mant in [1/2, 1)
+  const uint64_t M = (uint64_t)std::ldexp(mant, 53);        // 53-bit integer, bit 52 = the hidden bit
+  const int e = ex - 1;                                     // |x| = 2^e (1.f)
+  const uint64_t f = M - (1ULL << 52);
+  const double sign = x < 0 ? -1.0 : 1.0;
+  out4[0] = sign * std::ldexp((double)((1ULL << 13) + (f >> 39)), e - 13);
+  out4[1] = sign * std::ldexp((double)((f >> 26) & 8191), e - 26);
+  out4[2] = sign * std::ldexp((double)((f >> 13) & 8191), e - 39);
+  out4[3] = sign * std::ldexp((double)(f & 8191), e - 52);
+}
+
+static inline double ulp_of(double x) { return std::ldexp(1.0, std::ilogb(x) - 52); }
+
+// R18, eq. (7) for a multiple double x[0..limbs-1]: wherever a limb and the next one have opposite signs,
+// b := one ulp of the upper limb (with its sign); upper -= b; lower += b.  The paper's b = 2^-52 assumes |lower| below one ulp
+// of upper; after a borrow further up a limb can have shrunk by cancellation, so in general b = the smallest power of two that
+// is at least one ulp of upper AND exceeds |lower| (one ulp for a normalised pair), which makes lower + b take upper's sign.
+// "the last bit should then be added to the next double in the sequence ... using multiple double arithmetic": the rounding
+// error of lower + b is carried down by TwoSum; what falls off the last limb is returned in carry[l] (exact).  Value
+// invariant: sum x + sum carry is unchanged.  A pair that is not even weakly normalised (b would exceed |upper| / 2) is left.
+void oracle_eq7(int limbs, double* x, double* carry) {
+  for (int l = 0; l < limbs; l++) carry[l] = 0.0;
+  for (int l = 0; l + 1 < limbs; l++) {
+    if (x[l] == 0.0 || x[l + 1] == 0.0 || ((x[l] < 0) == (x[l + 1] < 0))) continue;
+    double mag = ulp_of(x[l]);
+    const double above = std::ldexp(1.0, std::ilogb(x[l + 1]) + 1);  // the power of two just above |lower|
+    if (above > mag) mag = above;
+    if (mag > 0.5 * std::fabs(x[l])) continue;
+    const double b = std::copysign(mag, x[l]);
+    x[l] = x[l] - b;  // exact: x[l] is a multiple of its ulp, b a multiple of that ulp below |x[l]|
+    double c = b;
+    for (int j = l + 1; j < limbs; j++) two_sum(x[j], c, &x[j], &c);
+    carry[l] = c;
+  }
+}
+
+// R19, eq. (8) on the quarters d[0..Q-1] of ONE element whose quarter q sits on the unit u_q = 2^(e - 13 (q+1)):
+// top down, if quarter q+1 has leading zeros (|d_{q+1}| < 2^12 u_{q+1}: its exponent is below the grid) it borrows
+// b = 2^12 u_{q+1} (the paper's b = 2^-14 for q = 0, e = 0) from quarter q: d_q -= b; d_{q+1} += b.  A zero quarter "keeps the
+// desired exponent: do nothing"; a quarter lends only if that "does not alter [its] exponent" (PAPER.md:137:
+// q = 0, or more than 2^12 units).  Afterwards d_q is a multiple of u_q / 2.  Value invariant.
+void oracle_eq8(int Q, int e, double* d) {
+  for (int q = 0; q + 1 < Q; q++) {
+    const double u_next = std::ldexp(1.0, e - 13 * (q + 2));
+    const double top = 4096.0 * u_next;  // 2^12 u_{q+1} = u_q / 2
+    if (d[q + 1] == 0.0 || std::fabs(d[q + 1]) >= top) continue;
+    if (d[q] == 0.0 || ((d[q] < 0) != (d[q + 1] < 0))) continue;
+    if (q > 0 && std::fabs(d[q]) <= 2.0 * top * 4096.0) continue;  // lender must keep its top bit: more than 2^12 units of u_q
+    const double b = std::copysign(top, d[q]);
+    d[q] -= b;
+    d[q + 1] += b;
+  }
+}
+
+// Algorithm L: the literal split of one element (limbs x[0..limbs-1]) into `quarters` parts on the element's OWN grid.
+//   L1  eq. (7): all limbs get one sign (oracle_eq7)
+//   L2  e = ilogb of the leading non-zero limb: the element's exponent (the paper's "exponent of the leading quarter")
+//   L3  for q = 0 .. quarters-1: u_q = 2^(e - 13 (q+1)); part q = sum over the limbs of the bits of that limb at or above u_q
+//       (truncation toward zero of what is left of each limb: the paper's bit fields, R17, re-cut on the element's grid),
+//       and those bits are taken off the limbs.  Exact: every piece is a multiple of u_q below 2^14 u_q.
+//   L4  eq. (8) (oracle_eq8), if apply_eq8
+//   d[q] = the quarters (true values); rem[0..limbs-1] = what is left of the limbs, rem[limbs..2 limbs-1] = eq. (7) carries:
+//   sum d + sum rem == sum x exactly.  Returns e (0 for a zero element).
+int oracle_split_literal_element(int limbs, int quarters, int apply_eq8, const double* x_in, double* d, double* rem) {
+  std::vector<double> x(x_in, x_in + limbs), carry(limbs);
+  oracle_eq7(limbs, x.data(), carry.data());
+  int lead = 0;
+  while (lead < limbs && x[lead] == 0.0) lead++;
+  for (int q = 0; q < quarters; q++) d[q] = 0.0;
+  int e = 0;
+  if (lead < limbs) {
+    e = std::ilogb(x[lead]);
+    for (int q = 0; q < quarters; q++) {
+      const int s = e - 13 * (q + 1);
+      double part = 0.0;
+      for (int l = 0; l < limbs; l++) {
+        const double piece = std::ldexp(std::trunc(std::ldexp(x[l], -s)), s);  // the bits of limb l at or above 2^s
+        x[l] -= piece;                                                            // exact
+        part += piece;                                                            // exact: multiples of 2^s below 2^(s+14)
+      }
+      d[q] = part;
+    }
+    if (apply_eq8) oracle_eq8(quarters, e, d);
+  }
+  if (rem) {
+    for (int l = 0; l < limbs; l++) rem[l] = x[l];
+    for (int l = 0; l < limbs; l++) rem[limbs + l] = carry[l];
+  }
+  return e;
+}
+
+// The whole matrix: quarter_planes [quarters][rows][cols], exps int32[rows*cols] (per ELEMENT), remainder [2*limbs][rows][cols] or NULL.
+void oracle_split_literal(int rows, int cols, int limbs, int quarters, int apply_eq8, const double* planes,
+                          double* quarter_planes, int32_t* exps, double* remainder) {
+  const size_t plane = (size_t)rows * cols;
+#pragma omp parallel for schedule(static)
+  for (int i = 0; i < rows; i++) {
+    std::vector<double> x(limbs), d(quarters), rem(2 * limbs);
+    for (int j = 0; j < cols; j++) {
+      const size_t at = (size_t)i * cols + j;
+      for (int l = 0; l < limbs; l++) x[l] = planes[l * plane + at];
+      exps[at] = oracle_split_literal_element(limbs, quarters, apply_eq8, x.data(), d.data(), rem.data());
+      for (int q = 0; q < quarters; q++) quarter_planes[(size_t)q * plane + at] = d[q];
+      if (remainder)
+        for (int l = 0; l < 2 * limbs; l++) remainder[(size_t)l * plane + at] = rem[l];
+    }
+  }
+}
+
+static inline int floor_div13(int e) { return (e >= 0) ? e / 13 : -((-e + 12) / 13); }
+
+// R20-R22: the literal product.  Every element has its class c = e mod 13 ("the index is the exponent of the
+// leading quarter", 13 possible values on a grid of spacing 13) and its level z = floor(e / 13); A = A_0 + ... + A_12,
+// B likewise, and A B = sum over the 169 class pairs of A_c B_d ("execute many matrix multiplications").  Inside a class all
+// parts of all elements lie on ONE grid 2^(c + 13 Z), so part q of an element of level z is part P = q + (zmax - z) of its
+// class matrix on the common grid anchored at zmax (R20), and the class-pair product is an ordinary quarter product whose
+// order t = P + P' collects terms of ONE unit 2^(c + d + 13 (zmaxA + zmaxB) - 13 (t + 2)): exact accumulations, as in
+// PAPER.md:95-99.  Kept orders: t < quarters + spanA + spanB (span = zmax - zmin over the non-zero elements), i.e. every
+// product p + q < quarters of every element pair and whatever else shares its order.  With sign_groups (eq. 6)
+// every class is further cut into its positive and its negative elements: four sign-pair products per class pair, each a sum of
+// terms of one sign.  C = all order sums of all pairs added into `limbs` limbs (here: exactly, then rounded limb by limb).
+//   info[0..5] (if not NULL) = zminA, zmaxA, zminB, zmaxB, planes per class matrix of A / of B is quarters + span.
+void oracle_md_gemm_literal(int m, int n, int k, int limbs, int quarters, int apply_eq8, int sign_groups, const double* A,
+                            const double* B, double* C, int32_t* info) {
+  const size_t pa = (size_t)m * k, pb = (size_t)k * n, pc = (size_t)m * n;
+  std::vector<double> Aq((size_t)quarters * pa), Bq((size_t)quarters * pb);
+  std::vector<int32_t> eA(pa), eB(pb);
+  oracle_split_literal(m, k, limbs, quarters, apply_eq8, A, Aq.data(), eA.data(), nullptr);
+  oracle_split_literal(k, n, limbs, quarters, apply_eq8, B, Bq.data(), eB.data(), nullptr);
+  auto nonzero = [&](const std::vector<double>& Xq, size_t plane, size_t at) {
+    for (int q = 0; q < quarters; q++)
+      if (Xq[(size_t)q * plane + at] != 0.0) return true;
+    return false;
+  };
+  int zminA = 1 << 30, zmaxA = -(1 << 30), zminB = 1 << 30, zmaxB = -(1 << 30);
+  for (size_t at = 0; at < pa; at++)
+    if (nonzero(Aq, pa, at)) zminA = std::min(zminA, floor_div13(eA[at])), zmaxA = std::max(zmaxA, floor_div13(eA[at]));
+  for (size_t at = 0; at < pb; at++)
+    if (nonzero(Bq, pb, at)) zminB = std::min(zminB, floor_div13(eB[at])), zmaxB = std::max(zmaxB, floor_div13(eB[at]));
+  if (zmaxA < zminA) zminA = zmaxA = 0;
+  if (zmaxB < zminB) zminB = zmaxB = 0;
+  if (info) info[0] = zminA, info[1] = zmaxA, info[2] = zminB, info[3] = zmaxB;
+  const int orders = quarters + (zmaxA - zminA) + (zmaxB - zminB);
+  const int groups = sign_groups ? 26 : 13;  // group id = class (+ 13 for a negative element)
+#pragma omp parallel for schedule(static)
+  for (int i = 0; i < m; i++) {
+    std::vector<int64_t> acc((size_t)groups * groups * orders);
+    LongAcc sum;
+    for (int j = 0; j < n; j++) {
+      std::fill(acc.begin(), acc.end(), 0);
+      for (int t = 0; t < k; t++) {
+        const size_t aa = (size_t)i * k + t, bb = (size_t)t * n + j;
+        const int ea = eA[aa], eb = eB[bb];
+        const int ca = ((ea % 13) + 13) % 13, cb = ((eb % 13) + 13) % 13;
+        const int za = floor_div13(ea), zb = floor_div13(eb);
+        int ga = ca, gb = cb;
+        if (sign_groups) {  // the sign of an element = the sign of its parts (all equal after eq. 7)
+          for (int q = 0; q < quarters; q++)
+            if (Aq[(size_t)q * pa + aa] != 0.0) { if (Aq[(size_t)q * pa + aa] < 0) ga += 13; break; }
+          for (int q = 0; q < quarters; q++)
+            if (Bq[(size_t)q * pb + bb] != 0.0) { if (Bq[(size_t)q * pb + bb] < 0) gb += 13; break; }
+        }
+        for (int p = 0; p < quarters; p++) {
+          // integer digit of part p in HALF units (eq. 8 leaves multiples of u / 2): D = d / 2^(e - 13 (p+1) - 1)
+          const int64_t Da = (int64_t)std::ldexp(Aq[(size_t)p * pa + aa], -(ea - 13 * (p + 1) - 1));
+          if (Da == 0) continue;
+          const int P = p + (zmaxA - za);
+          for (int q = 0; q < quarters; q++) {
+            const int ord = P + q + (zmaxB - zb);
+            if (ord >= orders) break;
+            const int64_t Db = (int64_t)std::ldexp(Bq[(size_t)q * pb + bb], -(eb - 13 * (q + 1) - 1));
+            acc[((size_t)ga * groups + gb) * orders + ord] += Da * Db;
+          }
+        }
+      }
+      // every order sum is an exact double (|acc| < 2^53 under the budget k * orders * 2^30 <= 2^53); add them all, exactly
+      sum.clear();
+      for (int ga = 0; ga < groups; ga++)
+        for (int gb = 0; gb < groups; gb++)
+          for (int ord = 0; ord < orders; ord++) {
+            const int64_t v = acc[((size_t)ga * groups + gb) * orders + ord];
+            if (v == 0) continue;
+            // unit of the sum: 2^(ca + cb + 13 (zmaxA + zmaxB) - 13 (ord + 2)) / 4
+            const int ex = (ga % 13) + (gb % 13) + 13 * (zmaxA + zmaxB) - 13 * (ord + 2) - 2;
+            sum.add_double(std::ldexp((double)v, ex));
+          }
+      for (int l = 0; l < limbs; l++) {
+        const double v = sum.to_double();
+        C[l * pc + (size_t)i * n + j] = v;
+        sum.add_double(v, -1);
+      }
+    }
+  }
 }
 
 int oracle_num_threads(void) {

@@ -196,3 +196,53 @@ def md_gemm_rows_chunked(A, B, chunk: int, quarters: int, bits: int, row0: int =
     C = np.empty((limbs, row1 - row0, n))
     lib().oracle_md_gemm_rows_chunked_w(m, n, k, limbs, quarters, quarters, bits, chunk, _d(A), _d(B), row0, row1, _d(C))
     return C
+
+
+def quarter_double(x: float):
+    """R17: the four 13-bit parts of one double on its own exponent."""
+    out = (ctypes.c_double * 4)()
+    f = lib().oracle_quarter_double
+    f.argtypes = [ctypes.c_double, ctypes.POINTER(ctypes.c_double)]
+    f(float(x), out)
+    return list(out)
+
+
+def eq7(limbs_values):
+    """R18, eq. (7) on one multiple double: returns (new limbs, carries)."""
+    x = _f64(np.array(limbs_values, dtype=np.float64))
+    carry = np.zeros_like(x)
+    lib().oracle_eq7(x.size, _d(x), _d(carry))
+    return x, carry
+
+
+def eq8(d, e: int):
+    """R19, eq. (8) on the quarters of one element of exponent e."""
+    d = _f64(np.array(d, dtype=np.float64))
+    lib().oracle_eq8(d.size, int(e), _d(d))
+    return d
+
+
+def split_literal(planes, quarters: int | None = None, apply_eq8: bool = True, want_remainder: bool = False):
+    """Algorithm L (R17-R19): planes [limbs, rows, cols] -> (quarter planes [Q, rows, cols], per-ELEMENT exponents
+    int32 [rows, cols], remainder [2 limbs, rows, cols] or None)."""
+    planes = _f64(planes)
+    limbs, rows, cols = planes.shape
+    Q = 4 * limbs if quarters is None else quarters
+    qp = np.empty((Q, rows, cols), dtype=np.float64)
+    exps = np.empty((rows, cols), dtype=np.int32)
+    rem = np.empty((2 * limbs, rows, cols), dtype=np.float64) if want_remainder else None
+    lib().oracle_split_literal(rows, cols, limbs, Q, int(apply_eq8), _d(planes), _d(qp), exps.ctypes.data_as(_ip), _d(rem))
+    return qp, exps, rem
+
+
+def md_gemm_literal(A, B, quarters: int | None = None, apply_eq8: bool = True, sign_groups: bool = False):
+    """The paper's literal product (R20-R22): exponent classes A_0..A_12 (x sign groups), exact order sums per class
+    pair, exact recombination.  Returns (C [limbs, m, n], info = (zminA, zmaxA, zminB, zmaxB))."""
+    A, B = _f64(A), _f64(B)
+    limbs, m, k = A.shape
+    n = B.shape[2]
+    Q = 4 * limbs if quarters is None else quarters
+    C = np.empty((limbs, m, n))
+    info = np.zeros(4, dtype=np.int32)
+    lib().oracle_md_gemm_literal(m, n, k, limbs, Q, int(apply_eq8), int(sign_groups), _d(A), _d(B), _d(C), info.ctypes.data_as(_ip))
+    return C, tuple(int(v) for v in info)

@@ -258,8 +258,8 @@ def test_flags_and_runtime_errors():
     with pytest.raises(md.MdError) as e:  # no workspace registered
         md.md_gemm(dev(A), dev(B))
     assert e.value.status == md.MD_ERR_WORKSPACE
-    with md.Workspace(8, 8, 8, 2):  # too small for 200 x 200 x 64
-        cfg2, A2, B2 = gen(0, 200, 200, 64)
+    with md.Workspace(8, 8, 8, 2):  # too small for 1500 x 1500 x 64
+        cfg2, A2, B2 = gen(0, 1500, 1500, 64)
         with pytest.raises(md.MdError) as e2:
             md.md_gemm(dev(A2), dev(B2))
         assert e2.value.status == md.MD_ERR_WORKSPACE

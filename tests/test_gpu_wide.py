@@ -143,12 +143,12 @@ def test_more_tiles_than_sms_uses_the_stream_k_tail():
 def test_unsupported_and_budget_errors():
     cfg, A, B = gen(5, 16, 16, 16)
     with md.Workspace(16, 16, 16, 8):
-        md.md_set_option(md.MD_OPT_QUARTERS, 33)  # octo double has a kernel for 32 quarters only
+        md.md_set_option(md.MD_OPT_QUARTERS, 41)  # octo double: tuned kernels for 32 / 22, the generic one up to 40 quarters
         with pytest.raises(md.MdError) as e:
             md.md_gemm(dev(A), dev(B))
         assert e.value.status == md.MD_ERR_UNSUPPORTED
         md.md_set_option(md.MD_OPT_QUARTERS, 0)
     Aq, Bq = dev(np.zeros((32, 8, 8))), dev(np.zeros((32, 8, 8)))
-    with pytest.raises(md.MdError) as e:  # plain-layout md_qgemm: double / quad double only
+    with pytest.raises(md.MdError) as e:  # md_qgemm repacks octo / hexa double planes into the registered workspace: none here
         md.md_qgemm(Aq, Bq, 8)
-    assert e.value.status == md.MD_ERR_UNSUPPORTED
+    assert e.value.status == md.MD_ERR_WORKSPACE
