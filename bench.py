@@ -72,6 +72,13 @@ def parse_args():
                     help="instead of the md_gemm step: time the public per-step entry points on this config's shapes -- "
                          "md_split (axis 0 on A, axis 1 on B) and md_renorm -- and print their achieved HBM GB/s against "
                          "MEASURED_PEAKS.json (north_star: 'achieved HBM GB/s for the split and epilogue')")
+    ap.add_argument("--balance-table", action="store_true",
+                    help="instead of the md_gemm step: the same problem through (a) the row / column grid with the paper's quarter "
+                         "count, (b) that with one more ORDER, (c) with one more QUARTER, (d) the paper's own per-element balancing "
+                         "with exponent classes (md_gemm_literal) -- time and sampled err / (tol (|A||B|)_ij) of each (DESIGN.md "
+                         "R5, R17-R22; the table VERDICT r1 asks for)")
+    ap.add_argument("--samples", type=int, default=20000, help="--balance-table: uniformly sampled positions (+ 1024 riskiest)")
+    ap.add_argument("--sign-groups", action="store_true", help="--balance-table: also the literal mode with the sign groups of eq. (6)")
     ap.add_argument("--lean", action="store_true", help="skip the context blocks beside the headline (quarter plan, adaptive slices)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -269,6 +276,80 @@ def run_micro(args):
     out["kernels"]["md_renorm"] = {"ms": ms, "algorithmic_bytes": nbytes, "gbs": nbytes / ms / 1e6, "frac_of_hbm_peak": nbytes / ms / 1e6 / peak,
                                    "note": "synthetic order planes of the right magnitudes (timing only)"}
     print(json.dumps(out))
+
+
+def run_balance_table(args):
+    """--balance-table: row / column grid at Q, (Q, Q+1), Q+1 against the paper's literal exponent classes on one workload."""
+    import dataclasses
+    import torch
+    from oracle import md_oracle as orc
+    from paper_2607_06881_b200 import binding as md
+    from paper_2607_06881_b200 import inputs
+    torch.cuda.set_device(0)
+    cfg = apply_overrides(args, inputs.CONFIGS[args.config])
+    L = cfg.limbs
+    Q0 = 4 * L
+    tol = {2: 1e-28, 4: 1e-58, 8: 1e-120, 16: 1e-245}[L]
+    A_h, B_h = inputs.generate(cfg, "A"), inputs.generate(cfg, "B")
+    A, B = torch.from_numpy(A_h).cuda(), torch.from_numpy(B_h).cuda()
+    stream = torch.cuda.current_stream()
+    si, sj = inputs.sample_indices(cfg, args.samples, salt=7)
+    Wt = A[0].abs() @ B[0].abs()
+    rel = Wt / (A[0].abs().amax(dim=1)[:, None] * B[0].abs().amax(dim=0)[None, :])
+    flat = torch.topk(rel.flatten(), min(1024, rel.numel()), largest=False).indices.cpu().numpy()
+    del Wt, rel
+    si = np.concatenate([si, flat // cfg.n]).astype(np.int64)
+    sj = np.concatenate([sj, flat % cfg.n]).astype(np.int64)
+
+    def timed(fn, steps, warmup):
+        for _ in range(warmup):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(steps):
+            out = fn()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / steps, out
+
+    def accuracy(C):
+        r = orc.exact_samples(A_h, B_h, si, sj, C.cpu().numpy())
+        ratio = r["err"] / (tol * r["W"])
+        return {"max_err_over_tol_W": float(ratio.max()), "median": float(np.median(ratio)), "positions": int(si.size),
+                "misses": int((ratio > 1.0).sum())}
+
+    rows = []
+    for name, Q, S in (("row/column grid, paper's quarters", Q0, Q0), ("row/column grid, one more ORDER", Q0, Q0 + 1),
+                       ("row/column grid, one more QUARTER", Q0 + 1, Q0 + 1)):
+        c = dataclasses.replace(cfg, quarters=Q, orders=S)
+        with md.Workspace(cfg.m, cfg.n, cfg.k, L, Q, orders=0 if S == Q else S):
+            ms, C = timed(lambda: md.md_gemm(A, B), args.steps, args.warmup)
+        rows.append({"mode": name, "quarters": Q, "orders": S, "quarter_products": c.products, "ms": ms,
+                     "md_gflops": cfg.md_flops / ms / 1e6, **accuracy(C)})
+        del C
+    variants = [("paper-literal: per-element exponents, eq. 7 + eq. 8, exponent classes A_0..A_12", 0)]
+    if args.sign_groups:
+        variants.append(("paper-literal with the sign groups of eq. 6", md.MD_LITERAL_SIGN_GROUPS))
+    for name, flags in variants:
+        box = {}
+
+        def call():
+            C, info = md.md_gemm_literal(A, B, flags=flags, scratch=box.get("scratch"))
+            box["info"] = info
+            return C
+        l0 = md.md_launch_count()
+        ms, C = timed(call, 1, 0)   # one timed call: it is hundreds of quarter GEMMs
+        info = box["info"]
+        T = sum(1 for p in range(info["planes"]) for q in range(info["planes"]) if p + q < info["orders"])
+        rows.append({"mode": name, "quarters": Q0, "planes_per_class": info["planes"], "orders": info["orders"],
+                     "class_pairs": info["pairs"], "quarter_products": info["pairs"] * T, "launches": md.md_launch_count() - l0, "ms": ms,
+                     "md_gflops": cfg.md_flops / ms / 1e6, "levels": [info["zminA"], info["zmaxA"], info["zminB"], info["zmaxB"]],
+                     **accuracy(C)})
+        del C
+    print(json.dumps({"impl": "ours", "mode": "balance-table",
+                      "config": {"workload": f"BASELINE.json configs[{cfg.index}] {cfg.name}: m={cfg.m} n={cfg.n} k={cfg.k}, limbs={L}, seed {cfg.seed}"},
+                      "tolerance": tol, "rows": rows}))
 
 
 def run_ours(args):
@@ -560,6 +641,8 @@ def main():
         run_reference(args)
     elif args.micro:
         run_micro(args)
+    elif args.balance_table:
+        run_balance_table(args)
     else:
         run_ours(args)
 

@@ -74,7 +74,7 @@ enum {
                            DESIGN.md R13); with MD_OPT_SLICE_BITS also 6, 7 / 11, 12 / 22 / 44.  Every other count runs on
                            the generic kernel (runtime counts; slower, same bits). */
   MD_OPT_ORDERS = 2,    /* kept product orders S: C^(s) for s = 0..S-1 (the paper's C_1..C_S).  Default = quarters
-                           (the paper keeps C_1..C_8 of 8 quarters).  1 <= S <= min(quarters + 2, 2*quarters - 1): S < quarters
+                           (the paper keeps C_1..C_8 of 8 quarters).  1 <= S <= min(2*quarters - 1, 24 / 32 / 42 / 74 for limbs 2 / 4 / 8 / 16): S < quarters
                            is a PRUNED set (fewer products, larger error), S > quarters an EXTENDED one -- order Q adds the Q - 1
                            products p + q = Q that the paper's set drops, for less work than another quarter (R5).
                            Tuned kernels for (8, 9), (8, 10), (16, 17), (16, 18); the generic kernel otherwise.  Error bound:
@@ -222,6 +222,49 @@ md_status md_plan_quarters(int m, int n, int k, int limbs, const double* A_plane
 size_t md_auto_scratch_bytes(int m, int n, int k, int limbs, int quarters);
 md_status md_gemm_auto(int m, int n, int k, int limbs, const double* A_planes, const double* B_planes, double* C_planes,
                        void* scratch, size_t scratch_bytes, double rel_tol, int* quarters_used, md_stream stream);
+
+/* ---------------------------------------------------------------------------------------------------------------------
+ * The paper's OWN balancing, element by element (section 3; R17-R22) -- a second
+ * split mode beside md_split / md_gemm, measured against them in profiles/ (it is far more work).
+ *
+ * md_split_literal -- Algorithm L on every element of a multiple-double matrix:
+ *   (1) eq. (7): where a limb and the next have opposite signs, the upper gives b (one ulp of it; in general the
+ *       smallest power of two >= that ulp above |lower|) to the lower; rounding errors travel down by TwoSum ("the last bit should
+ *       then be added to the next double");
+ *   (2) the element's exponent e = ilogb of its leading non-zero limb ("the exponent of the leading quarter");
+ *   (3) part q = the bits of the element on the unit 2^(e - 13 (q+1)) (13-bit parts with exponents 0, -13, -26,
+ *       -39, here of the ELEMENT and continued through all its limbs); the leading part also holds the hidden bit (14 bits);
+ *   (4) eq. (8), top down: a part below 2^12 of its units borrows b = 2^12 units (half a unit of the part above,
+ *       the paper's 2^-14) from the part above, provided that part keeps its own exponent; zero parts "do nothing".
+ *   planes          in   [limbs][rows][cols]
+ *   quarter_planes  out  [quarters][rows][cols]  true-valued parts, all of the element's sign, multiples of HALF their unit
+ *   exps            out  int32[rows * cols]      e per ELEMENT (0 for a zero element)
+ *   flags           MD_LITERAL_NO_EQ8: skip step (4)
+ *   The element equals the sum of its parts plus a remainder below limbs * 2^(e - 13 quarters).  limbs in {2, 4, 8, 16};
+ *   bit-exact against the oracle's Algorithm L.
+ *
+ * md_gemm_literal -- C = A * B through the exponent classes of PAPER.md:120-122: A = A_0 + ... + A_12 by e mod 13 (B likewise);
+ *   inside a class every part of every element lies on the grid 2^(c + 13 Z), so part q of an element of level z = floor(e / 13)
+ *   is plane q + (zmax - z) of the class matrix, a class pair A_c B_d is an ORDINARY quarter GEMM (md_gemm's kernels) with exact
+ *   accumulations, and all order sums of all non-empty pairs are added error free into C.  Planes per class matrix: quarters +
+ *   max(spanA, spanB); orders kept: quarters + spanA + spanB (span = zmax - zmin of an operand).  MD_LITERAL_SIGN_GROUPS adds the
+ *   sign groups of eq. (6): 26 groups per operand, four sign-pair products per class pair, same C (every
+ *   accumulation being exact, grouping by sign changes nothing but the cost).
+ *   Error: relative to (|A||B|)_ij term by term -- about (quarters + 3) 2^(-13 quarters + 2) -- whatever the dynamic range.
+ *   scratch      device, 256-byte aligned, caller-owned; md_literal_scratch_bytes(m, n, k, limbs, planes, orders) for given counts
+ *                (0, 0 = no spread: quarters planes and orders).  If the data needs more, MD_ERR_WORKSPACE with the counts in
+ *                info_host[4], [5]: size again and repeat.
+ *   info_host    HOST int32[8], may be NULL: zminA, zmaxA, zminB, zmaxB, planes, orders, class pairs run, kernels launched
+ *   MD_ERR_UNSUPPORTED when planes / orders exceed the generic kernel's maxima (16 / 24 for double double, 24 / 32 for quad
+ *   double: level spans up to 8, i.e. elements over about 2^+-50); uses MD_OPT_QUARTERS, needs MD_OPT_SLICE_BITS = 13.
+ *   SYNCHRONISES `stream` once (the counts come back to the host); not capturable in a CUDA graph.
+ * ------------------------------------------------------------------------------------------------------------------ */
+enum { MD_LITERAL_NO_EQ8 = 1, MD_LITERAL_SIGN_GROUPS = 2 };
+md_status md_split_literal(int rows, int cols, int limbs, int quarters, int flags, const double* planes, double* quarter_planes,
+                           int32_t* exps, md_stream stream);
+size_t md_literal_scratch_bytes(int m, int n, int k, int limbs, int planes_per_class, int orders);
+md_status md_gemm_literal(int m, int n, int k, int limbs, const double* A_planes, const double* B_planes, double* C_planes,
+                          void* scratch, size_t scratch_bytes, int flags, int32_t* info_host, md_stream stream);
 
 /* Workspace for md_gemm / md_gemm_orders: quarter planes of A and B, exponent vectors and the status word, for the
  * CURRENT option values.  The caller allocates (device memory, 256-byte aligned) and registers it FOR THE CURRENT DEVICE; the

@@ -28,6 +28,9 @@ _SIGNATURES = {
     "md_plan_quarters": (_c.c_int, [_c.c_int] * 4 + [_c.c_void_p] * 3 + [_c.c_size_t, _c.c_double] + [_c.c_void_p] * 3),
     "md_auto_scratch_bytes": (_c.c_size_t, [_c.c_int] * 5),
     "md_gemm_auto": (_c.c_int, [_c.c_int] * 4 + [_c.c_void_p] * 4 + [_c.c_size_t, _c.c_double, _c.c_void_p, _c.c_void_p]),
+    "md_split_literal": (_c.c_int, [_c.c_int] * 5 + [_c.c_void_p] * 4),
+    "md_literal_scratch_bytes": (_c.c_size_t, [_c.c_int] * 6),
+    "md_gemm_literal": (_c.c_int, [_c.c_int] * 4 + [_c.c_void_p] * 4 + [_c.c_size_t, _c.c_int, _c.c_void_p, _c.c_void_p]),
     "md_plan_slices_chunked": (_c.c_int, [_c.c_int] * 3 + [_c.c_void_p] * 3),
     "md_split": (_c.c_int, [_c.c_int] * 5 + [_c.c_void_p] * 4),
     "md_qgemm": (_c.c_int, [_c.c_int] * 6 + [_c.c_void_p] * 5),
@@ -201,6 +204,47 @@ def md_gemm_auto(A: torch.Tensor, B: torch.Tensor, C: torch.Tensor | None = None
         want = q.value
     _check(st, "md_gemm_auto")
     return C, q.value
+
+
+MD_LITERAL_NO_EQ8, MD_LITERAL_SIGN_GROUPS = 1, 2
+
+
+def md_split_literal(planes: torch.Tensor, quarters: int | None = None, flags: int = 0, stream=None):
+    """Algorithm L (include/mdgemm.h): planes [limbs, rows, cols] -> (parts [Q, rows, cols], per-element exponents int32 [rows, cols])."""
+    limbs, rows, cols = planes.shape
+    Q = 4 * limbs if quarters is None else quarters
+    qp = torch.empty((Q, rows, cols), dtype=torch.float64, device=planes.device)
+    exps = torch.empty((rows, cols), dtype=torch.int32, device=planes.device)
+    _check(lib().md_split_literal(rows, cols, limbs, Q, flags, _dev(planes), _dev(qp), _dev(exps, torch.int32), _stream(stream)),
+           "md_split_literal")
+    return qp, exps
+
+
+def md_gemm_literal(A: torch.Tensor, B: torch.Tensor, C: torch.Tensor | None = None, flags: int = 0, stream=None, scratch=None):
+    """The paper's exponent-class product (include/mdgemm.h).  Returns (C, info dict).  Sizes the scratch for no spread first and
+    again with the counts the data needs.  Synchronises."""
+    limbs, m, k = A.shape
+    n = B.shape[2]
+    if C is None:
+        C = torch.empty((limbs, m, n), dtype=torch.float64, device=A.device)
+    info = (ctypes.c_int32 * 8)()
+    planes = orders = 0
+    st = MD_ERR_WORKSPACE
+    for _ in range(2):
+        need = lib().md_literal_scratch_bytes(m, n, k, limbs, planes, orders)
+        if need == 0:
+            raise MdError(MD_ERR_UNSUPPORTED, "md_literal_scratch_bytes")
+        if scratch is None or scratch.numel() < need:
+            scratch = None
+            scratch = torch.empty(need, dtype=torch.uint8, device=A.device)
+        st = lib().md_gemm_literal(m, n, k, limbs, _dev(A), _dev(B), _dev(C), _dev(scratch, torch.uint8), scratch.numel(), flags,
+                                   ctypes.addressof(info), _stream(stream))
+        if st != MD_ERR_WORKSPACE:
+            break
+        planes, orders = info[4], info[5]
+    _check(st, "md_gemm_literal")
+    keys = ("zminA", "zmaxA", "zminB", "zmaxB", "planes", "orders", "pairs", "launches")
+    return C, dict(zip(keys, (int(v) for v in info)))
 
 
 def md_gemm_orders(A: torch.Tensor, B: torch.Tensor, stream=None) -> torch.Tensor:

@@ -66,10 +66,13 @@ bool qgemm_wide_supported(int limbs, int quarters);
 cudaError_t launch_qgemm_wide(int m, int n, int k, int limbs, int quarters, const double* Ap, const double* Bp,
                               double* order_planes, double* C_planes, void* sk_ws, cudaStream_t stream,
                               uint64_t* launches);
-// GENERIC instances of the same kernel (qgemm_wide.cu): quarter and order counts are runtime values up to these maxima, orders
-// <= quarters + 2 (and <= 2 quarters - 1); packed operands with the tile shape of pack_bx_generic and k-slab depth 4
+// GENERIC instances of the same kernel (qgemm_wide.cu): quarter and order counts are runtime values up to these maxima (and
+// orders <= 2 quarters - 1); packed operands with the tile shape of pack_bx_generic and k-slab depth 4.  Double and quad double
+// keep 8 orders beyond the quarter maximum: the class-pair products of the literal mode (literal.cu) need quarters + spans.
 constexpr int GENERIC_QMAX_DD = 16, GENERIC_QMAX_QD = 24, GENERIC_QMAX_OD = 40, GENERIC_QMAX_HD = 72;
+constexpr int GENERIC_SMAX_DD = 24, GENERIC_SMAX_QD = 32, GENERIC_SMAX_OD = 42, GENERIC_SMAX_HD = 74;
 int qgemm_generic_max_quarters(int limbs);
+int qgemm_generic_max_orders(int limbs);
 bool qgemm_generic_supported(int limbs, int quarters, int orders);
 cudaError_t launch_qgemm_generic(int m, int n, int k, int limbs, int quarters, int orders, const double* Ap, const double* Bp,
                                  double* order_planes, double* C_planes, void* sk_ws, cudaStream_t stream, uint64_t* launches);

@@ -19,7 +19,7 @@
 //     lane-private slot of shared memory, which performs exactly the operation sequence of the standalone md_renorm.
 //
 // GENERIC instances (WCfg<..., GENERIC = true>): the same kernel with the quarter count Q and the order count S as RUNTIME
-// values below compile-time maxima (double double Q <= 16, quad 24, octo 40, hexa 72; S <= Q + 2, so the pruned and
+// values below compile-time maxima (double double Q <= 16 / S <= 24, quad 24 / 32, octo 40 / 42, hexa 72 / 74, so the pruned and
 // extended order sets of MD_OPT_ORDERS run here too).  Every DMMA site of the maximal triangular set stays in the code
 // behind a warp-uniform predicate; the order ranges are those of the maximal set, so a smaller problem leaves the upper
 // ranges short of work.  Slower than a tuned instance (one 8x8 tile per warp, predicates, k-slab depth 4), but every
@@ -448,10 +448,10 @@ using WCfgOD22 = WCfg<22, 8, 4, 2, 1>; // octo double in 22 slices of 19 bits (M
 using WCfgHD = WCfg<64, 16, 2, 1, 4>;  // hexa double: 16 x 8 CTA tile, 2 tiles x 4 ranges
 using WCfgHD44 = WCfg<44, 16, 2, 2, 2>;  // hexa double in 44 slices of 19 bits: 16 x 16 CTA tile, 4 tiles x 2 ranges
 // GENERIC instances: runtime (Q, S) up to these maxima
-using WCfgGenDD = WCfg<GENERIC_QMAX_DD, 2, 4, 2, 1, GENERIC_QMAX_DD + 2, true>;
-using WCfgGenQD = WCfg<GENERIC_QMAX_QD, 4, 4, 2, 1, GENERIC_QMAX_QD + 2, true>;
-using WCfgGenOD = WCfg<GENERIC_QMAX_OD, 8, 2, 2, 2, GENERIC_QMAX_OD + 2, true>;
-using WCfgGenHD = WCfg<GENERIC_QMAX_HD, 16, 2, 1, 4, GENERIC_QMAX_HD + 2, true>;
+using WCfgGenDD = WCfg<GENERIC_QMAX_DD, 2, 4, 2, 1, GENERIC_SMAX_DD, true>;
+using WCfgGenQD = WCfg<GENERIC_QMAX_QD, 4, 4, 2, 1, GENERIC_SMAX_QD, true>;
+using WCfgGenOD = WCfg<GENERIC_QMAX_OD, 8, 2, 2, 2, GENERIC_SMAX_OD, true>;
+using WCfgGenHD = WCfg<GENERIC_QMAX_HD, 16, 2, 1, 4, GENERIC_SMAX_HD, true>;
 
 }  // namespace
 
@@ -462,9 +462,12 @@ bool qgemm_wide_supported(int limbs, int quarters) {
 int qgemm_generic_max_quarters(int limbs) {
   return limbs == 2 ? GENERIC_QMAX_DD : limbs == 4 ? GENERIC_QMAX_QD : limbs == 8 ? GENERIC_QMAX_OD : limbs == 16 ? GENERIC_QMAX_HD : 0;
 }
+int qgemm_generic_max_orders(int limbs) {
+  return limbs == 2 ? GENERIC_SMAX_DD : limbs == 4 ? GENERIC_SMAX_QD : limbs == 8 ? GENERIC_SMAX_OD : limbs == 16 ? GENERIC_SMAX_HD : 0;
+}
 bool qgemm_generic_supported(int limbs, int quarters, int orders) {
-  const int qmax = qgemm_generic_max_quarters(limbs);
-  return qmax > 0 && quarters >= 1 && quarters <= qmax && orders >= 1 && orders <= quarters + 2 && orders <= 2 * quarters - 1;
+  const int qmax = qgemm_generic_max_quarters(limbs), smax = qgemm_generic_max_orders(limbs);
+  return qmax > 0 && quarters >= 1 && quarters <= qmax && orders >= 1 && orders <= smax && orders <= 2 * quarters - 1;
 }
 
 cudaError_t launch_qgemm_wide(int m, int n, int k, int limbs, int quarters, const double* Ap, const double* Bp,

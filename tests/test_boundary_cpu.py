@@ -65,11 +65,12 @@ def test_argument_errors_need_no_gpu(lib):
     assert lib.md_qgemm(4, 4, 4, 2, 8, 7, fake, fake, fake, fake, None) == md.MD_ERR_WORKSPACE
     assert lib.md_qgemm(4, 4, 4, 2, 12, 12, fake, fake, fake, fake, None) == md.MD_ERR_WORKSPACE
     assert lib.md_qgemm(4, 4, 4, 2, 17, 17, fake, fake, fake, fake, None) == md.MD_ERR_UNSUPPORTED   # dd: at most 16 quarters
-    assert lib.md_qgemm(4, 4, 4, 2, 8, 11, fake, fake, fake, fake, None) == md.MD_ERR_UNSUPPORTED    # orders <= quarters + 2
+    assert lib.md_qgemm(4, 4, 4, 2, 8, 16, fake, fake, fake, fake, None) == md.MD_ERR_UNSUPPORTED    # orders <= 2 quarters - 1
+    assert lib.md_qgemm(4, 4, 4, 2, 16, 25, fake, fake, fake, fake, None) == md.MD_ERR_UNSUPPORTED   # dd: at most 24 orders
     assert lib.md_qgemm(4, 4, 4, 4, 25, 25, fake, fake, fake, fake, None) == md.MD_ERR_UNSUPPORTED   # qd: at most 24
     assert lib.md_qgemm(4, 4, 4, 2, 8, 8, fake, fake, None, None, None) == md.MD_ERR_BAD_ARG
     # every quarter count md_plan_quarters may return within the generic maxima has a kernel (R5, R15):
-    # dd 1..16, qd 1..24, od 1..40, hd 1..72, and MD_OPT_ORDERS in [Q - 2, Q + 2]
+    # dd 1..16, qd 1..24, od 1..40, hd 1..72, and MD_OPT_ORDERS in [Q - 2, Q + 2] (and further: DESIGN.md R22)
     try:
         for limbs, qmax in ((2, 16), (4, 24), (8, 40), (16, 72)):
             for Q in range(3, qmax + 1):
