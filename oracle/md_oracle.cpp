@@ -22,6 +22,7 @@
 //   --  oracle_md_gemm      O2 -> O3 (fp64 route) -> O4, the paper's 5-step algorithm
 //   --  oracle_md_gemm_rows_chunked_w   the same with the order sums formed exactly per chunk of k (R16)
 //   --  oracle_plan_quarters            the quarter count a given input needs for a tolerance (R15)
+//   O7  oracle_md_qr                   unblocked Householder QR in multiple-double arithmetic (PAPER.md:213 future work; ref [18])
 //   O6  oracle_split_literal, oracle_md_gemm_literal   the paper's own section-3 balancing, element by element: eq. 7, eq. 8,
 //                                       exponent classes A_0..A_12, sign groups of eq. 6 (R17-R22)
 // Parity status: every function above has an independent pin (tests/test_oracle_*.py: accumulator, split, orders,
@@ -773,6 +774,203 @@ void oracle_md_gemm_literal(int m, int n, int k, int limbs, int quarters, int ap
       }
     }
   }
+}
+
+// =====================================================================================================
+// O7 -- Householder QR in multiple-double arithmetic, the "second workload" the paper names as future work
+//   ("apply this multiple double tensor core matrix multiplication to accelerate the blocked Householder QR,
+//   extending [18]"; ref [18] PAPER.md:235, least squares on GPUs in multiple double precision).
+//   The oracle is the plain UNBLOCKED algorithm (one reflection per column, applied column by column), every scalar operation
+//   in multiple-double arithmetic built from the textbook error-free transformations of O5 (refs [2], [3], [15]):
+//     mdx_add   (L+1)-term TwoSum cascade, renormalised
+//     mdx_mul   partial products a_i b_j with i + j < L by TwoProd, those with i + j = L in plain fp64, cascaded
+//     mdx_div   long division: L + 1 quotient digits q_i = r_0 / b_0, r -= q_i b
+//     mdx_sqrt  Heron's iteration x <- (x + a / x) / 2 from the double-precision root
+//   A = Q R, A m x n (m >= n), Q m x n with orthonormal columns, R n x n upper triangular with diag(R) >= 0 (the sign of every
+//   row of R / column of Q is fixed that way, which makes the factorisation of a full-rank A unique).
+// =====================================================================================================
+namespace {
+
+void mdx_renorm(int terms, double* acc) {
+  for (int l = terms - 1; l > 0; l--) two_sum(acc[l - 1], acc[l], &acc[l - 1], &acc[l]);
+  for (int sweep = 0; sweep + 1 < terms; sweep++)
+    for (int l = 0; l + 1 < terms; l++) two_sum(acc[l], acc[l + 1], &acc[l], &acc[l + 1]);
+}
+void mdx_add(int L, const double* a, const double* b, double* out, double sign_b = 1.0) {
+  std::vector<double> acc(L + 1, 0.0);
+  for (int l = 0; l < L; l++) acc[l] = a[l];
+  for (int l = L - 1; l >= 0; l--) md_cascade_add(acc.data(), L + 1, sign_b * b[l]);
+  mdx_renorm(L + 1, acc.data());
+  for (int l = 0; l < L; l++) out[l] = acc[l];
+}
+void mdx_mul(int L, const double* a, const double* b, double* out) {
+  std::vector<double> acc(L + 1, 0.0);
+  for (int s = L; s >= 0; s--)  // smallest partial products first
+    for (int la = 0; la < L; la++) {
+      const int lb = s - la;
+      if (lb < 0 || lb >= L) continue;
+      if (s < L) {
+        double p, e;
+        two_prod(a[la], b[lb], &p, &e);
+        md_cascade_add(acc.data(), L + 1, e);
+        md_cascade_add(acc.data(), L + 1, p);
+      } else {
+        md_cascade_add(acc.data(), L + 1, a[la] * b[lb]);
+      }
+    }
+  mdx_renorm(L + 1, acc.data());
+  for (int l = 0; l < L; l++) out[l] = acc[l];
+}
+void mdx_div(int L, const double* a, const double* b, double* out) {
+  std::vector<double> r(a, a + L), q(L + 1, 0.0), qb(L), t(L);
+  for (int i = 0; i <= L; i++) {
+    q[i] = r[0] / b[0];
+    std::fill(t.begin(), t.end(), 0.0);
+    t[0] = q[i];
+    mdx_mul(L, t.data(), b, qb.data());
+    mdx_add(L, r.data(), qb.data(), r.data(), -1.0);
+  }
+  mdx_renorm(L + 1, q.data());
+  for (int l = 0; l < L; l++) out[l] = q[l];
+}
+void mdx_sqrt(int L, const double* a, double* out) {
+  std::fill(out, out + L, 0.0);
+  if (a[0] <= 0.0) return;
+  std::vector<double> x(L, 0.0), t(L);
+  x[0] = std::sqrt(a[0]);
+  int iters = 2;
+  for (int l = 1; l < L; l *= 2) iters++;
+  for (int it = 0; it < iters; it++) {
+    mdx_div(L, a, x.data(), t.data());
+    mdx_add(L, x.data(), t.data(), x.data());
+    for (int l = 0; l < L; l++) x[l] *= 0.5;
+  }
+  for (int l = 0; l < L; l++) out[l] = x[l];
+}
+
+}  // namespace
+
+// test access to the four scalar operations (a, b, out: `limbs` doubles each); op: 0 add, 1 sub, 2 mul, 3 div, 4 sqrt(a)
+void oracle_mdx_op(int limbs, int op, const double* a, const double* b, double* out) {
+  switch (op) {
+    case 0: mdx_add(limbs, a, b, out); break;
+    case 1: mdx_add(limbs, a, b, out, -1.0); break;
+    case 2: mdx_mul(limbs, a, b, out); break;
+    case 3: mdx_div(limbs, a, b, out); break;
+    default: mdx_sqrt(limbs, a, out); break;
+  }
+}
+
+// A [limbs][m][n] -> Q [limbs][m][n], R [limbs][n][n].  Reflections as in the textbook (Golub & Van Loan alg. 5.1.1 / LAPACK
+// dgeqr2): for column j, alpha = A_jj, sigma = sum_{i>j} A_ij^2, beta = -sign(alpha) sqrt(alpha^2 + sigma), tau = (beta - alpha) /
+// beta, v = (1, A_{j+1:,j} / (alpha - beta)); H_j = I - tau v v^T; R_jj = beta.  Q = H_0 H_1 ... H_{n-1} applied to the first n
+// columns of I, backwards.  Finally the signs: R_jj < 0 => row j of R and column j of Q are negated.
+void oracle_md_qr(int m, int n, int limbs, const double* A, double* Q, double* R) {
+  const int L = limbs;
+  const size_t pa = (size_t)m * n, pr = (size_t)n * n;
+  std::vector<double> W((size_t)L * pa);  // working copy: R above the diagonal, v below
+  std::memcpy(W.data(), A, sizeof(double) * (size_t)L * pa);
+  std::vector<double> tau((size_t)n * L, 0.0);
+  auto get = [&](const std::vector<double>& X, size_t plane, size_t at, double* out) {
+    for (int l = 0; l < L; l++) out[l] = X[l * plane + at];
+  };
+  auto put = [&](std::vector<double>& X, size_t plane, size_t at, const double* in) {
+    for (int l = 0; l < L; l++) X[l * plane + at] = in[l];
+  };
+  std::vector<double> a(L), b(L), c(L), d(L), alpha(L), beta(L), sigma(L), w(L), one(L, 0.0), zero(L, 0.0);
+  one[0] = 1.0;
+  for (int j = 0; j < n; j++) {
+    get(W, pa, (size_t)j * n + j, alpha.data());
+    std::fill(sigma.begin(), sigma.end(), 0.0);
+    for (int i = j + 1; i < m; i++) {
+      get(W, pa, (size_t)i * n + j, a.data());
+      mdx_mul(L, a.data(), a.data(), b.data());
+      mdx_add(L, sigma.data(), b.data(), sigma.data());
+    }
+    double* tj = &tau[(size_t)j * L];
+    if (sigma[0] == 0.0) {  // nothing below the diagonal: H = I (the sign of R_jj is fixed at the end)
+      std::fill(tj, tj + L, 0.0);
+      continue;
+    }
+    mdx_mul(L, alpha.data(), alpha.data(), b.data());
+    mdx_add(L, b.data(), sigma.data(), b.data());
+    mdx_sqrt(L, b.data(), beta.data());
+    if (alpha[0] >= 0.0)
+      for (int l = 0; l < L; l++) beta[l] = -beta[l];
+    mdx_add(L, beta.data(), alpha.data(), c.data(), -1.0);  // beta - alpha
+    mdx_div(L, c.data(), beta.data(), tj);                  // tau
+    mdx_add(L, alpha.data(), beta.data(), c.data(), -1.0);  // alpha - beta
+    for (int i = j + 1; i < m; i++) {
+      get(W, pa, (size_t)i * n + j, a.data());
+      mdx_div(L, a.data(), c.data(), b.data());
+      put(W, pa, (size_t)i * n + j, b.data());
+    }
+    put(W, pa, (size_t)j * n + j, beta.data());
+    // apply H_j to the columns to the right: w = v^T a_c, a_c -= tau w v
+#pragma omp parallel for schedule(static) firstprivate(a, b, c, d, w)
+    for (int col = j + 1; col < n; col++) {
+      get(W, pa, (size_t)j * n + col, w.data());
+      for (int i = j + 1; i < m; i++) {
+        get(W, pa, (size_t)i * n + j, a.data());
+        get(W, pa, (size_t)i * n + col, b.data());
+        mdx_mul(L, a.data(), b.data(), c.data());
+        mdx_add(L, w.data(), c.data(), w.data());
+      }
+      mdx_mul(L, tj, w.data(), d.data());  // tau w
+      get(W, pa, (size_t)j * n + col, b.data());
+      mdx_add(L, b.data(), d.data(), b.data(), -1.0);
+      put(W, pa, (size_t)j * n + col, b.data());
+      for (int i = j + 1; i < m; i++) {
+        get(W, pa, (size_t)i * n + j, a.data());
+        mdx_mul(L, a.data(), d.data(), c.data());
+        get(W, pa, (size_t)i * n + col, b.data());
+        mdx_add(L, b.data(), c.data(), b.data(), -1.0);
+        put(W, pa, (size_t)i * n + col, b.data());
+      }
+    }
+  }
+  // R
+  std::vector<double> Rv((size_t)L * pr, 0.0), Qv((size_t)L * pa, 0.0);
+  for (int i = 0; i < n; i++)
+    for (int col = i; col < n; col++)
+      for (int l = 0; l < L; l++) Rv[l * pr + (size_t)i * n + col] = W[l * pa + (size_t)i * n + col];
+  // Q = H_0 ... H_{n-1} I_{m x n}: apply the reflections backwards to the identity
+  for (int i = 0; i < n; i++) Qv[(size_t)i * n + i] = 1.0;
+  for (int j = n - 1; j >= 0; j--) {
+    const double* tj = &tau[(size_t)j * L];
+    if (tj[0] == 0.0) continue;
+#pragma omp parallel for schedule(static) firstprivate(a, b, c, d, w)
+    for (int col = j; col < n; col++) {
+      get(Qv, pa, (size_t)j * n + col, w.data());
+      for (int i = j + 1; i < m; i++) {
+        get(W, pa, (size_t)i * n + j, a.data());
+        get(Qv, pa, (size_t)i * n + col, b.data());
+        mdx_mul(L, a.data(), b.data(), c.data());
+        mdx_add(L, w.data(), c.data(), w.data());
+      }
+      mdx_mul(L, tj, w.data(), d.data());
+      get(Qv, pa, (size_t)j * n + col, b.data());
+      mdx_add(L, b.data(), d.data(), b.data(), -1.0);
+      put(Qv, pa, (size_t)j * n + col, b.data());
+      for (int i = j + 1; i < m; i++) {
+        get(W, pa, (size_t)i * n + j, a.data());
+        mdx_mul(L, a.data(), d.data(), c.data());
+        get(Qv, pa, (size_t)i * n + col, b.data());
+        mdx_add(L, b.data(), c.data(), b.data(), -1.0);
+        put(Qv, pa, (size_t)i * n + col, b.data());
+      }
+    }
+  }
+  // signs: diag(R) >= 0
+  for (int j = 0; j < n; j++) {
+    if (Rv[(size_t)j * n + j] >= 0.0) continue;
+    for (int l = 0; l < L; l++) {
+      for (int col = j; col < n; col++) Rv[l * pr + (size_t)j * n + col] = -Rv[l * pr + (size_t)j * n + col];
+      for (int i = 0; i < m; i++) Qv[l * pa + (size_t)i * n + j] = -Qv[l * pa + (size_t)i * n + j];
+    }
+  }
+  std::memcpy(Q, Qv.data(), sizeof(double) * (size_t)L * pa);
+  std::memcpy(R, Rv.data(), sizeof(double) * (size_t)L * pr);
 }
 
 int oracle_num_threads(void) {

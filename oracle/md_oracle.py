@@ -246,3 +246,24 @@ def md_gemm_literal(A, B, quarters: int | None = None, apply_eq8: bool = True, s
     info = np.zeros(4, dtype=np.int32)
     lib().oracle_md_gemm_literal(m, n, k, limbs, Q, int(apply_eq8), int(sign_groups), _d(A), _d(B), _d(C), info.ctypes.data_as(_ip))
     return C, tuple(int(v) for v in info)
+
+
+def mdx_op(op: str, a, b=None):
+    """One scalar multiple-double operation of O7 ('add', 'sub', 'mul', 'div', 'sqrt') on limb vectors."""
+    a = _f64(np.array(a, dtype=np.float64))
+    b = _f64(np.array(a if b is None else b, dtype=np.float64))
+    out = np.empty_like(a)
+    lib().oracle_mdx_op(a.size, {"add": 0, "sub": 1, "mul": 2, "div": 3, "sqrt": 4}[op], _d(a), _d(b), _d(out))
+    return out
+
+
+def md_qr(A):
+    """O7: unblocked Householder QR in multiple-double arithmetic.  A [limbs, m, n] (m >= n) -> (Q [limbs, m, n], R [limbs, n, n]),
+    diag(R) >= 0."""
+    A = _f64(A)
+    limbs, m, n = A.shape
+    assert m >= n
+    Q = np.empty((limbs, m, n))
+    R = np.empty((limbs, n, n))
+    lib().oracle_md_qr(m, n, limbs, _d(A), _d(Q), _d(R))
+    return Q, R
