@@ -79,6 +79,10 @@ def parse_args():
                          "R5, R17-R22; the table VERDICT r1 asks for)")
     ap.add_argument("--samples", type=int, default=20000, help="--balance-table: uniformly sampled positions (+ 1024 riskiest)")
     ap.add_argument("--sign-groups", action="store_true", help="--balance-table: also the literal mode with the sign groups of eq. (6)")
+    ap.add_argument("--qr", action="store_true",
+                    help="instead of the md_gemm step: md_qr (blocked Householder QR on top of md_gemm, PAPER.md:213) of the m x n "
+                         "matrix A of this config (--shape m,n,k; k unused): time, share of it inside the md_gemm path, md-GFLOP/s "
+                         "counting 2 m n^2 - 2 n^3 / 3 for R plus the same again for Q")
     ap.add_argument("--lean", action="store_true", help="skip the context blocks beside the headline (quarter plan, adaptive slices)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -350,6 +354,32 @@ def run_balance_table(args):
     print(json.dumps({"impl": "ours", "mode": "balance-table",
                       "config": {"workload": f"BASELINE.json configs[{cfg.index}] {cfg.name}: m={cfg.m} n={cfg.n} k={cfg.k}, limbs={L}, seed {cfg.seed}"},
                       "tolerance": tol, "rows": rows}))
+
+
+def run_qr(args):
+    import torch
+    from paper_2607_06881_b200 import binding as md
+    from paper_2607_06881_b200 import inputs
+    torch.cuda.set_device(0)
+    cfg = apply_overrides(args, inputs.CONFIGS[args.config])
+    m, n = cfg.m, cfg.n
+    cfg = cfg.with_shape(m, 3, n)
+    A = torch.from_numpy(inputs.generate(cfg, "A")).cuda()
+    l0 = md.md_launch_count()
+    rows = []
+    for i in range(args.warmup + args.steps):
+        Q, R, (total, in_gemm) = md.md_qr(A, want_times=True)
+        if i >= args.warmup:
+            rows.append((total, in_gemm))
+    launches = (md.md_launch_count() - l0) // (args.warmup + args.steps)
+    total = sum(r[0] for r in rows) / len(rows)
+    in_gemm = sum(r[1] for r in rows) / len(rows)
+    flops = 2 * (2.0 * m * n * n - 2.0 * n ** 3 / 3.0)
+    print(json.dumps({"impl": "ours", "mode": "qr", "metric": "md_qr: multiple-double GFLOP/s (4 m n^2 - 4 n^3 / 3 for R and Q)",
+                      "value": flops / total / 1e6, "unit": "GFLOP/s (multiple double)", "ms": total, "ms_in_md_gemm": in_gemm,
+                      "share_in_md_gemm": in_gemm / total, "launches_per_call": launches, "steps": args.steps, "warmup": args.warmup,
+                      "config": {"workload": f"{m} x {n} matrix A of BASELINE.json configs[{cfg.index}] ({cfg.name} recipe), limbs={cfg.limbs}, "
+                                             f"quarters={cfg.quarters}, panel width 32"}}))
 
 
 def run_ours(args):
@@ -643,6 +673,8 @@ def main():
         run_micro(args)
     elif args.balance_table:
         run_balance_table(args)
+    elif args.qr:
+        run_qr(args)
     else:
         run_ours(args)
 

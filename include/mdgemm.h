@@ -266,6 +266,28 @@ size_t md_literal_scratch_bytes(int m, int n, int k, int limbs, int planes_per_c
 md_status md_gemm_literal(int m, int n, int k, int limbs, const double* A_planes, const double* B_planes, double* C_planes,
                           void* scratch, size_t scratch_bytes, int flags, int32_t* info_host, md_stream stream);
 
+/* ---------------------------------------------------------------------------------------------------------------------
+ * md_qr -- blocked Householder QR of a multiple-double matrix on top of md_gemm: the application the paper announces.
+ *   PAPER.md:213 (conclusions): "Future work will apply this multiple double tensor core matrix multiplication to accelerate the
+ *   blocked Householder QR, extending [18]" (ref [18]: least squares on GPUs in multiple double precision).
+ *   A = Q R with A m x n (m >= n), Q m x n with orthonormal columns, R n x n upper triangular with diag(R) >= 0.
+ *   Panels of 32 columns are factored on the regular FP64 cores in multiple-double arithmetic (one cooperative launch per panel);
+ *   every trailing update and the accumulation of Q are products of limb-plane matrices through the SAME path as md_gemm
+ *   (split, fused quarter GEMM on the FP64 tensor pipe, renormalising epilogue; MD_OPT_QUARTERS / MD_OPT_ORDERS apply).
+ *   A_planes   in   [limbs][m][n]
+ *   Q_planes   out  [limbs][m][n]
+ *   R_planes   out  [limbs][n][n]
+ *   scratch    device, 256-byte aligned, md_qr_scratch_bytes(m, n, limbs) bytes, caller-owned (working copy of A, block reflectors,
+ *              compacted sub-matrices, the workspace of the products)
+ *   times_ms_host  HOST float[2] or NULL: when given the call records CUDA events, SYNCHRONISES `stream`, and stores the device
+ *              time of the whole factorisation and the part of it spent inside the md_gemm path (for bench.py)
+ *   limbs in {2, 4}.  Backward error: |A - Q R| and |Q^T Q - I| of the order n 2^-(52 limbs) (norm-wise; tests/test_gpu_qr.py).
+ *   Asynchronous unless times_ms_host is given; not capturable in a CUDA graph (cooperative launches).
+ * ------------------------------------------------------------------------------------------------------------------ */
+size_t md_qr_scratch_bytes(int m, int n, int limbs);
+md_status md_qr(int m, int n, int limbs, const double* A_planes, double* Q_planes, double* R_planes, void* scratch,
+                size_t scratch_bytes, float* times_ms_host, md_stream stream);
+
 /* Workspace for md_gemm / md_gemm_orders: quarter planes of A and B, exponent vectors and the status word, for the
  * CURRENT option values.  The caller allocates (device memory, 256-byte aligned) and registers it FOR THE CURRENT DEVICE; the
  * library keeps the pointer until it is replaced (ptr = NULL, bytes = 0 unregisters).  md_workspace_bytes returns 0 on bad

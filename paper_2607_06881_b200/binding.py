@@ -31,6 +31,8 @@ _SIGNATURES = {
     "md_split_literal": (_c.c_int, [_c.c_int] * 5 + [_c.c_void_p] * 4),
     "md_literal_scratch_bytes": (_c.c_size_t, [_c.c_int] * 6),
     "md_gemm_literal": (_c.c_int, [_c.c_int] * 4 + [_c.c_void_p] * 4 + [_c.c_size_t, _c.c_int, _c.c_void_p, _c.c_void_p]),
+    "md_qr_scratch_bytes": (_c.c_size_t, [_c.c_int] * 3),
+    "md_qr": (_c.c_int, [_c.c_int] * 3 + [_c.c_void_p] * 4 + [_c.c_size_t, _c.c_void_p, _c.c_void_p]),
     "md_plan_slices_chunked": (_c.c_int, [_c.c_int] * 3 + [_c.c_void_p] * 3),
     "md_split": (_c.c_int, [_c.c_int] * 5 + [_c.c_void_p] * 4),
     "md_qgemm": (_c.c_int, [_c.c_int] * 6 + [_c.c_void_p] * 5),
@@ -245,6 +247,22 @@ def md_gemm_literal(A: torch.Tensor, B: torch.Tensor, C: torch.Tensor | None = N
     _check(st, "md_gemm_literal")
     keys = ("zminA", "zmaxA", "zminB", "zmaxB", "planes", "orders", "pairs", "launches")
     return C, dict(zip(keys, (int(v) for v in info)))
+
+
+def md_qr(A: torch.Tensor, want_times: bool = False, stream=None):
+    """Blocked Householder QR on top of md_gemm (include/mdgemm.h): A [limbs, m, n] -> (Q [limbs, m, n], R [limbs, n, n]) with
+    diag(R) >= 0; with want_times also (total ms, ms inside the md_gemm path)."""
+    limbs, m, n = A.shape
+    Q = torch.empty((limbs, m, n), dtype=torch.float64, device=A.device)
+    R = torch.empty((limbs, n, n), dtype=torch.float64, device=A.device)
+    need = lib().md_qr_scratch_bytes(m, n, limbs)
+    if need == 0:
+        raise MdError(MD_ERR_UNSUPPORTED, "md_qr_scratch_bytes")
+    scratch = torch.empty(need, dtype=torch.uint8, device=A.device)
+    times = (ctypes.c_float * 2)()
+    _check(lib().md_qr(m, n, limbs, _dev(A), _dev(Q), _dev(R), _dev(scratch, torch.uint8), scratch.numel(),
+                       ctypes.addressof(times) if want_times else None, _stream(stream)), "md_qr")
+    return (Q, R, (float(times[0]), float(times[1]))) if want_times else (Q, R)
 
 
 def md_gemm_orders(A: torch.Tensor, B: torch.Tensor, stream=None) -> torch.Tensor:

@@ -80,16 +80,46 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
   const int dp_mine = plan.dp_waves - (cta >= plan.dp_tail ? 1 : 0);  // whole tiles of this CTA
   const int n_seg = n_sk + dp_mine;
   const int total_slabs = (g1 - g0) + dp_mine * KS;
+  // stream-K segment `i` of this CTA in slab order: tile, slab range [s0, s1)
+  auto sk_segment = [&](int i, int& tile, int& s0, int& s1) {
+    const int r = g0 / KS + i;
+    tile = plan.dp_waves * G + r;
+    s0 = i == 0 ? g0 - r * KS : 0;
+    s1 = min(KS, g1 - r * KS);
+  };
+  // Processing order.  Chunked kernel: the stream-K segments in slab order, then the whole tiles (partial sums meet in the
+  // scratch through red.add, R16).  Otherwise the HAND-OVER order: a tile that is cut along k is FINISHED by the CTA
+  // that owns its last slabs; every other contributor stores its partial sums to its own scratch slot and raises a flag.  A CTA
+  // has at most one segment that stops short of its tile's end (its last one in slab order: the HEAD of a tile) and at most one
+  // that finishes a tile begun elsewhere (its first one: a TAIL).  It runs the head FIRST and the tail LAST, so that (1) the
+  // partial sums a tail needs were written an entire run earlier -- the flag wait never spins in practice -- and (2) a CTA only
+  // ever waits for CTAs of LOWER index, none of which waits before raising its own flag: no deadlock even if the grid were not
+  // fully resident.  All sums are exact (R6), so the result is bit-identical to any other order.
+  bool has_head = false, has_tail = false;
+  if (!CHUNK && n_sk > 0) {
+    int t_, a_, b_;
+    sk_segment(n_sk - 1, t_, a_, b_);
+    has_head = b_ < KS;
+    sk_segment(0, t_, a_, b_);
+    has_tail = a_ > 0 && b_ == KS;
+  }
   auto segment = [&](int i, int& tile, int& s0, int& s1) {
-    if (i < n_sk) {
-      const int r = g0 / KS + i;
-      tile = plan.dp_waves * G + r;
-      s0 = i == 0 ? g0 - r * KS : 0;
-      s1 = min(KS, g1 - r * KS);
+    if constexpr (CHUNK) {
+      if (i < n_sk) sk_segment(i, tile, s0, s1);
+      else tile = (i - n_sk) * G + cta, s0 = 0, s1 = KS;
     } else {
-      tile = (i - n_sk) * G + cta;
-      s0 = 0;
-      s1 = KS;
+      if (has_head) {
+        if (i == 0) return sk_segment(n_sk - 1, tile, s0, s1);
+        i--;
+      }
+      if (i < dp_mine) {
+        tile = i * G + cta, s0 = 0, s1 = KS;
+        return;
+      }
+      i -= dp_mine;
+      const int mid = n_sk - (has_head ? 1 : 0) - (has_tail ? 1 : 0);
+      if (i < mid) return sk_segment((has_tail ? 1 : 0) + i, tile, s0, s1);
+      sk_segment(0, tile, s0, s1);
     }
   };
 
@@ -282,27 +312,31 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
       }
     } else if (c_s1 - c_s0 == KS) {  // whole tile in registers
       qgemm_epilogue<S, L, MT, NT>(acc, m, n, row_base, col_base, lane, order_planes, C_planes);
-    } else {                  // partial sums of a stream-K tile: exact fp64 reduction through the tile's scratch
-      const int r = c_tile - plan.dp_waves * G;
-      double* sc = sk_scratch + (size_t)r * (S * C::BM * C::BN) + (size_t)warp * (S * MT * NT * 64) + lane * 2;
+    } else if (c_s1 < KS) {   // the head (or a middle part) of a tile that another CTA finishes: hand the partial sums over
+      double* sc = sk_scratch + (size_t)cta * (S * C::BM * C::BN) + (size_t)warp * (S * MT * NT * 64) + lane * 2;
 #pragma unroll
       for (int s = 0; s < S; s++)
 #pragma unroll
         for (int i = 0; i < MT; i++)
 #pragma unroll
-          for (int j = 0; j < NT; j++) {
-            atomicAdd(sc + ((s * MT + i) * NT + j) * 64, acc[s][i][j][0]);
-            atomicAdd(sc + ((s * MT + i) * NT + j) * 64 + 1, acc[s][i][j][1]);
-          }
+          for (int j = 0; j < NT; j++)
+            __stcg(reinterpret_cast<double2*>(sc + ((s * MT + i) * NT + j) * 64), make_double2(acc[s][i][j][0], acc[s][i][j][1]));
       __threadfence();
       __syncthreads();
       if (tid == 0) {
-        const unsigned int mine = (unsigned int)(c_s1 - c_s0);
-        *last_flag = (atomicAdd(&sk_counters[r], mine) + mine == (unsigned int)KS);
-      }
-      __syncthreads();
-      if (*last_flag) {  // every slab of the tile has been added: read the totals back and finish the tile
         __threadfence();
+        atomicExch(&sk_counters[cta], 1u);  // the flag: this CTA's slot is complete
+      }
+    } else {                  // the tail of a tile: add what the CTAs before this one computed of it, then finish the tile
+      const int r = c_tile - plan.dp_waves * G;
+      const int first = (r * KS) / plan.sk_iters_per_cta;  // the CTA whose range holds the tile's first slab
+      for (int other = first; other < cta; other++) {
+        if (tid == 0) {
+          while (atomicAdd(&sk_counters[other], 0u) == 0u) __nanosleep(64);
+          __threadfence();
+        }
+        __syncthreads();
+        const double* sc = sk_scratch + (size_t)other * (S * C::BM * C::BN) + (size_t)warp * (S * MT * NT * 64) + lane * 2;
 #pragma unroll
         for (int s = 0; s < S; s++)
 #pragma unroll
@@ -310,11 +344,11 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
 #pragma unroll
             for (int j = 0; j < NT; j++) {
               const double2 v = __ldcg(reinterpret_cast<const double2*>(sc + ((s * MT + i) * NT + j) * 64));
-              acc[s][i][j][0] = v.x;
-              acc[s][i][j][1] = v.y;
+              acc[s][i][j][0] += v.x;  // exact: integers below 2^53 units (R6)
+              acc[s][i][j][1] += v.y;
             }
-        qgemm_epilogue<S, L, MT, NT>(acc, m, n, row_base, col_base, lane, order_planes, C_planes);
       }
+      qgemm_epilogue<S, L, MT, NT>(acc, m, n, row_base, col_base, lane, order_planes, C_planes);
     }
     zero_acc();
     if (++c_seg < n_seg) {
@@ -407,8 +441,8 @@ cudaError_t launch_cfg(int m, int n, int k, const double* Ap, const double* Bp, 
   unsigned int* counters = static_cast<unsigned int*>(sk_ws);
   double* scratch = reinterpret_cast<double*>(static_cast<char*>(sk_ws) + SK_COUNTER_BYTES);
   cudaError_t err;
-  if (plan.sk_tiles > 0) {  // counters and the scratch tiles in use start at zero (one contiguous region)
-    err = cudaMemsetAsync(sk_ws, 0, SK_COUNTER_BYTES + sizeof(double) * (size_t)plan.sk_tiles * C::S * C::BM * C::BN, stream);
+  if (plan.sk_tiles > 0) {  // the hand-over flags (one per CTA) start at zero; the scratch slots are written before they are read
+    err = cudaMemsetAsync(sk_ws, 0, SK_COUNTER_BYTES, stream);
     if (err != cudaSuccess) return err;
   }
   auto kern = qgemm_packed_kernel<C, false>;

@@ -161,9 +161,13 @@ __device__ __forceinline__ void k_step_range_rt(double (&acc)[S1 - S0][2], const
     const int lo = S0 - q > 0 ? S0 - q : 0;
     const int hi = S1 - 1 - q < QMAX - 1 ? S1 - 1 - q : QMAX - 1;
     const int pmax = min(Qr - 1, Sr - 1 - q);
+    // a BRANCH out of the live prefix, not a predicate per site: a predicated-off DMMA still takes its slot in the tensor pipe
+    // (measured: 83 % pipe-active at 38 % useful throughput with predication, profiles/r3d)
 #pragma unroll
-    for (int p = lo; p <= hi; p++)
-      if (p <= pmax) dmma_8x8x4(acc[p + q - S0], a[p % RW], b);
+    for (int p = lo; p <= hi; p++) {
+      if (p > pmax) break;
+      dmma_8x8x4(acc[p + q - S0], a[p % RW], b);
+    }
     b = b_next;
   }
 }
