@@ -476,7 +476,7 @@ def run_ours(args):
         plan_ms = (time.perf_counter() - t0) * 1e3
         md.md_set_option(md.MD_OPT_SLICE_BITS, 0)
         return {"spread_D": pd, "guaranteed_quarters": pq, "run_with": Q, "slice_bits": W, "ms": plan_ms,
-                "note": "smallest Q with k (Q+1) 2^(D - W Q - 2) <= the format's tolerance at every position "
+                "note": "smallest Q with k (Q+3) 2^(D - W Q - 2) <= the format's tolerance at every position "
                         "(worst case; measured errors are 2-3 orders of magnitude below the bound)"}
 
     quarter_plan = context_block(plan_block) if world == 1 and not args.lean else None

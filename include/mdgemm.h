@@ -174,12 +174,13 @@ md_status md_renorm(int m, int n, int limbs, int orders, const double* order_pla
  *   `limbs` limb planes.  Splits A by rows and B by columns into the registered workspace, then one fused kernel does
  *   the quarter products and writes the renormalised C once.  limbs in {2, 4, 8, 16} (double double, quad double, and the
  *   octo / hexa double of PAPER.md:196-205 Table 2).
- *   Accuracy: |C - A*B|_ij <= k (Q+1) 2^(E_i + F_j - 13Q - 2) + 2^-(53*limbs - 3) |C|_ij for any input (Q = quarters = orders;
+ *   Accuracy: |C - A*B|_ij <= k (Q+3) 2^(E_i + F_j - 13Q - 2) + 2^-(53*limbs - 3) |C|_ij for any input (Q = quarters = orders;
  *   E, F the exponent vectors of A's rows and B's columns).  THE BOUND IS RELATIVE TO 2^(E_i + F_j), NOT TO (|A||B|)_ij: on the
  *   BASELINE.json workloads it is within 1e-28 (|A||B|)_ij (double double; configs[3] with 9 quarters) and 1e-58 (quad
  *   double), but a row such as [2^60, 1 + 2^-70] loses the low limb of its small element -- no flag is raised; use
- *   md_plan_quarters / md_gemm_auto when the data is not known to be well scaled.  With orders S != Q the first term is
- *   k 2^(E_i + F_j - 2) [ 2^(1 - 13Q) + (2Q - 1 - S)+ 2^(-13S) ] (remainders of the split + dropped orders S..2Q-2).
+ *   md_plan_quarters / md_gemm_auto when the data is not known to be well scaled.  The Q + 3 units are: 2 + 2 from what the
+ *   split leaves of a and of b, Q - 1 from the dropped products of order Q.  With orders S > Q the last becomes
+ *   (2Q - 1 - S) 2^(-13 (S - Q)): about 4 units in all; with S < Q the bound is that of Q = S (R5).
  *   md_gemm_orders is the debug/parity variant: same split, then writes the order matrices C^(s) [orders][m][n] instead.
  * ------------------------------------------------------------------------------------------------------------------ */
 md_status md_gemm(int m, int n, int k, int limbs, const double* A_planes, const double* B_planes, double* C_planes,
@@ -190,10 +191,10 @@ md_status md_gemm_orders(int m, int n, int k, int limbs, const double* A_planes,
 /* ---------------------------------------------------------------------------------------------------------------------
  * md_plan_quarters -- how many quarters THIS data needs (R15; SURVEY.md 8(f) NEXT-1 "exponent-spread-driven quarter
  *   count").  With one exponent per row of A / column of B the error of md_gemm is bounded relative to 2^(E_i + F_j), not to
- *   (|A||B|)_ij (see md_gemm below): |C - A*B|_ij <= k (Q+1) 2^(E_i + F_j - W Q - 2) + renormalisation, W = slice width (13).
+ *   (|A||B|)_ij (see md_gemm below): |C - A*B|_ij <= k (Q+3) 2^(E_i + F_j - W Q - 2) + renormalisation, W = slice width (13).
  *   This call measures D = max over positions with (|A_0||B_0|)_ij > 0 of E_i + F_j - ilogb((|A_0||B_0|)_ij) -- the leading
  *   limb planes multiplied in plain fp64 on the same DMMA kernel, 1/36 of a double-double md_gemm -- and returns the
- *   smallest Q >= ceil(52 limbs / W) with k (Q+1) 2^(D - W Q - 2) <= rel_tol: with MD_OPT_QUARTERS = Q the first term of
+ *   smallest Q >= ceil(52 limbs / W) with k (Q+3) 2^(D - W Q - 2) <= rel_tol: with MD_OPT_QUARTERS = Q the first term of
  *   the bound is below rel_tol (|A||B|)_ij at EVERY position, for any input.  It is a worst-case guarantee (all dropped
  *   digit products at their bound with one sign); measured errors are 2-3 orders of magnitude below it.
  *   scratch        device, 256-byte aligned, md_plan_scratch_bytes(m, n, k) bytes (|A_0|, |B_0|, their product, exponents)

@@ -986,9 +986,9 @@ int oracle_num_threads(void) {
 // Planning the quarter count from the data (R15; SURVEY.md 8(f) NEXT-1 "exponent-spread-driven quarter count").
 //   With one exponent per row of A / column of B (R2) the error of the path is bounded relative to
 //   2^(E_i + F_j), not to (|A||B|)_ij (R5):
-//       |C - A*B|_ij <= k (Q+1) 2^(E_i + F_j - bits*Q - 2)  +  (renormalisation, 2^-(53 limbs - 1) |C|_ij).
+//       |C - A*B|_ij <= k (Q+3) 2^(E_i + F_j - bits*Q - 2)  +  (renormalisation, 2^-(53 limbs - 1) |C|_ij).
 //   The first term stays below rel_tol * W_ij, W = |A||B|, at every position iff
-//       k (Q+1) 2^(D - bits*Q - 2) <= rel_tol,     D >= log2 max_ij 2^(E_i + F_j) / W_ij.
+//       k (Q+3) 2^(D - bits*Q - 2) <= rel_tol,     D >= log2 max_ij 2^(E_i + F_j) / W_ij.
 //   Plain definition, written out: W~_ij = sum_k |A_0[i,k]| |B_0[k,j]| on the leading limbs in fp64 (k innermost),
 //   D = max over positions with W~_ij > 0 of E_i + F_j - ilogb(W~_ij) (an integer upper bound of the log2 above), and
 //   Q = the smallest Q >= ceil(52 limbs / bits) that satisfies the inequality.  Positions with W~_ij = 0 have C_ij = 0
@@ -1020,8 +1020,8 @@ int oracle_plan_quarters(int m, int n, int k, int limbs, int bits, const double*
   if (spread_out) *spread_out = D;
   int Q = (52 * limbs + bits - 1) / bits;
   if (D == INT32_MIN) return Q;
-  // k (Q+1) 2^(D - bits*Q - 2) <= rel_tol: the left side is exact in fp64 (an integer below 2^53 times a power of two)
-  while (Q < 4096 && std::ldexp((double)k * (Q + 1), D - bits * Q - 2) > rel_tol) Q++;
+  // k (Q+3) 2^(D - bits*Q - 2) <= rel_tol: the left side is exact in fp64 (an integer below 2^53 times a power of two)
+  while (Q < 4096 && std::ldexp((double)k * (Q + 3), D - bits * Q - 2) > rel_tol) Q++;
   return Q;
 }
 

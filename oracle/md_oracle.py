@@ -175,7 +175,7 @@ def md_gemm_rows(A, B, row0: int = 0, row1: int | None = None, quarters: int | N
 
 
 def plan_quarters(A, B, rel_tol: float, bits: int = 13):
-    """DESIGN.md R15: the smallest quarter count whose error bound k (Q+1) 2^(E_i+F_j-bits Q-2) stays below
+    """DESIGN.md R15: the smallest quarter count whose error bound k (Q+3) 2^(E_i+F_j-bits Q-2) stays below
     rel_tol (|A||B|)_ij at every position.  Returns (Q, D), D = max_ij E_i + F_j - ilogb((|A_0||B_0|)_ij)."""
     A, B = _f64(A), _f64(B)
     limbs, m, k = A.shape

@@ -490,10 +490,10 @@ md_status md_plan_quarters(int m, int n, int k, int limbs, const double* A_plane
   if (err == cudaSuccess) err = cudaMemcpyAsync(&D, spread, sizeof(D), cudaMemcpyDeviceToHost, st);
   if (err != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) return MD_ERR_CUDA;
   if (spread_out) *spread_out = D;
-  // the smallest Q >= ceil(52 limbs / W) with k (Q+1) 2^(D - W Q - 2) <= rel_tol (R15; the left side is exact)
+  // the smallest Q >= ceil(52 limbs / W) with k (Q+3) 2^(D - W Q - 2) <= rel_tol (R15; the left side is exact)
   int Q = (52 * limbs + W - 1) / W;
   if (D != INT32_MIN)
-    while (Q < 4096 && ldexp((double)k * (Q + 1), D - W * Q - 2) > rel_tol) Q++;
+    while (Q < 4096 && ldexp((double)k * (Q + 3), D - W * Q - 2) > rel_tol) Q++;
   *quarters_out = Q;
   return MD_OK;
 }

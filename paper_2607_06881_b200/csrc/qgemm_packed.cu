@@ -15,7 +15,7 @@
 //     __syncthreads, so the two warps of an SM sub-partition drift apart and one's LDS / barrier latency hides behind
 //     the other's DMMA stream.  The refill of a stage is issued two slabs after its last read, when its empty barrier
 //     has long completed, so the issuing thread never actually waits.
-// The r01 ncu capture of the cp.async kernel (profiles/r01_qgemm_ncu.md) showed exactly these three costs as the gap
+// The first ncu capture of the cp.async kernel of qgemm.cu (round 1) showed exactly these three costs as the gap
 // between 88 % and the DMMA peak.
 //
 // Exactness (eq. 5; R6): quarters are integers |D| <= 2^13 times the group unit and

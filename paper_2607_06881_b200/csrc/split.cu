@@ -134,7 +134,7 @@ __global__ void __launch_bounds__(256) split_kernel(size_t rows, size_t cols, in
 
 // 256-bit global accesses (sm_100: LDG.E.ENL2.256 / STG.E.ENL2.256); p must be 32-byte aligned.  A fragment row of the
 // packed layout is 4 doubles, so one store per quarter per thread fills whole 32-byte sectors (two 16-byte stores at a
-// 32-byte lane stride half-fill 32 sectors each and made the kernel L1-bound: profiles/r01c_split_ncu.md).
+// 32-byte lane stride half-fill 32 sectors each and made the kernel L1-bound at 0.55 of the HBM peak in an earlier capture).
 __device__ __forceinline__ void ldg_256(const double* p, double& a, double& b, double& c, double& d) {
   asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
 }

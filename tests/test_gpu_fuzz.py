@@ -67,7 +67,7 @@ def test_random_case(case):
     r = orc.exact_all(A, B, Cn)
     # the any-input bound (R5) always; the tolerance relative to (|A||B|)_ij wherever the data-driven plan
     # (R15) says this slice count guarantees it, and for the well-scaled distributions regardless
-    bound = k * (Q + 1) * np.ldexp(1.0, (eA[:, None] + eB[None, :] - W * Q - 2).astype(np.int32))
+    bound = k * (Q + 3) * np.ldexp(1.0, (eA[:, None] + eB[None, :] - W * Q - 2).astype(np.int32))
     assert (r["err"] <= bound + np.abs(Cn[0]) * 2.0 ** (-53 * L + 1)).all()
     Q_needed, _ = orc.plan_quarters(A, B, TOL[L], bits=W)
     if Q >= Q_needed or cfg.dist in ("uniform", "normal"):

@@ -179,14 +179,14 @@ def test_gemm_within_stated_tolerance_of_exact_product(cfg_idx, shape):
 @pytest.mark.parametrize("cfg_idx,Q", [(0, 8), (3, 8), (3, 9), (3, 10), (4, 16)])
 def test_gemm_error_bound_relative_to_group_exponents(cfg_idx, Q):
     """The guarantee for ANY input (include/mdgemm.h md_gemm; R5):
-    |C - A*B|_ij <= k (Q+1) 2^(E_i+F_j-13Q-2) + 2^-(53L-1) |C|_ij."""
+    |C - A*B|_ij <= k (Q+3) 2^(E_i+F_j-13Q-2) + 2^-(53L-1) |C|_ij."""
     cfg, A, B = gen(cfg_idx, 64, 64, 64)
     with md.Workspace(cfg.m, cfg.n, cfg.k, cfg.limbs, Q):
         C = host(md.md_gemm(dev(A), dev(B)))
     _, eA, _ = orc.split(A, 0)
     _, eB, _ = orc.split(B, 1)
     r = orc.exact_all(A, B, C)
-    bound = cfg.k * (Q + 1) * np.ldexp(1.0, (eA[:, None] + eB[None, :] - 13 * Q - 2).astype(np.int32))
+    bound = cfg.k * (Q + 3) * np.ldexp(1.0, (eA[:, None] + eB[None, :] - 13 * Q - 2).astype(np.int32))
     assert (r["err"] <= bound + np.abs(C[0]) * 2.0 ** (-53 * cfg.limbs + 1)).all()
 
 

@@ -20,7 +20,7 @@ def dev(x):
 
 def smallest_Q(k, limbs, bits, D, tol):
     Q = -(-(52 * limbs) // bits)
-    while k * (Q + 1) * 2.0 ** (D - bits * Q - 2) > tol:
+    while k * (Q + 3) * 2.0 ** (D - bits * Q - 2) > tol:
         Q += 1
     return Q
 

@@ -59,7 +59,7 @@ def test_orders_bit_exact_and_C_within_tolerance(cfg_idx, bits, Q, shape):
         # the 2^[-30,30] element range at a SMALL k makes (|A||B|)_ij << 2^(E_i+F_j) common; there the common-exponent
         # reading guarantees the any-input bound (R5 with W in place of 13).  The full-size config 3 is held to
         # 1e-28 (|A||B|)_ij below.
-        bound = cfg.k * (Q + 1) * np.ldexp(1.0, (eA[:, None] + eB[None, :] - bits * Q - 2).astype(np.int32))
+        bound = cfg.k * (Q + 3) * np.ldexp(1.0, (eA[:, None] + eB[None, :] - bits * Q - 2).astype(np.int32))
         assert (r["err"] <= bound + np.abs(Ch[0]) * 2.0 ** (-53 * cfg.limbs + 1)).all()
     else:
         assert (r["err"] <= TOL[cfg.limbs] * r["W"]).all()

@@ -1,7 +1,7 @@
 """Pins for the oracle's data-driven quarter count (oracle_plan_quarters; R15, SURVEY.md 8(f) NEXT-1
 "exponent-spread-driven quarter count").
 
-Pinned against: exact rational arithmetic (W = |A_0||B_0| and the inequality k (Q+1) 2^(D - bits Q - 2) <= rel_tol restated
+Pinned against: exact rational arithmetic (W = |A_0||B_0| and the inequality k (Q+3) 2^(D - bits Q - 2) <= rel_tol restated
 with Fractions), math.frexp for the exponents, closed-form special cases, the invariance of D under row / column scaling by
 powers of two, and -- what the plan is FOR -- the exact product: with the planned Q the five-step pipeline is within
 rel_tol (|A||B|)_ij at every position of an input on which the paper's count (8) is not."""
@@ -42,7 +42,7 @@ def exact_spread(A0, B0):
 
 def smallest_Q(k, limbs, bits, D, rel_tol):
     Q = -(-(52 * limbs) // bits)
-    while Fraction(k * (Q + 1)) * Fraction(2) ** (D - bits * Q - 2) > Fraction(rel_tol):
+    while Fraction(k * (Q + 3)) * Fraction(2) ** (D - bits * Q - 2) > Fraction(rel_tol):
         Q += 1
     return Q
 
@@ -97,5 +97,5 @@ def test_planned_count_delivers_the_tolerance_where_the_papers_count_does_not():
     _, eA, _ = orc.split(A, 0)
     _, eB, _ = orc.split(B, 1)
     for QQ, r in ((8, r8), (Q, rq)):
-        bound = cfg.k * (QQ + 1) * np.ldexp(1.0, (eA[:, None] + eB[None, :] - 13 * QQ - 2).astype(np.int32))
+        bound = cfg.k * (QQ + 3) * np.ldexp(1.0, (eA[:, None] + eB[None, :] - 13 * QQ - 2).astype(np.int32))
         assert (r["err"] <= bound + 2.0 ** -105 * r["W"]).all()

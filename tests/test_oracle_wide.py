@@ -126,7 +126,7 @@ def test_five_step_pipeline_reaches_the_derived_tolerance(cfg_idx, shape):
     _, eA, _ = orc.split(A, 0)
     _, eB, _ = orc.split(B, 1)
     Q = cfg.quarters  # the any-input bound of DESIGN.md R5
-    bound = cfg.k * (Q + 1) * np.ldexp(1.0, (eA[:, None] + eB[None, :] - 13 * Q - 2).astype(np.int32))
+    bound = cfg.k * (Q + 3) * np.ldexp(1.0, (eA[:, None] + eB[None, :] - 13 * Q - 2).astype(np.int32))
     assert (r["err"] <= bound + np.abs(C[0]) * 2.0 ** (-53 * cfg.limbs + 1)).all()
     for l in range(cfg.limbs - 1):
         assert (np.abs(C[l + 1]) <= np.spacing(np.abs(C[l])) / 2).all()
