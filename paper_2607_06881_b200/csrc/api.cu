@@ -130,6 +130,21 @@ static inline bool use_fused_prep(int m, int n, int k) {
   return ((long long)m + n) * k <= (1ll << 23);
 }
 
+// The whole path in ONE launch (fused_small.cu): where the 32 x 16 tiles of C number at most the SMs, so that a tile per CTA
+// (times the k-runs of its cluster) is a single wave, and a CTA's run of the contraction is short (at most 16 k-slabs: the CTA
+// splits its own operand slabs, which costs about 0.6 of the DMMA time of the slab -- measured: faster than prepare + multiply
+// up to 192^3, equal at 256^3, slower beyond).
+constexpr int ONE_LAUNCH_MAX_SLABS = 16;
+static bool use_one_launch(int m, int n, int k, int limbs, int Q, int S, int bits) {
+  if (g_opt.one_launch == 2 || !fused_small_supported(limbs, Q, S) || chunk_for(k, limbs, Q, S, bits) > 0) return false;
+  if (g_opt.one_launch == 1) return true;
+  const long long tiles = (((long long)m + 31) / 32) * (((long long)n + 15) / 16);
+  const int G = sk_grid();
+  if (G <= 0 || tiles > G) return false;
+  const int KS = (k + 7) / 8;
+  return (KS + fused_small_cluster(m, n, k) - 1) / fused_small_cluster(m, n, k) <= ONE_LAUNCH_MAX_SLABS;
+}
+
 // the fused quarter GEMM of one (block of a) problem on packed operands
 cudaError_t launch_fused(int m, int n, int k, int limbs, int Q, int S, const KernelPick& pick, const double* Aq, const double* Bq,
                          double* order_planes, double* C_planes, void* sk, cudaStream_t stream, uint64_t* launches) {
@@ -158,6 +173,20 @@ md_status gemm_impl(int m, int n, int k, int limbs, int Q, int S, const double* 
   cudaEvent_t* ev = (ds && ds->prof_count < ds->prof_capacity) ? &ds->prof_ev[3 * (size_t)ds->prof_count] : nullptr;
   if (ev) cudaEventRecord(ev[0], stream);
   cudaError_t err = cudaErrorUnknown;
+  if (allow_small && use_one_launch(m, n, k, limbs, Q, S, W)) {  // a1-a4 in one kernel, no quarter planes in HBM
+    if (ev) cudaEventRecord(ev[1], stream);
+    err = launch_fused_small(m, n, k, limbs, Q, S, W, A, B, order_planes, C_planes, c.flags, stream, &launches);
+    if (err == cudaSuccess) {
+      if (ev) {
+        cudaEventRecord(ev[2], stream);
+        ds->prof_count++;
+      }
+      g_launches += launches;
+      return MD_OK;
+    }
+    cudaGetLastError();  // a cluster launch the context cannot take: the two-launch path does the same work
+    err = cudaErrorUnknown;
+  }
   if (use_fused_prep(m, n, k)) {  // one launch instead of five: what matters below ~2048^3
     err = launch_prep_packed(m, n, k, limbs, Q, W, pick.bxA, pick.bxB, pick.bk, A, B, c.Aq, c.Bq, c.expA, c.expB, c.flags, stream, &launches);
     if (err != cudaSuccess) cudaGetLastError();  // a cooperative launch the context cannot take: the separate kernels do the same
@@ -258,6 +287,10 @@ md_status md_set_option(int key, int value) {
       if (value < 0 || value > 2) return MD_ERR_BAD_ARG;
       g_opt.fused_prep = value;
       return MD_OK;
+    case MD_OPT_ONE_LAUNCH:
+      if (value < 0 || value > 2) return MD_ERR_BAD_ARG;
+      g_opt.one_launch = value;
+      return MD_OK;
     case MD_OPT_HOST_BLOCKS:  // 0 = automatic, 1..32 blocks, or PR * 256 + PC (explicit panel counts, each <= 64)
       if (value < 0 || (value > 32 && (value < 256 || (value >> 8) > 64 || (value & 255) > 64))) return MD_ERR_BAD_ARG;
       g_opt.host_blocks = value;
@@ -286,6 +319,7 @@ int md_get_option(int key) {
     case MD_OPT_HOST_BLOCKS: return g_opt.host_blocks;
     case MD_OPT_K_CHUNK: return g_opt.k_chunk;
     case MD_OPT_FUSED_PREP: return g_opt.fused_prep;
+    case MD_OPT_ONE_LAUNCH: return g_opt.one_launch;
     case MD_OPT_TILE: return g_opt.tile;
     case MD_OPT_RASTER_GROUP: return g_opt.raster_group;
     default: return -1;

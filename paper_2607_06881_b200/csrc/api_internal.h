@@ -19,6 +19,7 @@ struct Options {
   int bits = 0;          // 0 = 13, the paper's quarter
   int tile = 0;          // 0 = automatic, 1 = the 32 x 16 tile instance wherever it exists, 2 = never
   int fused_prep = 0;    // 0 = automatic (small / medium operands), 1 = always, 2 = never
+  int one_launch = 0;    // 0 = automatic (single-wave problems), 1 = wherever the kernel exists, 2 = never
   int k_chunk = 0;       // 0 = chunked accumulation only when k exceeds the exactness budget; else the chunk length to force
   int host_blocks = 0;   // md_gemm_host: 0 = automatic panel plan, else the number of blocks of C (1 = no pipelining)
   int raster_group = 0;  // tile rows per raster group of the fused GEMM (0 = default 8)

@@ -155,7 +155,10 @@ int mdc_topdown_gemm(int m, int n, int k, int limbs, int quarters, const double*
   if (s1 != MD_OK) return s1;
   mark(1);
   // step 2 (eq. 4): store the convoluted A
-  build_atil_kernel<<<148 * 16, 256, 0, st>>>(m, k, Q, c.Aq, c.Atil);
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
+    return MD_ERR_CUDA;
+  build_atil_kernel<<<sms * 16, 256, 0, st>>>(m, k, Q, c.Aq, c.Atil);
   if (cudaGetLastError() != cudaSuccess) return MD_ERR_CUDA;
   mark(2);
   // step 3: one plain double-precision GEMM.  Row-major Cbar (Qm x n) = Atil (Qm x Qk) * Bstk (Qk x n) is the

@@ -54,6 +54,11 @@ inline bool sk_chunk_scratch_fits(size_t nchunks, int S, int BM, int BN) {
 }
 size_t sk_workspace_bytes(int orders, int bxA, int bxB, int k, int chunk);
 int sk_grid();
+// fused_small.cu: steps a1-a4 in one launch for single-wave problems (quarter planes only in shared memory)
+bool fused_small_supported(int limbs, int quarters, int orders);
+int fused_small_cluster(int m, int n, int k);
+cudaError_t launch_fused_small(int m, int n, int k, int limbs, int quarters, int orders, int bits, const double* A, const double* B,
+                               double* order_planes, double* C_planes, uint32_t* flags, cudaStream_t stream, uint64_t* launches);
 // chunk = 0: exact orders over the whole k.  chunk > 0 (R16; a multiple of 8, qgemm_chunk_supported instances
 // only, C_planes only): the accumulators are folded into the elements' expansions every `chunk` contraction indices.
 bool qgemm_chunk_supported(int limbs, int quarters);

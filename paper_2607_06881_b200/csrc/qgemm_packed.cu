@@ -58,7 +58,13 @@ struct PCfg {
 // tile's scratch (exact, like the unchunked stream-K: the total of a chunk is within the budget whoever contributes), and
 // the CTA that completes the slab count runs the same renorm_add sequence over the chunks' totals -- so the result is
 // bit-identical to a whole-tile run whatever the split.  No order planes (the order sums of the whole k are not doubles).
-template <class C, bool CHUNK>
+// HANDOVER: how the CTAs that share a stream-K tile combine their partial order sums (both exact, R6, hence the same
+// bits): false -- fp64 red.global.add into the tile's zeroed scratch, whoever completes the slab count re-reads the totals and
+// runs the epilogue, nobody waits (large problems: the stream-K tail is one wave in dozens); true -- per-CTA slots and flags, the
+// CTA that owns a tile's last slabs collects the others' sums (small problems, where every tile is cut and 16 KB of atomics per
+// warp through L2 were the critical path: 256^3 0.55 -> 0.66, 512^3 0.88 -> 0.92 of the peak).  Two instantiations rather than
+// one: at 254 registers the DMMA loop's schedule is sensitive to the code around it.
+template <class C, bool CHUNK, bool HANDOVER = false>
 __global__ void __launch_bounds__(C::THREADS, 1)
 qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, const double* __restrict__ Bp,
                     double* __restrict__ order_planes, double* __restrict__ C_planes, double* __restrict__ sk_scratch,
@@ -80,46 +86,51 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
   const int dp_mine = plan.dp_waves - (cta >= plan.dp_tail ? 1 : 0);  // whole tiles of this CTA
   const int n_seg = n_sk + dp_mine;
   const int total_slabs = (g1 - g0) + dp_mine * KS;
-  // stream-K segment `i` of this CTA in slab order: tile, slab range [s0, s1)
-  auto sk_segment = [&](int i, int& tile, int& s0, int& s1) {
-    const int r = g0 / KS + i;
-    tile = plan.dp_waves * G + r;
-    s0 = i == 0 ? g0 - r * KS : 0;
-    s1 = min(KS, g1 - r * KS);
-  };
-  // Processing order.  Chunked kernel: the stream-K segments in slab order, then the whole tiles (partial sums meet in the
-  // scratch through red.add, R16).  Otherwise the HAND-OVER order: a tile that is cut along k is FINISHED by the CTA
-  // that owns its last slabs; every other contributor stores its partial sums to its own scratch slot and raises a flag.  A CTA
-  // has at most one segment that stops short of its tile's end (its last one in slab order: the HEAD of a tile) and at most one
-  // that finishes a tile begun elsewhere (its first one: a TAIL).  It runs the head FIRST and the tail LAST, so that (1) the
-  // partial sums a tail needs were written an entire run earlier -- the flag wait never spins in practice -- and (2) a CTA only
-  // ever waits for CTAs of LOWER index, none of which waits before raising its own flag: no deadlock even if the grid were not
-  // fully resident.  All sums are exact (R6), so the result is bit-identical to any other order.
-  bool has_head = false, has_tail = false;
-  if (!CHUNK && n_sk > 0) {
-    int t_, a_, b_;
-    sk_segment(n_sk - 1, t_, a_, b_);
-    has_head = b_ < KS;
-    sk_segment(0, t_, a_, b_);
-    has_tail = a_ > 0 && b_ == KS;
+  // Segment list.  Without hand-over: the stream-K segments in slab order, then the whole tiles.
+  // With hand-over: a CTA's share of stream-K slabs is at most one tile long (sk_tiles < G), so it has at most TWO stream-K
+  // segments -- in slab order the TAIL of a tile begun by the CTAs before it (it ends at the tile's last slab) and / or the HEAD
+  // (or a middle part) of a tile that a later CTA finishes.  Thread 0 writes them to shared memory in PROCESSING order: head,
+  // whole tiles, tail.  A tile that is cut along k is FINISHED by the CTA that owns its last slabs; every other contributor
+  // stores its partial sums to its own scratch slot and raises a flag.  Running the head first and the tail last means (1) the
+  // partial sums a tail needs were written long before it asks for them -- the flag wait rarely spins -- and (2) a CTA only ever
+  // waits for CTAs of LOWER index, none of which waits before raising its own flag: no deadlock even if the grid were not fully
+  // resident.
+  __shared__ int sk_tab[8];  // HANDOVER: [0..2], [3..5] = tile, s0, s1 of the stream-K segments in processing order; [6] = 1 if the first is a head
+  if constexpr (HANDOVER) {
+    if (tid == 0) {
+      int seg[2][3] = {{0, 0, 0}, {0, 0, 0}};
+      for (int i = 0; i < n_sk && i < 2; i++) {
+        const int r = g0 / KS + i;
+        seg[i][0] = plan.dp_waves * G + r;
+        seg[i][1] = i == 0 ? g0 - r * KS : 0;
+        seg[i][2] = min(KS, g1 - r * KS);
+      }
+      const bool swap = n_sk == 2;  // the head is the last one in slab order
+#pragma unroll
+      for (int e = 0; e < 3; e++) sk_tab[e] = seg[swap ? 1 : 0][e], sk_tab[3 + e] = seg[swap ? 0 : 1][e];
+      sk_tab[6] = (n_sk > 0 && sk_tab[2] < KS) ? 1 : 0;
+    }
   }
   auto segment = [&](int i, int& tile, int& s0, int& s1) {
-    if constexpr (CHUNK) {
-      if (i < n_sk) sk_segment(i, tile, s0, s1);
-      else tile = (i - n_sk) * G + cta, s0 = 0, s1 = KS;
-    } else {
-      if (has_head) {
-        if (i == 0) return sk_segment(n_sk - 1, tile, s0, s1);
-        i--;
-      }
-      if (i < dp_mine) {
-        tile = i * G + cta, s0 = 0, s1 = KS;
+    if constexpr (HANDOVER) {
+      const int pre = sk_tab[6];  // the whole tiles come after the head
+      if (i >= pre && i < pre + dp_mine) {
+        tile = (i - pre) * G + cta, s0 = 0, s1 = KS;
         return;
       }
-      i -= dp_mine;
-      const int mid = n_sk - (has_head ? 1 : 0) - (has_tail ? 1 : 0);
-      if (i < mid) return sk_segment((has_tail ? 1 : 0) + i, tile, s0, s1);
-      sk_segment(0, tile, s0, s1);
+      if (i >= pre) i -= dp_mine;
+      tile = sk_tab[3 * i], s0 = sk_tab[3 * i + 1], s1 = sk_tab[3 * i + 2];
+    } else {
+      if (i < n_sk) {
+        const int r = g0 / KS + i;
+        tile = plan.dp_waves * G + r;
+        s0 = i == 0 ? g0 - r * KS : 0;
+        s1 = min(KS, g1 - r * KS);
+      } else {
+        tile = (i - n_sk) * G + cta;
+        s0 = 0;
+        s1 = KS;
+      }
     }
   };
 
@@ -312,31 +323,27 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
       }
     } else if (c_s1 - c_s0 == KS) {  // whole tile in registers
       qgemm_epilogue<S, L, MT, NT>(acc, m, n, row_base, col_base, lane, order_planes, C_planes);
-    } else if (c_s1 < KS) {   // the head (or a middle part) of a tile that another CTA finishes: hand the partial sums over
-      double* sc = sk_scratch + (size_t)cta * (S * C::BM * C::BN) + (size_t)warp * (S * MT * NT * 64) + lane * 2;
+    } else if constexpr (!HANDOVER) {  // partial sums of a stream-K tile: exact fp64 reduction through the tile's scratch
+      const int r = c_tile - plan.dp_waves * G;
+      double* sc = sk_scratch + (size_t)r * (S * C::BM * C::BN) + (size_t)warp * (S * MT * NT * 64) + lane * 2;
 #pragma unroll
       for (int s = 0; s < S; s++)
 #pragma unroll
         for (int i = 0; i < MT; i++)
 #pragma unroll
-          for (int j = 0; j < NT; j++)
-            __stcg(reinterpret_cast<double2*>(sc + ((s * MT + i) * NT + j) * 64), make_double2(acc[s][i][j][0], acc[s][i][j][1]));
+          for (int j = 0; j < NT; j++) {
+            atomicAdd(sc + ((s * MT + i) * NT + j) * 64, acc[s][i][j][0]);
+            atomicAdd(sc + ((s * MT + i) * NT + j) * 64 + 1, acc[s][i][j][1]);
+          }
       __threadfence();
       __syncthreads();
       if (tid == 0) {
-        __threadfence();
-        atomicExch(&sk_counters[cta], 1u);  // the flag: this CTA's slot is complete
+        const unsigned int mine = (unsigned int)(c_s1 - c_s0);
+        *last_flag = (atomicAdd(&sk_counters[r], mine) + mine == (unsigned int)KS);
       }
-    } else {                  // the tail of a tile: add what the CTAs before this one computed of it, then finish the tile
-      const int r = c_tile - plan.dp_waves * G;
-      const int first = (r * KS) / plan.sk_iters_per_cta;  // the CTA whose range holds the tile's first slab
-      for (int other = first; other < cta; other++) {
-        if (tid == 0) {
-          while (atomicAdd(&sk_counters[other], 0u) == 0u) __nanosleep(64);
-          __threadfence();
-        }
-        __syncthreads();
-        const double* sc = sk_scratch + (size_t)other * (S * C::BM * C::BN) + (size_t)warp * (S * MT * NT * 64) + lane * 2;
+      __syncthreads();
+      if (*last_flag) {  // every slab of the tile has been added: read the totals back and finish the tile
+        __threadfence();
 #pragma unroll
         for (int s = 0; s < S; s++)
 #pragma unroll
@@ -344,11 +351,50 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
 #pragma unroll
             for (int j = 0; j < NT; j++) {
               const double2 v = __ldcg(reinterpret_cast<const double2*>(sc + ((s * MT + i) * NT + j) * 64));
-              acc[s][i][j][0] += v.x;  // exact: integers below 2^53 units (R6)
-              acc[s][i][j][1] += v.y;
+              acc[s][i][j][0] = v.x;
+              acc[s][i][j][1] = v.y;
             }
+        qgemm_epilogue<S, L, MT, NT>(acc, m, n, row_base, col_base, lane, order_planes, C_planes);
       }
-      qgemm_epilogue<S, L, MT, NT>(acc, m, n, row_base, col_base, lane, order_planes, C_planes);
+    } else {
+      if (c_s1 < KS) {   // the head (or a middle part) of a tile that another CTA finishes: hand the partial sums over
+        double* sc = sk_scratch + (size_t)cta * (S * C::BM * C::BN) + (size_t)warp * (S * MT * NT * 64) + lane * 2;
+#pragma unroll
+        for (int s = 0; s < S; s++)
+#pragma unroll
+          for (int i = 0; i < MT; i++)
+#pragma unroll
+            for (int j = 0; j < NT; j++)
+              __stcg(reinterpret_cast<double2*>(sc + ((s * MT + i) * NT + j) * 64), make_double2(acc[s][i][j][0], acc[s][i][j][1]));
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) {
+          __threadfence();
+          atomicExch(&sk_counters[cta], 1u);  // the flag: this CTA's slot is complete
+        }
+      } else {                  // the tail of a tile: add what the CTAs before this one computed of it, then finish the tile
+        const int r = c_tile - plan.dp_waves * G;
+        const int first = (r * KS) / plan.sk_iters_per_cta;  // the CTA whose range holds the tile's first slab
+        for (int other = first; other < cta; other++) {
+          if (tid == 0) {
+            while (atomicAdd(&sk_counters[other], 0u) == 0u) __nanosleep(64);
+            __threadfence();
+          }
+          __syncthreads();
+          const double* sc = sk_scratch + (size_t)other * (S * C::BM * C::BN) + (size_t)warp * (S * MT * NT * 64) + lane * 2;
+#pragma unroll
+          for (int s = 0; s < S; s++)
+#pragma unroll
+            for (int i = 0; i < MT; i++)
+#pragma unroll
+              for (int j = 0; j < NT; j++) {
+                const double2 v = __ldcg(reinterpret_cast<const double2*>(sc + ((s * MT + i) * NT + j) * 64));
+                acc[s][i][j][0] += v.x;  // exact: integers below 2^53 units (R6)
+                acc[s][i][j][1] += v.y;
+              }
+        }
+        qgemm_epilogue<S, L, MT, NT>(acc, m, n, row_base, col_base, lane, order_planes, C_planes);
+      }
     }
     zero_acc();
     if (++c_seg < n_seg) {
@@ -426,6 +472,8 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
   }
 }
 
+constexpr int HANDOVER_MAX_WAVES = 8;  // whole-tile waves from which the stream-K tail goes through red.add (launch_cfg)
+
 // Exact orders over the whole k, persistent stream-K.
 template <class C>
 cudaError_t launch_cfg(int m, int n, int k, const double* Ap, const double* Bp, double* order_planes, double* C_planes,
@@ -441,19 +489,36 @@ cudaError_t launch_cfg(int m, int n, int k, const double* Ap, const double* Bp, 
   unsigned int* counters = static_cast<unsigned int*>(sk_ws);
   double* scratch = reinterpret_cast<double*>(static_cast<char*>(sk_ws) + SK_COUNTER_BYTES);
   cudaError_t err;
-  if (plan.sk_tiles > 0) {  // the hand-over flags (one per CTA) start at zero; the scratch slots are written before they are read
-    err = cudaMemsetAsync(sk_ws, 0, SK_COUNTER_BYTES, stream);
+  // hand-over between the CTAs of a stream-K tile while every tile is cut (small problems); fp64 red.add into the tile's scratch
+  // once whole-tile waves dominate (measured: 512^3 0.88 -> 0.92 with, dd 4096^3 134.65 against 134.88 ms without)
+  const bool handover = plan.dp_waves < HANDOVER_MAX_WAVES;
+  if (plan.sk_tiles > 0) {  // hand-over: the flags (one per CTA) start at zero, the slots are written before they are read;
+                            // red.add: counters and the scratch tiles in use start at zero (one contiguous region)
+    const size_t bytes = handover ? (size_t)SK_COUNTER_BYTES
+                                  : SK_COUNTER_BYTES + sizeof(double) * (size_t)plan.sk_tiles * C::S * C::BM * C::BN;
+    err = cudaMemsetAsync(sk_ws, 0, bytes, stream);
     if (err != cudaSuccess) return err;
   }
-  auto kern = qgemm_packed_kernel<C, false>;
-  static bool attr_done[MD_MAX_DEVICES] = {};  // the shared-memory opt-in is per function and device: once, not per launch
+  static bool attr_done[MD_MAX_DEVICES][2] = {};  // the shared-memory opt-in is per function and device: once, not per launch
   const int dev = current_device();
-  if (dev < 0 || dev >= MD_MAX_DEVICES || !attr_done[dev]) {
-    err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
-    if (err != cudaSuccess) return err;
-    if (dev >= 0 && dev < MD_MAX_DEVICES) attr_done[dev] = true;
+  const bool known = dev >= 0 && dev < MD_MAX_DEVICES;
+  if (handover) {
+    auto kern = qgemm_packed_kernel<C, false, true>;
+    if (!known || !attr_done[dev][1]) {
+      err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+      if (err != cudaSuccess) return err;
+      if (known) attr_done[dev][1] = true;
+    }
+    kern<<<G, C::THREADS, C::SMEM_BYTES, stream>>>(m, n, plan, Ap, Bp, order_planes, C_planes, scratch, counters);
+  } else {
+    auto kern = qgemm_packed_kernel<C, false, false>;
+    if (!known || !attr_done[dev][0]) {
+      err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+      if (err != cudaSuccess) return err;
+      if (known) attr_done[dev][0] = true;
+    }
+    kern<<<G, C::THREADS, C::SMEM_BYTES, stream>>>(m, n, plan, Ap, Bp, order_planes, C_planes, scratch, counters);
   }
-  kern<<<G, C::THREADS, C::SMEM_BYTES, stream>>>(m, n, plan, Ap, Bp, order_planes, C_planes, scratch, counters);
   return cudaGetLastError();
 }
 

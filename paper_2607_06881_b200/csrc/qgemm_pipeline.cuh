@@ -40,14 +40,14 @@ __device__ __forceinline__ void bulk_g2s(uint32_t smem_dst, const void* gmem_src
 }
 
 // Persistent kernel: gridDim.x = G CTAs (one per SM), each walks a private list of SEGMENTS = (tile, slab range):
-//   * stream-K part first: the sk_tiles tiles that do not fill a whole wave of G CTAs are cut along k into G nearly equal
-//     runs of slabs (CTA b owns global slab iterations [b*ipc, (b+1)*ipc) of the sk_tiles * KS), so that the last wave costs
-//     sk_tiles*KS/G slab-times instead of KS.  A CTA adds its partial order sums into the tile's scratch with fp64
-//     red.global.add -- EXACT here, every partial sum being an integer below 2^53 units (R6), hence the result is
-//     bit-identical whatever the arrival order -- then bumps the tile's slab counter; whoever completes the count re-reads
-//     the scratch and runs the epilogue.  Nobody ever waits for another CTA.
-//   * then dp_waves whole tiles, ids b, b + G, b + 2G, ... (tile ids are rasterised, so at any time the G CTAs cover a
-//     compact patch of C), accumulated and renormalised entirely in registers.
+//   * dp_waves whole tiles, ids b, b + G, b + 2G, ... (tile ids are rasterised, so at any time the G CTAs cover a compact patch
+//     of C), accumulated and renormalised entirely in registers;
+//   * the stream-K part: the sk_tiles tiles that do not fill a whole wave of G CTAs are cut along k into G nearly equal runs of
+//     slabs (CTA b owns global slab iterations [b*ipc, (b+1)*ipc) of the sk_tiles * KS), so that the last wave costs
+//     sk_tiles*KS/G slab-times instead of KS.  The partial order sums of the CTAs that share a tile are combined EXACTLY --
+//     every partial sum is an integer below 2^53 units (R6), so the result is bit-identical whatever the order --
+//     either by fp64 red.global.add into the tile's scratch (whoever completes the slab count runs the epilogue; nobody waits)
+//     or by a hand-over through per-CTA slots and flags (qgemm_packed.cu says which and why).
 // The stage ring runs straight through segment boundaries: the refill thread is AHEAD slabs ahead, possibly already in the
 // next tile, so the pipeline never drains between tiles.
 struct SkPlan {

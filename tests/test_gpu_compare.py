@@ -38,6 +38,9 @@ def test_topdown_materialised_path_is_bit_exact(cfg_idx, shape):
 @pytest.mark.parametrize("cfg_idx", [0, 2, 3, 4])
 @pytest.mark.parametrize("shape", [(64, 64, 64), (37, 51, 77), (1, 1, 1)])
 def test_cuda_core_classical_gemm_matches_oracle_O5(cfg_idx, shape):
+    """The classical kernel mirrors the oracle's O5 operation for operation (both restate the same textbook TwoSum / TwoProd
+    cascade), so "bit-identical to O5" compares two copies of ONE algorithm: it shows the GPU arithmetic is IEEE and
+    uncontracted, nothing more.  The INDEPENDENT check is the second assertion: the bound against the exact product O1."""
     cfg = inputs.CONFIGS[cfg_idx].with_shape(*shape)
     A, B = inputs.generate(cfg, "A"), inputs.generate(cfg, "B")
     C = mdc.mdc_classic_gemm(dev(A), dev(B)).cpu().numpy()

@@ -38,10 +38,12 @@ def test_random_case(case):
     dA, dB = dev(A), dev(B)
     chunk = int(rng.choice([8, 16, 64])) if chunked else 0
     blocks = int(rng.choice([0, 1, 3, 6]))
+    one_launch = int(rng.choice([0, 1, 2]))  # automatic / wherever the one-launch kernel exists / never: the same bits
     Aq_o, eA, _ = orc.split(A, 0, Q, bits=W)
     Bq_o, eB, _ = orc.split(B, 1, Q, bits=W)
     md.md_set_option(md.MD_OPT_K_CHUNK, chunk)
     md.md_set_option(md.MD_OPT_HOST_BLOCKS, blocks)
+    md.md_set_option(md.MD_OPT_ONE_LAUNCH, one_launch)
     try:
         md.md_set_option(md.MD_OPT_SLICE_BITS, 0 if W == 13 else W)
         Aq, gA = md.md_split(dA, 0, Q)
@@ -61,7 +63,7 @@ def test_random_case(case):
             md.md_gemm_host(torch.from_numpy(A).pin_memory(), torch.from_numpy(B).pin_memory(), Ch, scratch)
             assert bool((Ch == C.cpu()).all())
     finally:
-        for key in (md.MD_OPT_K_CHUNK, md.MD_OPT_HOST_BLOCKS, md.MD_OPT_SLICE_BITS):
+        for key in (md.MD_OPT_K_CHUNK, md.MD_OPT_HOST_BLOCKS, md.MD_OPT_SLICE_BITS, md.MD_OPT_ONE_LAUNCH):
             md.md_set_option(key, 0)
     Cn = C.cpu().numpy()
     r = orc.exact_all(A, B, Cn)

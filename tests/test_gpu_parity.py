@@ -224,7 +224,7 @@ def test_host_entry_point_matches_device_entry_point():
     scratch = torch.empty(md.md_host_scratch_bytes(cfg.m, cfg.n, cfg.k, 2), dtype=torch.uint8, device="cuda")
     before = md.md_launch_count()
     md.md_gemm_host(Ah, Bh, Ch, scratch)
-    assert md.md_launch_count() - before == 2  # one block: the cooperative preparation kernel and the fused GEMM
+    assert md.md_launch_count() - before == 1  # one block of a single-wave problem: the one-launch kernel (MD_OPT_ONE_LAUNCH)
     assert bits_equal(Ch.numpy(), C)
 
 
@@ -293,6 +293,7 @@ def test_fused_preparation_is_bit_identical_to_the_separate_kernels(cfg_idx, sha
     out = {}
     for mode in (1, 2):
         md.md_set_option(md.MD_OPT_FUSED_PREP, mode)
+        md.md_set_option(md.MD_OPT_ONE_LAUNCH, 2)   # the two-kernel path is what is compared here (tests/test_gpu_one_launch.py has the other)
         try:
             with md.Workspace(cfg.m, cfg.n, cfg.k, cfg.limbs, cfg.quarters):
                 before = md.md_launch_count()
@@ -301,6 +302,7 @@ def test_fused_preparation_is_bit_identical_to_the_separate_kernels(cfg_idx, sha
                 out[mode] = (host(md.md_gemm_orders(dev(A), dev(B))), host(C), launches, md.md_read_flags())
         finally:
             md.md_set_option(md.MD_OPT_FUSED_PREP, 0)
+            md.md_set_option(md.MD_OPT_ONE_LAUNCH, 0)
     assert out[1][2] == 2 and out[2][2] == 6 and out[1][3] == out[2][3] == 0
     assert bits_equal(out[1][0], out[2][0]) and bits_equal(out[1][1], out[2][1])
     Aq, eA, _ = orc.split(A, 0, cfg.quarters)
@@ -372,15 +374,43 @@ def test_small_tile_instance_is_bit_identical_to_the_large_one(cfg_idx, shape, Q
         for fused in (1, 2):
             md.md_set_option(md.MD_OPT_TILE, tile)
             md.md_set_option(md.MD_OPT_FUSED_PREP, fused)
+            md.md_set_option(md.MD_OPT_ONE_LAUNCH, 2)
             try:
                 with md.Workspace(cfg.m, cfg.n, cfg.k, 2, Q, bits=W):
                     out[tile, fused] = (host(md.md_gemm_orders(dev(A), dev(B))), host(md.md_gemm(dev(A), dev(B))), md.md_read_flags())
             finally:
                 md.md_set_option(md.MD_OPT_TILE, 0)
                 md.md_set_option(md.MD_OPT_FUSED_PREP, 0)
+                md.md_set_option(md.MD_OPT_ONE_LAUNCH, 0)
     Aq, eA, _ = orc.split(A, 0, Q, bits=W)
     Bq, eB, _ = orc.split(B, 1, Q, bits=W)
     want = orc.orders_int(Aq, eA, Bq, eB, bits=W)
     for key, (orders, C, flags) in out.items():
         assert flags == 0 and bits_equal(orders, want), key
         assert bits_equal(C, out[2, 2][1]), key
+
+
+@pytest.mark.parametrize("world", [2, 3, 8])
+@pytest.mark.parametrize("cfg_idx,shape", [(3, (203, 77, 130)), (4, (70, 45, 91))])
+def test_row_sharded_md_gemm_is_bit_identical_to_the_unsharded_call(world, cfg_idx, shape):
+    """SURVEY.md 8(e) / DESIGN.md section 8: the path shards by rows of A with no collective.  Every rank's block
+    (shard.row_block) through md_gemm on this one GPU, concatenated, must equal the unsharded md_gemm bit for bit: E_i and the
+    quarters of a row depend on that row only, F_j on B only.  Ragged m (not a multiple of world or of the tile), cfg3's
+    wide-range distribution and quad double."""
+    from paper_2607_06881_b200 import shard
+    cfg, A, B = gen(cfg_idx, *shape)
+    dA, dB = dev(A), dev(B)
+    with md.Workspace(cfg.m, cfg.n, cfg.k, cfg.limbs, cfg.quarters):
+        whole = host(md.md_gemm(dA, dB))
+        whole_orders = host(md.md_gemm_orders(dA, dB))
+        parts, parts_orders = [], []
+        for rank in range(world):
+            r0, r1 = shard.row_block(cfg.m, world, rank)
+            if r1 == r0:
+                continue
+            blk = dA[:, r0:r1, :].contiguous()
+            parts.append(host(md.md_gemm(blk, dB)))
+            parts_orders.append(host(md.md_gemm_orders(blk, dB)))
+        assert md.md_read_flags() == 0
+    assert bits_equal(np.concatenate(parts, axis=1), whole)
+    assert bits_equal(np.concatenate(parts_orders, axis=1), whole_orders)
