@@ -18,6 +18,7 @@ MD_OK = 0
 MD_ERR_BAD_ARG, MD_ERR_K_TOO_LARGE, MD_ERR_WORKSPACE, MD_ERR_CUDA, MD_ERR_UNSUPPORTED = -1, -2, -3, -4, -5
 MD_OPT_QUARTERS, MD_OPT_ORDERS, MD_OPT_SLICE_BITS, MD_OPT_HOST_BLOCKS, MD_OPT_K_CHUNK, MD_OPT_FUSED_PREP, MD_OPT_TILE, MD_OPT_RASTER_GROUP = 1, 2, 3, 4, 5, 6, 7, 8
 MD_OPT_ONE_LAUNCH = 9
+MD_OPT_TILE_SCHEDULE = 10
 
 # every symbol include/mdgemm.h declares: name -> (restype, argtypes)
 _c = ctypes

@@ -45,6 +45,7 @@ DeviceState* device_state() {
 }
 
 int raster_group() { return g_opt.raster_group ? g_opt.raster_group : 8; }
+int tile_schedule() { return g_opt.tile_schedule; }
 
 // Chunked accumulation (R16): the budget is kept per chunk of the contraction; the chunk md_gemm uses for
 // (limbs, S, W), a multiple of the k-slab depth 8, or 0 when the path stays unchunked / cannot be chunked.
@@ -147,12 +148,13 @@ static bool use_one_launch(int m, int n, int k, int limbs, int Q, int S, int bit
 
 // the fused quarter GEMM of one (block of a) problem on packed operands
 cudaError_t launch_fused(int m, int n, int k, int limbs, int Q, int S, const KernelPick& pick, const double* Aq, const double* Bq,
-                         double* order_planes, double* C_planes, void* sk, cudaStream_t stream, uint64_t* launches) {
+                         double* order_planes, double* C_planes, void* sk, bool counters_clear, cudaStream_t stream,
+                         uint64_t* launches) {
   switch (pick.family) {
     case GEMM_PACKED:
     case GEMM_PACKED_SMALL:
       return launch_qgemm_packed(m, n, k, limbs, Q, S, order_planes ? 0 : pick.chunk, pick.family == GEMM_PACKED_SMALL, Aq, Bq,
-                                 order_planes, C_planes, sk, stream, launches);
+                                 order_planes, C_planes, sk, counters_clear, stream, launches);
     case GEMM_WIDE: return launch_qgemm_wide(m, n, k, limbs, Q, Aq, Bq, order_planes, C_planes, sk, stream, launches);
     case GEMM_GENERIC: return launch_qgemm_generic(m, n, k, limbs, Q, S, Aq, Bq, order_planes, C_planes, sk, stream, launches);
     default: return cudaErrorInvalidValue;
@@ -187,9 +189,11 @@ md_status gemm_impl(int m, int n, int k, int limbs, int Q, int S, const double* 
     cudaGetLastError();  // a cluster launch the context cannot take: the two-launch path does the same work
     err = cudaErrorUnknown;
   }
+  bool counters_clear = false;
   if (use_fused_prep(m, n, k)) {  // one launch instead of five: what matters below ~2048^3
-    err = launch_prep_packed(m, n, k, limbs, Q, W, pick.bxA, pick.bxB, pick.bk, A, B, c.Aq, c.Bq, c.expA, c.expB, c.flags, stream, &launches);
+    err = launch_prep_packed(m, n, k, limbs, Q, W, pick.bxA, pick.bxB, pick.bk, A, B, c.Aq, c.Bq, c.expA, c.expB, c.flags, c.sk, stream, &launches);
     if (err != cudaSuccess) cudaGetLastError();  // a cooperative launch the context cannot take: the separate kernels do the same
+    else counters_clear = true;                  // the preparation kernel has also cleared the fused kernel's counter / flag words
   }
   if (err != cudaSuccess) {
     err = launch_exponents(m, k, 0, Q, W, A, c.expA, c.flags, stream, &launches);
@@ -198,7 +202,7 @@ md_status gemm_impl(int m, int n, int k, int limbs, int Q, int S, const double* 
     if (err == cudaSuccess) err = launch_split_packed(k, n, limbs, Q, W, 1, pick.bxB, pick.bk, B, c.Bq, c.expB, c.flags, stream, &launches);
   }
   if (ev) cudaEventRecord(ev[1], stream);
-  if (err == cudaSuccess) err = launch_fused(m, n, k, limbs, Q, S, pick, c.Aq, c.Bq, order_planes, C_planes, c.sk, stream, &launches);
+  if (err == cudaSuccess) err = launch_fused(m, n, k, limbs, Q, S, pick, c.Aq, c.Bq, order_planes, C_planes, c.sk, counters_clear, stream, &launches);
   if (ev) {
     cudaEventRecord(ev[2], stream);
     if (err == cudaSuccess) ds->prof_count++;
@@ -291,6 +295,10 @@ md_status md_set_option(int key, int value) {
       if (value < 0 || value > 2) return MD_ERR_BAD_ARG;
       g_opt.one_launch = value;
       return MD_OK;
+    case MD_OPT_TILE_SCHEDULE:
+      if (value < 0 || value > 2) return MD_ERR_BAD_ARG;
+      g_opt.tile_schedule = value;
+      return MD_OK;
     case MD_OPT_HOST_BLOCKS:  // 0 = automatic, 1..32 blocks, or PR * 256 + PC (explicit panel counts, each <= 64)
       if (value < 0 || (value > 32 && (value < 256 || (value >> 8) > 64 || (value & 255) > 64))) return MD_ERR_BAD_ARG;
       g_opt.host_blocks = value;
@@ -320,6 +328,7 @@ int md_get_option(int key) {
     case MD_OPT_K_CHUNK: return g_opt.k_chunk;
     case MD_OPT_FUSED_PREP: return g_opt.fused_prep;
     case MD_OPT_ONE_LAUNCH: return g_opt.one_launch;
+    case MD_OPT_TILE_SCHEDULE: return g_opt.tile_schedule;
     case MD_OPT_TILE: return g_opt.tile;
     case MD_OPT_RASTER_GROUP: return g_opt.raster_group;
     default: return -1;
@@ -367,7 +376,7 @@ md_status md_qgemm(int m, int n, int k, int limbs, int quarters, int orders, con
     err = launch_pack_planes(m, k, quarters, 0, pick.bxA, pick.bk, Aq, c.Aq, st, &launches);
     if (err == cudaSuccess) err = launch_pack_planes(k, n, quarters, 1, pick.bxB, pick.bk, Bq, c.Bq, st, &launches);
     if (err == cudaSuccess)
-      err = launch_fused(m, n, k, limbs, quarters, orders, pick, c.Aq, c.Bq, order_planes, C_planes, c.sk, st, &launches);
+      err = launch_fused(m, n, k, limbs, quarters, orders, pick, c.Aq, c.Bq, order_planes, C_planes, c.sk, false, st, &launches);
   }
   g_launches += launches;
   return err == cudaSuccess ? MD_OK : MD_ERR_CUDA;
@@ -699,7 +708,7 @@ md_status md_gemm_host(int m, int n, int k, int limbs, const double* A_host, con
       }
       // block (i, j): compact [limbs][mi][nj] at the position its elements have in a row-panel-major walk of C
       double* Cb = dC + (size_t)limbs * ((size_t)r0 * n + (size_t)mi * c0);
-      err = launch_fused(mi, nj, k, limbs, Q, S, pick, Aq, Bq, nullptr, Cb, c.sk, st, &launches);
+      err = launch_fused(mi, nj, k, limbs, Q, S, pick, Aq, Bq, nullptr, Cb, c.sk, false, st, &launches);
       if (err != cudaSuccess) break;
       cudaEvent_t done = ev_C[j * hp.PR + i];
       MD_TRY(cudaEventRecord(done, st));

@@ -20,6 +20,7 @@ struct Options {
   int tile = 0;          // 0 = automatic, 1 = the 32 x 16 tile instance wherever it exists, 2 = never
   int fused_prep = 0;    // 0 = automatic (small / medium operands), 1 = always, 2 = never
   int one_launch = 0;    // 0 = automatic (single-wave problems), 1 = wherever the kernel exists, 2 = never
+  int tile_schedule = 0; // 0 = static stream-K lists, 1 = hybrid (static waves, then a tile queue), 2 = tile queue only
   int k_chunk = 0;       // 0 = chunked accumulation only when k exceeds the exactness budget; else the chunk length to force
   int host_blocks = 0;   // md_gemm_host: 0 = automatic panel plan, else the number of blocks of C (1 = no pipelining)
   int raster_group = 0;  // tile rows per raster group of the fused GEMM (0 = default 8)
@@ -86,7 +87,8 @@ size_t workspace_bytes_for(int m, int n, int k, int limbs, int Q, int S);
 
 md_status check_gemm_args(int m, int n, int k, int limbs, const void* A, const void* B, const void* C, bool want_orders);
 cudaError_t launch_fused(int m, int n, int k, int limbs, int Q, int S, const KernelPick& pick, const double* Aq, const double* Bq,
-                         double* order_planes, double* C_planes, void* sk, cudaStream_t stream, uint64_t* launches);
+                         double* order_planes, double* C_planes, void* sk, bool counters_clear, cudaStream_t stream,
+                         uint64_t* launches);
 // a1-a4 on device-resident operands with explicit (Q, S) and workspace: what md_gemm / md_gemm_orders / md_gemm_host /
 // md_gemm_auto and md_geqrf's trailing updates all run
 md_status gemm_impl(int m, int n, int k, int limbs, int Q, int S, const double* A, const double* B, double* C_planes,

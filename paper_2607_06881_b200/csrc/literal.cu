@@ -389,7 +389,7 @@ md_status md_gemm_literal(int m, int n, int k, int limbs, const double* A_planes
       if (population(hB, gb) == 0) continue;
       const int argB = signs ? (gb < 13 ? 13 + gb : 39 + (gb - 13)) : gb;
       err = launch_literal_split_packed(k, n, limbs, Q, NP, eq8, argB, hB[1], 1, pick.bxB, pick.bk, B_planes, c.Bq, st, &launches);
-      if (err == cudaSuccess) err = launch_fused(m, n, k, limbs, NP, S, pick, c.Aq, c.Bq, c.orders, nullptr, c.sk, st, &launches);
+      if (err == cudaSuccess) err = launch_fused(m, n, k, limbs, NP, S, pick, c.Aq, c.Bq, c.orders, nullptr, c.sk, false, st, &launches);
       if (err != cudaSuccess) break;
       switch (limbs) {
         case 2: literal_accumulate_kernel<2><<<eblocks, 256, 0, st>>>(total, S, c.orders, c.r); break;

@@ -41,11 +41,15 @@ bool qgemm_small_supported(int limbs, int quarters, int orders);
 // exponent vectors + packed quarter planes of BOTH operands in one launch (small and medium problems: md_gemm's fused prep)
 cudaError_t launch_prep_packed(int m, int n, int k, int limbs, int quarters, int bits, int bxA, int bxB, int bk, const double* A,
                                const double* B, double* Ap, double* Bp, int32_t* expA, int32_t* expB, uint32_t* flags,
-                               cudaStream_t stream, uint64_t* launches);
+                               void* sk_counters, cudaStream_t stream, uint64_t* launches);  // sk_counters != nullptr: also clears the
+                               // SK_COUNTER_BYTES counter / flag words of the fused GEMM's stream-K scratch
 // sk_ws: sk_workspace_bytes(limbs, quarters) bytes of device scratch for the stream-K tail (slab counters + one
 // order-plane tile per stream-K tile); zeroed by the launcher (a memset node on `stream`) as far as it is used.
 constexpr int SK_MAX_TILES = 256;
-constexpr size_t SK_COUNTER_BYTES = 1024;  // SK_MAX_TILES unsigned ints
+constexpr size_t SK_COUNTER_BYTES = 2048;  // 512 unsigned ints: slab counters of the stream-K tiles (red.add hand-in) or one hand-over
+                                           // flag per CTA at [0, SK_MAX_TILES), the work-queue counter of the dynamic schedule at
+                                           // SK_QUEUE_INDEX
+constexpr int SK_QUEUE_INDEX = SK_MAX_TILES;
 // chunk > 0: the chunked kernel's stream-K tail keeps one slot per (tile, chunk of the contraction) while that fits
 // SK_CHUNK_CAP_BYTES; beyond, the chunked kernel runs whole tiles only
 constexpr size_t SK_CHUNK_CAP_BYTES = (size_t)512 << 20;
@@ -63,8 +67,10 @@ cudaError_t launch_fused_small(int m, int n, int k, int limbs, int quarters, int
 // only, C_planes only): the accumulators are folded into the elements' expansions every `chunk` contraction indices.
 bool qgemm_chunk_supported(int limbs, int quarters);
 bool qgemm_packed_supported(int limbs, int quarters, int orders);
+// counters_clear: the SK_COUNTER_BYTES words at sk_ws are already zero on `stream` (launch_prep_packed cleared them), so a launch
+// that needs nothing else zeroed (the hand-over schedule) enqueues no memset node
 cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, int orders, int chunk, bool small, const double* Ap,
-                                const double* Bp, double* order_planes, double* C_planes, void* sk_ws,
+                                const double* Bp, double* order_planes, double* C_planes, void* sk_ws, bool counters_clear,
                                 cudaStream_t stream, uint64_t* launches);
 // octo / hexa double (qgemm_wide.cu): same packed operands (k-slab depth 4), same stream-K scratch convention
 bool qgemm_wide_supported(int limbs, int quarters);

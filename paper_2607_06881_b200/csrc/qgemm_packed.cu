@@ -64,7 +64,18 @@ struct PCfg {
 // CTA that owns a tile's last slabs collects the others' sums (small problems, where every tile is cut and 16 KB of atomics per
 // warp through L2 were the critical path: 256^3 0.55 -> 0.66, 512^3 0.88 -> 0.92 of the peak).  Two instantiations rather than
 // one: at 254 registers the DMMA loop's schedule is sensitive to the code around it.
-template <class C, bool CHUNK, bool HANDOVER = false>
+// MODE: SCHED_STATIC (0) the static segment lists above with the red.add hand-in; SCHED_HANDOVER (1) static lists, hand-over;
+// SCHED_DYNAMIC (2) -- the segments are CLAIMED from a queue counter in global memory instead of computed from the CTA index:
+// first every whole tile in raster order, then the remaining tiles (the last partial wave plus, when that is short, one more
+// wave) cut along k into units of plan.dyn_unit slabs, red.add hand-in.  An SM that runs ahead simply claims more, and the run
+// ends within one unit's time on every SM (under the static lists the SMs of the quad-double run finish up to 1.3 % apart).
+// An OPTION, not the default: launch_cfg says what it costs.
+// Thread 0 claims one item ahead of the segment it is producing and publishes the descriptors through a ring in shared
+// memory; a descriptor is written before the bulk copies of the PRECEDING segment's first slab are issued, so any warp that
+// has passed that slab's full barrier (release / acquire through the mbarrier) may read it -- no extra synchronisation in the loop.
+constexpr int SCHED_STATIC = 0, SCHED_HANDOVER = 1, SCHED_DYNAMIC = 2;
+constexpr int DYN_RING = 8;  // > STAGES + 1: a descriptor is not overwritten while a warp may still read it
+template <class C, bool CHUNK, int MODE = SCHED_STATIC>
 __global__ void __launch_bounds__(C::THREADS, 1)
 qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, const double* __restrict__ Bp,
                     double* __restrict__ order_planes, double* __restrict__ C_planes, double* __restrict__ sk_scratch,
@@ -78,6 +89,9 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int wm = warp / C::WN, wn = warp % C::WN;
   const int G = gridDim.x, cta = blockIdx.x, KS = plan.KS;
+  constexpr bool HANDOVER = MODE == SCHED_HANDOVER, DYN = MODE == SCHED_DYNAMIC;
+  static_assert(!(CHUNK && MODE != SCHED_STATIC), "the chunked kernel keeps the static lists");
+  static_assert(DYN_RING > STAGES + 1, "descriptor ring");
 
   // ---- this CTA's segment list ---------------------------------------------------------------------------------------
   const int sk_total = plan.sk_tiles * KS;
@@ -85,7 +99,8 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
   const int n_sk = g1 > g0 ? (g1 - 1) / KS - g0 / KS + 1 : 0;
   const int dp_mine = plan.dp_waves - (cta >= plan.dp_tail ? 1 : 0);  // whole tiles of this CTA
   const int n_seg = n_sk + dp_mine;
-  const int total_slabs = (g1 - g0) + dp_mine * KS;
+  const int total_slabs = DYN ? 1 : (g1 - g0) + dp_mine * KS;
+  const int sk_base = DYN ? plan.dyn_whole : plan.dp_waves * G;  // first tile that is cut along k
   // Segment list.  Without hand-over: the stream-K segments in slab order, then the whole tiles.
   // With hand-over: a CTA's share of stream-K slabs is at most one tile long (sk_tiles < G), so it has at most TWO stream-K
   // segments -- in slab order the TAIL of a tile begun by the CTAs before it (it ends at the tile's last slab) and / or the HEAD
@@ -111,8 +126,32 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
       sk_tab[6] = (n_sk > 0 && sk_tab[2] < KS) ? 1 : 0;
     }
   }
+  __shared__ int dyn_tab[DYN ? DYN_RING : 1][4];  // DYNAMIC: descriptor of segment j at [j % DYN_RING] = tile (-1: no more work), s0, s1
+  auto dyn_claim = [&](int j) {  // thread 0: claim the next item of the queue and publish it as segment j
+    // the first dyn_static segments of a CTA are the whole tiles cta, cta + G, ... (no claim): the CTAs stay in lock-step on
+    // neighbouring tiles and share operand slabs through L2 for most of the run; only what follows is claimed from the queue
+    const int x = j < plan.dyn_static ? j * G + cta : plan.dyn_static * G + (int)atomicAdd(&sk_counters[SK_QUEUE_INDEX], 1u);
+    int tile = -1, s0 = 0, s1 = 0;
+    if (x < plan.dyn_whole) {
+      tile = x, s1 = KS;
+    } else if (x < plan.dyn_items) {
+      // unit `part` of EVERY cut tile before unit part + 1 of any: the CTAs that run at the same time then work on the same
+      // k-range of neighbouring tiles and share their operand slabs through L2, as in the whole-tile phase (with the 16 units
+      // of one tile claimed together nothing was shared and the tail ran at DRAM speed: dd 4096^3 137.5 against 134.4 ms)
+      const int cut = plan.dyn_items - plan.dyn_whole, u = x - plan.dyn_whole;
+      const int cut_tiles = cut / plan.dyn_upt, part = u / cut_tiles;
+      tile = plan.dyn_whole + (u - part * cut_tiles);
+      s0 = part * plan.dyn_unit;
+      s1 = min(KS, s0 + plan.dyn_unit);
+    }
+    volatile int* d = dyn_tab[j % DYN_RING];
+    d[0] = tile, d[1] = s0, d[2] = s1;
+  };
   auto segment = [&](int i, int& tile, int& s0, int& s1) {
-    if constexpr (HANDOVER) {
+    if constexpr (DYN) {
+      const volatile int* d = dyn_tab[i % DYN_RING];
+      tile = d[0], s0 = d[1], s1 = d[2];
+    } else if constexpr (HANDOVER) {
       const int pre = sk_tab[6];  // the whole tiles come after the head
       if (i >= pre && i < pre + dp_mine) {
         tile = (i - pre) * G + cta, s0 = 0, s1 = KS;
@@ -143,17 +182,29 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
       mbar_init(empty_u32 + 8 * s, C::WARPS);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    if constexpr (DYN) dyn_claim(0);
   }
   __syncthreads();
   if (total_slabs == 0) return;
+  if constexpr (DYN) {
+    if (dyn_tab[0][0] < 0) return;  // the queue was empty before this CTA's first claim
+  }
 
   // ---- producer side (thread 0): a cursor over the flat slab sequence, AHEAD slabs ahead of the consumers -------------
   int p_seg = -1, p_left = 0, p_flat = 0, pst = 0;
+  bool p_done = false;  // DYNAMIC: the producer has met the end of the queue
   const double *p_A = nullptr, *p_B = nullptr;
   auto produce_one = [&]() {  // issue the bulk copies of flat slab p_flat into stage pst (its empty barrier has completed)
     if (p_left == 0) {
       int tile, s0, s1, tm, tn;
       segment(++p_seg, tile, s0, s1);
+      if constexpr (DYN) {
+        if (tile < 0) {
+          p_done = true;
+          return;
+        }
+        dyn_claim(p_seg + 1);  // published before this segment's first slab is issued
+      }
       raster_tile(tile, plan.tiles_m, plan.tiles_n, tm, tn, plan.group_m);
       p_A = Ap + ((size_t)tm * KS + s0) * C::A_CHUNK;
       p_B = Bp + ((size_t)tn * KS + s0) * C::B_CHUNK;
@@ -172,10 +223,10 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
   if (tid == 0) {
 #pragma unroll
     for (int j = 0; j < C::AHEAD; j++)
-      if (p_flat < total_slabs) produce_one();
+      if (DYN ? !p_done : p_flat < total_slabs) produce_one();
   }
   auto produce = [&]() {  // top of consumer iteration `it`: refill for flat slab it + AHEAD
-    if (p_flat < total_slabs) {
+    if (DYN ? !p_done : p_flat < total_slabs) {
       // the stage was last read for flat slab (p_flat - STAGES) = it - 2: wait for its release (completed long ago)
       if (p_flat >= STAGES) mbar_wait(empty_u32 + 8 * pst, ((p_flat / STAGES) + 1) & 1);
       produce_one();
@@ -277,6 +328,15 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
   int c_seg = 0, c_tile, c_s0, c_s1;
   segment(0, c_tile, c_s0, c_s1);
   int c_left = c_s1 - c_s0;
+  // slabs this CTA is known to consume.  DYNAMIC (two fragment sets): the segments up to the one AFTER the current one -- its
+  // descriptor is readable once the current segment's first slab has arrived -- so that "a slab follows this one" is a register
+  // compare, as with the static lists
+  int total_known = total_slabs;
+  auto dyn_peek = [&]() {  // add the length of the segment after the current one (nothing is published after the end marker)
+    if (c_tile < 0) return;
+    const volatile int* d = dyn_tab[(c_seg + 1) % DYN_RING];
+    total_known += d[0] >= 0 ? d[2] - d[1] : 0;
+  };
   if constexpr (CHUNK) {
     c_chunk = c_s0 / plan.flush_slabs;
     to_flush = plan.flush_slabs - c_s0 % plan.flush_slabs;
@@ -291,7 +351,7 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
         chunk_epilogue<L, MT, NT>(rexp, m, n, row_base, col_base, lane, C_planes);
         zero_rexp();
       } else {                  // stream-K part: the last (possibly partial) chunk of this run, then the hand-over
-        const int r = c_tile - plan.dp_waves * G;
+        const int r = c_tile - sk_base;
         flush_partial(r, c_chunk);
         __threadfence();
         __syncthreads();
@@ -324,7 +384,7 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
     } else if (c_s1 - c_s0 == KS) {  // whole tile in registers
       qgemm_epilogue<S, L, MT, NT>(acc, m, n, row_base, col_base, lane, order_planes, C_planes);
     } else if constexpr (!HANDOVER) {  // partial sums of a stream-K tile: exact fp64 reduction through the tile's scratch
-      const int r = c_tile - plan.dp_waves * G;
+      const int r = c_tile - sk_base;
       double* sc = sk_scratch + (size_t)r * (S * C::BM * C::BN) + (size_t)warp * (S * MT * NT * 64) + lane * 2;
 #pragma unroll
       for (int s = 0; s < S; s++)
@@ -366,6 +426,11 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
 #pragma unroll
             for (int j = 0; j < NT; j++)
               __stcg(reinterpret_cast<double2*>(sc + ((s * MT + i) * NT + j) * 64), make_double2(acc[s][i][j][0], acc[s][i][j][1]));
+        // PER WARP: a warp's part of the slot is read by the same warp of the finishing CTA only, so each warp raises its own
+        // flag and goes on -- no block-wide barrier (ncu at 256^3: 0.76 barrier + 0.19 membar stall cycles per issued
+        // instruction with the block-wide version, about 3 us per warp of a 45 us kernel)
+        // (one flag per CTA behind a block-wide barrier.  A flag per WARP, without the barrier, was measured and not kept: 256^3
+        // unchanged, 1024^3 2.135 -> 2.201 ms -- profiles/r04_small_sizes.md)
         __threadfence();
         __syncthreads();
         if (tid == 0) {
@@ -397,9 +462,11 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
       }
     }
     zero_acc();
-    if (++c_seg < n_seg) {
-      segment(c_seg, c_tile, c_s0, c_s1);
+    if (DYN || ++c_seg < n_seg) {
+      if constexpr (DYN) ++c_seg;
+      segment(c_seg, c_tile, c_s0, c_s1);  // DYNAMIC: tile < 0 when the queue is exhausted (the loops below have stopped by then)
       c_left = c_s1 - c_s0;
+      if constexpr (DYN && C::PREFETCH) dyn_peek();
       if constexpr (CHUNK) {
         c_chunk = c_s0 / plan.flush_slabs;
         to_flush = plan.flush_slabs - c_s0 % plan.flush_slabs;
@@ -411,7 +478,7 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
     if constexpr (CHUNK) {
       if (--to_flush == 0 && c_left > 0) {
         if (c_s1 - c_s0 == KS) flush_chunk();
-        else flush_partial(c_tile - plan.dp_waves * G, c_chunk);
+        else flush_partial(c_tile - sk_base, c_chunk);
         c_chunk++;
         to_flush = plan.flush_slabs;
       }
@@ -423,8 +490,12 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
   if constexpr (C::PREFETCH) {
     Frags f0, f1;
     mbar_wait(full_u32, 0);
+    if constexpr (DYN) {
+      total_known = c_left;
+      dyn_peek();
+    }
     load_frags(f0, stages + a_off, stages + b_off, 0);
-    for (int it = 0; it < total_slabs; it++) {
+    for (int it = 0; it < total_known; it++) {
       if (tid == 0) produce();
       const double* As = stages + (size_t)st * (C::A_CHUNK + C::B_CHUNK) + a_off;
       const double* Bs = stages + (size_t)st * (C::A_CHUNK + C::B_CHUNK) + b_off;
@@ -433,7 +504,7 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
 
       const int nst = (st + 1 == STAGES) ? 0 : st + 1;
       const uint32_t nphase = (st + 1 == STAGES) ? phase ^ 1 : phase;
-      if (it + 1 < total_slabs) {  // next slab: its first k-step's fragments are fetched under this slab's second k-step
+      if (it + 1 < total_known) {  // next slab: its first k-step's fragments are fetched under this slab's second k-step
         mbar_wait(full_u32 + 8 * nst, nphase);
         load_frags(f0, stages + (size_t)nst * (C::A_CHUNK + C::B_CHUNK) + a_off,
                    stages + (size_t)nst * (C::A_CHUNK + C::B_CHUNK) + b_off, 0);
@@ -448,7 +519,7 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
       if (c_left == 0) end_of_segment();
     }
   } else {  // one fragment set (register budget): loads of a k-step are issued at its start
-    for (int it = 0; it < total_slabs; it++) {
+    for (int it = 0; DYN ? c_tile >= 0 : it < total_slabs; it++) {
       if (tid == 0) produce();
       mbar_wait(full_u32 + 8 * st, phase);
       const double* As = stages + (size_t)st * (C::A_CHUNK + C::B_CHUNK) + a_off;
@@ -477,7 +548,7 @@ constexpr int HANDOVER_MAX_WAVES = 8;  // whole-tile waves from which the stream
 // Exact orders over the whole k, persistent stream-K.
 template <class C>
 cudaError_t launch_cfg(int m, int n, int k, const double* Ap, const double* Bp, double* order_planes, double* C_planes,
-                       void* sk_ws, cudaStream_t stream) {
+                       void* sk_ws, bool counters_clear, cudaStream_t stream) {
   constexpr bool SMALL = C::L == 2 && C::MT == 1;
   static_assert(C::BM == pack_bx(C::L, C::Q, 0, SMALL) && C::BN == pack_bx(C::L, C::Q, 1, SMALL), "tile shape must match the packed layout");
   const int tiles_m = (m + C::BM - 1) / C::BM, tiles_n = (n + C::BN - 1) / C::BN;
@@ -485,40 +556,59 @@ cudaError_t launch_cfg(int m, int n, int k, const double* Ap, const double* Bp, 
   if (tiles > 0x7fffffffLL) return cudaErrorInvalidValue;
   const int G = sk_grid();
   if (G <= 0) return cudaErrorInvalidDevice;
-  const SkPlan plan = make_sk_plan(tiles_m, tiles_n, (k + C::BK - 1) / C::BK, G);
+  SkPlan plan = make_sk_plan(tiles_m, tiles_n, (k + C::BK - 1) / C::BK, G);
   unsigned int* counters = static_cast<unsigned int*>(sk_ws);
   double* scratch = reinterpret_cast<double*>(static_cast<char*>(sk_ws) + SK_COUNTER_BYTES);
   cudaError_t err;
-  // hand-over between the CTAs of a stream-K tile while every tile is cut (small problems); fp64 red.add into the tile's scratch
-  // once whole-tile waves dominate (measured: 512^3 0.88 -> 0.92 with, dd 4096^3 134.65 against 134.88 ms without)
-  const bool handover = plan.dp_waves < HANDOVER_MAX_WAVES;
-  if (plan.sk_tiles > 0) {  // hand-over: the flags (one per CTA) start at zero, the slots are written before they are read;
-                            // red.add: counters and the scratch tiles in use start at zero (one contiguous region)
+  // Which schedule (all three give the same bits):
+  //   hand-over between the CTAs of a stream-K tile while every tile is cut or nearly so (small problems; measured: 512^3
+  //   0.88 -> 0.92 of the peak with it, dd 4096^3 134.65 against 134.88 ms without);
+  //   the static lists with red.add once whole-tile waves dominate;
+  //   the dynamic queue only on request (MD_OPT_TILE_SCHEDULE 1 / 2, wherever there is a whole wave).  MEASURED AND NOT MADE THE
+  //   DEFAULT (profiles/r04_dynamic_schedule.md): it does level the SMs' finishing times (quad double 2048^3: active cycles
+  //   per SM 124.6-126.2 M under the static lists, 126.1-126.4 M with the queue), but CTAs that have fallen out of lock-step no
+  //   longer fetch the same operand slabs at the same time, the L2 hit rate drops (dd 4096^3: 84 % -> 52 %, 18 -> 70 GB of DRAM
+  //   reads) and the DMMA pipe loses more than the balance gains: dd 4096^3 134.42 ms static, 134.29-134.38 hybrid, 135.12 queue
+  //   only; qd 2048^3 64.35 / 64.32 / 65.26.
+  const int sched_opt = tile_schedule();
+  const bool dynamic = sched_opt != 0 && plan.dp_waves >= 1;
+  const bool handover = !dynamic && plan.dp_waves < HANDOVER_MAX_WAVES;
+  if (dynamic) {
+    // the tiles that are cut: the last partial wave, plus one whole wave when that is short -- the whole-tile phase ends with
+    // the SMs spread over one tile time, and the cut tiles have to fill that triangle (about G / 2 tile times)
+    int cut = plan.sk_tiles;
+    if (cut < (7 * G) / 10 && cut + G <= SK_MAX_TILES - 1) cut += G;
+    constexpr int units = 16;
+    plan.dyn_whole = (int)tiles - cut;
+    // 1: every whole-tile wave but the last one keeps the static assignment (lock-step, L2 sharing); 2: the queue from the start
+    plan.dyn_static = sched_opt == 1 && plan.dyn_whole / G > 0 ? plan.dyn_whole / G - 1 : 0;
+    plan.dyn_unit = (plan.KS + units - 1) / units;
+    plan.dyn_upt = (plan.KS + plan.dyn_unit - 1) / plan.dyn_unit;
+    plan.dyn_items = plan.dyn_whole + cut * plan.dyn_upt;
+    // queue counter, slab counters and the scratch tiles of the cut tiles start at zero
+    err = cudaMemsetAsync(sk_ws, 0, SK_COUNTER_BYTES + sizeof(double) * (size_t)(plan.dyn_upt > 1 ? cut : 0) * C::S * C::BM * C::BN, stream);
+    if (err != cudaSuccess) return err;
+  } else if (plan.sk_tiles > 0) {  // hand-over: the flags (one per CTA) start at zero, the slots are written before they are read;
+                                   // red.add: counters and the scratch tiles in use start at zero (one contiguous region)
     const size_t bytes = handover ? (size_t)SK_COUNTER_BYTES
                                   : SK_COUNTER_BYTES + sizeof(double) * (size_t)plan.sk_tiles * C::S * C::BM * C::BN;
-    err = cudaMemsetAsync(sk_ws, 0, bytes, stream);
-    if (err != cudaSuccess) return err;
+    if (!(handover && counters_clear)) {  // the fused preparation kernel has cleared the flags already (md_gemm below ~2048^3)
+      err = cudaMemsetAsync(sk_ws, 0, bytes, stream);
+      if (err != cudaSuccess) return err;
+    }
   }
-  static bool attr_done[MD_MAX_DEVICES][2] = {};  // the shared-memory opt-in is per function and device: once, not per launch
+  static bool attr_done[MD_MAX_DEVICES][3] = {};  // the shared-memory opt-in is per function and device: once, not per launch
   const int dev = current_device();
   const bool known = dev >= 0 && dev < MD_MAX_DEVICES;
-  if (handover) {
-    auto kern = qgemm_packed_kernel<C, false, true>;
-    if (!known || !attr_done[dev][1]) {
-      err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
-      if (err != cudaSuccess) return err;
-      if (known) attr_done[dev][1] = true;
-    }
-    kern<<<G, C::THREADS, C::SMEM_BYTES, stream>>>(m, n, plan, Ap, Bp, order_planes, C_planes, scratch, counters);
-  } else {
-    auto kern = qgemm_packed_kernel<C, false, false>;
-    if (!known || !attr_done[dev][0]) {
-      err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
-      if (err != cudaSuccess) return err;
-      if (known) attr_done[dev][0] = true;
-    }
-    kern<<<G, C::THREADS, C::SMEM_BYTES, stream>>>(m, n, plan, Ap, Bp, order_planes, C_planes, scratch, counters);
+  const int mode = dynamic ? SCHED_DYNAMIC : handover ? SCHED_HANDOVER : SCHED_STATIC;
+  auto kern = mode == SCHED_DYNAMIC ? qgemm_packed_kernel<C, false, SCHED_DYNAMIC>
+            : mode == SCHED_HANDOVER ? qgemm_packed_kernel<C, false, SCHED_HANDOVER> : qgemm_packed_kernel<C, false, SCHED_STATIC>;
+  if (!known || !attr_done[dev][mode]) {
+    err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+    if (err != cudaSuccess) return err;
+    if (known) attr_done[dev][mode] = true;
   }
+  kern<<<G, C::THREADS, C::SMEM_BYTES, stream>>>(m, n, plan, Ap, Bp, order_planes, C_planes, scratch, counters);
   return cudaGetLastError();
 }
 
@@ -611,10 +701,10 @@ bool qgemm_packed_supported(int limbs, int quarters, int orders) {
 }
 
 cudaError_t launch_qgemm_packed(int m, int n, int k, int limbs, int quarters, int orders, int chunk, bool small, const double* Ap,
-                                const double* Bp, double* order_planes, double* C_planes, void* sk_ws, cudaStream_t stream,
-                                uint64_t* launches) {
+                                const double* Bp, double* order_planes, double* C_planes, void* sk_ws, bool counters_clear,
+                                cudaStream_t stream, uint64_t* launches) {
   cudaError_t err = cudaErrorInvalidValue;
-#define MD_Q(...) err = launch_cfg<__VA_ARGS__>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream)
+#define MD_Q(...) err = launch_cfg<__VA_ARGS__>(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, counters_clear, stream)
   if (small) {
     if (chunk > 0 || !qgemm_small_supported(limbs, quarters, orders)) return cudaErrorInvalidValue;
     if (quarters == 8) MD_Q(PCfgDDS<8>);

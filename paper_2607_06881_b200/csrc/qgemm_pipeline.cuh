@@ -59,10 +59,18 @@ struct SkPlan {
   int dp_tail;           // CTAs 0 .. dp_tail-1 own a tile in the LAST of the dp_waves (all G of them unless chunked, below)
   int flush_slabs;       // chunked accumulation (qgemm_packed.cu, R16): slabs between two flushes; 0 = never
   int group_m;           // tile rows per raster group (raster_tile; MD_OPT_RASTER_GROUP, default 8)
+  // DYNAMIC schedule (qgemm_packed.cu, MODE 2): CTAs claim work items from a queue counter in item order --
+  // items [0, dyn_whole) are whole tiles (tile id = item), the others cut the remaining tiles along k into units of dyn_unit slabs
+  int dyn_whole;         // whole-tile items
+  int dyn_unit;          // slabs per unit of a cut tile
+  int dyn_upt;           // units per cut tile = ceil(KS / dyn_unit)
+  int dyn_items;         // all items
+  int dyn_static;        // the first dyn_static whole tiles of CTA b are b, b + G, ... without a claim; the queue starts at item dyn_static * G
 };
 
 // Plan for `tiles` output tiles of KS slabs each on a grid of G persistent CTAs.
 int raster_group();  // api.cu: MD_OPT_RASTER_GROUP (default 8)
+int tile_schedule();  // api.cu: MD_OPT_TILE_SCHEDULE (0 = static lists, 1 = hybrid, 2 = tile queue only)
 inline SkPlan make_sk_plan(int tiles_m, int tiles_n, int KS, int G) {
   const long long tiles = (long long)tiles_m * tiles_n;
   SkPlan plan;
@@ -75,6 +83,7 @@ inline SkPlan make_sk_plan(int tiles_m, int tiles_n, int KS, int G) {
   plan.dp_tail = G;
   plan.flush_slabs = 0;
   plan.group_m = raster_group();
+  plan.dyn_whole = plan.dyn_unit = plan.dyn_upt = plan.dyn_items = plan.dyn_static = 0;
   return plan;
 }
 

@@ -205,12 +205,16 @@ template <int L>
 __global__ void __launch_bounds__(256) prep_coop_kernel(int m, int n, int k, int Q, int bits, int bxA, int bxB, int bk,
                                                         const double* __restrict__ A, const double* __restrict__ B,
                                                         double* __restrict__ Ap, double* __restrict__ Bp, uint32_t* rawA,
-                                                        uint32_t* rawB, uint32_t* flags, int exp_lo) {
+                                                        uint32_t* rawB, uint32_t* flags, int exp_lo, uint32_t* zero_words,
+                                                        int zero_count) {
   cooperative_groups::grid_group grid = cooperative_groups::this_grid();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int gthreads = gridDim.x * blockDim.x, gtid = blockIdx.x * blockDim.x + threadIdx.x;
   for (int i = gtid; i < m; i += gthreads) rawA[i] = 0;
   for (int i = gtid; i < n; i += gthreads) rawB[i] = 0;
+  // the hand-over flags of the fused GEMM that follows on the stream (qgemm_packed.cu) start at zero: cleared here instead of
+  // by a memset node between the two kernels
+  for (int i = gtid; i < zero_count; i += gthreads) zero_words[i] = 0;
   grid.sync();
   // phase 1a: rows of A_0 in pieces of 1024 elements, a warp per piece, lanes along the row (coalesced)
   {
@@ -319,11 +323,13 @@ cudaError_t launch_split(int rows, int cols, int limbs, int quarters, int bits, 
 
 cudaError_t launch_prep_packed(int m, int n, int k, int limbs, int quarters, int bits, int bxA, int bxB, int bk, const double* A,
                                const double* B, double* Ap, double* Bp, int32_t* expA, int32_t* expB, uint32_t* flags,
-                               cudaStream_t stream, uint64_t* launches) {
+                               void* sk_counters, cudaStream_t stream, uint64_t* launches) {
   int exp_lo = exponent_floor(quarters, bits);
+  uint32_t* zero_words = static_cast<uint32_t*>(sk_counters);
+  int zero_count = sk_counters ? (int)(SK_COUNTER_BYTES / sizeof(uint32_t)) : 0;
   uint32_t* rawA = reinterpret_cast<uint32_t*>(expA);
   uint32_t* rawB = reinterpret_cast<uint32_t*>(expB);
-  void* args[] = {&m, &n, &k, &quarters, &bits, &bxA, &bxB, &bk, &A, &B, &Ap, &Bp, &rawA, &rawB, &flags, &exp_lo};
+  void* args[] = {&m, &n, &k, &quarters, &bits, &bxA, &bxB, &bk, &A, &B, &Ap, &Bp, &rawA, &rawB, &flags, &exp_lo, &zero_words, &zero_count};
   const void* kern = nullptr;
   switch (limbs) {
     case 2: kern = reinterpret_cast<const void*>(prep_coop_kernel<2>); break;

@@ -414,3 +414,41 @@ def test_row_sharded_md_gemm_is_bit_identical_to_the_unsharded_call(world, cfg_i
         assert md.md_read_flags() == 0
     assert bits_equal(np.concatenate(parts, axis=1), whole)
     assert bits_equal(np.concatenate(parts_orders, axis=1), whole_orders)
+
+
+@pytest.mark.parametrize("cfg_idx,shape,Q,S,schedule", [
+    (1, (1000, 700, 200), 8, 8, 1),     # dd, 64 x 32 tiles: 16 x 22 = 352 = 2.4 waves of 148; ragged m, n; 25 slabs in units of 2
+    (3, (1000, 700, 72), 9, 9, 1),      # cfg3's distribution with the ninth quarter
+    (3, (700, 1000, 40), 8, 9, 1),      # an extended order set
+    (4, (400, 300, 90), 16, 16, 2),     # qd, 32 x 16 tiles: 13 x 19 = 247 tiles
+    (4, (700, 500, 40), 16, 16, 1),     # qd, 22 x 32 = 704 tiles = 4.8 waves: static waves, then the queue
+    (0, (1600, 1600, 64), 8, 8, 2),     # 25 x 50 = 1250 tiles = 8.4 waves, the queue from the first tile on
+    (2, (1601, 1530, 8), 8, 8, 1),      # one slab per tile: the units are whole tiles; 7 static waves first
+    (2, (1024, 1024, 7), 6, 6, 1),      # 6 slices of 19 bits
+])
+def test_dynamic_tile_schedule_is_bit_identical_to_the_static_lists(cfg_idx, shape, Q, S, schedule):
+    """MD_OPT_TILE_SCHEDULE 1 / 2: the CTAs of the persistent kernel claim their tiles (and, at the end, k-units of the last tiles)
+    from a queue counter instead of walking static lists (an option; the static lists stay the default).  Every partial order sum is exact (R6), so the order matrices
+    and C must not differ in a bit from the static schedule, whichever CTA computed what -- repeated, because the assignment
+    differs from run to run -- and the order matrices must equal the oracle's."""
+    cfg, A, B = gen(cfg_idx, *shape)
+    W = 19 if Q == 6 else 13
+    dA, dB = dev(A), dev(B)
+    out = {}
+    try:
+        with md.Workspace(cfg.m, cfg.n, cfg.k, cfg.limbs, Q, bits=W, orders=S):
+            md.md_set_option(md.MD_OPT_TILE_SCHEDULE, 0)
+            out["static"] = (host(md.md_gemm_orders(dA, dB)), host(md.md_gemm(dA, dB)))
+            md.md_set_option(md.MD_OPT_TILE_SCHEDULE, schedule)
+            for rep in range(3):
+                out[rep] = (host(md.md_gemm_orders(dA, dB)), host(md.md_gemm(dA, dB)))
+            assert md.md_read_flags() == 0
+    finally:
+        md.md_set_option(md.MD_OPT_TILE_SCHEDULE, 0)
+    for rep in range(3):
+        assert bits_equal(out[rep][0], out["static"][0]) and bits_equal(out[rep][1], out["static"][1]), rep
+    si, sj = inputs.sample_indices(cfg, 4096, salt=7)
+    Aq, eA, _ = orc.split(A, 0, Q, bits=W)
+    Bq, eB, _ = orc.split(B, 1, Q, bits=W)
+    want = orc.orders_int_samples(Aq, eA, Bq, eB, si, sj, orders=S, bits=W)
+    assert bits_equal(out[0][0][:, si, sj].T, want)
