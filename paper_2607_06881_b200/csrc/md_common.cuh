@@ -43,6 +43,26 @@ __device__ __forceinline__ void renorm_add(double (&r)[L + 1], double x) {
   for (int l = 0; l < L; l++) two_sum(r[l], x, r[l], x);
   r[L] = __dadd_rn(r[L], x);
 }
+// renorm_add for the TWO elements a thread owns in a DMMA tile, interleaved (two independent dependency chains side by side:
+// a cascade is 5 L dependent additions long and latency-bound on its own), and cut short once there is nothing left to carry
+// down: after a group of four levels, if the carried term of BOTH elements is zero in EVERY lane of the warp, the remaining
+// TwoSums would add zero to their terms and are skipped.  Same values as two calls of renorm_add (a skipped TwoSum(r, 0) returns
+// (r, 0)); the orders arrive smallest first, so the early ones occupy only the top few terms of the 17-term accumulator of a
+// hexa double and most of the cascade moved zeros.  All 32 lanes must call it together.
+template <int L>
+__device__ __forceinline__ void renorm_add2(double (&r0)[L + 1], double (&r1)[L + 1], double x0, double x1) {
+#pragma unroll
+  for (int g = 0; g < L; g += 4) {
+#pragma unroll
+    for (int l = g; l < g + 4 && l < L; l++) {
+      two_sum(r0[l], x0, r0[l], x0);
+      two_sum(r1[l], x1, r1[l], x1);
+    }
+    if (g + 4 < L && __all_sync(0xffffffffu, x0 == 0.0 && x1 == 0.0)) return;
+  }
+  r0[L] = __dadd_rn(r0[L], x0);
+  r1[L] = __dadd_rn(r1[L], x1);
+}
 template <int L>
 __device__ __forceinline__ void renorm_finish(double (&r)[L + 1], double (&out)[L]) {
   // bottom-up: r[0] becomes fl(total), the rest the successive rounding errors
@@ -57,6 +77,26 @@ __device__ __forceinline__ void renorm_finish(double (&r)[L + 1], double (&out)[
   }
 #pragma unroll
   for (int l = 0; l < L; l++) out[l] = r[l];
+}
+
+// renorm_finish for two elements, interleaved (same operations per element)
+template <int L>
+__device__ __forceinline__ void renorm_finish2(double (&r0)[L + 1], double (&r1)[L + 1], double (&out0)[L], double (&out1)[L]) {
+#pragma unroll
+  for (int l = L; l >= 1; l--) {
+    two_sum(r0[l - 1], r0[l], r0[l - 1], r0[l]);
+    two_sum(r1[l - 1], r1[l], r1[l - 1], r1[l]);
+  }
+#pragma unroll(L <= 4 ? L : 1)
+  for (int sweep = 0; sweep < L; sweep++) {
+#pragma unroll
+    for (int l = 0; l < L; l++) {
+      two_sum(r0[l], r0[l + 1], r0[l], r0[l + 1]);
+      two_sum(r1[l], r1[l + 1], r1[l], r1[l + 1]);
+    }
+  }
+#pragma unroll
+  for (int l = 0; l < L; l++) out0[l] = r0[l], out1[l] = r1[l];
 }
 
 template <int L, int S>

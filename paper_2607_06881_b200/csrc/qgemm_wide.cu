@@ -242,22 +242,37 @@ __device__ __forceinline__ void wide_epilogue(const WideCtx& x, const double (&a
   // into an (L+1)-term accumulator; with R ranges the accumulator travels range R-1 -> ... -> range 0.
 #pragma unroll
   for (int rr = R - 1; rr >= 0; rr--) {
-    if (rr == RANGE) {
+    if (rr == RANGE) {  // both elements of the thread side by side, the cascades cut short where only zeros are left (renorm_add2)
+      double r0[L + 1], r1[L + 1];
+      double* slot0 = x.xchg + (size_t)((t * 2 + 0) * (L + 1)) * 32 + lane;
+      double* slot1 = x.xchg + (size_t)((t * 2 + 1) * (L + 1)) * 32 + lane;
 #pragma unroll
-      for (int e = 0; e < 2; e++) {
-        double r[L + 1];
-        double* slot = x.xchg + (size_t)((t * 2 + e) * (L + 1)) * 32 + lane;
+      for (int l = 0; l <= L; l++) {
+        r0[l] = (RANGE == R - 1) ? 0.0 : slot0[l * 32];
+        r1[l] = (RANGE == R - 1) ? 0.0 : slot1[l * 32];
+      }
+      // a ROLLED loop over the orders, fed from a copy of the accumulators in local memory: unrolled, the recombination of a
+      // hexa double was ~10 000 straight-line instructions per range executed once per tile -- every tile end re-fetched
+      // 160 KB of code per warp through the instruction cache
+      // (hexa double 512^3: 0.898 -> 0.931 of the peak; octo double's recombination is a quarter of the code and stays unrolled:
+      // rolled it measured 0.9886 -> 0.9862)
+      if constexpr (L >= 16) {
+        double tmp[S1 - S0][2];
 #pragma unroll
-        for (int l = 0; l <= L; l++) r[l] = (RANGE == R - 1) ? 0.0 : slot[l * 32];
+        for (int i = 0; i < S1 - S0; i++) tmp[i][0] = acc[i][0], tmp[i][1] = acc[i][1];
+        const int s_top = C::GENERIC ? (Sr < S1 ? Sr : S1) : S1;
+#pragma unroll 1
+        for (int s = s_top - 1; s >= S0; s--) renorm_add2<L>(r0, r1, tmp[s - S0][0], tmp[s - S0][1]);
+      } else {
 #pragma unroll
         for (int s = S1 - 1; s >= S0; s--)
-          if (!C::GENERIC || s < Sr) renorm_add<L>(r, acc[s - S0][e]);
-        if (RANGE > 0) {
+          if (!C::GENERIC || s < Sr) renorm_add2<L>(r0, r1, acc[s - S0][0], acc[s - S0][1]);
+      }
+      if (RANGE > 0) {
 #pragma unroll
-          for (int l = 0; l <= L; l++) slot[l * 32] = r[l];
-        } else {
-          renorm_finish<L>(r, out[e]);
-        }
+        for (int l = 0; l <= L; l++) slot0[l * 32] = r0[l], slot1[l * 32] = r1[l];
+      } else {
+        renorm_finish2<L>(r0, r1, out[0], out[1]);
       }
     }
     if (R > 1) __syncthreads();  // hand-over to the next range; the last one keeps the next tile's writers behind the readers
