@@ -68,6 +68,7 @@ def parse_args():
     ap.add_argument("--quarters", type=int, default=0, help="override the config's quarter count (MD_OPT_QUARTERS)")
     ap.add_argument("--orders", type=int, default=0, help="kept product orders S (MD_OPT_ORDERS); default = quarters")
     ap.add_argument("--raster-group", type=int, default=0, help="MD_OPT_RASTER_GROUP (tile rows per raster group; 0 = default)")
+    ap.add_argument("--host-blocks", type=int, default=0, help="MD_OPT_HOST_BLOCKS for the e2e leg (0 = automatic; n = blocks of C; PR * 256 + PC = explicit panels)")
     ap.add_argument("--tile-schedule", type=int, default=0, choices=(0, 1, 2),
                     help="MD_OPT_TILE_SCHEDULE: 0 = static stream-K lists (default), 1 = hybrid (static waves, then a tile queue), 2 = tile queue only")
     ap.add_argument("--one-launch", type=int, default=0, choices=[0, 1, 2],
@@ -409,6 +410,7 @@ def run_ours(args):
     md.md_set_option(md.MD_OPT_RASTER_GROUP, args.raster_group)
     md.md_set_option(md.MD_OPT_ONE_LAUNCH, args.one_launch)
     md.md_set_option(md.MD_OPT_TILE_SCHEDULE, args.tile_schedule)
+    md.md_set_option(md.MD_OPT_HOST_BLOCKS, args.host_blocks)
     # weak scaling: the global A has world * m rows, rank r owns one block of m rows (no collective on the data path)
     if args.slices == "adaptive":
         base = base.with_slices(*md.md_plan_slices(base.k, base.limbs))

@@ -1,7 +1,11 @@
 // split.cu -- steps a1 + a2 of the hot path: exponent vectors and quarter planes (include/mdgemm.h: md_split).
 //   PAPER.md:47-49 (13-bit quarters with exponents 0,-13,-26,-39), :95 (balanced = exponents on an equally spaced grid),
 //   :124-142 (moving bits between parts without changing the value; zeros keep the desired exponent).
-// HBM-bound: reads 8*limbs and writes 8*quarters bytes per element, once.
+// The splitters read 8*limbs and write 8*quarters bytes per element, once, and run at the HBM roofline from a few hundred MB on
+// (split_kernel 0.96, split_packed_kernel 0.95-0.98 of the measured copy peak at 4096^2: profiles/r04_split_renorm_ncu.md).  What is
+// NOT HBM-bound: row_exponent_kernel (134 MB in 36 us = 3.7 TB/s at 4096^2: a block per row leaves too few loads in flight;
+// 0.03 % of an md_gemm step) and the cooperative prep_coop_kernel below 1024^3, which is bound by its three grid-wide barriers
+// (12 us at 256^3 for 5 MB: profiles/r04_small_sizes.md section 4).
 #include <cooperative_groups.h>
 
 #include "md_common.cuh"
