@@ -23,7 +23,7 @@ constexpr int PACK_BK = 8, PACK_BK_WIDE = 4;
 __host__ __device__ constexpr int pack_bk(int limbs) { return limbs <= 4 ? PACK_BK : PACK_BK_WIDE; }
 
 // CTA tile extent along the group index: BM (axis 0) or BN (axis 1) of the fused GEMM configuration for (limbs, quarters)
-// (dd 64 x 32, qd 32 x 16 -- 64 x 32 with the 11 / 12 wide slices of MD_OPT_SLICE_BITS, whose accumulators leave room for
+// (dd 64 x 32, qd 32 x 32 -- 64 x 32 with the 11 / 12 wide slices of MD_OPT_SLICE_BITS, whose accumulators leave room for
 // four 8x8 tiles per warp: qgemm_packed.cu; od 32 x 16, hd 16 x 8 -- 16 x 16 in 44 wide slices: qgemm_wide.cu).
 // small = the 32 x 16 tile instance of the double-double kernel that md_gemm picks when the 64 x 32 tiles would not fill the
 // SMs (qgemm_packed.cu: PCfgDDS); every other format ignores it.
@@ -31,6 +31,7 @@ __host__ __device__ constexpr int pack_bx(int limbs, int quarters, int axis, boo
   return (small && limbs == 2) ? (axis == 0 ? 32 : 16)
          : (limbs == 4 && quarters <= 10) ? (axis == 0 ? 64 : 16)  // quad double, chunked accumulation: 16 x 8 warp tile
          : (limbs == 2 || (limbs == 4 && quarters <= 12)) ? (axis == 0 ? 64 : 32)
+         : limbs == 4 ? 32  // quad double with the paper's 16 (17, 18) quarters: 32 x 32 CTA tile, 8 x 16 warp tile
          : limbs == 16 ? (axis == 0 ? 16 : (quarters <= 44 ? 16 : 8)) : (axis == 0 ? 32 : 16);
 }
 

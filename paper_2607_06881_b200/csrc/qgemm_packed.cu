@@ -652,13 +652,13 @@ cudaError_t launch_chunked(int m, int n, int k, int chunk, const double* Ap, con
   return cudaGetLastError();
 }
 
-// double double: 64 x 32 CTA tile, 8 warps (4 x 2), 16 x 16 warp tile.  quad double: 32 x 16 CTA tile, 8 x 8 warp tile
+// double double: 64 x 32 CTA tile, 8 warps (4 x 2), 16 x 16 warp tile.  quad double: 32 x 32 CTA tile, 8 x 16 warp tile
 // (16 orders x 2 registers per 8x8 tile).
 template <int Q, int S = Q> using PCfgDD = PCfg<Q, 2, 4, 2, 2, 2, S>;
 // double double on 32 x 16 CTA tiles (8 x 8 warp tiles): four times the tiles, for problems whose 64 x 32 tiles would not
 // fill the SMs -- every tile would be cut along k and each CTA would flush a whole tile of partial sums through L2
 template <int Q> using PCfgDDS = PCfg<Q, 2, 4, 2, 1, 1>;
-template <int Q, int S = Q> using PCfgQD = PCfg<Q, 4, 4, 2, 1, 1, S>;
+template <int Q, int S = Q> using PCfgQD = PCfg<Q, 4, 4, 2, 1, 2, S>;
 // quad double in 11 / 12 wide slices (MD_OPT_SLICE_BITS): 22 / 24 accumulator registers per 8x8 tile leave room for the
 // double-double warp tile (16 x 16), which halves the LDS and L2 traffic per DMMA and doubles the DMMAs per slab
 template <int Q> using PCfgQDW = PCfg<Q, 4, 4, 2, 2, 2>;
