@@ -125,6 +125,33 @@ def test_identity_and_small_integer_products(cfg_idx):
     assert bool((got == orc.split(Bm, 1)[0]).all())
 
 
+@pytest.mark.parametrize("cfg_idx", WIDE)
+def test_recombination_when_only_some_lanes_carry_something(cfg_idx):
+    """The recombination of the wide formats stops a TwoSum cascade once EVERY lane of the warp carries zero (renorm_add2).  Rows
+    of zeros, rows with a single power of two and exactly cancelling pairs next to dense rows put lanes that carry nothing beside
+    lanes that do, in one 8 x 8 tile: the fused result must still equal the standalone md_renorm of the dumped orders bit for bit
+    (which adds every order through the whole cascade) and meet the tolerance against the exact product."""
+    cfg, A, B = gen(cfg_idx, 40, 24, 36)
+    L = cfg.limbs
+    A[:, 0::4, :] = 0.0                                  # zero rows
+    A[:, 1::4, :] = 0.0
+    A[0, 1::4, 5] = 2.0 ** -7                            # a single power of two: one non-zero order per element
+    A[:, 2::4, 1::2] = -A[:, 2::4, 0::2]                 # a_{2j+1} = -a_{2j} ...
+    B[:, 1::2, :8] = B[:, 0::2, :8]                      # ... against b_{2j+1} = b_{2j} in the first 8 columns: exact zeros
+    with md.Workspace(cfg.m, cfg.n, cfg.k, L, cfg.quarters):
+        dA, dB = dev(A), dev(B)
+        C = host(md.md_gemm(dA, dB))
+        orders = md.md_gemm_orders(dA, dB)
+        assert md.md_read_flags() == 0
+    assert bool((C == host(md.md_renorm(orders, L))).all())
+    assert not C[:, 0::4, :].any() and not C[:, 2::4, :8].any()
+    r = orc.exact_all(A, B, C)
+    assert (r["err"] <= TOL[L] * r["W"]).all()
+    Aq, eA, _ = orc.split(A, 0)
+    Bq, eB, _ = orc.split(B, 1)
+    assert bool((host(orders) == orc.orders_int(Aq, eA, Bq, eB)).all())
+
+
 def test_more_tiles_than_sms_uses_the_stream_k_tail():
     """hd 16x8 tiles: 200 x 160 outputs = 13 x 20 = 260 tiles on 148 CTAs -> 1 whole wave + 112 stream-K tiles."""
     cfg, A, B = gen(6, 200, 160, 40)
