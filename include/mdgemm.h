@@ -102,7 +102,7 @@ enum {
                             share their operand slabs through L2).  0 = default 8 (the best of the measured 4 / 8 / 16 / 32,
                             profiles/).  Same bits for any value. */
   MD_OPT_ONE_LAUNCH = 9,  /* md_gemm / md_gemm_orders, double double (8 quarters) and quad double (16): 0 = automatic -- when the
-                            32 x 16 tiles of C number at most the SMs (up to about 256^3) the WHOLE path runs in ONE launch: each
+                            32 x 16 tiles of C number at most the SMs and a CTA's run of the contraction is at most 16 k-slabs (cubes: up to 192^3) the WHOLE path runs in ONE launch: each
                             CTA derives the exponents of its rows / columns, splits its operand slabs into shared memory and
                             issues the quarter products; a thread-block cluster shares a tile along k (no quarter planes in
                             HBM); 1 = wherever that kernel exists (any size); 2 = never.  Same bits. */

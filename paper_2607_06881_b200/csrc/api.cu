@@ -134,7 +134,7 @@ static inline bool use_fused_prep(int m, int n, int k) {
 // The whole path in ONE launch (fused_small.cu): where the 32 x 16 tiles of C number at most the SMs, so that a tile per CTA
 // (times the k-runs of its cluster) is a single wave, and a CTA's run of the contraction is short (at most 16 k-slabs: the CTA
 // splits its own operand slabs, which costs about 0.6 of the DMMA time of the slab -- measured: faster than prepare + multiply
-// up to 192^3, equal at 256^3, slower beyond).
+// up to 192^3 and slower from 224^3 on, where a tile's contraction is no longer shared by a cluster).
 constexpr int ONE_LAUNCH_MAX_SLABS = 16;
 static bool use_one_launch(int m, int n, int k, int limbs, int Q, int S, int bits) {
   if (g_opt.one_launch == 2 || !fused_small_supported(limbs, Q, S) || chunk_for(k, limbs, Q, S, bits) > 0) return false;
