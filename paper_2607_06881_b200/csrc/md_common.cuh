@@ -63,6 +63,38 @@ __device__ __forceinline__ void renorm_add2(double (&r0)[L + 1], double (&r1)[L 
   r0[L] = __dadd_rn(r0[L], x0);
   r1[L] = __dadd_rn(r1[L], x1);
 }
+// N CONSECUTIVE orders (x[0] first) into both elements: order i runs i levels behind order 0 -- at step t order i adds into
+// r[t - i], which order i - 1 has left one step earlier -- so every term still receives the orders in their sequence, the values
+// are those of N calls of renorm_add2, and 2 N independent TwoSum chains are in flight instead of two (a TwoSum level is five
+// dependent additions; the recombination of a hexa double is latency-bound on exactly that chain).  x[i][e]: order i, element e.
+template <int L, int N>
+__device__ __forceinline__ void renorm_add2xN(double (&r0)[L + 1], double (&r1)[L + 1], double (&x)[N][2]) {
+#pragma unroll
+  for (int g = 0; g < L + N - 1; g += 4) {
+#pragma unroll
+    for (int t = g; t < g + 4 && t < L + N - 1; t++) {
+#pragma unroll
+      for (int i = 0; i < N; i++) {
+        const int l = t - i;
+        if (l >= 0 && l < L) {
+          two_sum(r0[l], x[i][0], r0[l], x[i][0]);
+          two_sum(r1[l], x[i][1], r1[l], x[i][1]);
+        }
+      }
+    }
+    if (g + 4 < L + N - 1) {
+      bool zero = true;
+#pragma unroll
+      for (int i = 0; i < N; i++) zero = zero && x[i][0] == 0.0 && x[i][1] == 0.0;
+      if (__all_sync(0xffffffffu, zero)) return;
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < N; i++) {
+    r0[L] = __dadd_rn(r0[L], x[i][0]);
+    r1[L] = __dadd_rn(r1[L], x[i][1]);
+  }
+}
 template <int L>
 __device__ __forceinline__ void renorm_finish(double (&r)[L + 1], double (&out)[L]) {
   // bottom-up: r[0] becomes fl(total), the rest the successive rounding errors

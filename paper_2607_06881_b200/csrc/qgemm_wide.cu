@@ -261,8 +261,19 @@ __device__ __forceinline__ void wide_epilogue(const WideCtx& x, const double (&a
 #pragma unroll
         for (int i = 0; i < S1 - S0; i++) tmp[i][0] = acc[i][0], tmp[i][1] = acc[i][1];
         const int s_top = C::GENERIC ? (Sr < S1 ? Sr : S1) : S1;
+        // orders per trip, each one level behind the one before it (renorm_add2xN): 2 took hd 512^3 from 0.931 to 0.938; 4, and
+        // staggering the final sweeps of renorm_finish2 the same way, measured no further gain (profiles/r04_qgemm_hd.md)
+        constexpr int NW = 2;
+        int s = s_top - 1;
 #pragma unroll 1
-        for (int s = s_top - 1; s >= S0; s--) renorm_add2<L>(r0, r1, tmp[s - S0][0], tmp[s - S0][1]);
+        for (; s - (NW - 1) >= S0; s -= NW) {
+          double xs[NW][2];
+#pragma unroll
+          for (int i = 0; i < NW; i++) xs[i][0] = tmp[s - i - S0][0], xs[i][1] = tmp[s - i - S0][1];
+          renorm_add2xN<L, NW>(r0, r1, xs);
+        }
+#pragma unroll 1
+        for (; s >= S0; s--) renorm_add2<L>(r0, r1, tmp[s - S0][0], tmp[s - S0][1]);
       } else {
 #pragma unroll
         for (int s = S1 - 1; s >= S0; s--)
