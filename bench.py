@@ -671,6 +671,18 @@ def run_ours(args):
                         "sample": f"first {CPU_SAMPLE_ROWS} rows of A ({CPU_SAMPLE_ROWS}x{base.n} outputs of the "
                                   f"{base.m}x{base.n}x{base.k} problem), all of B; oracle split + {base.products} plain "
                                   f"fp64 quarter GEMM loops + exact renorm, OpenMP over rows"}
+        # the same leg also checks the device result of THIS run against the oracle's exact product (long accumulator) at a few
+        # seeded positions: a bench line whose numbers come from a wrong C should say so
+        try:
+            from oracle import md_oracle as orc
+            si, sj = inputs.sample_indices(cfg, 64, salt=4242)
+            chk = orc.exact_samples(A_host.numpy(), B_host.numpy(), si, sj, C.cpu().numpy())
+            tol = {2: 1e-28, 4: 1e-58, 8: 1e-120, 16: 1e-245}[L]
+            ratio = float((chk["err"] / (tol * chk["W"])).max())
+            cpu_baseline["sampled_parity"] = {"positions": 64, "max_err_over_tol_W": ratio, "within_tolerance": bool(ratio <= 1.0),
+                                              "tolerance": f"{tol:g} (|A||B|)_ij, exact product from the oracle's long accumulator"}
+        except Exception as exc:  # noqa: BLE001
+            cpu_baseline["sampled_parity"] = {"error": f"{type(exc).__name__}: {exc}"}
 
     in_mib, qp_mib = (A.numel() + B.numel() + C.numel()) * 8 / 2 ** 20, 8.0 * Q * (m * k + k * n) / 2 ** 20
     if in_mib > 126:
