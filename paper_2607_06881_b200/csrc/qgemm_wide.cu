@@ -72,9 +72,14 @@ struct WCfg {
   __host__ __device__ static constexpr int hi(int r) { return bound(r + 1); }
   // warp -> (tile, range).  Warps w and w + 4 share an SM sub-partition: R = 4 pairs ranges (0,1) and (2,3) there (1035 /
   // 1045 DMMAs per k-step), R = 2 the two ranges of one tile (990).
-  __host__ __device__ static constexpr int tile_of(int w) { return R == 1 ? w : R == 2 ? w % 4 : w / 4; }
+  // R = 2: the two warps of a sub-partition (w, w + 4) run the SAME range on different tiles (the two ranges are balanced,
+  // 496 / 494 products): hd in 44 slices 0.929 -> 0.942 of the peak against one warp of each range per sub-partition.  R = 4
+  // keeps mixed pairs: its ranges are unequal (528 / 507 / 505 / 540) and pairing equal ranges puts 1080 products on one
+  // sub-partition against 1010 on another (measured 0.940 -> 0.913); with every warp forced onto ONE range body (a timing
+  // experiment) the k loop runs at 0.99 of the peak instead of 0.96 -- profiles/r04_qgemm_hd.md
+  __host__ __device__ static constexpr int tile_of(int w) { return R == 1 ? w : R == 2 ? (((w >> 2) << 1) | (w & 1)) : w / 4; }
   __host__ __device__ static constexpr int range_of(int w) {
-    return R == 1 ? 0 : R == 2 ? w / 4
+    return R == 1 ? 0 : R == 2 ? ((w & 3) >> 1)
                       : (w < 4 ? (w == 0 ? 0 : w == 1 ? 2 : w == 2 ? 1 : 3) : (w == 4 ? 1 : w == 5 ? 3 : w == 6 ? 0 : 2));
   }
 };
