@@ -141,6 +141,56 @@ __device__ __forceinline__ void k_step_range(double (&acc)[S1 - S0][2], const do
   }
 }
 
+// The same k-step for a range with S0 > 0, ROLLED over q where the range has its full width.  For q <= S0 every one of the
+// W = S1 - S0 orders receives a product (p = S0 - q + j into accumulator j) and the register ring of A fragments repeats with
+// period RW = W + 1 in q, so RW consecutive q-steps make one trip of a loop whose register indices are compile-time constants; only
+// the remaining full-width steps (at least one) and the triangle q > S0 stay straight-line code.  Same products, same accumulators
+// (exact sums, R6); the point is CODE SIZE: one fully unrolled k-step body of about 10 KB stays in the SM's instruction
+// cache, two (hexa double in 44 slices: 496 + 494 DMMAs) do so only partly and were streamed from the L1.5 at 9.5 KB per
+// iteration of the k loop.  With the upper range rolled (312 DMMA sites instead of 494) they fit: 0.942 -> 0.964 of the peak.
+// NOT used for the four ranges of hexa double with 64 quarters: 528 + 325 + 175 + 180 sites (24 KB) still do not fit and the
+// loop overhead costs more than the smaller stream saves (0.940 -> 0.935); rotating the window by register moves instead (one
+// q-step per trip, 751 sites) stalls on the DMMAs that still read the registers (0.852).  profiles/r04_qgemm_hd.md.
+template <int Q, int S0, int S1, int AQ, int BQ>
+__device__ __forceinline__ void k_step_range_rolled(double (&acc)[S1 - S0][2], const double* __restrict__ As,
+                                                    const double* __restrict__ Bs) {
+  constexpr int W = S1 - S0, RW = W + 1;
+  constexpr int NTRIPS = S0 / RW, Q0 = NTRIPS * RW;  // trips cover q = 0 .. Q0 - 1 (Q0 <= S0: the step q = S0 is never inside a trip)
+  static_assert(S0 > 0 && S1 <= Q && S0 > RW, "a range above the first one, inside the quarter count");
+  double a[RW];
+#pragma unroll
+  for (int p = S0; p <= S1 - 1; p++) a[p % RW] = As[p * AQ];  // window of q = 0
+  double b = Bs[0];
+  const double* pa = As + S0 * AQ;  // A fragment p = S0 - q0
+  const double* pb = Bs;            // B fragment q0
+#pragma unroll 1
+  for (int trip = 0; trip < NTRIPS; trip++) {
+#pragma unroll
+    for (int u = 0; u < RW; u++) {  // q = trip * RW + u; fragment p = S0 - q + j sits in ring slot (S0 - u + j) % RW
+      const double b_next = pb[(u + 1) * BQ];
+      a[(S0 - u - 1) % RW] = pa[-(u + 1) * AQ];  // p = S0 - (q + 1) >= 0 inside the trips: the operand of the next step
+#pragma unroll
+      for (int j = 0; j < W; j++) dmma_8x8x4(acc[j], a[(S0 - u + j) % RW], b);
+      b = b_next;
+    }
+    pa -= RW * AQ;
+    pb += RW * BQ;
+  }
+#pragma unroll
+  for (int q = Q0; q <= S1 - 1; q++) {  // the last full-width steps and the triangle, as in k_step_range
+    double b_next = 0.0;
+    if (q + 1 <= S1 - 1) {
+      b_next = Bs[(q + 1) * BQ];
+      if (S0 - (q + 1) >= 0) a[(S0 - (q + 1)) % RW] = As[(S0 - (q + 1)) * AQ];
+    }
+    const int lo = S0 - q > 0 ? S0 - q : 0;
+    const int hi = S1 - 1 - q;
+#pragma unroll
+    for (int p = lo; p <= hi; p++) dmma_8x8x4(acc[p + q - S0], a[p % RW], b);
+    b = b_next;
+  }
+}
+
 // The same for a GENERIC instance: QMAX, [S0, S1) are the compile-time maxima, Qr <= QMAX and Sr the counts of this launch
 // (warp-uniform).  Every site of the maximal set is predicated; for a given q the live products are a prefix
 // p = lo .. min(hi, Qr - 1, Sr - 1 - q) of the compile-time range.
@@ -334,6 +384,7 @@ __device__ __forceinline__ void wide_consume(const WideCtx& x, int t, int lane, 
     mbar_wait(x.full_u32 + 8 * st, phase);
     const double* stage = x.stages + (size_t)st * STAGE_DOUBLES;
     if constexpr (C::GENERIC) k_step_range_rt<C::Q, S0, S1, C::AQ, C::BQ>(acc, stage + a_off, stage + b_off, x.Q, x.S);
+    else if constexpr (S0 > 0 && C::R == 2) k_step_range_rolled<C::Q, S0, S1, C::AQ, C::BQ>(acc, stage + a_off, stage + b_off);
     else k_step_range<C::Q, S0, S1, C::AQ, C::BQ>(acc, stage + a_off, stage + b_off);
     __syncwarp();
     if (lane == 0) mbar_arrive(x.empty_u32 + 8 * st);  // this warp is done reading the stage
