@@ -257,14 +257,16 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
   };
   auto flush_chunk = [&]() {  // orders from the smallest to the largest, as in renorm_orders (R9)
     if constexpr (CHUNK) {
+      // order by order across ALL elements of the thread (each element still receives its orders from the smallest to the largest):
+      // the TwoSum cascade of one element is a chain of dependent additions, 2 * MT * NT independent chains side by side hide it
 #pragma unroll
-      for (int i = 0; i < MT; i++)
+      for (int s = S - 1; s >= 0; s--)
 #pragma unroll
-        for (int j = 0; j < NT; j++)
+        for (int i = 0; i < MT; i++)
 #pragma unroll
-          for (int e = 0; e < 2; e++)
+          for (int j = 0; j < NT; j++)
 #pragma unroll
-            for (int s = S - 1; s >= 0; s--) renorm_add<L>(rexp[i][j][e], acc[s][i][j][e]);
+            for (int e = 0; e < 2; e++) renorm_add<L>(rexp[i][j][e], acc[s][i][j][e]);
       zero_acc();
     }
   };
