@@ -32,7 +32,7 @@ __host__ __device__ constexpr int pack_bx(int limbs, int quarters, int axis, boo
          : (limbs == 4 && quarters <= 10) ? (axis == 0 ? 64 : 16)  // quad double, chunked accumulation: 16 x 8 warp tile
          : (limbs == 2 || (limbs == 4 && quarters <= 12)) ? (axis == 0 ? 64 : 32)
          : limbs == 4 ? 32  // quad double with the paper's 16 (17, 18) quarters: 32 x 32 CTA tile, 8 x 16 warp tile
-         : limbs == 16 ? (axis == 0 ? 16 : (quarters <= 44 ? 16 : 8)) : (axis == 0 ? 32 : 16);
+         : (limbs == 16 && quarters <= 44) ? 16 : (axis == 0 ? 32 : 16);  // hd with 64 quarters: 32 x 16, one order range at a time
 }
 
 // The GENERIC-Q instances of qgemm_wide.cu (runtime quarter / order counts, any (limbs, quarters, orders) md_gemm accepts

@@ -497,6 +497,304 @@ qgemm_wide_kernel(int m, int n, int Qr, int Sr, SkPlan plan, const double* __res
   }
 }
 
+// =====================================================================================================================
+// Hexa double with the paper's 64 quarters, ONE ORDER RANGE AT A TIME (HPCfg / qgemm_hd_passes_kernel).
+//
+// The 64 accumulator sets of an 8x8 tile do not fit one thread.  The kernel above therefore lets four warps share a tile, each
+// with its own order range and its own fully unrolled k-step body -- 45 KB of straight-line code that the SM's instruction
+// cache can not hold: it is streamed from the L1.5 on every iteration of the k loop (profiles/r04_qgemm_hd.md: 96.9 M instruction
+// requests against 1.07 M for octo double) and the loop runs at 0.96 of the DMMA peak where one resident body runs at 0.99.
+// Here every warp owns a whole 8x8 tile (32 x 16 CTA tile, as octo double) and walks the contraction FOUR times, once per order
+// range, smallest orders first: during a pass all eight warps run the same body (about 10 KB, resident), keep that range's
+// <= 32 accumulator sets in registers and at the end of the pass fold them into the element's (L+1)-term expansion -- exactly
+// the order-by-order sequence of the recombination (R9), so the result equals the standalone md_renorm bit for bit.
+// There is no chain across warps and no block-wide barrier at a tile end any more.  Price: the operand slabs are fetched from L2
+// once per pass (of pass r only the quarters 0 .. hi(r) - 1, a prefix of the packed chunk), about 3x the L2 -> SM traffic of a
+// kernel that is tensor-bound by two orders of magnitude.
+// Work is cut along a VIRTUAL contraction of 4 KS slabs per tile (slab v = pass v / KS, k-slab v % KS), so the persistent
+// stream-K schedule above applies unchanged: a CTA that owns part of a tile adds the order sums of its slabs into the tile's
+// scratch (exact, R6) and the CTA that completes the count folds the totals range by range.
+struct HPCfg {
+  static constexpr int Q = 64, S = 64, L = 16, TM = 4, TN = 2, TILES = 8, WARPS = 8, THREADS = 256, PASSES = 4;
+  static constexpr int BM = TM * 8, BN = TN * 8, BK = PACK_BK_WIDE;
+  static constexpr int AQ = BK * BM, BQ = BK * BN, A_CHUNK = Q * AQ, B_CHUNK = Q * BQ;
+  static constexpr int STAGE_BYTES = (A_CHUNK + B_CHUNK) * 8, BAR_BYTES = 128, STAGES = 2;
+  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES;
+  static_assert(SMEM_BYTES <= SMEM_LIMIT, "two stages of all 64 quarters");
+  // pass p works on range 3 - p: [55,64) [45,55) [32,45) [0,32) -- 540 / 505 / 507 / 528 products per k-step
+  __host__ __device__ static constexpr int lo(int r) { return r == 0 ? 0 : r == 1 ? 32 : r == 2 ? 45 : 55; }
+  __host__ __device__ static constexpr int hi(int r) { return r == 0 ? 32 : r == 1 ? 45 : r == 2 ? 55 : 64; }
+};
+
+// fold the orders [S0, S1) held in acc (smallest first) into the two (L+1)-term expansions of the thread
+template <int S0, int S1>
+__device__ __forceinline__ void hp_fold(const double (&acc)[32][2], double (&r0)[HPCfg::L + 1], double (&r1)[HPCfg::L + 1]) {
+  constexpr int L = HPCfg::L;
+  double tmp[S1 - S0][2];  // a local-memory copy: the loop over the orders is rolled (code size, see wide_epilogue)
+#pragma unroll
+  for (int i = 0; i < S1 - S0; i++) tmp[i][0] = acc[i][0], tmp[i][1] = acc[i][1];
+  int s = S1 - 1;
+#pragma unroll 1
+  for (; s - 1 >= S0; s -= 2) {
+    double xs[2][2] = {{tmp[s - S0][0], tmp[s - S0][1]}, {tmp[s - 1 - S0][0], tmp[s - 1 - S0][1]}};
+    renorm_add2xN<L, 2>(r0, r1, xs);
+  }
+  if (s == S0) renorm_add2<L>(r0, r1, tmp[0][0], tmp[0][1]);
+}
+
+// one k-step of range r (warp-uniform) on the warp's tile
+__device__ __forceinline__ void hp_k_step(int r, double (&acc)[32][2], const double* As, const double* Bs) {
+  using C = HPCfg;
+  switch (r) {
+    case 0: k_step_range<C::Q, C::lo(0), C::hi(0), C::AQ, C::BQ>(acc, As, Bs); break;
+    case 1: k_step_range<C::Q, C::lo(1), C::hi(1), C::AQ, C::BQ>(reinterpret_cast<double(&)[C::hi(1) - C::lo(1)][2]>(acc), As, Bs); break;
+    case 2: k_step_range<C::Q, C::lo(2), C::hi(2), C::AQ, C::BQ>(reinterpret_cast<double(&)[C::hi(2) - C::lo(2)][2]>(acc), As, Bs); break;
+    default: k_step_range<C::Q, C::lo(3), C::hi(3), C::AQ, C::BQ>(reinterpret_cast<double(&)[C::hi(3) - C::lo(3)][2]>(acc), As, Bs); break;
+  }
+}
+
+__global__ void __launch_bounds__(HPCfg::THREADS, 1)
+qgemm_hd_passes_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, const double* __restrict__ Bp,
+                       double* __restrict__ order_planes, double* __restrict__ C_planes, double* __restrict__ sk_scratch,
+                       unsigned int* __restrict__ sk_counters) {
+  using C = HPCfg;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  constexpr int L = C::L, STAGE_DOUBLES = C::A_CHUNK + C::B_CHUNK;
+  double* const stages = reinterpret_cast<double*>(smem_raw);
+  const uint32_t stages_u32 = smem_u32(stages);
+  const uint32_t full_u32 = smem_u32(smem_raw + C::STAGES * C::STAGE_BYTES), empty_u32 = full_u32 + 8 * C::STAGES;
+  volatile int* const last_flag = reinterpret_cast<volatile int*>(smem_raw + C::STAGES * C::STAGE_BYTES + C::BAR_BYTES - 8);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int G = gridDim.x, cta = blockIdx.x;
+  const int KSV = plan.KS, KSR = KSV / C::PASSES;  // virtual slabs per tile (plan.KS) = 4 x the real k-slabs
+
+  // this CTA's segment list over the virtual slabs: its share of the stream-K slabs first, then whole tiles cta, cta + G, ...
+  const int sk_total = plan.sk_tiles * KSV;
+  const int g0 = min(cta * plan.sk_iters_per_cta, sk_total), g1 = min(g0 + plan.sk_iters_per_cta, sk_total);
+  const int n_sk = g1 > g0 ? (g1 - 1) / KSV - g0 / KSV + 1 : 0;
+  const int n_seg = n_sk + plan.dp_waves, total_slabs = (g1 - g0) + plan.dp_waves * KSV;
+  auto segment = [&](int i, int& tile, int& s0, int& s1) {
+    if (i < n_sk) {
+      const int r = g0 / KSV + i;
+      tile = plan.dp_waves * G + r, s0 = i == 0 ? g0 - r * KSV : 0, s1 = min(KSV, g1 - r * KSV);
+    } else {
+      tile = (i - n_sk) * G + cta, s0 = 0, s1 = KSV;
+    }
+  };
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < C::STAGES; s++) {
+      mbar_init(full_u32 + 8 * s, 1);
+      mbar_init(empty_u32 + 8 * s, C::WARPS);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (total_slabs == 0) return;
+
+  const int t = warp, ti = t / C::TN, tj = t % C::TN;
+  const int a_off = ti * 32 + lane, b_off = C::A_CHUNK + tj * 32 + lane;
+
+  // ---- producer (thread 0): one slab ahead of the consumers in a two-stage ring ------------------------------------------
+  int p_seg = -1, p_v = 0, p_end = 0, p_flat = 0, pst = 0, p_tm = 0, p_tn = 0;
+  auto produce_one = [&]() {
+    if (p_v == p_end) {
+      int tile;
+      segment(++p_seg, tile, p_v, p_end);
+      raster_tile(tile, plan.tiles_m, plan.tiles_n, p_tm, p_tn, plan.group_m);
+    }
+    const int pass = p_v / KSR, ks = p_v - pass * KSR;
+    const int nq = pass == 0 ? C::hi(3) : pass == 1 ? C::hi(2) : pass == 2 ? C::hi(1) : C::hi(0);  // quarters 0 .. hi - 1: a prefix of the chunk
+    const uint32_t dst = stages_u32 + pst * C::STAGE_BYTES, bar = full_u32 + 8 * pst;
+    mbar_expect_tx(bar, nq * (C::AQ + C::BQ) * 8);
+    bulk_g2s(dst, Ap + ((size_t)p_tm * KSR + ks) * C::A_CHUNK, nq * C::AQ * 8, bar);
+    bulk_g2s(dst + C::A_CHUNK * 8, Bp + ((size_t)p_tn * KSR + ks) * C::B_CHUNK, nq * C::BQ * 8, bar);
+    p_v++;
+    p_flat++;
+    pst ^= 1;
+  };
+  auto produce = [&]() {  // top of consumer iteration `it`: slab it + 1 into the stage slab it - 1 was read from
+    if (p_flat < total_slabs) {
+      if (p_flat >= C::STAGES) mbar_wait(empty_u32 + 8 * pst, ((p_flat / C::STAGES) + 1) & 1);
+      produce_one();
+    }
+  };
+  if (tid == 0) produce_one();
+
+  // ---- consumers ---------------------------------------------------------------------------------------------------------
+  // The two (L+1)-term expansions of the thread live in LOCAL memory between the passes (68 registers that the k loop of range 0
+  // -- 128 accumulator and 64 operand registers -- does not have): ex is only ever indexed through `zoff`, a run-time zero the
+  // compiler can not fold, so it is never promoted to registers; they are loaded into registers for a fold and stored back.
+  double acc[32][2], ex[2 * (L + 1)];
+  const int zoff = plan.flush_slabs;  // 0 (make_sk_plan)
+  auto zero_acc = [&]() {
+#pragma unroll
+    for (int s = 0; s < 32; s++) acc[s][0] = acc[s][1] = 0.0;
+  };
+  auto zero_exp = [&]() {
+#pragma unroll
+    for (int l = 0; l < 2 * (L + 1); l++) ex[zoff + l] = 0.0;
+  };
+  auto load_exp = [&](double (&r0)[L + 1], double (&r1)[L + 1]) {
+#pragma unroll
+    for (int l = 0; l <= L; l++) r0[l] = ex[zoff + l], r1[l] = ex[zoff + L + 1 + l];
+  };
+  auto store_exp = [&](const double (&r0)[L + 1], const double (&r1)[L + 1]) {
+#pragma unroll
+    for (int l = 0; l <= L; l++) ex[zoff + l] = r0[l], ex[zoff + L + 1 + l] = r1[l];
+  };
+  zero_acc();
+  zero_exp();
+  int c_seg = 0, c_tile, c_s0, c_s1;
+  segment(0, c_tile, c_s0, c_s1);
+  int c_v = c_s0;
+  const size_t planeC = (size_t)m * n;
+  const bool vec_ok = (n % 2 == 0) && (((uintptr_t)C_planes | (uintptr_t)order_planes) % 16 == 0);
+  // what is done with the accumulators of range r at the end of a pass (or of the CTA's part of it)
+  auto range_done = [&](int r, bool whole, int rsk, size_t at, bool inside, bool two) {
+    const int S0 = r == 0 ? C::lo(0) : r == 1 ? C::lo(1) : r == 2 ? C::lo(2) : C::lo(3);
+    const int W = (r == 0 ? C::hi(0) : r == 1 ? C::hi(1) : r == 2 ? C::hi(2) : C::hi(3)) - S0;
+    if (!whole) {  // stream-K part: exact fp64 reduction through the tile's scratch
+      double* sc = sk_scratch + (size_t)rsk * (C::S * C::BM * C::BN) + (size_t)t * 64 + lane * 2;
+#pragma unroll
+      for (int i = 0; i < 32; i++)
+        if (i < W) {
+          atomicAdd(sc + (size_t)(S0 + i) * (C::TILES * 64), acc[i][0]);
+          atomicAdd(sc + (size_t)(S0 + i) * (C::TILES * 64) + 1, acc[i][1]);
+        }
+      return;
+    }
+    if (order_planes && inside) {
+#pragma unroll
+      for (int i = 0; i < 32; i++)
+        if (i < W) {
+          if (vec_ok) {
+            *reinterpret_cast<double2*>(order_planes + (size_t)(S0 + i) * planeC + at) = make_double2(acc[i][0], acc[i][1]);
+          } else {
+            order_planes[(size_t)(S0 + i) * planeC + at] = acc[i][0];
+            if (two) order_planes[(size_t)(S0 + i) * planeC + at + 1] = acc[i][1];
+          }
+        }
+    }
+    if (C_planes) {
+      double r0[L + 1], r1[L + 1];
+      load_exp(r0, r1);
+      switch (r) {
+        case 0: hp_fold<C::lo(0), C::hi(0)>(acc, r0, r1); break;
+        case 1: hp_fold<C::lo(1), C::hi(1)>(acc, r0, r1); break;
+        case 2: hp_fold<C::lo(2), C::hi(2)>(acc, r0, r1); break;
+        default: hp_fold<C::lo(3), C::hi(3)>(acc, r0, r1); break;
+      }
+      store_exp(r0, r1);
+    }
+  };
+  auto write_C = [&](size_t at, bool inside, bool two) {  // after range 0: finish the expansions and write the limb planes once
+    if (C_planes) {
+      double r0[L + 1], r1[L + 1], o0[L], o1[L];
+      load_exp(r0, r1);
+      renorm_finish2<L>(r0, r1, o0, o1);
+      if (inside) {
+#pragma unroll
+        for (int l = 0; l < L; l++) {
+          if (vec_ok) {
+            *reinterpret_cast<double2*>(C_planes + l * planeC + at) = make_double2(o0[l], o1[l]);
+          } else {
+            C_planes[l * planeC + at] = o0[l];
+            if (two) C_planes[l * planeC + at + 1] = o1[l];
+          }
+        }
+      }
+    }
+    zero_exp();
+  };
+
+  int st = 0;
+  uint32_t phase = 0;
+  for (int it = 0; it < total_slabs; it++) {
+    if (tid == 0) produce();
+    mbar_wait(full_u32 + 8 * st, phase);
+    const double* stage = stages + (size_t)st * STAGE_DOUBLES;
+    const int pass = c_v / KSR, r = C::PASSES - 1 - pass;
+    hp_k_step(r, acc, stage + a_off, stage + b_off);
+    __syncwarp();
+    if (lane == 0) mbar_arrive(empty_u32 + 8 * st);
+    st ^= 1;
+    if (st == 0) phase ^= 1;
+    c_v++;
+    const bool seg_end = c_v == c_s1;
+    if (seg_end || c_v == (pass + 1) * KSR) {
+      int tm, tn;
+      raster_tile(c_tile, plan.tiles_m, plan.tiles_n, tm, tn, plan.group_m);
+      const int row = tm * C::BM + ti * 8 + (lane >> 2), col = tn * C::BN + tj * 8 + 2 * (lane & 3);
+      const bool inside = row < m && col < n, two = col + 1 < n, whole = c_s1 - c_s0 == KSV;
+      const size_t at = (size_t)row * n + col;
+      const int rsk = c_tile - plan.dp_waves * G;
+      range_done(r, whole, rsk, at, inside, two);
+      zero_acc();
+      if (whole && r == 0) write_C(at, inside, two);
+      if (seg_end) {
+        if (!whole) {
+          __threadfence();
+          __syncthreads();
+          if (tid == 0) {
+            const unsigned int mine = (unsigned int)(c_s1 - c_s0);
+            *last_flag = (atomicAdd(&sk_counters[rsk], mine) + mine == (unsigned int)KSV);
+          }
+          __syncthreads();
+          if (*last_flag) {  // every virtual slab of the tile has been added: the totals, range by range, smallest orders first
+            __threadfence();
+            const double* sc = sk_scratch + (size_t)rsk * (C::S * C::BM * C::BN) + (size_t)t * 64 + lane * 2;
+            for (int rr = C::PASSES - 1; rr >= 0; rr--) {
+              const int S0 = rr == 0 ? C::lo(0) : rr == 1 ? C::lo(1) : rr == 2 ? C::lo(2) : C::lo(3);
+              const int W = (rr == 0 ? C::hi(0) : rr == 1 ? C::hi(1) : rr == 2 ? C::hi(2) : C::hi(3)) - S0;
+#pragma unroll
+              for (int i = 0; i < 32; i++)
+                if (i < W) {
+                  const double2 v = __ldcg(reinterpret_cast<const double2*>(sc + (size_t)(S0 + i) * (C::TILES * 64)));
+                  acc[i][0] = v.x, acc[i][1] = v.y;
+                }
+              range_done(rr, true, rsk, at, inside, two);
+            }
+            zero_acc();
+            write_C(at, inside, two);
+          }
+        }
+        if (++c_seg < n_seg) {
+          segment(c_seg, c_tile, c_s0, c_s1);
+          c_v = c_s0;
+        }
+      }
+    }
+  }
+}
+
+cudaError_t launch_hd_passes(int m, int n, int k, const double* Ap, const double* Bp, double* order_planes, double* C_planes,
+                             void* sk_ws, cudaStream_t stream) {
+  using C = HPCfg;
+  const int tiles_m = (m + C::BM - 1) / C::BM, tiles_n = (n + C::BN - 1) / C::BN;
+  const long long KSR = ((long long)k + C::BK - 1) / C::BK;
+  if ((long long)tiles_m * tiles_n > 0x7fffffffLL || KSR * C::PASSES > 0x7fffffffLL) return cudaErrorInvalidValue;
+  const int G = sk_grid();
+  if (G <= 0) return cudaErrorInvalidDevice;
+  const SkPlan plan = make_sk_plan(tiles_m, tiles_n, (int)(KSR * C::PASSES), G);  // the VIRTUAL slab count: four passes over k
+  unsigned int* counters = static_cast<unsigned int*>(sk_ws);
+  double* scratch = reinterpret_cast<double*>(static_cast<char*>(sk_ws) + SK_COUNTER_BYTES);
+  cudaError_t err;
+  if (plan.sk_tiles > 0) {
+    err = cudaMemsetAsync(sk_ws, 0, SK_COUNTER_BYTES + sizeof(double) * (size_t)plan.sk_tiles * C::S * C::BM * C::BN, stream);
+    if (err != cudaSuccess) return err;
+  }
+  static bool attr_done[MD_MAX_DEVICES] = {};
+  const int dev = current_device();
+  if (dev < 0 || dev >= MD_MAX_DEVICES || !attr_done[dev]) {
+    err = cudaFuncSetAttribute(qgemm_hd_passes_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+    if (err != cudaSuccess) return err;
+    if (dev >= 0 && dev < MD_MAX_DEVICES) attr_done[dev] = true;
+  }
+  qgemm_hd_passes_kernel<<<G, C::THREADS, C::SMEM_BYTES, stream>>>(m, n, plan, Ap, Bp, order_planes, C_planes, scratch, counters);
+  return cudaGetLastError();
+}
+
 template <class C>
 cudaError_t launch_wide_cfg(int m, int n, int k, int Q, int S, const double* Ap, const double* Bp, double* order_planes,
                             double* C_planes, void* sk_ws, cudaStream_t stream) {
@@ -564,7 +862,7 @@ cudaError_t launch_qgemm_wide(int m, int n, int k, int limbs, int quarters, cons
   if (limbs == 8 && quarters == 32) err = launch_wide_cfg<WCfgOD>(m, n, k, Q, Q, Ap, Bp, order_planes, C_planes, sk_ws, stream);
   if (limbs == 8 && quarters == 22) err = launch_wide_cfg<WCfgOD22>(m, n, k, Q, Q, Ap, Bp, order_planes, C_planes, sk_ws, stream);
   if (limbs == 16 && quarters == 44) err = launch_wide_cfg<WCfgHD44>(m, n, k, Q, Q, Ap, Bp, order_planes, C_planes, sk_ws, stream);
-  if (limbs == 16 && quarters == 64) err = launch_wide_cfg<WCfgHD>(m, n, k, Q, Q, Ap, Bp, order_planes, C_planes, sk_ws, stream);
+  if (limbs == 16 && quarters == 64) err = launch_hd_passes(m, n, k, Ap, Bp, order_planes, C_planes, sk_ws, stream);
   if (err == cudaSuccess) *launches += 1;
   return err;
 }
