@@ -27,6 +27,8 @@
 //
 // Exactness as in qgemm_packed.cu: k * S <= 2^27 keeps every partial sum an integer below 2^53 units (PAPER.md:95-99
 // eq. 5; R6), so the result does not depend on the order in which warps, slabs or the hardware add things.
+#include <type_traits>
+
 #include "md_kernels.h"
 #include "md_packed.cuh"
 #include "qgemm_common.cuh"
@@ -542,17 +544,6 @@ __device__ __forceinline__ void hp_fold(const double (&acc)[32][2], double (&r0)
   if (s == S0) renorm_add2<L>(r0, r1, tmp[0][0], tmp[0][1]);
 }
 
-// one k-step of range r (warp-uniform) on the warp's tile
-__device__ __forceinline__ void hp_k_step(int r, double (&acc)[32][2], const double* As, const double* Bs) {
-  using C = HPCfg;
-  switch (r) {
-    case 0: k_step_range<C::Q, C::lo(0), C::hi(0), C::AQ, C::BQ>(acc, As, Bs); break;
-    case 1: k_step_range<C::Q, C::lo(1), C::hi(1), C::AQ, C::BQ>(reinterpret_cast<double(&)[C::hi(1) - C::lo(1)][2]>(acc), As, Bs); break;
-    case 2: k_step_range<C::Q, C::lo(2), C::hi(2), C::AQ, C::BQ>(reinterpret_cast<double(&)[C::hi(2) - C::lo(2)][2]>(acc), As, Bs); break;
-    default: k_step_range<C::Q, C::lo(3), C::hi(3), C::AQ, C::BQ>(reinterpret_cast<double(&)[C::hi(3) - C::lo(3)][2]>(acc), As, Bs); break;
-  }
-}
-
 __global__ void __launch_bounds__(HPCfg::THREADS, 1)
 qgemm_hd_passes_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, const double* __restrict__ Bp,
                        double* __restrict__ order_planes, double* __restrict__ C_planes, double* __restrict__ sk_scratch,
@@ -710,19 +701,34 @@ qgemm_hd_passes_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap,
 
   int st = 0;
   uint32_t phase = 0;
-  for (int it = 0; it < total_slabs; it++) {
-    if (tid == 0) produce();
-    mbar_wait(full_u32 + 8 * st, phase);
-    const double* stage = stages + (size_t)st * STAGE_DOUBLES;
+  // a RUN = the slabs of one pass inside the current segment: a tight loop with the range fixed at compile time
+  auto run = [&](auto rc, int count) {
+    constexpr int R_ = decltype(rc)::value;
+    for (int i = 0; i < count; i++) {
+      if (tid == 0) produce();
+      mbar_wait(full_u32 + 8 * st, phase);
+      const double* stage = stages + (size_t)st * STAGE_DOUBLES;
+      k_step_range<C::Q, C::lo(R_), C::hi(R_), C::AQ, C::BQ>(reinterpret_cast<double(&)[C::hi(R_) - C::lo(R_)][2]>(acc), stage + a_off,
+                                                             stage + b_off);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(empty_u32 + 8 * st);
+      st ^= 1;
+      if (st == 0) phase ^= 1;
+    }
+  };
+  for (int it = 0; it < total_slabs;) {
     const int pass = c_v / KSR, r = C::PASSES - 1 - pass;
-    hp_k_step(r, acc, stage + a_off, stage + b_off);
-    __syncwarp();
-    if (lane == 0) mbar_arrive(empty_u32 + 8 * st);
-    st ^= 1;
-    if (st == 0) phase ^= 1;
-    c_v++;
+    const int run_end = min(c_s1, (pass + 1) * KSR), count = run_end - c_v;
+    switch (r) {
+      case 0: run(std::integral_constant<int, 0>{}, count); break;
+      case 1: run(std::integral_constant<int, 1>{}, count); break;
+      case 2: run(std::integral_constant<int, 2>{}, count); break;
+      default: run(std::integral_constant<int, 3>{}, count); break;
+    }
+    it += count;
+    c_v = run_end;
     const bool seg_end = c_v == c_s1;
-    if (seg_end || c_v == (pass + 1) * KSR) {
+    {
       int tm, tn;
       raster_tile(c_tile, plan.tiles_m, plan.tiles_n, tm, tn, plan.group_m);
       const int row = tm * C::BM + ti * 8 + (lane >> 2), col = tn * C::BN + tj * 8 + 2 * (lane & 3);
