@@ -24,7 +24,7 @@ __host__ __device__ constexpr int pack_bk(int limbs) { return limbs <= 4 ? PACK_
 
 // CTA tile extent along the group index: BM (axis 0) or BN (axis 1) of the fused GEMM configuration for (limbs, quarters)
 // (dd 64 x 32, qd 32 x 32 -- 64 x 32 with the 11 / 12 wide slices of MD_OPT_SLICE_BITS, whose accumulators leave room for
-// four 8x8 tiles per warp: qgemm_packed.cu; od 32 x 16, hd 16 x 8 -- 16 x 16 in 44 wide slices: qgemm_wide.cu).
+// four 8x8 tiles per warp: qgemm_packed.cu; od 32 x 16, hd 32 x 16 -- 16 x 16 in 44 wide slices: qgemm_wide.cu).
 // small = the 32 x 16 tile instance of the double-double kernel that md_gemm picks when the 64 x 32 tiles would not fill the
 // SMs (qgemm_packed.cu: PCfgDDS); every other format ignores it.
 __host__ __device__ constexpr int pack_bx(int limbs, int quarters, int axis, bool small = false) {

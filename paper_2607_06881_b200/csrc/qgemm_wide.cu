@@ -9,9 +9,13 @@
 // order per thread, so 32 orders fill 128 registers and 64 orders do not fit a thread at all.  Hence
 //   * a warp owns ONE 8x8 tile of C and a contiguous ORDER RANGE [S0, S1) of at most 32 orders;
 //   * octo double: one range [0, 32) per tile, 8 tiles (32 x 16) per CTA;
-//   * hexa double: four ranges [0,32) [32,45) [45,55) [55,64) -- 528 / 507 / 505 / 540 products, balanced -- so the 8 warps
-//     of a CTA are 2 tiles (16 x 8) x 4 ranges, all fed from the same staged quarter tiles, and ranges are paired on the
-//     SM sub-partitions so that each issues 1035 or 1045 DMMAs per k-step (ideal 1040);
+//   * hexa double with the paper's 64 quarters: the four ranges [0,32) [32,45) [45,55) [55,64) -- 528 / 507 / 505 / 540
+//     products -- are walked ONE AFTER THE OTHER by every warp on its own 8x8 tile (qgemm_hd_passes_kernel, further down): four
+//     passes over the contraction, one resident k-step body at a time.  Four warps sharing a tile, each with its own range and
+//     body (WCfg<.., R = 4>: what round 1 ran, still used by the GENERIC hexa-double instance), lose 4 % of the k loop to the SM's
+//     instruction cache;
+//   * hexa double in 44 slices of 19 bits: two ranges [0,31) [31,44) per tile, 4 tiles (16 x 16) per CTA, both warps of an SM
+//     sub-partition on the same range, the upper range's k-step rolled (k_step_range_rolled) so that both bodies stay resident;
 //   * inside a k-step a range walks q = 0, 1, ... and needs the A fragments p in [S0-q, S1-1-q]: a window of S1-S0 quarters
 //     that slides down by one per q, kept in a register ring (one new LDS per q, issued one step ahead);
 //   * the recombination of a hexa double element is a chain over its four warps: the (L+1)-term accumulator of
