@@ -839,7 +839,7 @@ cudaError_t launch_wide_cfg(int m, int n, int k, int Q, int S, const double* Ap,
 
 using WCfgOD = WCfg<32, 8, 4, 2, 1>;   // octo double: 32 x 16 CTA tile, 8 tiles x 1 range
 using WCfgOD22 = WCfg<22, 8, 4, 2, 1>; // octo double in 22 slices of 19 bits (MD_OPT_SLICE_BITS; R14)
-using WCfgHD = WCfg<64, 16, 2, 1, 4>;  // hexa double: 16 x 8 CTA tile, 2 tiles x 4 ranges
+using WCfgHD = WCfg<64, 16, 2, 1, 4>;  // hexa double, 16 x 8 CTA tile, 2 tiles x 4 ranges: round 1's kernel, no longer launched (qgemm_hd_passes_kernel)
 using WCfgHD44 = WCfg<44, 16, 2, 2, 2>;  // hexa double in 44 slices of 19 bits: 16 x 16 CTA tile, 4 tiles x 2 ranges
 // GENERIC instances: runtime (Q, S) up to these maxima
 using WCfgGenDD = WCfg<GENERIC_QMAX_DD, 2, 4, 2, 1, GENERIC_SMAX_DD, true>;
