@@ -152,12 +152,20 @@ def test_recombination_when_only_some_lanes_carry_something(cfg_idx):
     assert bool((host(orders) == orc.orders_int(Aq, eA, Bq, eB)).all())
 
 
-def test_more_tiles_than_sms_uses_the_stream_k_tail():
-    """hd 16x8 tiles: 200 x 160 outputs = 13 x 20 = 260 tiles on 148 CTAs -> 1 whole wave + 112 stream-K tiles."""
-    cfg, A, B = gen(6, 200, 160, 40)
+@pytest.mark.parametrize("shape", [(200, 160, 40), (600, 300, 20), (600, 300, 3), (33, 17, 5)])
+def test_hexa_double_passes_kernel_whole_tiles_and_stream_k_parts(shape):
+    """Hexa double runs one order range at a time (qgemm_hd_passes_kernel: 32 x 16 CTA tiles, four passes over the contraction, the
+    stream-K schedule over a virtual contraction of 4 KS slabs).  (200, 160): 70 tiles on 148 CTAs, every tile cut, the cuts fall
+    inside and between passes; (600, 300): 19 x 19 = 361 tiles = two whole waves + 65 cut tiles; k = 3: one real k-slab, so a pass
+    is a single virtual slab; (33, 17): ragged edge tiles.  Order matrices bit-exact against the oracle, C within tolerance of
+    the exact product and equal to the standalone md_renorm of the dumped orders bit for bit."""
+    cfg, A, B = gen(6, *shape)
     with md.Workspace(cfg.m, cfg.n, cfg.k, 16):
-        got = host(md.md_gemm_orders(dev(A), dev(B)))
+        orders = md.md_gemm_orders(dev(A), dev(B))
         C = host(md.md_gemm(dev(A), dev(B)))
+        assert md.md_read_flags() == 0
+    assert bool((C == host(md.md_renorm(orders, 16))).all())
+    got = host(orders)
     si, sj = inputs.sample_indices(cfg, 300)
     Aq, eA, _ = orc.split(A, 0)
     Bq, eB, _ = orc.split(B, 1)
