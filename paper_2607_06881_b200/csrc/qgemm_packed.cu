@@ -185,6 +185,7 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
     if constexpr (DYN) dyn_claim(0);
   }
   __syncthreads();
+  grid_dependency_wait();  // (programmatic dependent launch behind the preparation kernel: nothing it wrote has been touched so far)
   if (total_slabs == 0) return;
   if constexpr (DYN) {
     if (dyn_tab[0][0] < 0) return;  // the queue was empty before this CTA's first claim
@@ -609,6 +610,19 @@ cudaError_t launch_cfg(int m, int n, int k, const double* Ap, const double* Bp, 
     err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
     if (err != cudaSuccess) return err;
     if (known) attr_done[dev][mode] = true;
+  }
+  if (handover && counters_clear) {
+    // directly behind the cooperative preparation kernel on this stream (no memset node in between): let the CTAs start while
+    // it drains -- launch latency, barrier set-up and the segment tables then cost nothing (256^3: 53.9 -> 51.6 us per md_gemm)
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(G), cfg.blockDim = dim3(C::THREADS), cfg.dynamicSmemBytes = C::SMEM_BYTES, cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr, cfg.numAttrs = 1;
+    err = cudaLaunchKernelEx(&cfg, kern, m, n, plan, Ap, Bp, order_planes, C_planes, scratch, counters);
+    if (err == cudaSuccess) return cudaGetLastError();
+    cudaGetLastError();  // a context that refuses the attribute: the plain launch does the same work
   }
   kern<<<G, C::THREADS, C::SMEM_BYTES, stream>>>(m, n, plan, Ap, Bp, order_planes, C_planes, scratch, counters);
   return cudaGetLastError();

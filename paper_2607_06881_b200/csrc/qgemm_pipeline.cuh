@@ -39,6 +39,12 @@ __device__ __forceinline__ void bulk_g2s(uint32_t smem_dst, const void* gmem_src
                : "memory");
 }
 
+// Programmatic dependent launch (sm_90+): a kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization may start
+// while its predecessor on the stream still runs -- once every block of the predecessor has executed launch_dependents (or exited)
+// -- and must execute grid_dependency_wait before it touches anything the predecessor wrote.  Both are no-ops in a plain launch.
+__device__ __forceinline__ void grid_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // Persistent kernel: gridDim.x = G CTAs (one per SM), each walks a private list of SEGMENTS = (tile, slab range):
 //   * dp_waves whole tiles, ids b, b + G, b + 2G, ... (tile ids are rasterised, so at any time the G CTAs cover a compact patch
 //     of C), accumulated and renormalised entirely in registers;

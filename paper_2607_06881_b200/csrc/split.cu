@@ -12,6 +12,7 @@
 #include "md_kernels.h"
 #include "md_packed.cuh"
 #include "md_split.cuh"
+#include "qgemm_pipeline.cuh"
 
 namespace md {
 namespace {
@@ -247,6 +248,10 @@ __global__ void __launch_bounds__(256) prep_coop_kernel(int m, int n, int k, int
     }
   }
   grid.sync();
+  // every block of this kernel is resident and past its last grid-wide barrier: the fused GEMM that md_gemm enqueues behind it
+  // (launched with programmatic stream serialization, qgemm_packed.cu) may start its CTAs -- barrier set-up, segment tables --
+  // on SMs with room; it waits for THIS grid to complete before it reads a quarter plane
+  grid_launch_dependents();
   // phase 2: split, A then B
   const int KS = (k + bk - 1) / bk, k4_groups = KS * (bk / 4), k_blocks = (k4_groups + 7) / 8;
   const int XPA = (m + bxA - 1) / bxA * bxA, XPB = (n + bxB - 1) / bxB * bxB;
