@@ -60,7 +60,8 @@ enum {
                                call cannot chunk the contraction (md_gemm_orders, md_qgemm, quad double and wider) */
   MD_ERR_WORKSPACE = -3,    /* no workspace registered, or it is too small (md_workspace_bytes) */
   MD_ERR_CUDA = -4,         /* a CUDA call failed */
-  MD_ERR_UNSUPPORTED = -5   /* combination of (limbs, quarters, orders) that has no kernel instantiation */
+  MD_ERR_UNSUPPORTED = -5,  /* combination of (limbs, quarters, orders) that has no kernel instantiation */
+  MD_ERR_STATIC_LIMIT = -6  /* md_gemm_static: the problem needs more than the built-in scratch (md_static_scratch_bytes) */
 };
 
 typedef void* md_stream;    /* a cudaStream_t */
@@ -352,6 +353,28 @@ int md_profile_read(float* split_ms_host, float* gemm_ms_host, int capacity);
  *   1 <= blocks; 1 <= warps_per_block <= 32; 1 <= iters < 2^25.
  * ------------------------------------------------------------------------------------------------------------------ */
 md_status md_probe_dmma(int blocks, int warps_per_block, int iters, double* sink, uint64_t* flops_host, md_stream stream);
+
+/* ---------------------------------------------------------------------------------------------------------------------
+ * md_gemm_static -- md_gemm (steps a1-a4: split, triangular quarter GEMM, recombination) for callers that can
+ *   NOT allocate device memory: code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  The
+ *   workspace md_gemm takes from md_set_workspace is a file-scope device array inside the library here (md_static_scratch_bytes()
+ *   = 64 MiB); the call allocates nothing (no cudaMalloc / cudaFree / allocating library routine), needs no md_set_workspace, and
+ *   runs the same kernels as md_gemm: the result is bit-identical.
+ *   A_planes / B_planes / C_planes, limbs, stream, options (MD_OPT_QUARTERS, ...): as md_gemm.
+ *   Limit: md_gemm_static_bytes(m, n, k, limbs) -- what this problem needs of the array with the current options, 0 for bad
+ *   arguments -- must not exceed md_static_scratch_bytes(): with the default options cubes up to 496^3 (double double), 352^3
+ *   (quad double), 192^3 (octo double); hexa double never fits (its stream-K scratch alone is 64 MiB).  Otherwise
+ *   MD_ERR_STATIC_LIMIT, with nothing enqueued.
+ *   Every GPU on which the library is used holds the 64 MiB until the process exits.  ALL calls on a device share the array, and
+ *   it keeps the last call's contents (each call clears what must start at zero, on `stream`): two calls that overlap on the
+ *   GPU -- different streams with no ordering between them -- RACE; serialise them.  The status word of the LAST call
+ *   (md_read_flags's bits) is read with md_gemm_static_read_flags, which synchronises `stream`.
+ * ------------------------------------------------------------------------------------------------------------------ */
+size_t md_static_scratch_bytes(void);
+size_t md_gemm_static_bytes(int m, int n, int k, int limbs);
+md_status md_gemm_static(int m, int n, int k, int limbs, const double* A_planes, const double* B_planes, double* C_planes,
+                         md_stream stream);
+md_status md_gemm_static_read_flags(uint32_t* flags_host, md_stream stream);
 
 /* Number of kernels this library has launched since load (all entry points), for launch accounting. */
 uint64_t md_launch_count(void);

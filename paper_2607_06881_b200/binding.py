@@ -16,6 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libmdgemm.so")
 
 MD_OK = 0
 MD_ERR_BAD_ARG, MD_ERR_K_TOO_LARGE, MD_ERR_WORKSPACE, MD_ERR_CUDA, MD_ERR_UNSUPPORTED = -1, -2, -3, -4, -5
+MD_ERR_STATIC_LIMIT = -6
 MD_OPT_QUARTERS, MD_OPT_ORDERS, MD_OPT_SLICE_BITS, MD_OPT_HOST_BLOCKS, MD_OPT_K_CHUNK, MD_OPT_FUSED_PREP, MD_OPT_TILE, MD_OPT_RASTER_GROUP = 1, 2, 3, 4, 5, 6, 7, 8
 MD_OPT_ONE_LAUNCH = 9
 MD_OPT_TILE_SCHEDULE = 10
@@ -49,6 +50,10 @@ _SIGNATURES = {
     "md_profile_enable": (_c.c_int, [_c.c_int]),
     "md_profile_read": (_c.c_int, [_c.c_void_p, _c.c_void_p, _c.c_int]),
     "md_probe_dmma": (_c.c_int, [_c.c_int] * 3 + [_c.c_void_p] * 3),
+    "md_static_scratch_bytes": (_c.c_size_t, []),
+    "md_gemm_static_bytes": (_c.c_size_t, [_c.c_int] * 4),
+    "md_gemm_static": (_c.c_int, [_c.c_int] * 4 + [_c.c_void_p] * 4),
+    "md_gemm_static_read_flags": (_c.c_int, [_c.c_void_p, _c.c_void_p]),
     "md_launch_count": (_c.c_uint64, []),
     "md_status_string": (_c.c_char_p, [_c.c_int]),
 }
@@ -188,6 +193,32 @@ def md_gemm(A: torch.Tensor, B: torch.Tensor, C: torch.Tensor | None = None, str
         C = torch.empty((limbs, m, n), dtype=torch.float64, device=A.device)
     _check(lib().md_gemm(m, n, k, limbs, _dev(A), _dev(B), _dev(C), _stream(stream)), "md_gemm")
     return C
+
+
+def md_static_scratch_bytes() -> int:
+    return lib().md_static_scratch_bytes()
+
+
+def md_gemm_static_bytes(m: int, n: int, k: int, limbs: int) -> int:
+    return lib().md_gemm_static_bytes(m, n, k, limbs)
+
+
+def md_gemm_static(A: torch.Tensor, B: torch.Tensor, C: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+    """md_gemm with the library's built-in scratch (include/mdgemm.h): no workspace, no allocation inside the call (pass C to
+    keep this wrapper from allocating the result either).  MdError(MD_ERR_STATIC_LIMIT) when the problem does not fit."""
+    limbs, m, k = A.shape
+    n = B.shape[2]
+    assert B.shape[0] == limbs and B.shape[1] == k
+    if C is None:
+        C = torch.empty((limbs, m, n), dtype=torch.float64, device=A.device)
+    _check(lib().md_gemm_static(m, n, k, limbs, _dev(A), _dev(B), _dev(C), _stream(stream)), "md_gemm_static")
+    return C
+
+
+def md_gemm_static_read_flags(stream=None) -> int:
+    out = ctypes.c_uint32(0)
+    _check(lib().md_gemm_static_read_flags(ctypes.addressof(out), _stream(stream)), "md_gemm_static_read_flags")
+    return out.value
 
 
 def md_gemm_auto(A: torch.Tensor, B: torch.Tensor, C: torch.Tensor | None = None, rel_tol: float = 0.0, stream=None):

@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmdgemm.so")
 COMPARE_LIB = os.path.join(HERE, "libmdcompare.so")
-SOURCES = ["api.cu", "split.cu", "renorm.cu", "qgemm.cu", "qgemm_packed.cu", "qgemm_wide.cu", "probe.cu", "plan.cu", "literal.cu", "qr.cu", "fused_small.cu"]
+SOURCES = ["api.cu", "split.cu", "renorm.cu", "qgemm.cu", "qgemm_packed.cu", "qgemm_wide.cu", "probe.cu", "plan.cu", "literal.cu", "qr.cu", "fused_small.cu", "static_gemm.cu"]
 HEADERS = [os.path.join(CSRC, "api_internal.h"), os.path.join(CSRC, "md_common.cuh"), os.path.join(CSRC, "md_arith.cuh"), os.path.join(CSRC, "md_kernels.h"), os.path.join(CSRC, "md_packed.cuh"), os.path.join(CSRC, "md_split.cuh"),
            os.path.join(CSRC, "qgemm_common.cuh"), os.path.join(CSRC, "qgemm_pipeline.cuh"),
            os.path.join(os.path.dirname(HERE), "include", "mdgemm.h")]

@@ -783,6 +783,7 @@ const char* md_status_string(md_status status) {
     case MD_ERR_WORKSPACE: return "MD_ERR_WORKSPACE: workspace missing or too small (md_workspace_bytes / md_host_scratch_bytes)";
     case MD_ERR_CUDA: return "MD_ERR_CUDA: a CUDA call failed (see cudaGetLastError)";
     case MD_ERR_UNSUPPORTED: return "MD_ERR_UNSUPPORTED: no kernel for this (limbs, quarters, orders)";
+    case MD_ERR_STATIC_LIMIT: return "MD_ERR_STATIC_LIMIT: the problem needs more than the 64 MiB built-in scratch of md_gemm_static (md_gemm_static_bytes > md_static_scratch_bytes); use md_gemm with a workspace";
     default: return "unknown md_status";
   }
 }
