@@ -69,8 +69,8 @@ def parse_args():
     ap.add_argument("--orders", type=int, default=0, help="kept product orders S (MD_OPT_ORDERS); default = quarters")
     ap.add_argument("--raster-group", type=int, default=0, help="MD_OPT_RASTER_GROUP (tile rows per raster group; 0 = default)")
     ap.add_argument("--host-blocks", type=int, default=0, help="MD_OPT_HOST_BLOCKS for the e2e leg (0 = automatic; n = blocks of C; PR * 256 + PC = explicit panels)")
-    ap.add_argument("--tile-schedule", type=int, default=0, choices=(0, 1, 2),
-                    help="MD_OPT_TILE_SCHEDULE: 0 = static stream-K lists (default), 1 = hybrid (static waves, then a tile queue), 2 = tile queue only")
+    ap.add_argument("--tile-schedule", type=int, default=0, choices=(0, 1, 2, 3),
+                    help="MD_OPT_TILE_SCHEDULE: 0 = automatic (hybrid from many whole-tile waves on), 1 = hybrid wherever possible, 2 = tile queue only, 3 = static lists")
     ap.add_argument("--one-launch", type=int, default=0, choices=[0, 1, 2],
                     help="MD_OPT_ONE_LAUNCH: 0 = automatic (single-wave problems run a1-a4 in one kernel), 1 = wherever it exists, 2 = never")
     ap.add_argument("--micro", action="store_true",

@@ -108,13 +108,13 @@ enum {
                             issues the quarter products; a thread-block cluster shares a tile along k (no quarter planes in
                             HBM); 1 = wherever that kernel exists (any size); 2 = never.  Same bits. */
   MD_OPT_TILE_SCHEDULE = 10, /* fused quarter GEMM of double / quad double (the persistent kernel), problems of at least one whole wave
-                            of tiles: 0 = the static stream-K lists (default: the CTAs stay in lock-step and share operand slabs
-                            through L2); 1 = hybrid -- every whole-tile wave but the last one static, then the CTAs CLAIM what is
-                            left from a queue (whole tiles, then the last one to two waves cut along k into 16 units per tile,
-                            partial order sums combined by exact fp64 red.add), so that all SMs finish within one unit's time;
-                            2 = the queue from the first tile on.  Same bits for all three (every partial sum is exact, DESIGN.md
-                            R6).  Measured: the queue levels the finishing times but costs L2 locality; 1 is within 0.1 % of 0,
-                            2 is 0.5-1.4 % slower (profiles/r04_dynamic_schedule.md). */
+                            of tiles.  The static stream-K lists keep the CTAs in lock-step on neighbouring tiles (they share operand
+                            slabs through L2); a queue lets a CTA that has fallen behind take less.  0 = automatic: HYBRID -- every
+                            whole tile keeps its static place, only the k-units (16 per tile) of the last, partial wave's tiles
+                            are claimed from a queue, partial order sums combined by exact fp64 red.add -- from about 10 whole waves
+                            on for quad double and 48 for double double, the static lists below; 1 = hybrid wherever there is a
+                            whole wave; 2 = the queue for every tile; 3 = static lists always.  Same bits for all (every partial
+                            sum is exact, R6).  Measured: profiles/r04_dynamic_schedule.md. */
   MD_OPT_HOST_BLOCKS = 4 /* md_gemm_host only: number of blocks C is cut into for overlapping copies and kernels.
                             Default 0 = automatic (about one wave of CTA tiles per block, at most 32); 1 = no overlap;
                             PR * 256 + PC = explicit numbers of row panels and column panels (each <= 64). */

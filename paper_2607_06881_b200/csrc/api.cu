@@ -296,7 +296,7 @@ md_status md_set_option(int key, int value) {
       g_opt.one_launch = value;
       return MD_OK;
     case MD_OPT_TILE_SCHEDULE:
-      if (value < 0 || value > 2) return MD_ERR_BAD_ARG;
+      if (value < 0 || value > 3) return MD_ERR_BAD_ARG;
       g_opt.tile_schedule = value;
       return MD_OK;
     case MD_OPT_HOST_BLOCKS:  // 0 = automatic, 1..32 blocks, or PR * 256 + PC (explicit panel counts, each <= 64)

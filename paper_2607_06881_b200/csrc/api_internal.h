@@ -20,7 +20,7 @@ struct Options {
   int tile = 0;          // 0 = automatic, 1 = the 32 x 16 tile instance wherever it exists, 2 = never
   int fused_prep = 0;    // 0 = automatic (small / medium operands), 1 = always, 2 = never
   int one_launch = 0;    // 0 = automatic (single-wave problems), 1 = wherever the kernel exists, 2 = never
-  int tile_schedule = 0; // 0 = static stream-K lists, 1 = hybrid (static waves, then a tile queue), 2 = tile queue only
+  int tile_schedule = 0; // 0 = automatic (hybrid from many whole-tile waves on), 1 = hybrid wherever possible, 2 = tile queue only, 3 = static lists
   int k_chunk = 0;       // 0 = chunked accumulation only when k exceeds the exactness budget; else the chunk length to force
   int host_blocks = 0;   // md_gemm_host: 0 = automatic panel plan, else the number of blocks of C (1 = no pipelining)
   int raster_group = 0;  // tile rows per raster group of the fused GEMM (0 = default 8)

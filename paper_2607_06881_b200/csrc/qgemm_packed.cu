@@ -563,28 +563,40 @@ cudaError_t launch_cfg(int m, int n, int k, const double* Ap, const double* Bp, 
   unsigned int* counters = static_cast<unsigned int*>(sk_ws);
   double* scratch = reinterpret_cast<double*>(static_cast<char*>(sk_ws) + SK_COUNTER_BYTES);
   cudaError_t err;
-  // Which schedule (all three give the same bits):
+  // Which schedule (all give the same bits):
   //   hand-over between the CTAs of a stream-K tile while every tile is cut or nearly so (small problems; measured: 512^3
   //   0.88 -> 0.92 of the peak with it, dd 4096^3 134.65 against 134.88 ms without);
   //   the static lists with red.add once whole-tile waves dominate;
-  //   the dynamic queue only on request (MD_OPT_TILE_SCHEDULE 1 / 2, wherever there is a whole wave).  MEASURED AND NOT MADE THE
-  //   DEFAULT (profiles/r04_dynamic_schedule.md): it does level the SMs' finishing times (quad double 2048^3: active cycles
-  //   per SM 124.6-126.2 M under the static lists, 126.1-126.4 M with the queue), but CTAs that have fallen out of lock-step no
-  //   longer fetch the same operand slabs at the same time, the L2 hit rate drops (dd 4096^3: 84 % -> 52 %, 18 -> 70 GB of DRAM
-  //   reads) and the DMMA pipe loses more than the balance gains: dd 4096^3 134.42 ms static, 134.29-134.38 hybrid, 135.12 queue
-  //   only; qd 2048^3 64.35 / 64.32 / 65.26.
+  //   the HYBRID from many waves on: every whole tile keeps its static place (tile = wave * G + cta: the CTAs stay in lock-step
+  //   and share operand slabs through L2) and only the k-units of the last, partial wave's tiles are claimed from the queue, so
+  //   that a CTA which has fallen behind claims fewer and all SMs finish within one unit's time.  It costs a red.add of the
+  //   accumulators per unit (16 per cut tile instead of about 2) and pays once the spread it removes is larger than that:
+  //   measured (profiles/r04_dynamic_schedule.md) quad double from about 10 whole waves on (1280^3 +0.001, 1536^3 +0.005,
+  //   2048^3 0.9747 -> 0.9796 of the peak; 1024^3, 6.9 waves: -0.012), double double, whose SMs finish within 0.1 % anyway, from
+  //   about 48 (3072^3, 31 waves: -0.0004; 4096^3, 55: +0.0003; 8192 x 8192 x 2048 with 9 quarters, 221: +0.002);
+  //   the queue for EVERYTHING only on request: it levels the finishing times too, but CTAs that claim whole tiles at their own
+  //   pace no longer fetch the same slabs at the same time (dd 4096^3: L2 hit rate 84 % -> 63 %, DRAM reads x 3) and lose more than
+  //   the balance returns (dd 4096^3 135.17 against 134.41 ms, qd 2048^3 65.31 against 64.40).
+  // MD_OPT_TILE_SCHEDULE: 0 = this rule, 1 = hybrid wherever there is a whole wave, 2 = queue only, 3 = never (static lists).
   const int sched_opt = tile_schedule();
-  const bool dynamic = sched_opt != 0 && plan.dp_waves >= 1;
+  const int hybrid_from = C::L >= 4 ? 10 : 48;  // whole-tile waves
+  const bool hybrid = (sched_opt == 1 && plan.dp_waves >= 1) || (sched_opt == 0 && plan.dp_waves >= hybrid_from);
+  const bool dynamic = hybrid || (sched_opt == 2 && plan.dp_waves >= 1);
   const bool handover = !dynamic && plan.dp_waves < HANDOVER_MAX_WAVES;
   if (dynamic) {
     // the tiles that are cut: the last partial wave, plus one whole wave when that is short -- the whole-tile phase ends with
     // the SMs spread over one tile time, and the cut tiles have to fill that triangle (about G / 2 tile times)
     int cut = plan.sk_tiles;
-    if (cut < (7 * G) / 10 && cut + G <= SK_MAX_TILES - 1) cut += G;
+    if (hybrid) {
+      if (cut == 0) cut = G;  // no partial wave: the last whole wave is the one that is cut
+    } else if (cut < (7 * G) / 10 && cut + G <= SK_MAX_TILES - 1) {
+      cut += G;
+    }
     constexpr int units = 16;
     plan.dyn_whole = (int)tiles - cut;
-    // 1: every whole-tile wave but the last one keeps the static assignment (lock-step, L2 sharing); 2: the queue from the start
-    plan.dyn_static = sched_opt == 1 && plan.dyn_whole / G > 0 ? plan.dyn_whole / G - 1 : 0;
+    // 1: EVERY whole tile keeps the static assignment (lock-step, L2 sharing) and only the k-units of the cut tiles are claimed;
+    // 2: the queue from the start
+    plan.dyn_static = hybrid ? plan.dyn_whole / G : 0;
     plan.dyn_unit = (plan.KS + units - 1) / units;
     plan.dyn_upt = (plan.KS + plan.dyn_unit - 1) / plan.dyn_unit;
     plan.dyn_items = plan.dyn_whole + cut * plan.dyn_upt;

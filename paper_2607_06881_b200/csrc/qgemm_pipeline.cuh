@@ -76,7 +76,7 @@ struct SkPlan {
 
 // Plan for `tiles` output tiles of KS slabs each on a grid of G persistent CTAs.
 int raster_group();  // api.cu: MD_OPT_RASTER_GROUP (default 8)
-int tile_schedule();  // api.cu: MD_OPT_TILE_SCHEDULE (0 = static lists, 1 = hybrid, 2 = tile queue only)
+int tile_schedule();  // api.cu: MD_OPT_TILE_SCHEDULE (0 = automatic, 1 = hybrid, 2 = tile queue only, 3 = static lists)
 inline SkPlan make_sk_plan(int tiles_m, int tiles_n, int KS, int G) {
   const long long tiles = (long long)tiles_m * tiles_n;
   SkPlan plan;

@@ -425,10 +425,11 @@ def test_row_sharded_md_gemm_is_bit_identical_to_the_unsharded_call(world, cfg_i
     (0, (1600, 1600, 64), 8, 8, 2),     # 25 x 50 = 1250 tiles = 8.4 waves, the queue from the first tile on
     (2, (1601, 1530, 8), 8, 8, 1),      # one slab per tile: the units are whole tiles; 7 static waves first
     (2, (1024, 1024, 7), 6, 6, 1),      # 6 slices of 19 bits
+    (4, (1100, 1500, 24), 16, 16, 0),   # qd, 35 x 47 = 1645 tiles = 11.1 waves: the AUTOMATIC rule takes the hybrid here
 ])
 def test_dynamic_tile_schedule_is_bit_identical_to_the_static_lists(cfg_idx, shape, Q, S, schedule):
-    """MD_OPT_TILE_SCHEDULE 1 / 2: the CTAs of the persistent kernel claim their tiles (and, at the end, k-units of the last tiles)
-    from a queue counter instead of walking static lists (an option; the static lists stay the default).  Every partial order sum is exact (R6), so the order matrices
+    """MD_OPT_TILE_SCHEDULE: the CTAs of the persistent kernel claim k-units of the last tiles (hybrid: 1, and 0 from many waves
+    on) or every tile (2) from a queue counter instead of walking static lists (3) -- DESIGN.md section 6.  Every partial order sum is exact (R6), so the order matrices
     and C must not differ in a bit from the static schedule, whichever CTA computed what -- repeated, because the assignment
     differs from run to run -- and the order matrices must equal the oracle's."""
     cfg, A, B = gen(cfg_idx, *shape)
@@ -437,7 +438,7 @@ def test_dynamic_tile_schedule_is_bit_identical_to_the_static_lists(cfg_idx, sha
     out = {}
     try:
         with md.Workspace(cfg.m, cfg.n, cfg.k, cfg.limbs, Q, bits=W, orders=S):
-            md.md_set_option(md.MD_OPT_TILE_SCHEDULE, 0)
+            md.md_set_option(md.MD_OPT_TILE_SCHEDULE, 3)
             out["static"] = (host(md.md_gemm_orders(dA, dB)), host(md.md_gemm(dA, dB)))
             md.md_set_option(md.MD_OPT_TILE_SCHEDULE, schedule)
             for rep in range(3):
