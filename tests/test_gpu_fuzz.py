@@ -76,3 +76,54 @@ def test_random_case(case):
         assert (r["err"] <= TOL[L] * r["W"]).all(), float((r["err"] / (TOL[L] * r["W"])).max())
     for l in range(L - 1):
         assert (np.abs(Cn[l + 1]) <= np.spacing(np.abs(Cn[l])) / 2).all()
+
+
+@pytest.mark.parametrize("case", range(20))
+def test_random_multiwave_case(case):
+    """Larger random shapes (short contractions, so that the oracle stays cheap): several to dozens of whole-tile waves on the
+    persistent kernels.  Double / quad double: every tile schedule (MD_OPT_TILE_SCHEDULE automatic, hybrid, queue only) against
+    the static lists bit for bit, C and order matrices; all formats: sampled order matrices against the oracle and the fused
+    epilogue against the standalone md_renorm.  (A one-off run of this generator over 24 182 cases, incl. hexa double through
+    its one-range-at-a-time kernel and md_gemm_static, found no difference.)"""
+    rng = np.random.default_rng(5000 + case)
+    kind = ("dd", "qd", "dd", "hd", "od")[case % 5]
+    if kind == "dd":
+        L, Q, cfg_idx = 2, int(rng.choice([8, 9])), int(rng.choice([0, 1, 2, 3]))
+        m, n, k = int(rng.integers(1200, 4200)), int(rng.integers(1200, 4200)), int(rng.integers(1, 70))
+    elif kind == "qd":
+        L, Q, cfg_idx = 4, 16, 4
+        m, n, k = int(rng.integers(700, 2400)), int(rng.integers(700, 2400)), int(rng.integers(1, 50))
+    elif kind == "hd":
+        L, Q, cfg_idx = 16, 64, 6
+        m, n, k = int(rng.integers(33, 800)), int(rng.integers(17, 600)), int(rng.integers(1, 40))
+    else:
+        L, Q, cfg_idx = 8, 32, 5
+        m, n, k = int(rng.integers(33, 1200)), int(rng.integers(17, 1000)), int(rng.integers(1, 40))
+    S = Q + 1 if (kind == "dd" and Q == 8 and case % 2) else Q
+    base = inputs.CONFIGS[cfg_idx]
+    cfg = inputs.Config(base.index, base.name, m, n, k, L, 9000 + case, base.dist)
+    A, B = inputs.generate(cfg, "A"), inputs.generate(cfg, "B")
+    dA, dB = dev(A), dev(B)
+    schedules = (3, 0, 1, 2) if L <= 4 else (0,)
+    res = {}
+    try:
+        with md.Workspace(m, n, k, L, Q, orders=(S if S != Q else 0)):
+            for ts in schedules:
+                md.md_set_option(md.MD_OPT_TILE_SCHEDULE, ts)
+                res[ts] = (md.md_gemm(dA, dB), md.md_gemm_orders(dA, dB))
+            assert md.md_read_flags() == 0
+    finally:
+        md.md_set_option(md.MD_OPT_TILE_SCHEDULE, 0)
+    C, orders = res[schedules[0]]
+    for ts in schedules[1:]:
+        assert bool((res[ts][0] == C).all()) and bool((res[ts][1] == orders).all()), ts
+    si, sj = rng.integers(0, m, 1500), rng.integers(0, n, 1500)
+    Aq, eA, _ = orc.split(A, 0, Q)
+    Bq, eB, _ = orc.split(B, 1, Q)
+    want = orc.orders_int_samples(Aq, eA, Bq, eB, si, sj, orders=S)
+    assert bool((orders[:, si, sj].T.cpu().numpy() == want).all())
+    if S == Q:
+        assert bool((C == md.md_renorm(orders, L)).all())
+    r = orc.exact_samples(A, B, si[:200], sj[:200], C.cpu().numpy())
+    bound = k * (Q + 3) * np.ldexp(1.0, (eA[si[:200]] + eB[sj[:200]] - 13 * Q - 2).astype(np.int32))
+    assert (r["err"] <= bound + np.abs(C[0, si[:200], sj[:200]].cpu().numpy()) * 2.0 ** (-53 * L + 1)).all()
