@@ -265,10 +265,17 @@ def test_flags_and_runtime_errors():
         assert e2.value.status == md.MD_ERR_WORKSPACE
 
 
-def test_on_a_side_stream_and_in_a_cuda_graph():
-    cfg, A, B = gen(2, 100, 60, 140)
+@pytest.mark.parametrize("cfg_idx,shape", [
+    (2, (100, 60, 140)),      # the one-launch kernel
+    (2, (700, 500, 90)),      # cooperative preparation kernel + the GEMM behind it as a programmatic dependent launch
+    (4, (1100, 1500, 24)),    # quad double, 11 whole-tile waves: the hybrid tile schedule (queue counter cleared by a memset node)
+])
+def test_on_a_side_stream_and_in_a_cuda_graph(cfg_idx, shape):
+    """md_gemm only enqueues: on a side stream, captured in a CUDA graph and REPLAYED TWICE (what a call leaves behind in the
+    workspace -- counters, flags, the tile queue -- must not leak into the next replay)."""
+    cfg, A, B = gen(cfg_idx, *shape)
     dA, dB = dev(A), dev(B)
-    with md.Workspace(cfg.m, cfg.n, cfg.k, 2):
+    with md.Workspace(cfg.m, cfg.n, cfg.k, cfg.limbs, 4 * cfg.limbs):
         ref = md.md_gemm(dA, dB).clone()
         s = torch.cuda.Stream()
         s.wait_stream(torch.cuda.current_stream())
@@ -279,6 +286,10 @@ def test_on_a_side_stream_and_in_a_cuda_graph():
             out.zero_()
             with torch.cuda.graph(graph, stream=s):
                 md.md_gemm(dA, dB, out)
+            graph.replay()
+            s.synchronize()
+            assert bool((out == ref).all())
+            out.zero_()
             graph.replay()
         s.synchronize()
         assert bool((out == ref).all())
