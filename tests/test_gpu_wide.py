@@ -175,6 +175,21 @@ def test_hexa_double_passes_kernel_whole_tiles_and_stream_k_parts(shape):
     assert (r["err"] <= TOL[16] * r["W"]).all()
 
 
+@pytest.mark.parametrize("cfg_idx,shape", [(6, (200, 160, 40)), (6, (600, 300, 12)), (5, (300, 200, 24))])
+def test_md_qgemm_on_oracle_quarters_with_both_outputs(cfg_idx, shape):
+    """The public md_qgemm on PLAIN quarter planes (the oracle's) for the wide formats: they are repacked into the workspace in the
+    tile shape of the kernel that runs them (hexa double: 32 x 16, one order range at a time), and one launch writes BOTH the order
+    matrices and C -- whole tiles and stream-K parts.  Orders bit-exact against the oracle, C == md_renorm of them."""
+    cfg, A, B = gen(cfg_idx, *shape)
+    L, Q = cfg.limbs, cfg.quarters
+    Aq, eA, _ = orc.split(A, 0)
+    Bq, eB, _ = orc.split(B, 1)
+    with md.Workspace(cfg.m, cfg.n, cfg.k, L, Q):
+        orders, C = md.md_qgemm(dev(Aq), dev(Bq), L, want_orders=True, want_C=True)
+    assert bool((host(orders) == orc.orders_int(Aq, eA, Bq, eB)).all())
+    assert bool((C == md.md_renorm(orders, L)).all())
+
+
 def test_unsupported_and_budget_errors():
     cfg, A, B = gen(5, 16, 16, 16)
     with md.Workspace(16, 16, 16, 8):
