@@ -69,6 +69,8 @@ def parse_args():
     ap.add_argument("--orders", type=int, default=0, help="kept product orders S (MD_OPT_ORDERS); default = quarters")
     ap.add_argument("--raster-group", type=int, default=0, help="MD_OPT_RASTER_GROUP (tile rows per raster group; 0 = default)")
     ap.add_argument("--host-blocks", type=int, default=0, help="MD_OPT_HOST_BLOCKS for the e2e leg (0 = automatic; n = blocks of C; PR * 256 + PC = explicit panels)")
+    ap.add_argument("--tile", type=int, default=0, choices=(0, 1, 2),
+                    help="MD_OPT_TILE (double double): 0 = automatic, 1 = the 32 x 16 CTA tile wherever it exists, 2 = never")
     ap.add_argument("--tile-schedule", type=int, default=0, choices=(0, 1, 2, 3),
                     help="MD_OPT_TILE_SCHEDULE: 0 = automatic (hybrid from many whole-tile waves on), 1 = hybrid wherever possible, 2 = tile queue only, 3 = static lists")
     ap.add_argument("--one-launch", type=int, default=0, choices=[0, 1, 2],
@@ -410,6 +412,7 @@ def run_ours(args):
     md.md_set_option(md.MD_OPT_RASTER_GROUP, args.raster_group)
     md.md_set_option(md.MD_OPT_ONE_LAUNCH, args.one_launch)
     md.md_set_option(md.MD_OPT_TILE_SCHEDULE, args.tile_schedule)
+    md.md_set_option(md.MD_OPT_TILE, args.tile)
     md.md_set_option(md.MD_OPT_HOST_BLOCKS, args.host_blocks)
     # weak scaling: the global A has world * m rows, rank r owns one block of m rows (no collective on the data path)
     if args.slices == "adaptive":

@@ -97,8 +97,8 @@ enum {
                             in ONE cooperative launch when (m + n) * k <= 2^23 elements, five launches otherwise; 1 = always; 2 = never.
                             Same bits either way. */
   MD_OPT_TILE = 7,       /* md_gemm / md_gemm_orders, double double with 8 or 6 slices: 0 = automatic -- the 32 x 16 CTA tile
-                            instance of the fused kernel when the 64 x 32 tiles would number at most two thirds of the SMs
-                            (up to about 448^3), 64 x 32 otherwise; 1 = 32 x 16 wherever it exists; 2 = never.  Same bits. */
+                            instance of the fused kernel when the 64 x 32 tiles would number at most 0.45 of the SMs
+                            (up to about 352^3), 64 x 32 otherwise; 1 = 32 x 16 wherever it exists; 2 = never.  Same bits. */
   MD_OPT_RASTER_GROUP = 8, /* fused quarter GEMM: tile rows per raster group (the CTAs in flight cover GROUP x (SMs / GROUP) tiles of C and
                             share their operand slabs through L2).  0 = default 8 (the best of the measured 4 / 8 / 16 / 32,
                             profiles/).  Same bits for any value. */

@@ -67,7 +67,10 @@ static bool use_small_tiles(int m, int n, int limbs, int Q, int S) {
   if (g_opt.tile == 1) return true;
   const int G = sk_grid();
   const long long tiles = ((long long)m + 63) / 64 * (((long long)n + 31) / 32);
-  return G > 0 && 3 * tiles <= 2 * G;  // measured on dd n^3: faster up to n = 448 (98 tiles), slower from n = 512 (128 tiles)
+  // measured on dd n^3 with the stream-K hand-over in place (profiles/r04_small_sizes.md section 8): the small tile is faster up
+  // to n = 352 (66 large tiles: 0.80 against 0.75 of the peak), even at 368 and slower from n = 384 (72 tiles: 0.82 against 0.85).
+  // (Before the hand-over, when every cut tile went through L2 atomics, it won up to 448.)
+  return G > 0 && 20 * tiles <= 9 * G;
 }
 
 // Which fused kernel runs (limbs, Q, S) on an m x n x k problem, and hence the packed layout the splitter writes for it:
