@@ -546,7 +546,11 @@ qgemm_packed_kernel(int m, int n, SkPlan plan, const double* __restrict__ Ap, co
   }
 }
 
-constexpr int HANDOVER_MAX_WAVES = 8;  // whole-tile waves from which the stream-K tail goes through red.add (launch_cfg)
+// whole-tile waves from which the stream-K tail goes through red.add (launch_cfg).  Re-measured on the final build (hand-over
+// against red.add, fraction of the peak): dd 768^3 (1 whole wave) 0.965 / 0.952, qd 768^3 (3) 0.9715 / 0.9699, dd 1024^3 (3)
+// 0.9724 / 0.9733, dd 1280^3 (5) 0.9788 / 0.9799, qd 1024^3 (6) 0.9729 / 0.9763, dd 1536^3 (7) 0.9819 / 0.9831, dd 2048^3 (13)
+// 0.9841 / 0.9862 -- the hand-over pays while the cut tiles are a large part of the work
+constexpr int HANDOVER_MAX_WAVES = 4;
 
 // Exact orders over the whole k, persistent stream-K.
 template <class C>
